@@ -1,0 +1,133 @@
+/*
+ * lrux.h -- C ABI of the B200-native low-rank determinant / Pfaffian update library.
+ *
+ * Hot path of "lrux: Fast low-rank updates of determinants and Pfaffians"
+ * (arxiv/paper_2602_05255; citations are PAPER.md line numbers) for W independent
+ * Monte-Carlo walkers, every step running in hand-written sm_100a CUDA kernels.
+ *
+ * Conventions
+ *  - Every d_* pointer is DEVICE memory owned by the caller.  The library never
+ *    allocates or frees device memory and holds no global state; the only host
+ *    allocation is the small handle.  `d_state` and `d_info` must outlive the handle.
+ *  - `stream` is a cudaStream_t passed as void*.  Every call is asynchronous and
+ *    stream-ordered on it; no call synchronises the device.
+ *  - Matrices are row-major.  LRUX_C128 data is interleaved (re,im) doubles at the
+ *    ABI.  All transposes in the method are plain, never conjugate.
+ *  - Host-detectable misuse returns a status and does nothing.  Conditions only
+ *    visible on the device set sticky bits in d_info[w] and never trap:
+ *      1 = singular A0 at init (zero pivot)
+ *      2 = proposal index out of range or duplicated (ratio returned as NaN)
+ *      4 = accepted update with singular / non-finite R (state left unchanged,
+ *          treated as rejected)
+ */
+#ifndef LRUX_H_
+#define LRUX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LRUX_MAX_K 8 /* largest kmax accepted by *_init */
+
+typedef struct lrux_handle_s* lrux_handle_t; /* small HOST object */
+typedef enum { LRUX_F64 = 0, LRUX_C128 = 1 } lrux_dtype_t;
+typedef enum {
+  LRUX_OK = 0,
+  LRUX_EINVAL = 1,      /* bad size / odd n for Pf / k > kmax / null pointer */
+  LRUX_ESTATE = 2,      /* accept without a pending ratio; det call on a pf handle */
+  LRUX_EWORKSPACE = 3,  /* state_bytes too small */
+  LRUX_EUNSUPPORTED = 4,
+  LRUX_ECUDA = 5        /* a CUDA launch failed */
+} lrux_status_t;
+
+/* ---------------------------------------------------------------- determinant
+ * State per walker: A^{-1} (stored transposed, so that the k columns a row
+ * replacement needs are contiguous), the amplitude det A as (phase, log|det|)
+ * (cf. slogpf), a pending proposal, and -- when K > 0 -- the delay
+ * buffers a_t, b_t of Eq. 10-11.
+ */
+
+/* Bytes of d_state needed for W walkers of n x n matrices, proposals of at most
+ * kmax rows and delay depth K (0 = immediate updates). */
+lrux_status_t lrux_det_state_bytes(int64_t W, int32_t n, int32_t kmax, int32_t K,
+                                   lrux_dtype_t dt, size_t* bytes);
+
+/* Build A^{-1} and (phase, log|det A|) per walker by partial-pivot elimination
+ * (the O(n^3) seed of PAPER.md:74-75, 97-98, 203).
+ *   d_A0    [W][n][n] row-major, read only
+ *   d_state caller-owned buffer of >= state_bytes bytes, 256-byte aligned
+ *   d_info  [W] int32, zeroed by this call, then sticky (see bits above) */
+lrux_status_t lrux_det_init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, int32_t K,
+                            lrux_dtype_t dt, const void* d_A0, void* d_state,
+                            size_t state_bytes, int32_t* d_info, void* stream);
+
+/* One proposal per walker: replace the k rows d_idx[w][0..k) of A_w by the new
+ * rows d_rows[w][a][0..n) (Eq. 8 with one-hot v).  Writes
+ * r_w = det A'_w / det A_w = det(1 + u^T A^{-1} v) (Eq. 2-4) to
+ * d_ratio[w], evaluated against the effective current inverse (Eq. 13 when the
+ * delay buffer is non-empty), and leaves the proposal pending.
+ * 1 <= k <= kmax, indices distinct in [0,n).  A second ratio before accept
+ * replaces the pending proposal.  d_idx/d_rows need only stay valid until this
+ * call's work completes on `stream`. */
+lrux_status_t lrux_det_ratio(lrux_handle_t h, int32_t k, const int32_t* d_idx /*[W][k]*/,
+                             const void* d_rows /*[W][k][n]*/, void* d_ratio /*[W]*/,
+                             void* stream);
+
+/* Apply the pending proposal where d_mask[w] != 0: Woodbury update of the stored
+ * inverse (Eq. 5) when K == 0, else append (a_t, b_t) to the delay
+ * buffer (Eq. 14-15) and fold the buffer of every walker whose
+ * depth reached K (Eq. 12).  Amplitude *= r.  Clears the pending
+ * proposal of every walker. */
+lrux_status_t lrux_det_accept(lrux_handle_t h, const uint8_t* d_mask /*[W]*/, void* stream);
+
+/* Fold every non-empty delay buffer into A^{-1} (Eq. 12). No-op when K == 0. */
+lrux_status_t lrux_det_flush(lrux_handle_t h, void* stream);
+
+/* d_phase [W] elements (+-1 real, unit complex), d_logabs [W] doubles. */
+lrux_status_t lrux_det_get_amplitude(lrux_handle_t h, void* d_phase, double* d_logabs,
+                                     void* stream);
+/* d_out [W][n][n] row-major A^{-1}.  Implies flush. */
+lrux_status_t lrux_det_get_inverse(lrux_handle_t h, void* d_out, void* stream);
+
+/* ---------------------------------------------------------------- Pfaffian
+ * A_w is skew-symmetric, n even.  Replacing the orbital in slot p changes row p
+ * and column p of A (Eq. 23-24): a rank-2k skew update
+ * A' = A - u J u^T (Eq. 16).  State: A^{-1} (exactly skew), the
+ * amplitude pf A as (phase, log|pf|), pending proposal, and for K > 0 the
+ * buffers a_t, R_t^{-1} of Eq. 25-26.
+ */
+lrux_status_t lrux_pf_state_bytes(int64_t W, int32_t n, int32_t kmax, int32_t K,
+                                  lrux_dtype_t dt, size_t* bytes);
+/* d_A0 [W][n][n]: only the strict upper triangle is read.  pf by Parlett-Reid
+ * elimination with pivoting (PAPER.md:445 leaves the algorithm open). */
+lrux_status_t lrux_pf_init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, int32_t K,
+                           lrux_dtype_t dt, const void* d_A0, void* d_state,
+                           size_t state_bytes, int32_t* d_info, void* stream);
+/* d_rows[w][a][0..n) is the NEW row d_idx[w][a] of A' (so column d_idx[w][a] is
+ * its negative), including the crossing entries A'[p_a][p_b]; the entry at its
+ * own index p_a is ignored (zero diagonal).  r_w = pf A'/pf A = pf R / pf J
+ * (Eq. 19-20). */
+lrux_status_t lrux_pf_ratio(lrux_handle_t h, int32_t k, const int32_t* d_idx,
+                            const void* d_rows, void* d_ratio, void* stream);
+/* Eq. 21 (k=1: Eq. 22), with an exactly skew R^{-1}; delayed:
+ * Eq. 28 append, Eq. 26 fold. */
+lrux_status_t lrux_pf_accept(lrux_handle_t h, const uint8_t* d_mask, void* stream);
+lrux_status_t lrux_pf_flush(lrux_handle_t h, void* stream);
+lrux_status_t lrux_pf_get_amplitude(lrux_handle_t h, void* d_phase, double* d_logabs,
+                                    void* stream);
+lrux_status_t lrux_pf_get_inverse(lrux_handle_t h, void* d_out, void* stream);
+
+/* ---------------------------------------------------------------- common */
+/* Number of kernel launches the library has enqueued through this handle so far
+ * (host counter; bench.py reports it as gpu_launches). */
+lrux_status_t lrux_launch_count(lrux_handle_t h, int64_t* count);
+lrux_status_t lrux_destroy(lrux_handle_t h);
+const char* lrux_status_string(lrux_status_t s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LRUX_H_ */

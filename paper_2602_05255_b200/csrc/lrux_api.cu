@@ -1,0 +1,239 @@
+// C-ABI entry points (include/lrux.h): argument checks, state layout, dispatch.
+#include <new>
+
+#include "lrux_internal.h"
+
+namespace lrux {
+
+static inline size_t align_up(size_t x) { return (x + 255) & ~size_t(255); }
+
+size_t state_layout(State* st, void* base, int64_t W, int32_t n, int32_t kmax, int32_t K,
+                    int32_t dt, int32_t kind) {
+  const size_t e = dt == LRUX_C128 ? 16 : 8;
+  const size_t kc = kind == KIND_PF ? 2 * (size_t)kmax : (size_t)kmax;
+  const size_t cap = (size_t)K * kc;
+  size_t off = 0;
+  char* b = (char*)base;
+  auto take = [&](size_t bytes) {
+    void* p = b ? (void*)(b + off) : nullptr;
+    off = align_up(off + bytes);
+    return p;
+  };
+  State s{};
+  s.W = W; s.n = n; s.kmax = kmax; s.K = K; s.kc = (int32_t)kc; s.cap = (int32_t)cap;
+  s.dt = dt; s.kind = kind;
+  s.Ti = take((size_t)W * n * n * e);
+  s.phase = take((size_t)W * e);
+  s.logabs = (double*)take((size_t)W * 8);
+  s.fill = (int32_t*)take((size_t)W * 4);
+  s.nupd = (int32_t*)take((size_t)W * 4);
+  s.pend_idx = (int32_t*)take((size_t)W * kmax * 4);
+  s.pend_ok = (uint8_t*)take((size_t)W);
+  s.pend_ratio = take((size_t)W * e);
+  s.pend_Rinv = take((size_t)W * kc * kc * e);
+  s.pend_C = take((size_t)W * kmax * n * e);
+  s.pend_N = take((size_t)W * kmax * n * e);
+  if (kind == KIND_PF) {
+    s.pend_Y = take((size_t)W * kmax * n * e);
+    s.pend_AN = cap ? take((size_t)W * kmax * cap * e) : nullptr;
+  } else {
+    s.pend_Y = cap ? take((size_t)W * kmax * cap * e) : nullptr;
+    s.pend_AN = nullptr;
+  }
+  s.Abuf = cap ? take((size_t)W * cap * n * e) : nullptr;
+  s.Bbuf = cap ? take((size_t)W * cap * n * e) : nullptr;
+  s.list = (int32_t*)take((size_t)W * 4);
+  s.flist = (int32_t*)take((size_t)W * 4);
+  s.counters = (int32_t*)take(8 * 4);
+  if (st) *st = s;
+  return off;
+}
+
+static lrux_status_t check_dims(int64_t W, int32_t n, int32_t kmax, int32_t K, int dt, int kind) {
+  if (W <= 0 || n <= 0 || kmax <= 0 || kmax > LRUX_MAX_K || K < 0) return LRUX_EINVAL;
+  if (dt != LRUX_F64 && dt != LRUX_C128) return LRUX_EINVAL;
+  if (kind == KIND_PF && (n % 2 != 0)) return LRUX_EINVAL;
+  if (kmax > n) return LRUX_EINVAL;
+  if (W > (int64_t)2000000000) return LRUX_EINVAL;
+  return LRUX_OK;
+}
+
+static lrux_status_t state_bytes(int64_t W, int32_t n, int32_t kmax, int32_t K, lrux_dtype_t dt,
+                                 size_t* bytes, int kind) {
+  if (!bytes) return LRUX_EINVAL;
+  lrux_status_t s = check_dims(W, n, kmax, K, dt, kind);
+  if (s != LRUX_OK) return s;
+  *bytes = state_layout(nullptr, nullptr, W, n, kmax, K, dt, kind);
+  return LRUX_OK;
+}
+
+static lrux_status_t init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, int32_t K,
+                          lrux_dtype_t dt, const void* d_A0, void* d_state, size_t sb,
+                          int32_t* d_info, void* stream, int kind) {
+  if (!h || !d_A0 || !d_state || !d_info) return LRUX_EINVAL;
+  lrux_status_t s = check_dims(W, n, kmax, K, dt, kind);
+  if (s != LRUX_OK) return s;
+  if (((uintptr_t)d_state & 255) != 0) return LRUX_EINVAL;
+  size_t need = state_layout(nullptr, nullptr, W, n, kmax, K, dt, kind);
+  if (sb < need) return LRUX_EWORKSPACE;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return LRUX_ECUDA;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return LRUX_ECUDA;
+  lrux_handle_s* hh = new (std::nothrow) lrux_handle_s();
+  if (!hh) return LRUX_EINVAL;
+  state_layout(&hh->st, d_state, W, n, kmax, K, dt, kind);
+  hh->st.info = d_info;
+  hh->pending_k = 0;
+  hh->launches = 0;
+  hh->num_sms = sms;
+  int nl = kind == KIND_DET ? launch_det_init(hh->st, d_A0, (cudaStream_t)stream)
+                            : launch_pf_init(hh->st, d_A0, (cudaStream_t)stream);
+  if (nl < 0) {
+    delete hh;
+    return LRUX_ECUDA;
+  }
+  hh->launches += nl;
+  *h = hh;
+  return LRUX_OK;
+}
+
+}  // namespace lrux
+
+using namespace lrux;
+
+#define LRUX_CHECK_HANDLE(h, KIND_)          \
+  if (!(h)) return LRUX_EINVAL;              \
+  if ((h)->st.kind != (KIND_)) return LRUX_ESTATE;
+
+#define LRUX_COUNT(h, expr)          \
+  do {                               \
+    int nl__ = (expr);               \
+    if (nl__ < 0) return LRUX_ECUDA; \
+    (h)->launches += nl__;           \
+  } while (0)
+
+extern "C" {
+
+lrux_status_t lrux_det_state_bytes(int64_t W, int32_t n, int32_t kmax, int32_t K, lrux_dtype_t dt,
+                                   size_t* bytes) {
+  return state_bytes(W, n, kmax, K, dt, bytes, KIND_DET);
+}
+lrux_status_t lrux_pf_state_bytes(int64_t W, int32_t n, int32_t kmax, int32_t K, lrux_dtype_t dt,
+                                  size_t* bytes) {
+  return state_bytes(W, n, kmax, K, dt, bytes, KIND_PF);
+}
+
+lrux_status_t lrux_det_init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, int32_t K,
+                            lrux_dtype_t dt, const void* d_A0, void* d_state, size_t state_bytes,
+                            int32_t* d_info, void* stream) {
+  return init(h, W, n, kmax, K, dt, d_A0, d_state, state_bytes, d_info, stream, KIND_DET);
+}
+lrux_status_t lrux_pf_init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, int32_t K,
+                           lrux_dtype_t dt, const void* d_A0, void* d_state, size_t state_bytes,
+                           int32_t* d_info, void* stream) {
+  return init(h, W, n, kmax, K, dt, d_A0, d_state, state_bytes, d_info, stream, KIND_PF);
+}
+
+lrux_status_t lrux_det_ratio(lrux_handle_t h, int32_t k, const int32_t* d_idx, const void* d_rows,
+                             void* d_ratio, void* stream) {
+  LRUX_CHECK_HANDLE(h, KIND_DET);
+  if (k < 1 || k > h->st.kmax || !d_idx || !d_rows || !d_ratio) return LRUX_EINVAL;
+  LRUX_COUNT(h, launch_det_ratio(h->st, k, d_idx, d_rows, d_ratio, (cudaStream_t)stream));
+  h->pending_k = k;
+  return LRUX_OK;
+}
+lrux_status_t lrux_pf_ratio(lrux_handle_t h, int32_t k, const int32_t* d_idx, const void* d_rows,
+                            void* d_ratio, void* stream) {
+  LRUX_CHECK_HANDLE(h, KIND_PF);
+  if (k < 1 || k > h->st.kmax || !d_idx || !d_rows || !d_ratio) return LRUX_EINVAL;
+  LRUX_COUNT(h, launch_pf_ratio(h->st, k, d_idx, d_rows, d_ratio, h->num_sms, (cudaStream_t)stream));
+  h->pending_k = k;
+  return LRUX_OK;
+}
+
+lrux_status_t lrux_det_accept(lrux_handle_t h, const uint8_t* d_mask, void* stream) {
+  LRUX_CHECK_HANDLE(h, KIND_DET);
+  if (!d_mask) return LRUX_EINVAL;
+  if (h->pending_k == 0) return LRUX_ESTATE;
+  LRUX_COUNT(h, launch_det_accept(h->st, h->pending_k, d_mask, h->num_sms, (cudaStream_t)stream));
+  h->pending_k = 0;
+  return LRUX_OK;
+}
+lrux_status_t lrux_pf_accept(lrux_handle_t h, const uint8_t* d_mask, void* stream) {
+  LRUX_CHECK_HANDLE(h, KIND_PF);
+  if (!d_mask) return LRUX_EINVAL;
+  if (h->pending_k == 0) return LRUX_ESTATE;
+  LRUX_COUNT(h, launch_pf_accept(h->st, h->pending_k, d_mask, h->num_sms, (cudaStream_t)stream));
+  h->pending_k = 0;
+  return LRUX_OK;
+}
+
+lrux_status_t lrux_det_flush(lrux_handle_t h, void* stream) {
+  LRUX_CHECK_HANDLE(h, KIND_DET);
+  if (h->st.K == 0) return LRUX_OK;
+  LRUX_COUNT(h, launch_det_flush(h->st, true, h->num_sms, (cudaStream_t)stream));
+  return LRUX_OK;
+}
+lrux_status_t lrux_pf_flush(lrux_handle_t h, void* stream) {
+  LRUX_CHECK_HANDLE(h, KIND_PF);
+  if (h->st.K == 0) return LRUX_OK;
+  LRUX_COUNT(h, launch_pf_flush(h->st, true, h->num_sms, (cudaStream_t)stream));
+  return LRUX_OK;
+}
+
+lrux_status_t lrux_det_get_amplitude(lrux_handle_t h, void* d_phase, double* d_logabs,
+                                     void* stream) {
+  LRUX_CHECK_HANDLE(h, KIND_DET);
+  if (!d_phase || !d_logabs) return LRUX_EINVAL;
+  LRUX_COUNT(h, launch_get_amplitude(h->st, d_phase, d_logabs, (cudaStream_t)stream));
+  return LRUX_OK;
+}
+lrux_status_t lrux_pf_get_amplitude(lrux_handle_t h, void* d_phase, double* d_logabs,
+                                    void* stream) {
+  LRUX_CHECK_HANDLE(h, KIND_PF);
+  if (!d_phase || !d_logabs) return LRUX_EINVAL;
+  LRUX_COUNT(h, launch_get_amplitude(h->st, d_phase, d_logabs, (cudaStream_t)stream));
+  return LRUX_OK;
+}
+
+lrux_status_t lrux_det_get_inverse(lrux_handle_t h, void* d_out, void* stream) {
+  LRUX_CHECK_HANDLE(h, KIND_DET);
+  if (!d_out) return LRUX_EINVAL;
+  if (h->st.K > 0) LRUX_COUNT(h, launch_det_flush(h->st, true, h->num_sms, (cudaStream_t)stream));
+  LRUX_COUNT(h, launch_get_inverse(h->st, d_out, (cudaStream_t)stream));
+  return LRUX_OK;
+}
+lrux_status_t lrux_pf_get_inverse(lrux_handle_t h, void* d_out, void* stream) {
+  LRUX_CHECK_HANDLE(h, KIND_PF);
+  if (!d_out) return LRUX_EINVAL;
+  if (h->st.K > 0) LRUX_COUNT(h, launch_pf_flush(h->st, true, h->num_sms, (cudaStream_t)stream));
+  LRUX_COUNT(h, launch_get_inverse(h->st, d_out, (cudaStream_t)stream));
+  return LRUX_OK;
+}
+
+lrux_status_t lrux_launch_count(lrux_handle_t h, int64_t* count) {
+  if (!h || !count) return LRUX_EINVAL;
+  *count = h->launches;
+  return LRUX_OK;
+}
+
+lrux_status_t lrux_destroy(lrux_handle_t h) {
+  if (!h) return LRUX_EINVAL;
+  delete h;
+  return LRUX_OK;
+}
+
+const char* lrux_status_string(lrux_status_t s) {
+  switch (s) {
+    case LRUX_OK: return "LRUX_OK";
+    case LRUX_EINVAL: return "LRUX_EINVAL: invalid argument";
+    case LRUX_ESTATE: return "LRUX_ESTATE: call not valid in this state";
+    case LRUX_EWORKSPACE: return "LRUX_EWORKSPACE: state buffer too small";
+    case LRUX_EUNSUPPORTED: return "LRUX_EUNSUPPORTED";
+    case LRUX_ECUDA: return "LRUX_ECUDA: CUDA error";
+  }
+  return "LRUX_?";
+}
+
+}  // extern "C"

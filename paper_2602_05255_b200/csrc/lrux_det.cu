@@ -1,0 +1,657 @@
+// Determinant hot path.
+//
+// New-rows-only forms used here (readings 5/5b), with P the k
+// replaced row indices, N (k x n) the new rows, C = A^-1[:,P]:
+//   R = 1 + u^T A^-1 v = N C                                  (Eq. 4)
+//   u^T A^-1 = N A^-1 - I[P,:]  =: Wm
+//   A'^-1 = A^-1 - C R^-1 Wm                                  (Eq. 5)
+// State Ti = A^-T row-major, so C[:,a] is the contiguous row P[a] of Ti and column
+// j of Wm depends only on row j of Ti: the update is a single pass over Ti.
+#include "lrux_common.cuh"
+#include "lrux_internal.h"
+
+namespace lrux {
+
+// ---------------------------------------------------------------- ratio (a1, a2, a5)
+// One CTA per walker.  Gathers C_eff = A_eff^-1[:,P] (Eq. 14 when the delay buffer
+// holds factors), stashes C_eff and N in the pending area, R = N C_eff, r = det R.
+template <typename T>
+__global__ void __launch_bounds__(128)
+det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __restrict__ rows,
+                 T* __restrict__ ratio_out) {
+  using S = Sc<T>;
+  __shared__ T Rs[kMaxK * kMaxK];
+  __shared__ T Ri[kMaxK * kMaxK];
+  __shared__ int sidx[kMaxK];
+  __shared__ int bad;
+  const int w = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
+  const int warp = tid >> 5, lane = tid & 31, nw = nt >> 5;
+  const int n = st.n, kmax = st.kmax;
+  if (w == 0 && tid == 0) st.counters[0] = 0;
+  if (tid == 0) {
+    int b = 0;
+    for (int a = 0; a < k; ++a) {
+      int p = idx[(size_t)w * k + a];
+      sidx[a] = p;
+      if (p < 0 || p >= n) b = 1;
+      for (int c = 0; c < a; ++c)
+        if (sidx[c] == p) b = 1;
+    }
+    bad = b;
+  }
+  __syncthreads();
+  if (bad) {
+    if (tid == 0) {
+      ratio_out[w] = S::nan();
+      ((T*)st.pend_ratio)[w] = S::nan();
+      st.pend_ok[w] = 0;
+      atomicOr(&st.info[w], 2);
+    }
+    return;
+  }
+  const int fill = st.cap ? st.fill[w] : 0;
+  const T* Tw = (const T*)st.Ti + (size_t)w * n * n;
+  const T* Ab = st.cap ? (const T*)st.Abuf + (size_t)w * st.cap * n : nullptr;
+  const T* Bb = st.cap ? (const T*)st.Bbuf + (size_t)w * st.cap * n : nullptr;
+  T* pC = (T*)st.pend_C + (size_t)w * kmax * n;
+  T* pN = (T*)st.pend_N + (size_t)w * kmax * n;
+  for (int a = 0; a < k; ++a) {
+    const int p = sidx[a];
+    for (int i = tid; i < n; i += nt) {
+      T c = Tw[(size_t)p * n + i];
+      for (int s = 0; s < fill; ++s)   // Eq. 14: a_tau = A0^-1 v - sum_t a_t (b_t^T v)
+        c = S::fnma(Bb[(size_t)s * n + p], Ab[(size_t)s * n + i], c);
+      pC[(size_t)a * n + i] = c;
+      pN[(size_t)a * n + i] = rows[((size_t)w * k + a) * n + i];
+    }
+  }
+  __syncthreads();
+  for (int pr = warp; pr < k * k; pr += nw) {
+    const int a = pr / k, b = pr % k;
+    T acc = S::zero();
+    for (int i = lane; i < n; i += 32) acc = S::fma(pN[(size_t)a * n + i], pC[(size_t)b * n + i], acc);
+    acc = warp_sum(acc);
+    if (lane == 0) Rs[a * kMaxK + b] = acc;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    bool ok;
+    T det = small_det_inv(Rs, Ri, k, kMaxK, &ok);
+    ratio_out[w] = det;
+    ((T*)st.pend_ratio)[w] = det;
+    st.pend_ok[w] = ok ? 1 : 0;
+    T* pR = (T*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
+    for (int a = 0; a < k; ++a) {
+      st.pend_idx[(size_t)w * kmax + a] = sidx[a];
+      for (int b = 0; b < k; ++b) pR[a * st.kc + b] = Ri[a * kMaxK + b];
+    }
+  }
+}
+
+// ---------------------------------------------------------------- select + amplitude (a8)
+// Compacts the accepted walkers into st.list and multiplies the amplitude by r,
+// kept as (phase, log|.|)  (detA *= r).
+template <typename T>
+__global__ void select_kernel(State st, const uint8_t* __restrict__ mask) {
+  using S = Sc<T>;
+  const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (w == 0) st.counters[1] = 0;
+  if (w >= st.W) return;
+  bool acc = mask[w] != 0;
+  if (acc && !st.pend_ok[w]) {
+    atomicOr(&st.info[w], 4);
+    acc = false;
+  }
+  st.pend_ok[w] = 0;
+  if (!acc) return;
+  const int slot = atomicAdd(&st.counters[0], 1);
+  st.list[slot] = (int32_t)w;
+  const T r = ((const T*)st.pend_ratio)[w];
+  const double ar = S::abs(r);
+  st.logabs[w] += log(ar);
+  T* ph = (T*)st.phase;
+  ph[w] = S::mul(ph[w], S::scale(r, 1.0 / ar));
+}
+template __global__ void select_kernel<double>(State, const uint8_t*);
+template __global__ void select_kernel<cplx>(State, const uint8_t*);
+
+// ---------------------------------------------------------------- immediate update (a3)
+// Work item = (accepted walker, tile of rows of Ti).  Persistent grid.  Each warp
+// owns whole rows: row j is loaded once into registers, its k dot products with N
+// give column j of Wm, and the row is written back once:
+//   Ti[j][:] -= sum_a g[a] C[a][:],   g = R^-1 (N Ti[j][:] - [j == P])
+// N, C (k x n each) are staged in shared memory once per item.
+// VEC elements per 16-byte lane access; CH chunks of 32*VEC elements cover a row.
+template <typename T, int VEC>
+struct RowVec;
+template <>
+struct RowVec<double, 2> {
+  using type = double2;
+  static __device__ __forceinline__ double get(const double2& v, int e) { return e ? v.y : v.x; }
+  static __device__ __forceinline__ void set(double2& v, int e, double x) { if (e) v.y = x; else v.x = x; }
+};
+template <>
+struct RowVec<double, 1> {
+  using type = double;
+  static __device__ __forceinline__ double get(const double& v, int) { return v; }
+  static __device__ __forceinline__ void set(double& v, int, double x) { v = x; }
+};
+template <>
+struct RowVec<cplx, 1> {
+  using type = double2;
+  static __device__ __forceinline__ cplx get(const double2& v, int) { return cplx{v.x, v.y}; }
+  static __device__ __forceinline__ void set(double2& v, int, cplx x) { v.x = x.re; v.y = x.im; }
+};
+
+template <typename T, int KT, int VEC, int CH, int RW>
+__global__ void __launch_bounds__(256)
+det_update_kernel(State st, int k, int tiles, int rows_per_tile) {
+  using S = Sc<T>;
+  using RV = RowVec<T, VEC>;
+  using V = typename RV::type;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int n = st.n, kmax = st.kmax;
+  T* Ns = (T*)smem_raw;            // [k][n]
+  T* Cs = Ns + (size_t)k * n;      // [k][n]
+  __shared__ T Ri[KT * KT];
+  __shared__ int sidx[KT];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
+  const int count = st.counters[0];
+  const int nvec = n / VEC;  // vectors per row
+  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
+    const int w = st.list[item / tiles];
+    const int tile = item % tiles;
+    __syncthreads();
+    {
+      const V* gN = (const V*)((const T*)st.pend_N + (size_t)w * kmax * n);
+      const V* gC = (const V*)((const T*)st.pend_C + (size_t)w * kmax * n);
+      for (int q = tid; q < k * nvec; q += blockDim.x) {
+        ((V*)Ns)[q] = gN[q];
+        ((V*)Cs)[q] = gC[q];
+      }
+      if (tid < KT * KT) {
+        const int a = tid / KT, b = tid % KT;
+        Ri[tid] = (a < k && b < k) ? ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + a * st.kc + b]
+                                   : S::zero();
+      }
+      if (tid < KT) sidx[tid] = tid < k ? st.pend_idx[(size_t)w * kmax + tid] : -1;
+    }
+    __syncthreads();
+    T* Tw = (T*)st.Ti + (size_t)w * n * n;
+    const int j_end = min(n, (tile + 1) * rows_per_tile);
+    for (int j0 = tile * rows_per_tile + warp * RW; j0 < j_end; j0 += nw * RW) {
+      V x[RW][CH];
+      T d[RW][KT];
+#pragma unroll
+      for (int r = 0; r < RW; ++r) {
+        const bool rv = j0 + r < j_end;
+        const V* row = (const V*)(Tw + (size_t)(j0 + r) * n);
+#pragma unroll
+        for (int m = 0; m < CH; ++m) {
+          const int q = lane + 32 * m;
+          if (rv && q < nvec) x[r][m] = row[q];
+          else { RV::set(x[r][m], 0, S::zero()); if (VEC == 2) RV::set(x[r][m], 1, S::zero()); }
+        }
+#pragma unroll
+        for (int a = 0; a < KT; ++a) d[r][a] = S::zero();
+      }
+#pragma unroll
+      for (int m = 0; m < CH; ++m) {
+        const int q = lane + 32 * m;
+        if (q < nvec) {
+#pragma unroll
+          for (int a = 0; a < KT; ++a) {
+            if (a < k) {
+              const V nv = ((const V*)(Ns + (size_t)a * n))[q];
+#pragma unroll
+              for (int e = 0; e < VEC; ++e)
+#pragma unroll
+                for (int r = 0; r < RW; ++r)
+                  d[r][a] = S::fma(RV::get(x[r][m], e), RV::get(nv, e), d[r][a]);
+            }
+          }
+        }
+      }
+      T g[RW][KT];
+#pragma unroll
+      for (int r = 0; r < RW; ++r) {
+#pragma unroll
+        for (int a = 0; a < KT; ++a) {
+          d[r][a] = warp_sum(d[r][a]);
+          if (j0 + r == sidx[a]) d[r][a] = S::sub(d[r][a], S::one());
+        }
+#pragma unroll
+        for (int a = 0; a < KT; ++a) {
+          T acc = S::zero();
+#pragma unroll
+          for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], d[r][b], acc);
+          g[r][a] = acc;
+        }
+      }
+#pragma unroll
+      for (int m = 0; m < CH; ++m) {
+        const int q = lane + 32 * m;
+        if (q < nvec) {
+#pragma unroll
+          for (int a = 0; a < KT; ++a) {
+            if (a < k) {
+              const V cv = ((const V*)(Cs + (size_t)a * n))[q];
+#pragma unroll
+              for (int e = 0; e < VEC; ++e)
+#pragma unroll
+                for (int r = 0; r < RW; ++r)
+                  RV::set(x[r][m], e, S::fnma(g[r][a], RV::get(cv, e), RV::get(x[r][m], e)));
+            }
+          }
+#pragma unroll
+          for (int r = 0; r < RW; ++r)
+            if (j0 + r < j_end) ((V*)(Tw + (size_t)(j0 + r) * n))[q] = x[r][m];
+        }
+      }
+    }
+  }
+}
+
+// Generic fallback for rows that do not fit in registers: the row is read twice
+// (second read hits L1/L2), N and C come from global memory.
+template <typename T, int KT>
+__global__ void __launch_bounds__(256)
+det_update_stream_kernel(State st, int k, int tiles, int rows_per_tile) {
+  using S = Sc<T>;
+  __shared__ T Ri[KT * KT];
+  __shared__ int sidx[KT];
+  const int n = st.n, kmax = st.kmax;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
+  const int count = st.counters[0];
+  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
+    const int w = st.list[item / tiles];
+    const int tile = item % tiles;
+    __syncthreads();
+    if (tid < KT * KT) {
+      const int a = tid / KT, b = tid % KT;
+      Ri[tid] = (a < k && b < k) ? ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + a * st.kc + b]
+                                 : S::zero();
+    }
+    if (tid < KT) sidx[tid] = tid < k ? st.pend_idx[(size_t)w * kmax + tid] : -1;
+    __syncthreads();
+    const T* gN = (const T*)st.pend_N + (size_t)w * kmax * n;
+    const T* gC = (const T*)st.pend_C + (size_t)w * kmax * n;
+    T* Tw = (T*)st.Ti + (size_t)w * n * n;
+    const int j_end = min(n, (tile + 1) * rows_per_tile);
+    for (int j = tile * rows_per_tile + warp; j < j_end; j += nw) {
+      T* row = Tw + (size_t)j * n;
+      T d[KT];
+#pragma unroll
+      for (int a = 0; a < KT; ++a) d[a] = S::zero();
+      for (int i = lane; i < n; i += 32) {
+        const T x = row[i];
+#pragma unroll
+        for (int a = 0; a < KT; ++a)
+          if (a < k) d[a] = S::fma(x, gN[(size_t)a * n + i], d[a]);
+      }
+      T g[KT];
+#pragma unroll
+      for (int a = 0; a < KT; ++a) {
+        d[a] = warp_sum(d[a]);
+        if (j == sidx[a]) d[a] = S::sub(d[a], S::one());
+      }
+#pragma unroll
+      for (int a = 0; a < KT; ++a) {
+        T acc = S::zero();
+#pragma unroll
+        for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], d[b], acc);
+        g[a] = acc;
+      }
+      for (int i = lane; i < n; i += 32) {
+        T x = row[i];
+#pragma unroll
+        for (int a = 0; a < KT; ++a)
+          if (a < k) x = S::fnma(g[a], gC[(size_t)a * n + i], x);
+        row[i] = x;
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------- delayed append (a6)
+// prep: per accepted walker, NA = N Abuf^T (k x fill) into pend_Y and
+// a_tau = C_eff copied into Abuf[fill .. fill+k)   (Eq. 14).
+template <typename T>
+__global__ void __launch_bounds__(256) det_prep_kernel(State st, int k) {
+  using S = Sc<T>;
+  const int n = st.n, kmax = st.kmax, cap = st.cap;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
+  const int count = st.counters[0];
+  for (int it = blockIdx.x; it < count; it += gridDim.x) {
+    const int w = st.list[it];
+    const int fill = st.fill[w];
+    const T* gN = (const T*)st.pend_N + (size_t)w * kmax * n;
+    const T* gC = (const T*)st.pend_C + (size_t)w * kmax * n;
+    T* Ab = (T*)st.Abuf + (size_t)w * cap * n;
+    T* NA = (T*)st.pend_Y + (size_t)w * kmax * cap;
+    for (int pr = warp; pr < k * fill; pr += nw) {
+      const int b = pr / fill, s = pr % fill;
+      T acc = S::zero();
+      for (int i = lane; i < n; i += 32) acc = S::fma(gN[(size_t)b * n + i], Ab[(size_t)s * n + i], acc);
+      acc = warp_sum(acc);
+      if (lane == 0) NA[(size_t)b * cap + s] = acc;
+    }
+    for (int q = tid; q < k * n; q += blockDim.x) Ab[(size_t)fill * n + q] = gC[q];
+  }
+}
+
+// append: b_tau^T = R^-1 (N A0^-1 - (N Abuf) Bbuf^T - I[P,:])   (Eq. 15 in new-rows form,
+// PAPER.md:194; reading 5b) -> Bbuf[fill .. fill+k).  One read-only pass over Ti.
+template <typename T, int KT>
+__global__ void __launch_bounds__(256)
+det_append_kernel(State st, int k, int tiles, int rows_per_tile) {
+  using S = Sc<T>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* dsm = (T*)smem_raw;  // [KT][rows_per_tile]
+  __shared__ T Ri[KT * KT];
+  __shared__ int sidx[KT];
+  const int n = st.n, kmax = st.kmax, cap = st.cap;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
+  const int count = st.counters[0];
+  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
+    const int w = st.list[item / tiles];
+    const int tile = item % tiles;
+    const int fill = st.fill[w];
+    __syncthreads();
+    if (tid < KT * KT) {
+      const int a = tid / KT, b = tid % KT;
+      Ri[tid] = (a < k && b < k) ? ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + a * st.kc + b]
+                                 : S::zero();
+    }
+    if (tid < KT) sidx[tid] = tid < k ? st.pend_idx[(size_t)w * kmax + tid] : -1;
+    const T* gN = (const T*)st.pend_N + (size_t)w * kmax * n;
+    const T* Tw = (const T*)st.Ti + (size_t)w * n * n;
+    const int j_beg = tile * rows_per_tile, j_end = min(n, j_beg + rows_per_tile);
+    for (int j = j_beg + warp; j < j_end; j += nw) {
+      const T* row = Tw + (size_t)j * n;
+      T d[KT];
+#pragma unroll
+      for (int a = 0; a < KT; ++a) d[a] = S::zero();
+      for (int i = lane; i < n; i += 32) {
+        const T x = row[i];
+#pragma unroll
+        for (int a = 0; a < KT; ++a)
+          if (a < k) d[a] = S::fma(x, gN[(size_t)a * n + i], d[a]);
+      }
+#pragma unroll
+      for (int a = 0; a < KT; ++a) {
+        d[a] = warp_sum(d[a]);
+        if (lane == 0) dsm[a * rows_per_tile + (j - j_beg)] = d[a];
+      }
+    }
+    __syncthreads();
+    const T* NA = (const T*)st.pend_Y + (size_t)w * kmax * cap;
+    T* Bb = (T*)st.Bbuf + (size_t)w * cap * n;
+    for (int jj = tid; jj < j_end - j_beg; jj += blockDim.x) {
+      const int j = j_beg + jj;
+      T m[KT];
+#pragma unroll
+      for (int b = 0; b < KT; ++b) {
+        m[b] = b < k ? dsm[b * rows_per_tile + jj] : S::zero();
+        if (j == sidx[b]) m[b] = S::sub(m[b], S::one());
+      }
+      for (int s = 0; s < fill; ++s) {
+        const T bv = Bb[(size_t)s * n + j];
+#pragma unroll
+        for (int b = 0; b < KT; ++b)
+          if (b < k) m[b] = S::fnma(NA[(size_t)b * cap + s], bv, m[b]);
+      }
+#pragma unroll
+      for (int a = 0; a < KT; ++a) {
+        if (a < k) {
+          T acc = S::zero();
+#pragma unroll
+          for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], m[b], acc);
+          Bb[(size_t)(fill + a) * n + j] = acc;
+        }
+      }
+    }
+  }
+}
+
+// post: fill += k for accepted walkers; walkers whose depth reached K (or whose
+// buffer cannot take another kmax columns) go to the flush list (reading 9).
+__global__ void post_kernel(State st, int k) {
+  const int it = blockIdx.x * blockDim.x + threadIdx.x;
+  if (it >= st.counters[0]) return;
+  const int w = st.list[it];
+  const int f = st.fill[w] + k, u = st.nupd[w] + 1;
+  st.fill[w] = f;
+  st.nupd[w] = u;
+  if (u >= st.K || f + st.kc > st.cap) st.flist[atomicAdd(&st.counters[1], 1)] = w;
+}
+
+// flush-all selection: every walker with a non-empty buffer.
+__global__ void flush_all_select_kernel(State st) {
+  const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= st.W) return;
+  if (st.fill[w] > 0) st.flist[atomicAdd(&st.counters[1], 1)] = (int32_t)w;
+}
+__global__ void reset_counter_kernel(State st, int which) { st.counters[which] = 0; }
+
+__global__ void flush_clear_kernel(State st) {
+  const int it = blockIdx.x * blockDim.x + threadIdx.x;
+  if (it >= st.counters[1]) return;
+  const int w = st.flist[it];
+  st.fill[w] = 0;
+  st.nupd[w] = 0;
+}
+
+// ---------------------------------------------------------------- flush (a7), FMA version
+// Ti[j][i] -= sum_s Bbuf[s][j] Abuf[s][i]   (Eq. 12), 64x64 tiles.
+template <typename T>
+__global__ void __launch_bounds__(256) det_flush_kernel(State st, int tiles_1d) {
+  using S = Sc<T>;
+  constexpr int BT = 64, BK = 16;
+  __shared__ T Bs[BK][BT];
+  __shared__ T As[BK][BT];
+  const int n = st.n, cap = st.cap;
+  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  const int count = st.counters[1];
+  const int tiles = tiles_1d * tiles_1d;
+  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
+    const int w = st.flist[item / tiles];
+    const int tile = item % tiles;
+    const int j0 = (tile / tiles_1d) * BT, i0 = (tile % tiles_1d) * BT;
+    const int fill = st.fill[w];
+    const T* Ab = (const T*)st.Abuf + (size_t)w * cap * n;
+    const T* Bb = (const T*)st.Bbuf + (size_t)w * cap * n;
+    T* Tw = (T*)st.Ti + (size_t)w * n * n;
+    T acc[4][4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+      for (int b = 0; b < 4; ++b) acc[a][b] = S::zero();
+    for (int s0 = 0; s0 < fill; s0 += BK) {
+      __syncthreads();
+      for (int q = tid; q < BK * BT; q += 256) {
+        const int kk = q / BT, c = q % BT;
+        const bool sv = s0 + kk < fill;
+        Bs[kk][c] = (sv && j0 + c < n) ? Bb[(size_t)(s0 + kk) * n + j0 + c] : S::zero();
+        As[kk][c] = (sv && i0 + c < n) ? Ab[(size_t)(s0 + kk) * n + i0 + c] : S::zero();
+      }
+      __syncthreads();
+#pragma unroll
+      for (int kk = 0; kk < BK; ++kk) {
+        T bv[4], av[4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) { bv[a] = Bs[kk][ty + 16 * a]; av[a] = As[kk][tx + 16 * a]; }
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+          for (int b = 0; b < 4; ++b) acc[a][b] = S::fma(bv[a], av[b], acc[a][b]);
+      }
+    }
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+      const int j = j0 + ty + 16 * a;
+      if (j >= n) continue;
+#pragma unroll
+      for (int b = 0; b < 4; ++b) {
+        const int i = i0 + tx + 16 * b;
+        if (i < n) Tw[(size_t)j * n + i] = S::sub(Tw[(size_t)j * n + i], acc[a][b]);
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------- shared helpers
+int launch_select(const State& st, const uint8_t* mask, cudaStream_t s) {
+  const unsigned gw = (unsigned)((st.W + 255) / 256);
+  if (st.dt == LRUX_F64) select_kernel<double><<<gw, 256, 0, s>>>(st, mask);
+  else select_kernel<cplx><<<gw, 256, 0, s>>>(st, mask);
+  return 1;
+}
+int launch_post(const State& st, int ncols, cudaStream_t s) {
+  post_kernel<<<(unsigned)((st.W + 255) / 256), 256, 0, s>>>(st, ncols);
+  return 1;
+}
+int launch_flush_select_all(const State& st, cudaStream_t s) {
+  reset_counter_kernel<<<1, 1, 0, s>>>(st, 1);
+  flush_all_select_kernel<<<(unsigned)((st.W + 255) / 256), 256, 0, s>>>(st);
+  return 2;
+}
+int launch_flush_clear(const State& st, cudaStream_t s) {
+  flush_clear_kernel<<<(unsigned)((st.W + 255) / 256), 256, 0, s>>>(st);
+  return 1;
+}
+
+// ---------------------------------------------------------------- launchers
+static inline int round_kt(int k) { return k <= 1 ? 1 : k <= 2 ? 2 : k <= 4 ? 4 : 8; }
+
+static inline int persistent_grid(int num_sms, int ctas_per_sm, int64_t max_items) {
+  int64_t g = (int64_t)num_sms * ctas_per_sm;
+  if (g > max_items) g = max_items;
+  return g < 1 ? 1 : (int)g;
+}
+
+template <typename T, int KT, int VEC, int CH, int RW>
+static int launch_update_reg(const State& st, int k, int num_sms, cudaStream_t s) {
+  const int n = st.n;
+  const size_t smem = 2 * (size_t)k * n * sizeof(T);
+  auto kern = det_update_kernel<T, KT, VEC, CH, RW>;
+  if (smem > 48 * 1024 &&
+      cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return -1;
+  int rows_per_tile = 64;
+  if (rows_per_tile > n) rows_per_tile = n;
+  const int tiles = (n + rows_per_tile - 1) / rows_per_tile;
+  int occ = 1;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, smem);
+  if (occ < 1) occ = 1;
+  const int grid = persistent_grid(num_sms, occ, (int64_t)st.W * tiles);
+  kern<<<grid, 256, smem, s>>>(st, k, tiles, rows_per_tile);
+  return 1;
+}
+
+template <typename T, int KT>
+static int launch_update_kt(const State& st, int k, int num_sms, cudaStream_t s) {
+  const int n = st.n;
+  constexpr int VECMAX = sizeof(T) == 8 ? 2 : 1;
+  const size_t smem = 2 * (size_t)k * n * sizeof(T);
+  const bool vec_ok = (n % VECMAX) == 0;
+  const int nvec = n / VECMAX;
+  if (vec_ok && smem <= 160 * 1024) {
+    if (nvec <= 32 * 1) return launch_update_reg<T, KT, VECMAX, 1, 2>(st, k, num_sms, s);
+    if (nvec <= 32 * 2) return launch_update_reg<T, KT, VECMAX, 2, 2>(st, k, num_sms, s);
+    if (nvec <= 32 * 4) return launch_update_reg<T, KT, VECMAX, 4, 2>(st, k, num_sms, s);
+    if (nvec <= 32 * 8) return launch_update_reg<T, KT, VECMAX, 8, 1>(st, k, num_sms, s);
+    if (nvec <= 32 * 16) return launch_update_reg<T, KT, VECMAX, 16, 1>(st, k, num_sms, s);
+  }
+  int rows_per_tile = 64;
+  if (rows_per_tile > n) rows_per_tile = n;
+  const int tiles = (n + rows_per_tile - 1) / rows_per_tile;
+  const int grid = persistent_grid(num_sms, 4, (int64_t)st.W * tiles);
+  det_update_stream_kernel<T, KT><<<grid, 256, 0, s>>>(st, k, tiles, rows_per_tile);
+  return 1;
+}
+
+template <typename T, int KT>
+static int launch_append_kt(const State& st, int k, int num_sms, cudaStream_t s) {
+  const int n = st.n;
+  int rows_per_tile = 64;
+  if (rows_per_tile > n) rows_per_tile = n;
+  const int tiles = (n + rows_per_tile - 1) / rows_per_tile;
+  const size_t smem = (size_t)KT * rows_per_tile * sizeof(T);
+  const int grid = persistent_grid(num_sms, 4, (int64_t)st.W * tiles);
+  det_append_kernel<T, KT><<<grid, 256, smem, s>>>(st, k, tiles, rows_per_tile);
+  return 1;
+}
+
+template <typename T>
+static int flush_impl(const State& st, bool all, int num_sms, cudaStream_t s) {
+  int nl = 0;
+  const unsigned gw = (unsigned)((st.W + 255) / 256);
+  if (all) {
+    reset_counter_kernel<<<1, 1, 0, s>>>(st, 1); ++nl;
+    flush_all_select_kernel<<<gw, 256, 0, s>>>(st); ++nl;
+  }
+  const int t1 = (st.n + 63) / 64;
+  const int grid = persistent_grid(num_sms, 4, (int64_t)st.W * t1 * t1);
+  det_flush_kernel<T><<<grid, 256, 0, s>>>(st, t1); ++nl;
+  flush_clear_kernel<<<gw, 256, 0, s>>>(st); ++nl;
+  return cudaGetLastError() == cudaSuccess ? nl : -1;
+}
+
+template <typename T>
+static int accept_impl(const State& st, int k, const uint8_t* mask, int num_sms, cudaStream_t s) {
+  int nl = 0;
+  const unsigned gw = (unsigned)((st.W + 255) / 256);
+  select_kernel<T><<<gw, 256, 0, s>>>(st, mask); ++nl;
+  const int kt = round_kt(k);
+  int r = 0;
+  if (st.K == 0) {
+    switch (kt) {
+      case 1: r = launch_update_kt<T, 1>(st, k, num_sms, s); break;
+      case 2: r = launch_update_kt<T, 2>(st, k, num_sms, s); break;
+      case 4: r = launch_update_kt<T, 4>(st, k, num_sms, s); break;
+      default: r = launch_update_kt<T, 8>(st, k, num_sms, s); break;
+    }
+    if (r < 0) return -1;
+    nl += r;
+  } else {
+    const int grid = persistent_grid(num_sms, 4, st.W);
+    det_prep_kernel<T><<<grid, 256, 0, s>>>(st, k); ++nl;
+    switch (kt) {
+      case 1: r = launch_append_kt<T, 1>(st, k, num_sms, s); break;
+      case 2: r = launch_append_kt<T, 2>(st, k, num_sms, s); break;
+      case 4: r = launch_append_kt<T, 4>(st, k, num_sms, s); break;
+      default: r = launch_append_kt<T, 8>(st, k, num_sms, s); break;
+    }
+    if (r < 0) return -1;
+    nl += r;
+    post_kernel<<<gw, 256, 0, s>>>(st, k); ++nl;
+    r = flush_impl<T>(st, false, num_sms, s);
+    if (r < 0) return -1;
+    nl += r;
+  }
+  return cudaGetLastError() == cudaSuccess ? nl : -1;
+}
+
+int launch_det_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
+                     void* d_ratio, cudaStream_t s) {
+  if (st.dt == LRUX_F64)
+    det_ratio_kernel<double><<<(unsigned)st.W, 128, 0, s>>>(st, k, d_idx, (const double*)d_rows,
+                                                            (double*)d_ratio);
+  else
+    det_ratio_kernel<cplx><<<(unsigned)st.W, 128, 0, s>>>(st, k, d_idx, (const cplx*)d_rows,
+                                                          (cplx*)d_ratio);
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+int launch_det_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? accept_impl<double>(st, k, d_mask, num_sms, s)
+                           : accept_impl<cplx>(st, k, d_mask, num_sms, s);
+}
+
+int launch_det_flush(const State& st, bool all, int num_sms, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? flush_impl<double>(st, all, num_sms, s)
+                           : flush_impl<cplx>(st, all, num_sms, s);
+}
+
+}  // namespace lrux

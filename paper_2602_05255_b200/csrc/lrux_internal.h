@@ -1,0 +1,76 @@
+// Host-side handle, state layout and kernel-launcher declarations.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "lrux.h"
+
+namespace lrux {
+
+enum Kind { KIND_DET = 0, KIND_PF = 1 };
+
+// Views into the caller-owned d_state buffer (all device pointers, 256 B aligned).
+// Element type is double (LRUX_F64) or interleaved complex (LRUX_C128); sizes
+// below are in elements of that type unless noted.
+struct State {
+  int64_t W;
+  int32_t n, kmax, K, kc;  // kc = core size: kmax (det) or 2*kmax (pf)
+  int32_t cap;             // delay-buffer capacity in columns: K*kmax (det), K*2*kmax (pf)
+  int32_t dt, kind;
+  // det: Ti[w][j][i] = (A^-1)[i][j]  (A^-T row-major);  pf: Ti[w] = A^-1 row-major
+  void* Ti;
+  void* phase;       // [W] elem
+  double* logabs;    // [W]
+  int32_t* fill;     // [W] columns in use in the delay buffer
+  int32_t* nupd;     // [W] updates held in the delay buffer
+  int32_t* pend_idx; // [W][kmax]
+  uint8_t* pend_ok;  // [W] 1 = valid proposal with finite non-zero R
+  void* pend_ratio;  // [W] elem
+  void* pend_Rinv;   // [W][kc][kc]
+  void* pend_C;      // [W][kmax][n]  det: effective A^-1[:,P] (= a_tau, Eq. 14); pf: A^-1[:,P]
+  void* pend_N;      // [W][kmax][n]  new rows
+  void* pend_Y;      // pf: [W][kmax][n]  A^-1 N ; det delayed: [W][kmax][cap] N * Abuf^T
+  void* pend_AN;     // pf delayed: [W][kmax][cap]  N * Abuf^T
+  void* Abuf;        // [W][cap][n]  det: a_t (Eq. 10);  pf: a'_t (Eq. 25)
+  void* Bbuf;        // [W][cap][n]  det: b_t (Eq. 11);  pf: a'_t R_t^-1
+  int32_t* list;     // [W] accepted walkers (compacted)
+  int32_t* flist;    // [W] walkers to flush (compacted)
+  int32_t* counters; // [8]: 0 = accepted count, 1 = flush count
+  int32_t* info;     // caller's d_info
+};
+
+}  // namespace lrux
+
+struct lrux_handle_s {
+  lrux::State st;
+  int32_t pending_k;  // 0 = nothing pending
+  int64_t launches;
+  int32_t num_sms;
+};
+
+namespace lrux {
+
+size_t state_layout(State* st, void* base, int64_t W, int32_t n, int32_t kmax, int32_t K,
+                    int32_t dt, int32_t kind);
+
+// launchers (each returns the number of kernels it enqueued, or -1 on a CUDA error)
+int launch_det_init(const State& st, const void* d_A0, cudaStream_t s);
+int launch_pf_init(const State& st, const void* d_A0, cudaStream_t s);
+int launch_det_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
+                     void* d_ratio, cudaStream_t s);
+int launch_det_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s);
+int launch_det_flush(const State& st, bool all, int num_sms, cudaStream_t s);
+int launch_pf_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
+                    void* d_ratio, int num_sms, cudaStream_t s);
+int launch_pf_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s);
+int launch_pf_flush(const State& st, bool all, int num_sms, cudaStream_t s);
+// shared between det and pf (defined in lrux_det.cu)
+int launch_select(const State& st, const uint8_t* mask, cudaStream_t s);
+int launch_post(const State& st, int ncols, cudaStream_t s);
+int launch_flush_select_all(const State& st, cudaStream_t s);
+int launch_flush_clear(const State& st, cudaStream_t s);
+int launch_get_amplitude(const State& st, void* d_phase, double* d_logabs, cudaStream_t s);
+int launch_get_inverse(const State& st, void* d_out, cudaStream_t s);
+
+}  // namespace lrux

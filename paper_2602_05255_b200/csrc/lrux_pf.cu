@@ -1,0 +1,508 @@
+// Pfaffian hot path.
+//
+// State Ti = A^-1 row-major, exactly skew.  New-rows-only forms (DESIGN.md §3,
+// readings 5/5b), P the k replaced slots, N[a][:] the new row P[a] of A' (with
+// N[a][P[a]] = 0), Aeff = A0^-1 + sum_s Bbuf[s][.] Abuf[s][.] the effective inverse:
+//   C[a][i] = Aeff[i][P[a]]          Y[a][i] = sum_j Aeff[i][j] N[a][j]
+//   R' = [[G, Tm], [-Tm^T, S]],  G[a][b] = N_a.Y_b + N[a][P[b]],  Tm[a][b] = N_a.C_b,
+//        S[a][b] = Aeff[P[a]][P[b]]          (= J + u^T A^-1 u up to a congruence, Eq. 20)
+//   r = (-1)^(k(k-1)/2) pf R'                                   (Eq. 19)
+//   A'^-1 = Aeff + Y' R'^-1 Y'^T,  Y' = (Y + E_P, C)             (Eq. 21)
+// R' is assembled from its strict upper triangle and mirrored, R'^-1 is skew
+// projected, and the update writes the upper triangle and its exact negative, so
+// the stored inverse stays exactly skew.
+#include "lrux_common.cuh"
+#include "lrux_internal.h"
+
+namespace lrux {
+
+constexpr int kMaxC = 2 * kMaxK;  // largest core size
+
+// ---------------------------------------------------------------- gather (+ ratio for k = 1)
+template <typename T>
+__global__ void __launch_bounds__(128)
+pf_gather_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __restrict__ rows,
+                 T* __restrict__ ratio_out) {
+  using S = Sc<T>;
+  __shared__ int sidx[kMaxK];
+  __shared__ int bad;
+  __shared__ T red[4];
+  const int w = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
+  const int warp = tid >> 5, lane = tid & 31;
+  const int n = st.n, kmax = st.kmax;
+  if (w == 0 && tid == 0) st.counters[0] = 0;
+  if (tid == 0) {
+    int b = 0;
+    for (int a = 0; a < k; ++a) {
+      int p = idx[(size_t)w * k + a];
+      sidx[a] = p;
+      if (p < 0 || p >= n) b = 1;
+      for (int c = 0; c < a; ++c)
+        if (sidx[c] == p) b = 1;
+    }
+    bad = b;
+  }
+  __syncthreads();
+  if (bad) {
+    if (tid == 0) {
+      ratio_out[w] = S::nan();
+      ((T*)st.pend_ratio)[w] = S::nan();
+      st.pend_ok[w] = 0;
+      st.pend_idx[(size_t)w * kmax] = -1;
+      atomicOr(&st.info[w], 2);
+    }
+    return;
+  }
+  const int fill = st.cap ? st.fill[w] : 0;
+  const T* Tw = (const T*)st.Ti + (size_t)w * n * n;
+  const T* Ab = st.cap ? (const T*)st.Abuf + (size_t)w * st.cap * n : nullptr;
+  const T* Bb = st.cap ? (const T*)st.Bbuf + (size_t)w * st.cap * n : nullptr;
+  T* pC = (T*)st.pend_C + (size_t)w * kmax * n;
+  T* pN = (T*)st.pend_N + (size_t)w * kmax * n;
+  T t1 = S::zero();
+  for (int a = 0; a < k; ++a) {
+    const int p = sidx[a];
+    for (int i = tid; i < n; i += nt) {
+      T c = S::neg(Tw[(size_t)p * n + i]);  // A0^-1[i][p] = -A0^-1[p][i]
+      for (int s = 0; s < fill; ++s) c = S::fma(Bb[(size_t)s * n + i], Ab[(size_t)s * n + p], c);
+      T x = (i == p) ? S::zero() : rows[((size_t)w * k + a) * n + i];
+      pC[(size_t)a * n + i] = c;
+      pN[(size_t)a * n + i] = x;
+      if (k == 1) t1 = S::fma(x, c, t1);
+    }
+  }
+  if (tid < k) st.pend_idx[(size_t)w * kmax + tid] = sidx[tid];
+  if (k > 1) return;
+  t1 = warp_sum(t1);
+  if (lane == 0) red[warp] = t1;
+  __syncthreads();
+  if (tid == 0) {
+    T t = red[0];
+    for (int q = 1; q < (nt >> 5); ++q) t = S::add(t, red[q]);
+    // k = 1: R' = [[0,t],[-t,0]], r = t; R'^-1 = [[0,-1/t],[1/t,0]]   (Eq. 22)
+    ratio_out[w] = t;
+    ((T*)st.pend_ratio)[w] = t;
+    const bool ok = S::finite(t) && !S::is_zero(t);
+    st.pend_ok[w] = ok ? 1 : 0;
+    T* pR = (T*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
+    const T ti = ok ? S::inv(t) : S::zero();
+    pR[0] = S::zero();
+    pR[1] = S::neg(ti);
+    pR[st.kc] = ti;
+    pR[st.kc + 1] = S::zero();
+  }
+}
+
+// ---------------------------------------------------------------- AN = N Abuf^T (delayed)
+template <typename T>
+__global__ void __launch_bounds__(256) pf_an_kernel(State st, int k, int use_list) {
+  using S = Sc<T>;
+  const int n = st.n, kmax = st.kmax, cap = st.cap;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
+  const int count = use_list ? st.counters[0] : (int)st.W;
+  for (int it = blockIdx.x; it < count; it += gridDim.x) {
+    const int w = use_list ? st.list[it] : it;
+    if (st.pend_idx[(size_t)w * kmax] < 0) continue;
+    const int fill = st.fill[w];
+    const T* gN = (const T*)st.pend_N + (size_t)w * kmax * n;
+    const T* Ab = (const T*)st.Abuf + (size_t)w * cap * n;
+    T* AN = (T*)st.pend_AN + (size_t)w * kmax * cap;
+    for (int pr = warp; pr < k * fill; pr += nw) {
+      const int a = pr / fill, s = pr % fill;
+      T acc = S::zero();
+      for (int j = lane; j < n; j += 32) acc = S::fma(gN[(size_t)a * n + j], Ab[(size_t)s * n + j], acc);
+      acc = warp_sum(acc);
+      if (lane == 0) AN[(size_t)a * cap + s] = acc;
+    }
+  }
+}
+
+// ---------------------------------------------------------------- Y = Aeff N
+// Work item = (walker, tile of rows).  One read-only pass over Ti.
+template <typename T, int KT>
+__global__ void __launch_bounds__(256)
+pf_y_kernel(State st, int k, int tiles, int rows_per_tile, int use_list) {
+  using S = Sc<T>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* dsm = (T*)smem_raw;  // [KT][rows_per_tile]
+  const int n = st.n, kmax = st.kmax, cap = st.cap;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
+  const int count = use_list ? st.counters[0] : (int)st.W;
+  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
+    const int w = use_list ? st.list[item / tiles] : item / tiles;
+    const int tile = item % tiles;
+    if (st.pend_idx[(size_t)w * kmax] < 0) continue;  // invalid proposal (uniform per CTA)
+    const int fill = cap ? st.fill[w] : 0;
+    const T* gN = (const T*)st.pend_N + (size_t)w * kmax * n;
+    const T* Tw = (const T*)st.Ti + (size_t)w * n * n;
+    const int i_beg = tile * rows_per_tile, i_end = min(n, i_beg + rows_per_tile);
+    __syncthreads();
+    for (int i = i_beg + warp; i < i_end; i += nw) {
+      const T* row = Tw + (size_t)i * n;
+      T d[KT];
+#pragma unroll
+      for (int a = 0; a < KT; ++a) d[a] = S::zero();
+      for (int j = lane; j < n; j += 32) {
+        const T x = row[j];
+#pragma unroll
+        for (int a = 0; a < KT; ++a)
+          if (a < k) d[a] = S::fma(x, gN[(size_t)a * n + j], d[a]);
+      }
+#pragma unroll
+      for (int a = 0; a < KT; ++a) {
+        d[a] = warp_sum(d[a]);
+        if (lane == 0) dsm[a * rows_per_tile + (i - i_beg)] = d[a];
+      }
+    }
+    __syncthreads();
+    const T* AN = cap ? (const T*)st.pend_AN + (size_t)w * kmax * cap : nullptr;
+    const T* Bb = cap ? (const T*)st.Bbuf + (size_t)w * cap * n : nullptr;
+    T* pY = (T*)st.pend_Y + (size_t)w * kmax * n;
+    for (int ii = tid; ii < i_end - i_beg; ii += blockDim.x) {
+      const int i = i_beg + ii;
+      T y[KT];
+#pragma unroll
+      for (int a = 0; a < KT; ++a) y[a] = a < k ? dsm[a * rows_per_tile + ii] : S::zero();
+      for (int s = 0; s < fill; ++s) {
+        const T bv = Bb[(size_t)s * n + i];
+#pragma unroll
+        for (int a = 0; a < KT; ++a)
+          if (a < k) y[a] = S::fma(bv, AN[(size_t)a * cap + s], y[a]);
+      }
+#pragma unroll
+      for (int a = 0; a < KT; ++a)
+        if (a < k) pY[(size_t)a * n + i] = y[a];
+    }
+  }
+}
+
+// ---------------------------------------------------------------- core (k >= 2)
+// Builds the exactly skew 2k x 2k core R', r = (-1)^(k(k-1)/2) pf R', R'^-1.
+template <typename T>
+__global__ void __launch_bounds__(128)
+pf_core_kernel(State st, int k, T* __restrict__ ratio_out) {
+  using S = Sc<T>;
+  __shared__ T R[kMaxC * kMaxC];
+  __shared__ T R2[kMaxC * kMaxC];
+  __shared__ T Ri[kMaxC * kMaxC];
+  const int w = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
+  const int warp = tid >> 5, lane = tid & 31, nw = nt >> 5;
+  const int n = st.n, kmax = st.kmax, m = 2 * k;
+  if (st.pend_idx[(size_t)w * kmax] < 0) return;
+  const T* pC = (const T*)st.pend_C + (size_t)w * kmax * n;
+  const T* pN = (const T*)st.pend_N + (size_t)w * kmax * n;
+  const T* pY = (const T*)st.pend_Y + (size_t)w * kmax * n;
+  const int32_t* P = st.pend_idx + (size_t)w * kmax;
+  for (int q = tid; q < kMaxC * kMaxC; q += nt) R[q] = S::zero();
+  __syncthreads();
+  // upper-right block Tm (all a,b) and strict upper triangle of G
+  for (int pr = warp; pr < 2 * k * k; pr += nw) {
+    const bool isG = pr >= k * k;
+    const int q = isG ? pr - k * k : pr;
+    const int a = q / k, b = q % k;
+    if (isG && a >= b) continue;
+    const T* other = isG ? pY + (size_t)b * n : pC + (size_t)b * n;
+    T acc = S::zero();
+    for (int i = lane; i < n; i += 32) acc = S::fma(pN[(size_t)a * n + i], other[i], acc);
+    acc = warp_sum(acc);
+    if (lane == 0) {
+      if (isG) {
+        acc = S::add(acc, pN[(size_t)a * n + P[b]]);
+        R[a * kMaxC + b] = acc;
+        R[b * kMaxC + a] = S::neg(acc);
+      } else {
+        R[a * kMaxC + (k + b)] = acc;
+        R[(k + b) * kMaxC + a] = S::neg(acc);
+      }
+    }
+  }
+  // S block: Aeff[P[a]][P[b]] = C[b][P[a]], strict upper triangle mirrored
+  if (tid < k * k) {
+    const int a = tid / k, b = tid % k;
+    if (a < b) {
+      const T v = pC[(size_t)b * n + P[a]];
+      R[(k + a) * kMaxC + (k + b)] = v;
+      R[(k + b) * kMaxC + (k + a)] = S::neg(v);
+    }
+  }
+  __syncthreads();
+  for (int q = tid; q < kMaxC * kMaxC; q += nt) R2[q] = R[q];
+  __syncthreads();
+  if (tid == 0) {
+    T pfv = small_pf(R2, m, kMaxC);
+    if ((k * (k - 1) / 2) & 1) pfv = S::neg(pfv);
+    bool ok;
+    small_det_inv(R, Ri, m, kMaxC, &ok);
+    ok = ok && S::finite(pfv) && !S::is_zero(pfv);
+    ratio_out[w] = pfv;
+    ((T*)st.pend_ratio)[w] = pfv;
+    st.pend_ok[w] = ok ? 1 : 0;
+    T* pR = (T*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
+    for (int a = 0; a < m; ++a) {
+      pR[a * st.kc + a] = S::zero();
+      for (int b = a + 1; b < m; ++b) {
+        const T v = ok ? S::scale(S::sub(Ri[a * kMaxC + b], Ri[b * kMaxC + a]), 0.5) : S::zero();
+        pR[a * st.kc + b] = v;
+        pR[b * st.kc + a] = S::neg(v);
+      }
+    }
+  }
+}
+
+// Y'[alpha][i] for alpha in [0,2k): (Y + E_P, C)
+template <typename T>
+__device__ __forceinline__ T yprime(const T* pY, const T* pC, const int* P, int k, int n, int alpha,
+                                    int i) {
+  if (alpha < k) {
+    T y = pY[(size_t)alpha * n + i];
+    return (i == P[alpha]) ? Sc<T>::add(y, Sc<T>::one()) : y;
+  }
+  return pC[(size_t)(alpha - k) * n + i];
+}
+
+// ---------------------------------------------------------------- immediate update (a4)
+// Work item = (accepted walker, upper tile pair I <= J of 32x32 tiles).
+//   Ti[i][j] += sum_beta g[beta][i] Y'[beta][j],  g[beta][i] = sum_alpha Y'[alpha][i] R'^-1[alpha][beta]
+// for j > i only; the mirrored entry receives the exact negative.
+template <typename T>
+__global__ void __launch_bounds__(256) pf_update_kernel(State st, int k, int t1) {
+  using S = Sc<T>;
+  constexpr int TS = 32;
+  __shared__ T gI[kMaxC][TS];
+  __shared__ T yJ[kMaxC][TS];
+  __shared__ T tile[TS][TS + 1];
+  __shared__ T Ri[kMaxC * kMaxC];
+  __shared__ int P[kMaxK];
+  const int n = st.n, kmax = st.kmax, m = 2 * k;
+  const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5;
+  const int count = st.counters[0];
+  const int tiles = t1 * (t1 + 1) / 2;
+  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
+    const int w = st.list[item / tiles];
+    int rem = item % tiles, I = 0;
+    while (rem >= t1 - I) { rem -= t1 - I; ++I; }
+    const int J = I + rem;
+    const int i0 = I * TS, j0 = J * TS;
+    const T* pC = (const T*)st.pend_C + (size_t)w * kmax * n;
+    const T* pY = (const T*)st.pend_Y + (size_t)w * kmax * n;
+    T* Tw = (T*)st.Ti + (size_t)w * n * n;
+    __syncthreads();
+    for (int q = tid; q < m * m; q += 256)
+      Ri[(q / m) * kMaxC + (q % m)] = ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + (q / m) * st.kc + (q % m)];
+    if (tid < k) P[tid] = st.pend_idx[(size_t)w * kmax + tid];
+    __syncthreads();
+    for (int q = tid; q < m * TS; q += 256) {
+      const int beta = q / TS, c = q % TS;
+      const int j = j0 + c, i = i0 + c;
+      yJ[beta][c] = j < n ? yprime(pY, pC, P, k, n, beta, j) : S::zero();
+      T g = S::zero();
+      if (i < n)
+        for (int alpha = 0; alpha < m; ++alpha)
+          g = S::fma(yprime(pY, pC, P, k, n, alpha, i), Ri[alpha * kMaxC + beta], g);
+      gI[beta][c] = g;
+    }
+    __syncthreads();
+    for (int r = ty; r < TS; r += 8) {
+      const int i = i0 + r, j = j0 + tx;
+      T v = S::zero();
+      if (i < n && j < n && j > i) {
+        v = Tw[(size_t)i * n + j];
+        for (int beta = 0; beta < m; ++beta) v = S::fma(gI[beta][r], yJ[beta][tx], v);
+        Tw[(size_t)i * n + j] = v;
+      }
+      tile[r][tx] = v;
+    }
+    __syncthreads();
+    // mirrored write: Ti[j][i] = -new(i,j)
+    for (int r = ty; r < TS; r += 8) {
+      const int j = j0 + r, i = i0 + tx;  // element (j,i) <- -tile[tx][r]
+      if (i < n && j < n && j > i) Tw[(size_t)j * n + i] = S::neg(tile[tx][r]);
+    }
+  }
+}
+
+// ---------------------------------------------------------------- delayed append (a6)
+// Abuf[fill+alpha][:] = Y'[alpha][:]  (a'_tau, Eq. 28), Bbuf[fill+beta][:] = (a'_tau R'^-1)[:, beta].
+template <typename T>
+__global__ void __launch_bounds__(256) pf_append_kernel(State st, int k) {
+  using S = Sc<T>;
+  __shared__ T Ri[kMaxC * kMaxC];
+  __shared__ int P[kMaxK];
+  const int n = st.n, kmax = st.kmax, cap = st.cap, m = 2 * k;
+  const int tid = threadIdx.x;
+  const int count = st.counters[0];
+  for (int it = blockIdx.x; it < count; it += gridDim.x) {
+    const int w = st.list[it];
+    const int fill = st.fill[w];
+    __syncthreads();
+    for (int q = tid; q < m * m; q += 256)
+      Ri[(q / m) * kMaxC + (q % m)] = ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + (q / m) * st.kc + (q % m)];
+    if (tid < k) P[tid] = st.pend_idx[(size_t)w * kmax + tid];
+    __syncthreads();
+    const T* pC = (const T*)st.pend_C + (size_t)w * kmax * n;
+    const T* pY = (const T*)st.pend_Y + (size_t)w * kmax * n;
+    T* Ab = (T*)st.Abuf + (size_t)w * cap * n;
+    T* Bb = (T*)st.Bbuf + (size_t)w * cap * n;
+    for (int i = tid; i < n; i += 256) {
+      T yp[kMaxC];
+      for (int alpha = 0; alpha < m; ++alpha) {
+        yp[alpha] = yprime(pY, pC, P, k, n, alpha, i);
+        Ab[(size_t)(fill + alpha) * n + i] = yp[alpha];
+      }
+      for (int beta = 0; beta < m; ++beta) {
+        T g = S::zero();
+        for (int alpha = 0; alpha < m; ++alpha) g = S::fma(yp[alpha], Ri[alpha * kMaxC + beta], g);
+        Bb[(size_t)(fill + beta) * n + i] = g;
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------- flush (a7), FMA version
+// Ti[i][j] += sum_s Bbuf[s][i] Abuf[s][j] for j > i, mirrored exactly (Eq. 26).
+template <typename T>
+__global__ void __launch_bounds__(256) pf_flush_kernel(State st, int t1) {
+  using S = Sc<T>;
+  constexpr int BT = 64, BK = 16;
+  __shared__ T Bs[BK][BT];
+  __shared__ T As[BK][BT];
+  const int n = st.n, cap = st.cap;
+  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  const int count = st.counters[1];
+  const int tiles = t1 * (t1 + 1) / 2;
+  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
+    const int w = st.flist[item / tiles];
+    int rem = item % tiles, I = 0;
+    while (rem >= t1 - I) { rem -= t1 - I; ++I; }
+    const int J = I + rem;
+    const int i0 = I * BT, j0 = J * BT;
+    const int fill = st.fill[w];
+    const T* Ab = (const T*)st.Abuf + (size_t)w * cap * n;
+    const T* Bb = (const T*)st.Bbuf + (size_t)w * cap * n;
+    T* Tw = (T*)st.Ti + (size_t)w * n * n;
+    T acc[4][4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+      for (int b = 0; b < 4; ++b) acc[a][b] = S::zero();
+    for (int s0 = 0; s0 < fill; s0 += BK) {
+      __syncthreads();
+      for (int q = tid; q < BK * BT; q += 256) {
+        const int kk = q / BT, c = q % BT;
+        const bool sv = s0 + kk < fill;
+        Bs[kk][c] = (sv && i0 + c < n) ? Bb[(size_t)(s0 + kk) * n + i0 + c] : S::zero();
+        As[kk][c] = (sv && j0 + c < n) ? Ab[(size_t)(s0 + kk) * n + j0 + c] : S::zero();
+      }
+      __syncthreads();
+#pragma unroll
+      for (int kk = 0; kk < BK; ++kk) {
+        T bv[4], av[4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) { bv[a] = Bs[kk][ty + 16 * a]; av[a] = As[kk][tx + 16 * a]; }
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+          for (int b = 0; b < 4; ++b) acc[a][b] = S::fma(bv[a], av[b], acc[a][b]);
+      }
+    }
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+      const int i = i0 + ty + 16 * a;
+#pragma unroll
+      for (int b = 0; b < 4; ++b) {
+        const int j = j0 + tx + 16 * b;
+        if (i < n && j < n && j > i) {
+          const T v = S::add(Tw[(size_t)i * n + j], acc[a][b]);
+          Tw[(size_t)i * n + j] = v;
+          Tw[(size_t)j * n + i] = S::neg(v);
+        }
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------- launchers
+static inline int round_kt(int k) { return k <= 1 ? 1 : k <= 2 ? 2 : k <= 4 ? 4 : 8; }
+static inline int pgrid(int num_sms, int per_sm, int64_t max_items) {
+  int64_t g = (int64_t)num_sms * per_sm;
+  if (g > max_items) g = max_items;
+  return g < 1 ? 1 : (int)g;
+}
+
+template <typename T>
+static int launch_y(const State& st, int k, int use_list, int num_sms, cudaStream_t s) {
+  int nl = 0;
+  if (st.cap) {
+    pf_an_kernel<T><<<pgrid(num_sms, 4, st.W), 256, 0, s>>>(st, k, use_list); ++nl;
+  }
+  int rpt = 64;
+  if (rpt > st.n) rpt = st.n;
+  const int tiles = (st.n + rpt - 1) / rpt;
+  const int grid = pgrid(num_sms, 4, (int64_t)st.W * tiles);
+  const int kt = round_kt(k);
+  const size_t smem = (size_t)kt * rpt * sizeof(T);
+  switch (kt) {
+    case 1: pf_y_kernel<T, 1><<<grid, 256, smem, s>>>(st, k, tiles, rpt, use_list); break;
+    case 2: pf_y_kernel<T, 2><<<grid, 256, smem, s>>>(st, k, tiles, rpt, use_list); break;
+    case 4: pf_y_kernel<T, 4><<<grid, 256, smem, s>>>(st, k, tiles, rpt, use_list); break;
+    default: pf_y_kernel<T, 8><<<grid, 256, smem, s>>>(st, k, tiles, rpt, use_list); break;
+  }
+  return nl + 1;
+}
+
+template <typename T>
+static int pf_ratio_impl(const State& st, int k, const int32_t* idx, const void* rows, void* ratio,
+                         int num_sms, cudaStream_t s) {
+  int nl = 0;
+  pf_gather_kernel<T><<<(unsigned)st.W, 128, 0, s>>>(st, k, idx, (const T*)rows, (T*)ratio); ++nl;
+  if (k > 1) {
+    nl += launch_y<T>(st, k, 0, num_sms, s);
+    pf_core_kernel<T><<<(unsigned)st.W, 128, 0, s>>>(st, k, (T*)ratio); ++nl;
+  }
+  return cudaGetLastError() == cudaSuccess ? nl : -1;
+}
+
+template <typename T>
+static int pf_flush_impl(const State& st, bool all, int num_sms, cudaStream_t s) {
+  int nl = 0;
+  if (all) nl += launch_flush_select_all(st, s);
+  const int t1 = (st.n + 63) / 64;
+  const int grid = pgrid(num_sms, 4, (int64_t)st.W * (t1 * (t1 + 1) / 2));
+  pf_flush_kernel<T><<<grid, 256, 0, s>>>(st, t1); ++nl;
+  nl += launch_flush_clear(st, s);
+  return cudaGetLastError() == cudaSuccess ? nl : -1;
+}
+
+template <typename T>
+static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_sms, cudaStream_t s) {
+  int nl = launch_select(st, mask, s);
+  if (k == 1) nl += launch_y<T>(st, k, 1, num_sms, s);  // Y only for accepted walkers
+  if (st.K == 0) {
+    const int t1 = (st.n + 31) / 32;
+    const int grid = pgrid(num_sms, 4, (int64_t)st.W * (t1 * (t1 + 1) / 2));
+    pf_update_kernel<T><<<grid, 256, 0, s>>>(st, k, t1); ++nl;
+  } else {
+    pf_append_kernel<T><<<pgrid(num_sms, 4, st.W), 256, 0, s>>>(st, k); ++nl;
+    nl += launch_post(st, 2 * k, s);
+    int r = pf_flush_impl<T>(st, false, num_sms, s);
+    if (r < 0) return -1;
+    nl += r;
+  }
+  return cudaGetLastError() == cudaSuccess ? nl : -1;
+}
+
+int launch_pf_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows, void* d_ratio,
+                    int num_sms, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? pf_ratio_impl<double>(st, k, d_idx, d_rows, d_ratio, num_sms, s)
+                           : pf_ratio_impl<cplx>(st, k, d_idx, d_rows, d_ratio, num_sms, s);
+}
+int launch_pf_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? pf_accept_impl<double>(st, k, d_mask, num_sms, s)
+                           : pf_accept_impl<cplx>(st, k, d_mask, num_sms, s);
+}
+int launch_pf_flush(const State& st, bool all, int num_sms, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? pf_flush_impl<double>(st, all, num_sms, s)
+                           : pf_flush_impl<cplx>(st, all, num_sms, s);
+}
+
+}  // namespace lrux

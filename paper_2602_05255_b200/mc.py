@@ -1,0 +1,61 @@
+"""Stream-ordered Metropolis chains driving the C-ABI library (harness level).
+
+One step = lruxh_*_propose -> lrux_*_ratio -> lruxh_decide -> lrux_*_accept, all
+enqueued on the current CUDA stream without host synchronisation.  This is the
+"step" bench.py times and the parity tests replay against the oracle.
+"""
+from __future__ import annotations
+
+import torch
+
+from . import lrux
+
+
+class Chain:
+    """Determinant (orbitals=Phi [W][M][n]) or Pfaffian (orbitals=F [W][M][M]) chain.
+
+    occ [W][n], unocc [W][M-n] int32 device tensors are updated in place.
+    """
+
+    def __init__(self, kind, orbitals, occ, unocc, k, K=0, seed=0, w0=0, kmax=None):
+        assert kind in ("det", "pf")
+        self.kind, self.k, self.K, self.seed, self.w0 = kind, int(k), int(K), int(seed), int(w0)
+        self.orb = orbitals.contiguous()
+        self.occ = occ.to(torch.int32).contiguous()
+        self.unocc = unocc.to(torch.int32).contiguous()
+        dev, dt = self.orb.device, self.orb.dtype
+        self.W, self.n = self.occ.shape
+        self.M = self.orb.shape[1]
+        W, n = self.W, self.n
+        ar = torch.arange(W, device=dev)[:, None]
+        occl = self.occ.long()
+        if kind == "det":
+            A0 = self.orb[ar, occl]                                   # [W][n][n]
+        else:
+            A0 = self.orb[ar[:, :, None], occl[:, :, None], occl[:, None, :]]
+        cls = lrux.DetWalkers if kind == "det" else lrux.PfWalkers
+        self.walkers = cls(A0, kmax=self.k if kmax is None else kmax, K=self.K)
+        del A0
+        self.idx = torch.zeros((W, self.k), dtype=torch.int32, device=dev)
+        self.upos = torch.zeros((W, self.k), dtype=torch.int32, device=dev)
+        self.rows = torch.zeros((W, self.k, n), dtype=dt, device=dev)
+        self.mask = torch.zeros(W, dtype=torch.uint8, device=dev)
+        self.naccept = torch.zeros(1, dtype=torch.int64, device=dev)
+        self.ratio = self.walkers.ratio
+        self.harness_launches = 0
+
+    def propose(self, t):
+        fn = lrux.det_propose if self.kind == "det" else lrux.pf_propose
+        fn(self.seed, self.w0, t, self.orb, self.occ, self.unocc, self.idx, self.upos, self.rows)
+        self.harness_launches += 1
+
+    def step(self, t):
+        self.propose(t)
+        self.walkers.ratio_(self.idx, self.rows)
+        lrux.decide(self.seed, self.w0, t, self.ratio, self.idx, self.upos, self.occ, self.unocc,
+                    self.mask, self.naccept)
+        self.harness_launches += 1
+        self.walkers.accept(self.mask)
+
+    def launches(self):
+        return self.walkers.launch_count() + self.harness_launches

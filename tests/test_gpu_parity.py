@@ -1,0 +1,156 @@
+"""GPU parity: the CUDA path (through the C ABI) vs the oracle, element by element
+on the same seeded inputs.  Tolerance: relative 1e-10 (BASELINE.json north_star)
+with the conditioning slack of parity_util.compare; decisions exact."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2602_05255_b200 import lrux
+from paper_2602_05255_b200 import workload as wl
+
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+
+
+def _run(kind, seed, W, n, M, k, K, steps, cplx=False, walkers=None, scratch_every=1):
+    orb, occ, unocc = pu.make_inputs(kind, seed, W, n, M, cplx)
+    rec = pu.run_gpu_chain(kind, orb, occ, unocc, k, K, seed, steps)
+    assert not rec["info"].any(), rec["info"]
+    walkers = list(range(W)) if walkers is None else walkers
+    oracle = pu.run_oracle(kind, orb, occ, unocc, k, seed, steps, walkers, scratch_every)
+    stats = pu.compare(kind, rec, oracle)
+    assert stats["dropped"] == 0
+    acc = rec["mask"].mean()
+    assert 0.05 < acc < 0.8, acc
+    assert rec["naccept"] == rec["mask"].sum()
+    return stats
+
+
+def test_det_config1():
+    """BASELINE.json configs[0]: 1 walker, n=32, M=64, k=1, 200 steps, no delay."""
+    stats = _run("det", wl.BASE_SEED + 1, 1, 32, 64, 1, 0, 200)
+    assert stats["points"] == 200
+
+
+@pytest.mark.parametrize("n,M,k,K,cplx", [
+    (32, 64, 1, 0, False),
+    (50, 100, 2, 0, False),      # ragged: n not a multiple of the 64-element chunk
+    (33, 70, 3, 0, False),       # odd n: scalar (VEC=1) path
+    (96, 192, 4, 0, False),
+    (64, 128, 8, 0, False),
+    (40, 80, 2, 0, True),
+    (64, 128, 4, 0, True),
+    (48, 96, 1, 4, False),       # delayed, K=4
+    (50, 100, 2, 3, False),
+    (64, 128, 4, 2, True),
+    (40, 90, 3, 5, True),
+])
+def test_det_small(n, M, k, K, cplx):
+    _run("det", 1234 + n + k, 6, n, M, k, K, 60, cplx)
+
+
+def test_det_config2_shape_reduced():
+    """configs[1] shape (n=256, M=512, k=2) on 40 walkers, 60 steps; oracle on 4 of
+    them; spans 4 row tiles x several waves of the update kernel."""
+    for K in (0, 16):
+        _run("det", wl.BASE_SEED + 2, 40, 256, 512, 2, K, 60, walkers=[0, 13, 27, 39])
+
+
+def test_det_large_n_stream_path():
+    """n=1100 > register-row limit: generic streaming update kernel."""
+    _run("det", 77, 3, 1100, 2200, 1, 0, 12, walkers=[0, 2], scratch_every=4)
+
+
+@pytest.mark.parametrize("n,M,k,K,cplx", [
+    (32, 64, 1, 0, False),
+    (50, 100, 1, 0, False),
+    (34, 70, 2, 0, False),
+    (64, 128, 3, 0, False),
+    (40, 80, 4, 0, False),
+    (32, 64, 1, 0, True),
+    (36, 72, 2, 0, True),
+    (48, 96, 1, 4, False),
+    (50, 100, 2, 3, False),
+    (32, 64, 2, 2, True),
+])
+def test_pf_small(n, M, k, K, cplx):
+    _run("pf", 4321 + n + k, 6, n, M, k, K, 60, cplx)
+
+
+def test_pf_config3_shape_reduced():
+    """configs[2] shape (n=128, M=256, k=1) on 24 walkers, 80 steps; oracle on 4."""
+    _run("pf", wl.BASE_SEED + 3, 24, 128, 256, 1, 0, 80, walkers=[0, 7, 15, 23])
+
+
+def test_det_config4_shape_reduced():
+    """configs[3] shape reduced: complex128, k=4, delay K=32, n=256."""
+    _run("det", wl.BASE_SEED + 4, 6, 256, 512, 4, 32, 80, cplx=True, walkers=[0, 5], scratch_every=5)
+
+
+# ---------------------------------------------------------------- error paths
+def test_errors_and_info_bits():
+    dev = "cuda"
+    W, n = 4, 16
+    rng = np.random.default_rng(3)
+    A0 = rng.standard_normal((W, n, n))
+    A0[2] = 0.0                                           # singular walker
+    wk = lrux.DetWalkers(torch.as_tensor(A0, device=dev), kmax=2, K=0)
+    torch.cuda.synchronize()
+    assert wk.info.cpu().tolist() == [0, 0, 1, 0]
+    mask = torch.ones(W, dtype=torch.uint8, device=dev)
+    with pytest.raises(lrux.LruxError) as e:              # accept without pending ratio
+        wk.accept(mask)
+    assert e.value.status == lrux.ESTATE
+    idx = torch.tensor([[0, 1], [3, 3], [0, 1], [0, 99]], dtype=torch.int32, device=dev)
+    rows = torch.as_tensor(rng.standard_normal((W, 2, n)), device=dev)
+    r = wk.ratio_(idx, rows).cpu().numpy()
+    assert np.isfinite(r[0]) and np.isnan(r[1]) and np.isnan(r[3])
+    inv_before = wk.get_inverse().cpu().numpy()
+    wk.ratio_(idx, rows)
+    wk.accept(mask)
+    info = wk.info.cpu().numpy()
+    assert info[0] == 0 and (info[1] & 2) and (info[3] & 2)
+    inv_after = wk.get_inverse().cpu().numpy()
+    assert not np.array_equal(inv_after[0], inv_before[0])          # walker 0 moved
+    assert np.array_equal(inv_after[1], inv_before[1])              # bad proposals left untouched
+    assert np.array_equal(inv_after[3], inv_before[3])
+    with pytest.raises(lrux.LruxError):                   # k > kmax
+        wk.ratio_(torch.zeros((W, 3), dtype=torch.int32, device=dev),
+                  torch.zeros((W, 3, n), dtype=torch.float64, device=dev))
+    with pytest.raises(lrux.LruxError):                   # odd n for a Pfaffian
+        lrux.PfWalkers(torch.zeros((2, 5, 5), dtype=torch.float64, device=dev))
+
+
+def test_init_amplitude_and_inverse():
+    """Step a0 alone: A^-1 and (phase, log|det|), (phase, log|pf|) vs the oracle."""
+    from oracle import lrux_oracle as orc
+
+    rng = np.random.default_rng(11)
+    for cplx in (False, True):
+        for n in (1, 2, 7, 64, 130):
+            A = rng.standard_normal((3, n, n))
+            if cplx:
+                A = A + 1j * rng.standard_normal((3, n, n))
+            wk = lrux.DetWalkers(torch.as_tensor(A, device="cuda"), kmax=1)
+            ph, la = wk.get_amplitude()
+            inv = wk.get_inverse().cpu().numpy()
+            for w in range(3):
+                oph, ola = orc.slogdet(A[w])
+                assert abs(ph[w].item() - oph) < 1e-9
+                assert abs(la[w].item() - ola) <= 1e-10 * max(1.0, abs(ola))
+                assert np.abs(inv[w] @ A[w] - np.eye(n)).max() < 1e-8
+        for n in (2, 8, 64, 130):
+            g = rng.standard_normal((3, n, n))
+            if cplx:
+                g = g + 1j * rng.standard_normal((3, n, n))
+            A = np.triu(g, 1) - np.triu(g, 1).transpose(0, 2, 1)
+            wk = lrux.PfWalkers(torch.as_tensor(A, device="cuda"), kmax=1)
+            ph, la = wk.get_amplitude()
+            inv = wk.get_inverse().cpu().numpy()
+            for w in range(3):
+                oph, ola = orc.slogpf(A[w])
+                assert abs(ph[w].item() - oph) < 1e-9
+                assert abs(la[w].item() - ola) <= 1e-10 * max(1.0, abs(ola))
+                assert np.abs(inv[w] @ A[w] - np.eye(n)).max() < 1e-8
+                assert np.array_equal(inv[w], -inv[w].T)
