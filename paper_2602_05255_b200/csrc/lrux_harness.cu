@@ -8,18 +8,21 @@ namespace lrux {
 constexpr uint64_t STREAM_SLOT = 2, STREAM_ORB = 3, STREAM_ACCEPT = 4;
 
 // k distinct values in [0,m): rho_a in [0,m-a) with counter step*k+a, skipping
-// previously chosen values in ascending order (workload._distinct).
-__device__ inline void draw_distinct(uint64_t seed, uint64_t w, uint64_t stream, uint64_t step,
-                                     int k, int m, int* out) {
-  int sorted[kMaxK];
+// previously chosen values in ascending order (workload._distinct), i.e. the
+// rho_a-th smallest value not chosen yet = least fixpoint of
+// v = rho_a + #{c < a : out[c] <= v}.
+__device__ __forceinline__ void draw_distinct(uint64_t seed, uint64_t w, uint64_t stream,
+                                              uint64_t step, int k, int m, int* out) {
   for (int a = 0; a < k; ++a) {
-    int rho = (int)to_below(rnd64(seed, w, stream, step * (uint64_t)k + a), (uint32_t)(m - a));
-    for (int c = 0; c < a; ++c)
-      if (rho >= sorted[c]) ++rho;
-    out[a] = rho;
-    int pos = a;  // insert into the sorted list
-    while (pos > 0 && sorted[pos - 1] > rho) { sorted[pos] = sorted[pos - 1]; --pos; }
-    sorted[pos] = rho;
+    const int rho = (int)to_below(rnd64(seed, w, stream, step * (uint64_t)k + a), (uint32_t)(m - a));
+    int v = rho;
+    for (int it = 0; it <= a; ++it) {
+      int cnt = 0;
+      for (int c = 0; c < a; ++c) cnt += (out[c] <= v) ? 1 : 0;
+      if (rho + cnt == v) break;
+      v = rho + cnt;
+    }
+    out[a] = v;
   }
 }
 
