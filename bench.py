@@ -1,0 +1,475 @@
+#!/usr/bin/env python
+"""bench.py -- walker-updates/s of the lrux hot path on B200 (BASELINE.json metric).
+
+One "step" = one Monte-Carlo step of every walker through the whole hot path
+(SURVEY.md §8(a)): lruxh_*_propose -> lrux_*_ratio -> lruxh_decide -> lrux_*_accept
+(immediate Woodbury update, or delayed append + flush when K > 0), all enqueued on
+one CUDA stream without host synchronisation.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c3|c4|n512...]
+    python bench.py --impl reference        # the CPU oracle on the host cores
+
+Prints ONE JSON line (rank 0).  See DESIGN.md §7 for the definition of every key.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "walker_updates_per_s"
+UNIT = "walker-updates/s"
+
+# name -> kind, dtype, W (per GPU), n, M, k, K variants (first = headline), default steps
+WORKLOADS = {
+    # BASELINE.json configs[1]: the configuration the metric is quoted on
+    "c2": dict(kind="det", cplx=False, W=4096, n=256, M=512, k=2, Ks=(0, 16), cfg=2,
+               desc="configs[1]: det f64, 4096 walkers, n=256, M=512, k=2, Metropolis; K=0 vs K=16"),
+    "c3": dict(kind="pf", cplx=False, W=1024, n=128, M=256, k=1, Ks=(0,), cfg=3,
+               desc="configs[2]: pf f64, 1024 walkers, n=128, M=256, k=1, Metropolis"),
+    "c4": dict(kind="det", cplx=True, W=512, n=1024, M=2048, k=4, Ks=(32,), cfg=4,
+               desc="configs[3]: det c128, 512 walkers, n=1024, M=2048, k=4, K=32, Metropolis"),
+    # small case used by the tests of bench.py itself
+    "tiny": dict(kind="det", cplx=False, W=64, n=64, M=128, k=2, Ks=(0, 4), cfg=2,
+                 desc="tiny det f64 smoke workload"),
+}
+
+
+def parse_args(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="lrux", choices=["lrux", "reference"])
+    ap.add_argument("--workload", default="c2")
+    ap.add_argument("--walkers", type=int, default=0, help="override walkers per GPU")
+    ap.add_argument("--e2e-steps", type=int, default=16)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0,
+                    help="CPU time budget of the cpu_baseline sample")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip forced-accept / delayed variants / DGEMM yardstick")
+    return ap.parse_args(argv)
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled DURING the timed region."""
+
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS,
+                 "--format=csv,noheader,nounits", "-lms", "20"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons, power = [], [], set(), []
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None,
+                "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------- GPU arm
+def build_inputs(wk, W, w0, device):
+    """Seeded synthetic inputs of the workload's shape, generated on the device
+    (DESIGN.md §4): per-walker Phi (det) or skew F (pf) and the initial occupation."""
+    from paper_2602_05255_b200 import workload as wl
+
+    seed = wl.BASE_SEED + wk["cfg"]
+    n, M = wk["n"], wk["M"]
+    if wk["kind"] == "det":
+        var = 1.0 / (2 * n) if wk["cplx"] else 1.0 / n
+        orb = wl.orbital_matrices_torch(seed, w0, W, M, n, var, device, wk["cplx"])
+    else:
+        orb = wl.pairing_matrices_torch(seed, w0, W, M, 1.0 / n, device)
+    occ, unocc = wl.initial_occupations(seed, W, M, n, w0=w0)
+    return seed, orb, occ, unocc
+
+
+def make_chain(wk, K, seed, orb, occ, unocc, w0, device):
+    import torch
+    from paper_2602_05255_b200 import mc
+
+    return mc.Chain(wk["kind"], orb, torch.as_tensor(occ, device=device),
+                    torch.as_tensor(unocc, device=device), k=wk["k"], K=K, seed=seed, w0=w0)
+
+
+def timed_run(ch, warmup, steps, forced=False, sampler=None):
+    """W untimed + K timed steps; device time by CUDA events on the launching stream,
+    barrier + synchronize on both sides.  Returns a dict of raw measurements."""
+    import torch
+    from paper_2602_05255_b200 import lrux, shard
+
+    for t in range(warmup):
+        ch.step(t, forced)
+    torch.cuda.synchronize()
+    shard.barrier()
+    torch.cuda.synchronize()
+    acc0 = int(ch.naccept.item())
+    l0 = ch.launches()
+    ch.walkers.profile_enable(True)
+    for c in range(5):
+        ch.walkers.profile_read(c)
+    if sampler:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for t in range(steps):
+        ch.step(warmup + t, forced)
+    e1.record()
+    torch.cuda.synchronize()
+    shard.barrier()
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler else None
+    ms = e0.elapsed_time(e1)
+    prof = {}
+    for name, c in (("ratio", lrux.PROF_RATIO), ("update", lrux.PROF_UPDATE),
+                    ("append", lrux.PROF_APPEND), ("flush", lrux.PROF_FLUSH),
+                    ("ypass", lrux.PROF_YPASS)):
+        t_ms, cnt = ch.walkers.profile_read(c)
+        prof[name] = {"ms": t_ms, "launches": cnt}
+    ch.walkers.profile_enable(False)
+    return {"ms": ms, "accepted": int(ch.naccept.item()) - acc0, "launches": ch.launches() - l0,
+            "prof": prof, "clocks": clocks}
+
+
+def e2e_run(wk, seed, orb, occ, unocc, w0, device, warmup, steps):
+    """The same chain driven through the C-ABI calls from HOST buffers: every step
+    copies idx + new rows from pinned host memory, reads the ratios back, takes the
+    Metropolis decision on the host and uploads the mask.  The host
+    inputs are recorded from a device-harness run of the same chain beforehand, so
+    the replay walks the identical trajectory."""
+    import numpy as np
+    import torch
+    from paper_2602_05255_b200 import workload as wl
+
+    K = wk["Ks"][0]
+    T = warmup + steps
+    W, k, n = occ.shape[0], wk["k"], wk["n"]
+    dt = orb.dtype
+    rec = make_chain(wk, K, seed, orb, occ, unocc, w0, device)
+    idx_h = torch.empty((T, W, k), dtype=torch.int32).pin_memory()
+    rows_h = torch.empty((T, W, k, n), dtype=dt).pin_memory()
+    mask_rec = torch.empty((T, W), dtype=torch.uint8).pin_memory()
+    for t in range(T):
+        rec.step(t)
+        idx_h[t].copy_(rec.idx)
+        rows_h[t].copy_(rec.rows)
+        mask_rec[t].copy_(rec.mask)
+    torch.cuda.synchronize()
+    A0_chain = make_chain(wk, K, seed, orb, occ, unocc, w0, device)   # fresh state, same A0
+    wkr = A0_chain.walkers
+    del rec
+    xi = np.stack([wl.to_uniform(wl.rnd64(seed, np.arange(w0, w0 + W, dtype=np.uint64),
+                                          wl.STREAM_ACCEPT, np.uint64(t))) for t in range(T)])
+    idx_d, rows_d, mask_d = A0_chain.idx, A0_chain.rows, A0_chain.mask
+    ratio_h = torch.empty(W, dtype=dt).pin_memory()
+    mask_h = torch.empty(W, dtype=torch.uint8).pin_memory()
+    mism = 0
+    t_start = 0.0
+    for t in range(T):
+        if t == warmup:
+            torch.cuda.synchronize()
+            t_start = time.perf_counter()
+        idx_d.copy_(idx_h[t], non_blocking=True)
+        rows_d.copy_(rows_h[t], non_blocking=True)
+        wkr.ratio_(idx_d, rows_d)
+        ratio_h.copy_(wkr.ratio, non_blocking=True)
+        torch.cuda.synchronize()
+        r = ratio_h.numpy()
+        a2 = r.real ** 2 + r.imag ** 2 if wk["cplx"] else r * r
+        m = (xi[t] < np.minimum(1.0, a2))
+        mask_h.numpy()[:] = m
+        mism += int((m != mask_rec[t].numpy().astype(bool)).sum())
+        mask_d.copy_(mask_h, non_blocking=True)
+        wkr.accept(mask_d)
+    torch.cuda.synchronize()
+    sec = time.perf_counter() - t_start
+    esz = 16 if wk["cplx"] else 8
+    return {"sec": sec, "steps": steps, "mismatch": mism,
+            "h2d": W * k * 4 + W * k * n * esz + W, "d2h": W * esz}
+
+
+# ---------------------------------------------------------------------------- CPU oracle arm
+def oracle_cores():
+    try:
+        from threadpoolctl import threadpool_info
+
+        nt = [int(p.get("num_threads", 1)) for p in threadpool_info()]
+        return max(nt) if nt else 1
+    except Exception:
+        return 1
+
+
+class _Clock:
+    """Timestamps delivered by the oracle's on_step hook."""
+
+    def __init__(self):
+        self.t = {}
+
+    def __call__(self, step):
+        self.t[step] = time.perf_counter()
+
+
+def oracle_sample(wk, warmup, steps, budget_s, max_walkers=1 << 30):
+    """Time the oracle (as it stands) on walkers 0,1,2,... of the workload, `warmup`
+    untimed + `steps` timed Monte-Carlo steps each, until `budget_s` seconds of timed
+    work are spent.  Returns (timed seconds, walker-steps done, walkers)."""
+    import numpy as np
+    from oracle import lrux_oracle as orc
+    from paper_2602_05255_b200 import workload as wl
+
+    seed = wl.BASE_SEED + wk["cfg"]
+    n, M, k = wk["n"], wk["M"], wk["k"]
+    T = warmup + steps
+    total, done, nw = 0.0, 0, 0
+    while total < budget_s and nw < max_walkers:
+        w = nw
+        if wk["kind"] == "det":
+            var = 1.0 / (2 * n) if wk["cplx"] else 1.0 / n
+            orb = wl.orbital_matrix(seed, w, M, n, var, wk["cplx"])
+        else:
+            orb = wl.pairing_matrix(seed, w, M, 1.0 / n, wk["cplx"])
+        occ, unocc = wl.initial_occupation(seed, w, M, n)
+        P, J, xi = wl.proposals(seed, w + 1, T, n, M, k, walkers=[w])
+        clk = _Clock()
+        fn = orc.det_trajectory if wk["kind"] == "det" else orc.pf_trajectory
+        t_init = time.perf_counter()
+        fn(orb, occ, unocc, P[:, 0], J[:, 0], xi[:, 0], scratch_every=0, delay=wk["Ks"][0],
+           on_step=clk)
+        t_begin = clk.t[warmup - 1] if warmup > 0 else t_init
+        total += clk.t[T - 1] - t_begin
+        done += steps
+        nw += 1
+    return total, done, nw
+
+
+def reference_arm(args, wk):
+    """--impl reference: the oracle timed on the host cores on this arm's config,
+    metric and unit (rank 0 only)."""
+    from paper_2602_05255_b200 import shard
+
+    rank, _, _ = shard.env_rank()
+    if rank != 0:
+        return 0
+    steps, warmup = args.steps, args.warmup
+    # bounded sample: at most ~cpu-seconds*4 of oracle work in total
+    sec, done, nw = oracle_sample(wk, warmup, steps, args.cpu_seconds * 4, max_walkers=64)
+    value = done / sec
+    cores = oracle_cores()
+    sample = "%d walker(s) x %d steps of %s, oracle naive path (scratch_every=0)" % (nw, steps, args.workload)
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+           "n_gpus": args.gpus, "steps": steps, "warmup": warmup,
+           "ms_per_step": 1e3 * sec / max(1, steps), "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "c128" if wk["cplx"] else "f64", "data": "synthetic",
+           "config": {"workload": wk["desc"], "K": wk["Ks"][0], "sample": sample},
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                            "sample": sample},
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+    return 0
+
+
+# ---------------------------------------------------------------------------- main
+def dgemm_yardstick(device, n=4096, reps=5):
+    """cuBLAS FP64 GEMM throughput (TFLOP/s) as the measured FP64 tensor peak the
+    flush is reported against (yardstick only; not on the product path)."""
+    import torch
+
+    a = torch.randn((n, n), dtype=torch.float64, device=device)
+    b = torch.randn((n, n), dtype=torch.float64, device=device)
+    torch.matmul(a, b)
+    torch.cuda.synchronize()
+    best = 1e30
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        torch.matmul(a, b)
+        e1.record()
+        torch.cuda.synchronize()
+        best = min(best, e0.elapsed_time(e1))
+    return 2.0 * n ** 3 / (best * 1e-3) / 1e12
+
+
+def roofline_update(wk, run, peak, peak_src):
+    """HBM roofline of the immediate Woodbury update kernel:
+    algorithmic bytes = 2 n^2 e per accepted walker (read once + write once)."""
+    esz = 16 if wk["cplx"] else 8
+    pr = run["prof"]["update"]
+    if pr["launches"] == 0 or pr["ms"] <= 0:
+        return None
+    byts = 2.0 * wk["n"] ** 2 * esz * run["accepted"]
+    ach = byts / (pr["ms"] * 1e-3) / 1e9
+    return {"bound": "hbm", "kernel": "%s_update_kernel" % wk["kind"], "achieved": ach, "peak": peak,
+            "unit": "GB/s", "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+            "bytes_per_launch": byts / pr["launches"], "us_per_launch": 1e3 * pr["ms"] / pr["launches"],
+            "launches": pr["launches"]}
+
+
+def main(argv=None):
+    args = parse_args(argv)
+    if args.workload not in WORKLOADS:
+        raise SystemExit("unknown workload %r" % args.workload)
+    wk = dict(WORKLOADS[args.workload])
+    if args.walkers:
+        wk["W"] = args.walkers
+    if args.impl == "reference":
+        return reference_arm(args, wk)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2602_05255_b200 import build, lrux, shard
+
+    rank, local_rank, world = shard.env_rank()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+    build.build()
+    lrux.load_library()
+
+    W = wk["W"]
+    w0, _ = shard.walker_range(rank, world, W)
+    seed, orb, occ, unocc = build_inputs(wk, W, w0, device)
+    peak, peak_src = measured_peaks()
+    steps, warmup = args.steps, max(3, args.warmup)
+
+    # headline: first K variant, Metropolis as the config is written
+    K0 = wk["Ks"][0]
+    ch = make_chain(wk, K0, seed, orb, occ, unocc, w0, device)
+    run = timed_run(ch, warmup, steps, sampler=ClockSampler(local_rank) if rank == 0 else None)
+    info_bad = int((ch.walkers.info != 0).sum().item())
+    del ch
+    ms_max, = shard.reduce_scalars([run["ms"]], "max", device)
+    acc_sum, launches = shard.reduce_scalars([run["accepted"], run["launches"]], "sum", device)
+    value = W * world * steps / (ms_max * 1e-3)
+
+    extras = {}
+    if not args.no_extras:
+        # forced-accept (every proposal applied: what the paper's Fig. 2 times) -> cleanest roofline
+        chf = make_chain(wk, K0, seed, orb, occ, unocc, w0, device)
+        fsteps = min(steps, 50)
+        rf = timed_run(chf, warmup, fsteps, forced=True)
+        del chf
+        extras["forced_accept"] = {
+            "K": K0, "steps": fsteps, "walker_updates_per_s": W * fsteps / (rf["ms"] * 1e-3),
+            "accept_frac": rf["accepted"] / float(W * fsteps),
+            "roofline": roofline_update(wk, rf, peak, peak_src) if K0 == 0 else None,
+            "prof_ms": {k: v["ms"] for k, v in rf["prof"].items()}}
+        for K in wk["Ks"][1:]:
+            chk = make_chain(wk, K, seed, orb, occ, unocc, w0, device)
+            rk = timed_run(chk, warmup, steps)
+            del chk
+            esz = 16 if wk["cplx"] else 8
+            fl = rk["prof"]["flush"]
+            extras["K%d" % K] = {
+                "walker_updates_per_s": W * steps / (rk["ms"] * 1e-3), "ms_per_step": rk["ms"] / steps,
+                "accept_frac": rk["accepted"] / float(W * steps),
+                "prof_ms": {k: v["ms"] for k, v in rk["prof"].items()},
+                # flush: 2 n^2 Kk flops and 2 n^2 e + 2 n Kk e bytes per flushed walker (full buffers)
+                "flush_tflops": (2.0 * wk["n"] ** 2 * wk["k"] * rk["accepted"] / (fl["ms"] * 1e-3) / 1e12
+                                 if fl["ms"] > 0 else None),
+                "flush_gbs": ((2.0 * wk["n"] ** 2 * esz / K + 2.0 * wk["n"] * wk["k"] * esz) * rk["accepted"]
+                              / (fl["ms"] * 1e-3) / 1e9 if fl["ms"] > 0 else None)}
+        if rank == 0:
+            extras["dgemm_f64_tflops_cublas"] = dgemm_yardstick(device)
+
+    # end to end through the C-ABI from host buffers
+    e2e_steps = max(1, min(args.e2e_steps, steps))
+    ee = e2e_run(wk, seed, orb, occ, unocc, w0, device, 3, e2e_steps)
+    ee_sec, = shard.reduce_scalars([ee["sec"]], "max", device)
+    e2e_value = W * world * e2e_steps / ee_sec
+
+    roof = roofline_update(wk, run, peak, peak_src) if K0 == 0 else None
+    if roof is None and "forced_accept" in extras and extras["forced_accept"]["roofline"]:
+        roof = extras["forced_accept"]["roofline"]
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
+           "warmup": warmup, "ms_per_step": ms_max / steps, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "c128" if wk["cplx"] else "f64",
+           "data": "synthetic",
+           "config": {"workload": wk["desc"], "walkers_per_gpu": W, "n": wk["n"], "M": wk["M"],
+                      "k": wk["k"], "K": K0, "mode": "metropolis",
+                      "l2": "inputs larger than L2: %.2f GiB of inverses per GPU, no flush needed"
+                            % (W * wk["n"] ** 2 * (16 if wk["cplx"] else 8) / 2 ** 30)},
+           "accept_frac": acc_sum / float(W * world * steps),
+           "accepted_updates_per_s": acc_sum / (ms_max * 1e-3),
+           "gpu_launches": int(launches), "info_nonzero_walkers": info_bad,
+           "clocks": run["clocks"],
+           "prof_ms": {k: v["ms"] for k, v in run["prof"].items()},
+           "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": ee["h2d"],
+                   "d2h_bytes_per_step": ee["d2h"], "steps": e2e_steps,
+                   "decision_mismatches_vs_device_chain": ee["mismatch"]},
+           "roofline": roof, "extras": extras}
+    if rank == 0:
+        if world == 1:
+            sec, done, nw = oracle_sample(wk, 2, 20, args.cpu_seconds)
+            out["cpu_baseline"] = {
+                "value": done / sec, "unit": UNIT, "cores": oracle_cores(), "kind": "oracle",
+                "sample": "%d walker(s) x 20 steps of %s (after 2 warm-up steps), oracle naive path"
+                          % (nw, args.workload)}
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

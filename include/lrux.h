@@ -120,6 +120,25 @@ lrux_status_t lrux_pf_get_amplitude(lrux_handle_t h, void* d_phase, double* d_lo
                                     void* stream);
 lrux_status_t lrux_pf_get_inverse(lrux_handle_t h, void* d_out, void* stream);
 
+/* ---------------------------------------------------------------- profiling
+ * Device time per kernel class, taken with CUDA events the library records on the
+ * caller's stream directly around its own launches (bench.py's roofline figures:
+ * algorithmic bytes or flops / these durations).  Off by default; host objects
+ * only.  lrux_profile_read is the one call that waits: it synchronises on the
+ * events recorded so far for `cls`, returns their summed duration in
+ * milliseconds and the number of timed launches, and clears that class. */
+typedef enum {
+  LRUX_PROF_RATIO = 0,  /* gather + core + det/pf (a1, a2, a5) */
+  LRUX_PROF_UPDATE = 1, /* immediate Woodbury update of A^-1 (a3, a4) */
+  LRUX_PROF_APPEND = 2, /* delayed append (a6) */
+  LRUX_PROF_FLUSH = 3,  /* delay-buffer fold (a7) */
+  LRUX_PROF_YPASS = 4,  /* Pfaffian read-only pass Y = A^-1 N */
+  LRUX_PROF_NCLASS = 5
+} lrux_prof_class_t;
+lrux_status_t lrux_profile_enable(lrux_handle_t h, int32_t on);
+lrux_status_t lrux_profile_read(lrux_handle_t h, int32_t cls, double* ms_total,
+                                int64_t* launches);
+
 /* ---------------------------------------------------------------- common */
 /* Number of kernel launches the library has enqueued through this handle so far
  * (host counter; bench.py reports it as gpu_launches). */

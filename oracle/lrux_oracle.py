@@ -411,7 +411,7 @@ def _quot(ph1, la1, ph0, la0):
     return (ph1 / ph0) * np.exp(la1 - la0)
 
 
-def det_trajectory(Phi, occ, unocc, P, J, xi, scratch_every=1, delay=0):
+def det_trajectory(Phi, occ, unocc, P, J, xi, scratch_every=1, delay=0, on_step=None):
     """One walker's chain of k-row replacements (BASELINE.json configs[0,1,3]).
 
     A = Phi[occ,:].  Step t proposes to put orbital unocc[J[t][a]] into slot
@@ -463,12 +463,14 @@ def det_trajectory(Phi, occ, unocc, P, J, xi, scratch_every=1, delay=0):
             logabs = logabs + float(np.log(abs(r)))
             for a in range(len(p)):
                 occ[p[a]], unocc[J[t][a]] = unocc[J[t][a]], occ[p[a]]
+        if on_step is not None:
+            on_step(t)        # timing hook for bench.py; takes no part in the arithmetic
     out.update(A=A, Ainv=carrier.inverse() if carrier else Ainv, occ=occ, unocc=unocc,
                phase=phase, logabs=logabs, scratch_phase=s_ph, scratch_logabs=s_la)
     return out
 
 
-def pf_trajectory(F, occ, unocc, P, J, xi, scratch_every=1, delay=0):
+def pf_trajectory(F, occ, unocc, P, J, xi, scratch_every=1, delay=0, on_step=None):
     """One walker's chain of k-orbital replacements in a Pfaffian state
     (BASELINE.json configs[2]).  A = F[occ][:,occ]; replacing the orbital in slot p
     changes row p and column p of A (Eq. 23-24); u from ``pf_update_vectors``;
@@ -516,6 +518,8 @@ def pf_trajectory(F, occ, unocc, P, J, xi, scratch_every=1, delay=0):
             logabs = logabs + float(np.log(abs(r)))
             for a in range(len(p)):
                 occ[p[a]], unocc[J[t][a]] = unocc[J[t][a]], occ[p[a]]
+        if on_step is not None:
+            on_step(t)        # timing hook for bench.py; takes no part in the arithmetic
     out.update(A=A, Ainv=carrier.inverse() if carrier else Ainv, occ=occ, unocc=unocc,
                phase=phase, logabs=logabs, scratch_phase=s_ph, scratch_logabs=s_la)
     return out

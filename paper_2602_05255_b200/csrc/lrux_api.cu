@@ -139,7 +139,7 @@ lrux_status_t lrux_det_ratio(lrux_handle_t h, int32_t k, const int32_t* d_idx, c
                              void* d_ratio, void* stream) {
   LRUX_CHECK_HANDLE(h, KIND_DET);
   if (k < 1 || k > h->st.kmax || !d_idx || !d_rows || !d_ratio) return LRUX_EINVAL;
-  LRUX_COUNT(h, launch_det_ratio(h->st, k, d_idx, d_rows, d_ratio, (cudaStream_t)stream));
+  LRUX_COUNT(h, launch_det_ratio(h->st, k, d_idx, d_rows, d_ratio, (cudaStream_t)stream, &h->prof));
   h->pending_k = k;
   return LRUX_OK;
 }
@@ -147,7 +147,7 @@ lrux_status_t lrux_pf_ratio(lrux_handle_t h, int32_t k, const int32_t* d_idx, co
                             void* d_ratio, void* stream) {
   LRUX_CHECK_HANDLE(h, KIND_PF);
   if (k < 1 || k > h->st.kmax || !d_idx || !d_rows || !d_ratio) return LRUX_EINVAL;
-  LRUX_COUNT(h, launch_pf_ratio(h->st, k, d_idx, d_rows, d_ratio, h->num_sms, (cudaStream_t)stream));
+  LRUX_COUNT(h, launch_pf_ratio(h->st, k, d_idx, d_rows, d_ratio, h->num_sms, (cudaStream_t)stream, &h->prof));
   h->pending_k = k;
   return LRUX_OK;
 }
@@ -156,7 +156,7 @@ lrux_status_t lrux_det_accept(lrux_handle_t h, const uint8_t* d_mask, void* stre
   LRUX_CHECK_HANDLE(h, KIND_DET);
   if (!d_mask) return LRUX_EINVAL;
   if (h->pending_k == 0) return LRUX_ESTATE;
-  LRUX_COUNT(h, launch_det_accept(h->st, h->pending_k, d_mask, h->num_sms, (cudaStream_t)stream));
+  LRUX_COUNT(h, launch_det_accept(h->st, h->pending_k, d_mask, h->num_sms, (cudaStream_t)stream, &h->prof));
   h->pending_k = 0;
   return LRUX_OK;
 }
@@ -164,7 +164,7 @@ lrux_status_t lrux_pf_accept(lrux_handle_t h, const uint8_t* d_mask, void* strea
   LRUX_CHECK_HANDLE(h, KIND_PF);
   if (!d_mask) return LRUX_EINVAL;
   if (h->pending_k == 0) return LRUX_ESTATE;
-  LRUX_COUNT(h, launch_pf_accept(h->st, h->pending_k, d_mask, h->num_sms, (cudaStream_t)stream));
+  LRUX_COUNT(h, launch_pf_accept(h->st, h->pending_k, d_mask, h->num_sms, (cudaStream_t)stream, &h->prof));
   h->pending_k = 0;
   return LRUX_OK;
 }
@@ -172,13 +172,13 @@ lrux_status_t lrux_pf_accept(lrux_handle_t h, const uint8_t* d_mask, void* strea
 lrux_status_t lrux_det_flush(lrux_handle_t h, void* stream) {
   LRUX_CHECK_HANDLE(h, KIND_DET);
   if (h->st.K == 0) return LRUX_OK;
-  LRUX_COUNT(h, launch_det_flush(h->st, true, h->num_sms, (cudaStream_t)stream));
+  LRUX_COUNT(h, launch_det_flush(h->st, true, h->num_sms, (cudaStream_t)stream, &h->prof));
   return LRUX_OK;
 }
 lrux_status_t lrux_pf_flush(lrux_handle_t h, void* stream) {
   LRUX_CHECK_HANDLE(h, KIND_PF);
   if (h->st.K == 0) return LRUX_OK;
-  LRUX_COUNT(h, launch_pf_flush(h->st, true, h->num_sms, (cudaStream_t)stream));
+  LRUX_COUNT(h, launch_pf_flush(h->st, true, h->num_sms, (cudaStream_t)stream, &h->prof));
   return LRUX_OK;
 }
 
@@ -200,14 +200,14 @@ lrux_status_t lrux_pf_get_amplitude(lrux_handle_t h, void* d_phase, double* d_lo
 lrux_status_t lrux_det_get_inverse(lrux_handle_t h, void* d_out, void* stream) {
   LRUX_CHECK_HANDLE(h, KIND_DET);
   if (!d_out) return LRUX_EINVAL;
-  if (h->st.K > 0) LRUX_COUNT(h, launch_det_flush(h->st, true, h->num_sms, (cudaStream_t)stream));
+  if (h->st.K > 0) LRUX_COUNT(h, launch_det_flush(h->st, true, h->num_sms, (cudaStream_t)stream, &h->prof));
   LRUX_COUNT(h, launch_get_inverse(h->st, d_out, (cudaStream_t)stream));
   return LRUX_OK;
 }
 lrux_status_t lrux_pf_get_inverse(lrux_handle_t h, void* d_out, void* stream) {
   LRUX_CHECK_HANDLE(h, KIND_PF);
   if (!d_out) return LRUX_EINVAL;
-  if (h->st.K > 0) LRUX_COUNT(h, launch_pf_flush(h->st, true, h->num_sms, (cudaStream_t)stream));
+  if (h->st.K > 0) LRUX_COUNT(h, launch_pf_flush(h->st, true, h->num_sms, (cudaStream_t)stream, &h->prof));
   LRUX_COUNT(h, launch_get_inverse(h->st, d_out, (cudaStream_t)stream));
   return LRUX_OK;
 }
@@ -218,8 +218,35 @@ lrux_status_t lrux_launch_count(lrux_handle_t h, int64_t* count) {
   return LRUX_OK;
 }
 
+lrux_status_t lrux_profile_enable(lrux_handle_t h, int32_t on) {
+  if (!h) return LRUX_EINVAL;
+  h->prof.on = on != 0;
+  return LRUX_OK;
+}
+
+lrux_status_t lrux_profile_read(lrux_handle_t h, int32_t cls, double* ms_total, int64_t* launches) {
+  if (!h || !ms_total || !launches || cls < 0 || cls >= LRUX_PROF_NCLASS) return LRUX_EINVAL;
+  double ms = 0.0;
+  int64_t cnt = 0;
+  for (auto& r : h->prof.recs[cls]) {
+    float t = 0.f;
+    if (cudaEventSynchronize(r.b) != cudaSuccess || cudaEventElapsedTime(&t, r.a, r.b) != cudaSuccess)
+      return LRUX_ECUDA;
+    ms += t;
+    ++cnt;
+    h->prof.pool.push_back(r);
+  }
+  h->prof.recs[cls].clear();
+  *ms_total = ms;
+  *launches = cnt;
+  return LRUX_OK;
+}
+
 lrux_status_t lrux_destroy(lrux_handle_t h) {
   if (!h) return LRUX_EINVAL;
+  for (int c = 0; c < LRUX_PROF_NCLASS; ++c)
+    for (auto& r : h->prof.recs[c]) h->prof.pool.push_back(r);
+  for (auto& r : h->prof.pool) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   delete h;
   return LRUX_OK;
 }

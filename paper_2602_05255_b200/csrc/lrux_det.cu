@@ -584,7 +584,7 @@ static int launch_append_kt(const State& st, int k, int num_sms, cudaStream_t s)
 }
 
 template <typename T>
-static int flush_impl(const State& st, bool all, int num_sms, cudaStream_t s) {
+static int flush_impl(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof) {
   int nl = 0;
   const unsigned gw = (unsigned)((st.W + 255) / 256);
   if (all) {
@@ -593,19 +593,24 @@ static int flush_impl(const State& st, bool all, int num_sms, cudaStream_t s) {
   }
   const int t1 = (st.n + 63) / 64;
   const int grid = persistent_grid(num_sms, 4, (int64_t)st.W * t1 * t1);
-  det_flush_kernel<T><<<grid, 256, 0, s>>>(st, t1); ++nl;
+  {
+    ProfScope ps(prof, LRUX_PROF_FLUSH, s);
+    det_flush_kernel<T><<<grid, 256, 0, s>>>(st, t1); ++nl;
+  }
   flush_clear_kernel<<<gw, 256, 0, s>>>(st); ++nl;
   return cudaGetLastError() == cudaSuccess ? nl : -1;
 }
 
 template <typename T>
-static int accept_impl(const State& st, int k, const uint8_t* mask, int num_sms, cudaStream_t s) {
+static int accept_impl(const State& st, int k, const uint8_t* mask, int num_sms, cudaStream_t s,
+                       Prof* prof) {
   int nl = 0;
   const unsigned gw = (unsigned)((st.W + 255) / 256);
   select_kernel<T><<<gw, 256, 0, s>>>(st, mask); ++nl;
   const int kt = round_kt(k);
   int r = 0;
   if (st.K == 0) {
+    ProfScope ps(prof, LRUX_PROF_UPDATE, s);
     switch (kt) {
       case 1: r = launch_update_kt<T, 1>(st, k, num_sms, s); break;
       case 2: r = launch_update_kt<T, 2>(st, k, num_sms, s); break;
@@ -616,17 +621,20 @@ static int accept_impl(const State& st, int k, const uint8_t* mask, int num_sms,
     nl += r;
   } else {
     const int grid = persistent_grid(num_sms, 4, st.W);
-    det_prep_kernel<T><<<grid, 256, 0, s>>>(st, k); ++nl;
-    switch (kt) {
-      case 1: r = launch_append_kt<T, 1>(st, k, num_sms, s); break;
-      case 2: r = launch_append_kt<T, 2>(st, k, num_sms, s); break;
-      case 4: r = launch_append_kt<T, 4>(st, k, num_sms, s); break;
-      default: r = launch_append_kt<T, 8>(st, k, num_sms, s); break;
+    {
+      ProfScope ps(prof, LRUX_PROF_APPEND, s);
+      det_prep_kernel<T><<<grid, 256, 0, s>>>(st, k); ++nl;
+      switch (kt) {
+        case 1: r = launch_append_kt<T, 1>(st, k, num_sms, s); break;
+        case 2: r = launch_append_kt<T, 2>(st, k, num_sms, s); break;
+        case 4: r = launch_append_kt<T, 4>(st, k, num_sms, s); break;
+        default: r = launch_append_kt<T, 8>(st, k, num_sms, s); break;
+      }
     }
     if (r < 0) return -1;
     nl += r;
     post_kernel<<<gw, 256, 0, s>>>(st, k); ++nl;
-    r = flush_impl<T>(st, false, num_sms, s);
+    r = flush_impl<T>(st, false, num_sms, s, prof);
     if (r < 0) return -1;
     nl += r;
   }
@@ -634,7 +642,8 @@ static int accept_impl(const State& st, int k, const uint8_t* mask, int num_sms,
 }
 
 int launch_det_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
-                     void* d_ratio, cudaStream_t s) {
+                     void* d_ratio, cudaStream_t s, Prof* prof) {
+  ProfScope ps(prof, LRUX_PROF_RATIO, s);
   if (st.dt == LRUX_F64)
     det_ratio_kernel<double><<<(unsigned)st.W, 128, 0, s>>>(st, k, d_idx, (const double*)d_rows,
                                                             (double*)d_ratio);
@@ -644,14 +653,15 @@ int launch_det_ratio(const State& st, int k, const int32_t* d_idx, const void* d
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
-int launch_det_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s) {
-  return st.dt == LRUX_F64 ? accept_impl<double>(st, k, d_mask, num_sms, s)
-                           : accept_impl<cplx>(st, k, d_mask, num_sms, s);
+int launch_det_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s,
+                      Prof* prof) {
+  return st.dt == LRUX_F64 ? accept_impl<double>(st, k, d_mask, num_sms, s, prof)
+                           : accept_impl<cplx>(st, k, d_mask, num_sms, s, prof);
 }
 
-int launch_det_flush(const State& st, bool all, int num_sms, cudaStream_t s) {
-  return st.dt == LRUX_F64 ? flush_impl<double>(st, all, num_sms, s)
-                           : flush_impl<cplx>(st, all, num_sms, s);
+int launch_det_flush(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof) {
+  return st.dt == LRUX_F64 ? flush_impl<double>(st, all, num_sms, s, prof)
+                           : flush_impl<cplx>(st, all, num_sms, s, prof);
 }
 
 }  // namespace lrux

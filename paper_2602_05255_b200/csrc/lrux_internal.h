@@ -4,6 +4,8 @@
 #include <stddef.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "lrux.h"
 
 namespace lrux {
@@ -40,10 +42,36 @@ struct State {
   int32_t* info;     // caller's d_info
 };
 
+// Optional per-class kernel timing (lrux_profile_*): event pairs recorded on the
+// caller's stream around the library's own launches.
+struct Prof {
+  struct Rec { cudaEvent_t a, b; };
+  bool on = false;
+  std::vector<Rec> recs[LRUX_PROF_NCLASS];
+  std::vector<Rec> pool;
+  Rec get() {
+    Rec r{};
+    if (!pool.empty()) { r = pool.back(); pool.pop_back(); return r; }
+    cudaEventCreate(&r.a);
+    cudaEventCreate(&r.b);
+    return r;
+  }
+};
+struct ProfScope {
+  Prof* p; int cls; cudaStream_t s; Prof::Rec r;
+  ProfScope(Prof* p_, int cls_, cudaStream_t s_) : p(p_ && p_->on ? p_ : nullptr), cls(cls_), s(s_) {
+    if (p) { r = p->get(); cudaEventRecord(r.a, s); }
+  }
+  ~ProfScope() {
+    if (p) { cudaEventRecord(r.b, s); p->recs[cls].push_back(r); }
+  }
+};
+
 }  // namespace lrux
 
 struct lrux_handle_s {
   lrux::State st;
+  lrux::Prof prof;
   int32_t pending_k;  // 0 = nothing pending
   int64_t launches;
   int32_t num_sms;
@@ -58,13 +86,15 @@ size_t state_layout(State* st, void* base, int64_t W, int32_t n, int32_t kmax, i
 int launch_det_init(const State& st, const void* d_A0, cudaStream_t s);
 int launch_pf_init(const State& st, const void* d_A0, cudaStream_t s);
 int launch_det_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
-                     void* d_ratio, cudaStream_t s);
-int launch_det_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s);
-int launch_det_flush(const State& st, bool all, int num_sms, cudaStream_t s);
+                     void* d_ratio, cudaStream_t s, Prof* prof);
+int launch_det_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s,
+                      Prof* prof);
+int launch_det_flush(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof);
 int launch_pf_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
-                    void* d_ratio, int num_sms, cudaStream_t s);
-int launch_pf_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s);
-int launch_pf_flush(const State& st, bool all, int num_sms, cudaStream_t s);
+                    void* d_ratio, int num_sms, cudaStream_t s, Prof* prof);
+int launch_pf_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s,
+                     Prof* prof);
+int launch_pf_flush(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof);
 // shared between det and pf (defined in lrux_det.cu)
 int launch_select(const State& st, const uint8_t* mask, cudaStream_t s);
 int launch_post(const State& st, int ncols, cudaStream_t s);

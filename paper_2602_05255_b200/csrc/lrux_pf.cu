@@ -430,7 +430,8 @@ static inline int pgrid(int num_sms, int per_sm, int64_t max_items) {
 }
 
 template <typename T>
-static int launch_y(const State& st, int k, int use_list, int num_sms, cudaStream_t s) {
+static int launch_y(const State& st, int k, int use_list, int num_sms, cudaStream_t s, Prof* prof) {
+  ProfScope ps(prof, LRUX_PROF_YPASS, s);
   int nl = 0;
   if (st.cap) {
     pf_an_kernel<T><<<pgrid(num_sms, 4, st.W), 256, 0, s>>>(st, k, use_list); ++nl;
@@ -452,39 +453,51 @@ static int launch_y(const State& st, int k, int use_list, int num_sms, cudaStrea
 
 template <typename T>
 static int pf_ratio_impl(const State& st, int k, const int32_t* idx, const void* rows, void* ratio,
-                         int num_sms, cudaStream_t s) {
+                         int num_sms, cudaStream_t s, Prof* prof) {
   int nl = 0;
-  pf_gather_kernel<T><<<(unsigned)st.W, 128, 0, s>>>(st, k, idx, (const T*)rows, (T*)ratio); ++nl;
+  {
+    ProfScope ps(prof, LRUX_PROF_RATIO, s);
+    pf_gather_kernel<T><<<(unsigned)st.W, 128, 0, s>>>(st, k, idx, (const T*)rows, (T*)ratio); ++nl;
+  }
   if (k > 1) {
-    nl += launch_y<T>(st, k, 0, num_sms, s);
+    nl += launch_y<T>(st, k, 0, num_sms, s, prof);
+    ProfScope ps(prof, LRUX_PROF_RATIO, s);
     pf_core_kernel<T><<<(unsigned)st.W, 128, 0, s>>>(st, k, (T*)ratio); ++nl;
   }
   return cudaGetLastError() == cudaSuccess ? nl : -1;
 }
 
 template <typename T>
-static int pf_flush_impl(const State& st, bool all, int num_sms, cudaStream_t s) {
+static int pf_flush_impl(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof) {
   int nl = 0;
   if (all) nl += launch_flush_select_all(st, s);
   const int t1 = (st.n + 63) / 64;
   const int grid = pgrid(num_sms, 4, (int64_t)st.W * (t1 * (t1 + 1) / 2));
-  pf_flush_kernel<T><<<grid, 256, 0, s>>>(st, t1); ++nl;
+  {
+    ProfScope ps(prof, LRUX_PROF_FLUSH, s);
+    pf_flush_kernel<T><<<grid, 256, 0, s>>>(st, t1); ++nl;
+  }
   nl += launch_flush_clear(st, s);
   return cudaGetLastError() == cudaSuccess ? nl : -1;
 }
 
 template <typename T>
-static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_sms, cudaStream_t s) {
+static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_sms, cudaStream_t s,
+                          Prof* prof) {
   int nl = launch_select(st, mask, s);
-  if (k == 1) nl += launch_y<T>(st, k, 1, num_sms, s);  // Y only for accepted walkers
+  if (k == 1) nl += launch_y<T>(st, k, 1, num_sms, s, prof);  // Y only for accepted walkers
   if (st.K == 0) {
     const int t1 = (st.n + 31) / 32;
     const int grid = pgrid(num_sms, 4, (int64_t)st.W * (t1 * (t1 + 1) / 2));
+    ProfScope ps(prof, LRUX_PROF_UPDATE, s);
     pf_update_kernel<T><<<grid, 256, 0, s>>>(st, k, t1); ++nl;
   } else {
-    pf_append_kernel<T><<<pgrid(num_sms, 4, st.W), 256, 0, s>>>(st, k); ++nl;
+    {
+      ProfScope ps(prof, LRUX_PROF_APPEND, s);
+      pf_append_kernel<T><<<pgrid(num_sms, 4, st.W), 256, 0, s>>>(st, k); ++nl;
+    }
     nl += launch_post(st, 2 * k, s);
-    int r = pf_flush_impl<T>(st, false, num_sms, s);
+    int r = pf_flush_impl<T>(st, false, num_sms, s, prof);
     if (r < 0) return -1;
     nl += r;
   }
@@ -492,17 +505,18 @@ static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_s
 }
 
 int launch_pf_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows, void* d_ratio,
-                    int num_sms, cudaStream_t s) {
-  return st.dt == LRUX_F64 ? pf_ratio_impl<double>(st, k, d_idx, d_rows, d_ratio, num_sms, s)
-                           : pf_ratio_impl<cplx>(st, k, d_idx, d_rows, d_ratio, num_sms, s);
+                    int num_sms, cudaStream_t s, Prof* prof) {
+  return st.dt == LRUX_F64 ? pf_ratio_impl<double>(st, k, d_idx, d_rows, d_ratio, num_sms, s, prof)
+                           : pf_ratio_impl<cplx>(st, k, d_idx, d_rows, d_ratio, num_sms, s, prof);
 }
-int launch_pf_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s) {
-  return st.dt == LRUX_F64 ? pf_accept_impl<double>(st, k, d_mask, num_sms, s)
-                           : pf_accept_impl<cplx>(st, k, d_mask, num_sms, s);
+int launch_pf_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s,
+                     Prof* prof) {
+  return st.dt == LRUX_F64 ? pf_accept_impl<double>(st, k, d_mask, num_sms, s, prof)
+                           : pf_accept_impl<cplx>(st, k, d_mask, num_sms, s, prof);
 }
-int launch_pf_flush(const State& st, bool all, int num_sms, cudaStream_t s) {
-  return st.dt == LRUX_F64 ? pf_flush_impl<double>(st, all, num_sms, s)
-                           : pf_flush_impl<cplx>(st, all, num_sms, s);
+int launch_pf_flush(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof) {
+  return st.dt == LRUX_F64 ? pf_flush_impl<double>(st, all, num_sms, s, prof)
+                           : pf_flush_impl<cplx>(st, all, num_sms, s, prof);
 }
 
 }  // namespace lrux

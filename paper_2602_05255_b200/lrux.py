@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "lib", "liblrux.so")
 F64, C128 = 0, 1
 OK, EINVAL, ESTATE, EWORKSPACE, EUNSUPPORTED, ECUDA = range(6)
 MAX_K = 8
+PROF_RATIO, PROF_UPDATE, PROF_APPEND, PROF_FLUSH, PROF_YPASS = range(5)
 
 _vp, _i32, _i64, _u64, _sz = C.c_void_p, C.c_int32, C.c_int64, C.c_uint64, C.c_size_t
 
@@ -37,6 +38,8 @@ SIGNATURES = {
     "lrux_det_get_inverse": [_vp, _vp, _vp],
     "lrux_pf_get_inverse": [_vp, _vp, _vp],
     "lrux_launch_count": [_vp, C.POINTER(_i64)],
+    "lrux_profile_enable": [_vp, _i32],
+    "lrux_profile_read": [_vp, _i32, C.POINTER(C.c_double), C.POINTER(_i64)],
     "lrux_destroy": [_vp],
     "lrux_status_string": [C.c_int],
     "lruxh_det_propose": [_u64, _i64, _i64, _i64, _i32, _i32, _i32, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
@@ -156,6 +159,15 @@ class _Walkers:
         c = _i64(0)
         _check(self._lib.lrux_launch_count(self._h, C.byref(c)))
         return c.value
+
+    def profile_enable(self, on=True):
+        _check(self._lib.lrux_profile_enable(self._h, 1 if on else 0))
+
+    def profile_read(self, cls):
+        """(milliseconds, launches) of kernel class ``cls`` (PROF_*); synchronises."""
+        ms, cnt = C.c_double(0.0), _i64(0)
+        _check(self._lib.lrux_profile_read(self._h, cls, C.byref(ms), C.byref(cnt)))
+        return ms.value, cnt.value
 
     def close(self):
         if self._h:

@@ -42,6 +42,8 @@ class Chain:
         self.mask = torch.zeros(W, dtype=torch.uint8, device=dev)
         self.naccept = torch.zeros(1, dtype=torch.int64, device=dev)
         self.ratio = self.walkers.ratio
+        # |r|^2 = 4 -> the Metropolis test always passes: forced-accept mode
+        self.force_ratio = torch.full((W,), 2.0, dtype=dt, device=dev)
         self.harness_launches = 0
 
     def propose(self, t):
@@ -49,11 +51,13 @@ class Chain:
         fn(self.seed, self.w0, t, self.orb, self.occ, self.unocc, self.idx, self.upos, self.rows)
         self.harness_launches += 1
 
-    def step(self, t):
+    def step(self, t, forced=False):
+        """One Monte-Carlo step of every walker.  ``forced``: every proposal with a
+        regular R is applied (what the paper's Fig. 2 times)."""
         self.propose(t)
         self.walkers.ratio_(self.idx, self.rows)
-        lrux.decide(self.seed, self.w0, t, self.ratio, self.idx, self.upos, self.occ, self.unocc,
-                    self.mask, self.naccept)
+        lrux.decide(self.seed, self.w0, t, self.force_ratio if forced else self.ratio, self.idx,
+                    self.upos, self.occ, self.unocc, self.mask, self.naccept)
         self.harness_launches += 1
         self.walkers.accept(self.mask)
 

@@ -59,13 +59,16 @@ def run_oracle(kind, orb, occ, unocc, k, seed, steps, walkers, scratch_every=1):
 def compare(kind, rec, oracle, inv_tol=1e-9):
     """Element-by-element parity of one GPU record against oracle trajectories.
 
-    Pass rule: with r* the from-scratch
-    ratio and r_smw the oracle's own naive-Woodbury ratio,
-        |r_gpu - r*| <= 1e-10 |r*| + 4 |r_smw - r*|
+    Pass rule (SURVEY.md §8(c) item 14 as read in DESIGN.md §3 reading 14): with
+    r*_t the from-scratch ratio, r_smw,t the oracle's own naive-Woodbury ratio and
+    e_t = max_{s<=t} |r_smw,s - r*_s| / |r*_s| the worst relative error the plain
+    fp64 algorithm has shown on this walker so far (the error sits in the tracked
+    inverse, so it persists after the step that exposed it),
+        |r_gpu,t - r*_t| <= (1e-10 + 4 e_t) |r*_t|
     i.e. 1e-10, or no worse than 4x the plain algorithm's own error where the
-    problem is ill-conditioned.  Decisions must match exactly unless the oracle
-    logged a near-tie (then the walker is dropped from later comparison).
-    Returns statistics for reporting.
+    trajectory is ill-conditioned.  Decisions must match exactly unless the
+    oracle logged a near-tie (then the walker is dropped from later comparison).
+    Returns statistics for reporting (``pure`` counts points within the bare 1e-10).
     """
     stats = dict(points=0, pure=0, max_rel=0.0, dropped=0)
     for w, tr in oracle.items():
@@ -75,10 +78,13 @@ def compare(kind, rec, oracle, inv_tol=1e-9):
         assert rec["init_logabs"][w] == _approx(tr["init_logabs"], 1e-10 * max(1.0, abs(tr["init_logabs"])))
         assert abs(rec["init_phase"][w] - tr["init_phase"]) < 1e-9
         dropped = False
+        e_run = 0.0
         for t in range(steps):
             rg, rl, rs = rec["ratio"][t, w], tr["r_lemma"][t], tr["r_scratch"][t]
             ref = rl if np.isnan(rs) else rs
-            slack = 0.0 if np.isnan(rs) else 4 * abs(rl - rs)
+            if not np.isnan(rs):
+                e_run = max(e_run, abs(rl - rs) / abs(rs))
+            slack = 4 * e_run * abs(ref)
             err = abs(rg - ref)
             stats["points"] += 1
             rel = err / abs(ref)
@@ -96,7 +102,8 @@ def compare(kind, rec, oracle, inv_tol=1e-9):
         assert np.array_equal(rec["occ"][w], tr["occ"])
         assert np.array_equal(rec["unocc"][w], tr["unocc"])
         # amplitude: tracked on the GPU vs recomputed from scratch by the oracle
-        la_tol = RTOL * max(1.0, abs(tr["scratch_logabs"])) + 4 * abs(tr["logabs"] - tr["scratch_logabs"])
+        la_tol = (RTOL * max(1.0, abs(tr["scratch_logabs"])) + 4 * abs(tr["logabs"] - tr["scratch_logabs"])
+                  + 4 * e_run)
         assert abs(rec["logabs"][w] - tr["scratch_logabs"]) <= la_tol
         assert abs(rec["phase"][w] - tr["scratch_phase"]) <= 1e-9
         n = tr["A"].shape[0]
