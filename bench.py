@@ -54,6 +54,8 @@ def parse_args(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=16)
     ap.add_argument("--cpu-seconds", type=float, default=15.0,
                     help="CPU time budget of the cpu_baseline sample")
+    ap.add_argument("--mode", default="metropolis", choices=["metropolis", "forced"],
+                    help="forced: every proposal is applied (ncu captures, Fig. 2-style runs)")
     ap.add_argument("--no-extras", action="store_true",
                     help="skip forced-accept / delayed variants / DGEMM yardstick")
     return ap.parse_args(argv)
@@ -167,11 +169,15 @@ def timed_run(ch, warmup, steps, forced=False, sampler=None):
     if sampler:
         sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if sampler:
+        torch.cuda.profiler.start()   # ncu --profile-from-start off sees the timed region only
     e0.record()
     for t in range(steps):
         ch.step(warmup + t, forced)
     e1.record()
     torch.cuda.synchronize()
+    if sampler:
+        torch.cuda.profiler.stop()
     shard.barrier()
     torch.cuda.synchronize()
     clocks = sampler.stop() if sampler else None
@@ -346,6 +352,21 @@ def dgemm_yardstick(device, n=4096, reps=5):
     return 2.0 * n ** 3 / (best * 1e-3) / 1e12
 
 
+def ncu_traffic_per_walker(kernel, workload):
+    """DRAM bytes per updated walker from the committed ncu --set full capture
+    (profiles/*_traffic.csv, newest round last); None when there is no capture."""
+    import csv
+    import glob
+
+    best = None
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
+        for row in csv.DictReader(open(path)):
+            if row["kernel"] == kernel and row["workload"] == workload:
+                best = ((float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]))
+                        / float(row["walkers_updated_per_launch"]))
+    return best
+
+
 def roofline_update(wk, run, peak, peak_src):
     """HBM roofline of the immediate Woodbury update kernel:
     algorithmic bytes = 2 n^2 e per accepted walker (read once + write once)."""
@@ -355,8 +376,11 @@ def roofline_update(wk, run, peak, peak_src):
         return None
     byts = 2.0 * wk["n"] ** 2 * esz * run["accepted"]
     ach = byts / (pr["ms"] * 1e-3) / 1e9
-    return {"bound": "hbm", "kernel": "%s_update_kernel" % wk["kind"], "achieved": ach, "peak": peak,
-            "unit": "GB/s", "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+    kern = "%s_update_kernel" % wk["kind"]
+    tpw = ncu_traffic_per_walker(kern, wk.get("name", ""))
+    traffic = tpw * run["accepted"] / pr["launches"] if tpw else None
+    return {"bound": "hbm", "kernel": kern, "achieved": ach, "peak": peak,
+            "unit": "GB/s", "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
             "bytes_per_launch": byts / pr["launches"], "us_per_launch": 1e3 * pr["ms"] / pr["launches"],
             "launches": pr["launches"]}
 
@@ -365,7 +389,7 @@ def main(argv=None):
     args = parse_args(argv)
     if args.workload not in WORKLOADS:
         raise SystemExit("unknown workload %r" % args.workload)
-    wk = dict(WORKLOADS[args.workload])
+    wk = dict(WORKLOADS[args.workload], name=args.workload)
     if args.walkers:
         wk["W"] = args.walkers
     if args.impl == "reference":
@@ -394,7 +418,8 @@ def main(argv=None):
     # headline: first K variant, Metropolis as the config is written
     K0 = wk["Ks"][0]
     ch = make_chain(wk, K0, seed, orb, occ, unocc, w0, device)
-    run = timed_run(ch, warmup, steps, sampler=ClockSampler(local_rank) if rank == 0 else None)
+    run = timed_run(ch, warmup, steps, forced=args.mode == "forced",
+                    sampler=ClockSampler(local_rank) if rank == 0 else None)
     info_bad = int((ch.walkers.info != 0).sum().item())
     del ch
     ms_max, = shard.reduce_scalars([run["ms"]], "max", device)
@@ -446,7 +471,7 @@ def main(argv=None):
            "scaling": "weak", "vs_baseline": None, "dtype": "c128" if wk["cplx"] else "f64",
            "data": "synthetic",
            "config": {"workload": wk["desc"], "walkers_per_gpu": W, "n": wk["n"], "M": wk["M"],
-                      "k": wk["k"], "K": K0, "mode": "metropolis",
+                      "k": wk["k"], "K": K0, "mode": args.mode,
                       "l2": "inputs larger than L2: %.2f GiB of inverses per GPU, no flush needed"
                             % (W * wk["n"] ** 2 * (16 if wk["cplx"] else 8) / 2 ** 30)},
            "accept_frac": acc_sum / float(W * world * steps),
