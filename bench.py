@@ -56,6 +56,8 @@ def parse_args(argv=None):
                     help="CPU time budget of the cpu_baseline sample")
     ap.add_argument("--mode", default="metropolis", choices=["metropolis", "forced"],
                     help="forced: every proposal is applied (ncu captures, Fig. 2-style runs)")
+    ap.add_argument("--delay", type=int, default=-1,
+                    help="override the workload's delay depth K (headline variant only)")
     ap.add_argument("--no-extras", action="store_true",
                     help="skip forced-accept / delayed variants / DGEMM yardstick")
     return ap.parse_args(argv)
@@ -392,6 +394,8 @@ def main(argv=None):
     wk = dict(WORKLOADS[args.workload], name=args.workload)
     if args.walkers:
         wk["W"] = args.walkers
+    if args.delay >= 0:
+        wk["Ks"] = (args.delay,)
     if args.impl == "reference":
         return reference_arm(args, wk)
 

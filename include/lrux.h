@@ -39,7 +39,7 @@ typedef enum {
   LRUX_EINVAL = 1,      /* bad size / odd n for Pf / k > kmax / null pointer */
   LRUX_ESTATE = 2,      /* accept without a pending ratio; det call on a pf handle */
   LRUX_EWORKSPACE = 3,  /* state_bytes too small */
-  LRUX_EUNSUPPORTED = 4,
+  LRUX_EUNSUPPORTED = 4, /* delay depth too large: K*kmax^2*sizeof(elem) (x4 for Pf) > 48 KiB */
   LRUX_ECUDA = 5        /* a CUDA launch failed */
 } lrux_status_t;
 

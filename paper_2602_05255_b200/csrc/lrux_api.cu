@@ -54,6 +54,9 @@ static lrux_status_t check_dims(int64_t W, int32_t n, int32_t kmax, int32_t K, i
   if (dt != LRUX_F64 && dt != LRUX_C128) return LRUX_EINVAL;
   if (kind == KIND_PF && (n % 2 != 0)) return LRUX_EINVAL;
   if (kmax > n) return LRUX_EINVAL;
+  // the delayed ratio stages K*kmax*kmax coefficients in shared memory (48 KiB static limit)
+  if ((size_t)K * kmax * kmax * (kind == KIND_PF ? 4 : 1) * (dt == LRUX_C128 ? 16 : 8) > 48 * 1024)
+    return LRUX_EUNSUPPORTED;
   if (W > (int64_t)2000000000) return LRUX_EINVAL;
   return LRUX_OK;
 }

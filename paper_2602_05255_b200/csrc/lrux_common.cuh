@@ -16,7 +16,8 @@ struct cplx {
   double re, im;
 };
 
-__host__ __device__ inline double sc_make(double, double re, double) { return re; }
+__device__ __forceinline__ double sc_from(double re, double, double) { return re; }
+__device__ __forceinline__ cplx sc_from(double re, double im, cplx) { return cplx{re, im}; }
 
 template <typename T>
 struct Sc;

@@ -16,10 +16,12 @@ namespace lrux {
 // One CTA per walker.  Gathers C_eff = A_eff^-1[:,P] (Eq. 14 when the delay buffer
 // holds factors), stashes C_eff and N in the pending area, R = N C_eff, r = det R.
 template <typename T>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(256)
 det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __restrict__ rows,
                  T* __restrict__ ratio_out) {
   using S = Sc<T>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* Bp = (T*)smem_raw;  // [fill][k]: b_t^T v = Bbuf[s][P[a]]  (Eq. 14)
   __shared__ T Rs[kMaxK * kMaxK];
   __shared__ T Ri[kMaxK * kMaxK];
   __shared__ int sidx[kMaxK];
@@ -55,15 +57,27 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
   const T* Bb = st.cap ? (const T*)st.Bbuf + (size_t)w * st.cap * n : nullptr;
   T* pC = (T*)st.pend_C + (size_t)w * kmax * n;
   T* pN = (T*)st.pend_N + (size_t)w * kmax * n;
-  for (int a = 0; a < k; ++a) {
-    const int p = sidx[a];
-    for (int i = tid; i < n; i += nt) {
-      T c = Tw[(size_t)p * n + i];
-      for (int s = 0; s < fill; ++s)   // Eq. 14: a_tau = A0^-1 v - sum_t a_t (b_t^T v)
-        c = S::fnma(Bb[(size_t)s * n + p], Ab[(size_t)s * n + i], c);
-      pC[(size_t)a * n + i] = c;
-      pN[(size_t)a * n + i] = rows[((size_t)w * k + a) * n + i];
+  for (int q = tid; q < fill * k; q += nt) Bp[q] = Bb[(size_t)(q / k) * n + sidx[q % k]];
+  __syncthreads();
+  // one pass over Abuf for all k columns: a_tau = A0^-1 v - sum_t a_t (b_t^T v)   (Eq. 14)
+  for (int i = tid; i < n; i += nt) {
+    T c[kMaxK];
+#pragma unroll
+    for (int a = 0; a < kMaxK; ++a)
+      if (a < k) c[a] = Tw[(size_t)sidx[a] * n + i];
+#pragma unroll 4
+    for (int s = 0; s < fill; ++s) {
+      const T av = Ab[(size_t)s * n + i];
+#pragma unroll
+      for (int a = 0; a < kMaxK; ++a)
+        if (a < k) c[a] = S::fnma(Bp[s * k + a], av, c[a]);
     }
+#pragma unroll
+    for (int a = 0; a < kMaxK; ++a)
+      if (a < k) {
+        pC[(size_t)a * n + i] = c[a];
+        pN[(size_t)a * n + i] = rows[((size_t)w * k + a) * n + i];
+      }
   }
   __syncthreads();
   for (int pr = warp; pr < k * k; pr += nw) {
@@ -314,102 +328,156 @@ det_update_stream_kernel(State st, int k, int tiles, int rows_per_tile) {
 }
 
 // ---------------------------------------------------------------- delayed append (a6)
-// prep: per accepted walker, NA = N Abuf^T (k x fill) into pend_Y and
-// a_tau = C_eff copied into Abuf[fill .. fill+k)   (Eq. 14).
-template <typename T>
-__global__ void __launch_bounds__(256) det_prep_kernel(State st, int k) {
+// prep: work item = (accepted walker, group of 8 buffer rows).  Each warp reads one
+// row a_s of Abuf once and forms NA[b][s] = N_b . a_s for all b (-> pend_Y); group 0
+// also copies a_tau = C_eff into Abuf[fill .. fill+k)   (Eq. 14).
+template <typename T, int KT>
+__global__ void __launch_bounds__(256) det_prep_kernel(State st, int k, int groups) {
   using S = Sc<T>;
   const int n = st.n, kmax = st.kmax, cap = st.cap;
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int count = st.counters[0];
-  for (int it = blockIdx.x; it < count; it += gridDim.x) {
-    const int w = st.list[it];
+  for (int item = blockIdx.x; item < count * groups; item += gridDim.x) {
+    const int w = st.list[item / groups];
+    const int grp = item % groups;
     const int fill = st.fill[w];
     const T* gN = (const T*)st.pend_N + (size_t)w * kmax * n;
-    const T* gC = (const T*)st.pend_C + (size_t)w * kmax * n;
     T* Ab = (T*)st.Abuf + (size_t)w * cap * n;
-    T* NA = (T*)st.pend_Y + (size_t)w * kmax * cap;
-    for (int pr = warp; pr < k * fill; pr += nw) {
-      const int b = pr / fill, s = pr % fill;
-      T acc = S::zero();
-      for (int i = lane; i < n; i += 32) acc = S::fma(gN[(size_t)b * n + i], Ab[(size_t)s * n + i], acc);
-      acc = warp_sum(acc);
-      if (lane == 0) NA[(size_t)b * cap + s] = acc;
+    if (grp == 0) {
+      const T* gC = (const T*)st.pend_C + (size_t)w * kmax * n;
+      for (int q = tid; q < k * n; q += blockDim.x) Ab[(size_t)fill * n + q] = gC[q];
     }
-    for (int q = tid; q < k * n; q += blockDim.x) Ab[(size_t)fill * n + q] = gC[q];
+    const int s = grp * 8 + warp;
+    if (s >= fill) continue;
+    T acc[KT];
+#pragma unroll
+    for (int b = 0; b < KT; ++b) acc[b] = S::zero();
+    for (int i = lane; i < n; i += 32) {
+      const T x = Ab[(size_t)s * n + i];
+#pragma unroll
+      for (int b = 0; b < KT; ++b)
+        if (b < k) acc[b] = S::fma(gN[(size_t)b * n + i], x, acc[b]);
+    }
+    T* NA = (T*)st.pend_Y + (size_t)w * kmax * cap;
+#pragma unroll
+    for (int b = 0; b < KT; ++b) {
+      if (b < k) {
+        const T v = warp_sum(acc[b]);
+        if (lane == 0) NA[(size_t)b * cap + s] = v;
+      }
+    }
   }
 }
 
 // append: b_tau^T = R^-1 (N A0^-1 - (N Abuf) Bbuf^T - I[P,:])   (Eq. 15 in new-rows form,
-// PAPER.md:194; reading 5b) -> Bbuf[fill .. fill+k).  One read-only pass over Ti.
-template <typename T, int KT>
+// PAPER.md:194; reading 5b) -> Bbuf[fill .. fill+k).  One read-only pass over
+// Ti: work item = (accepted walker, tile of RPT rows); N staged in shared memory, each
+// warp streams RW rows at a time with 16-byte loads.
+template <typename T, int KT, int VEC, int RW>
 __global__ void __launch_bounds__(256)
-det_append_kernel(State st, int k, int tiles, int rows_per_tile) {
+det_append_kernel(State st, int k, int tiles, int rows_per_tile, int n_in_smem) {
   using S = Sc<T>;
+  using RV = RowVec<T, VEC>;
+  using V = typename RV::type;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  T* dsm = (T*)smem_raw;  // [KT][rows_per_tile]
+  const int n = st.n, kmax = st.kmax, cap = st.cap;
+  T* dsm = (T*)smem_raw;                         // [4][KT][rows_per_tile] partial sums
+  T* Ns = dsm + 4 * KT * rows_per_tile;          // [k][n] (when it fits)
   __shared__ T Ri[KT * KT];
   __shared__ int sidx[KT];
-  const int n = st.n, kmax = st.kmax, cap = st.cap;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
   const int count = st.counters[0];
+  const int nvec = n / VEC;
   for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
     const int w = st.list[item / tiles];
     const int tile = item % tiles;
     const int fill = st.fill[w];
     __syncthreads();
-    if (tid < KT * KT) {
-      const int a = tid / KT, b = tid % KT;
-      Ri[tid] = (a < k && b < k) ? ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + a * st.kc + b]
-                                 : S::zero();
-    }
-    if (tid < KT) sidx[tid] = tid < k ? st.pend_idx[(size_t)w * kmax + tid] : -1;
-    const T* gN = (const T*)st.pend_N + (size_t)w * kmax * n;
-    const T* Tw = (const T*)st.Ti + (size_t)w * n * n;
-    const int j_beg = tile * rows_per_tile, j_end = min(n, j_beg + rows_per_tile);
-    for (int j = j_beg + warp; j < j_end; j += nw) {
-      const T* row = Tw + (size_t)j * n;
-      T d[KT];
-#pragma unroll
-      for (int a = 0; a < KT; ++a) d[a] = S::zero();
-      for (int i = lane; i < n; i += 32) {
-        const T x = row[i];
-#pragma unroll
-        for (int a = 0; a < KT; ++a)
-          if (a < k) d[a] = S::fma(x, gN[(size_t)a * n + i], d[a]);
+    {
+      const V* gN = (const V*)((const T*)st.pend_N + (size_t)w * kmax * n);
+      if (n_in_smem)
+        for (int q = tid; q < k * nvec; q += blockDim.x) ((V*)Ns)[q] = gN[q];
+      if (tid < KT * KT) {
+        const int a = tid / KT, b = tid % KT;
+        Ri[tid] = (a < k && b < k) ? ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + a * st.kc + b]
+                                   : S::zero();
       }
-#pragma unroll
-      for (int a = 0; a < KT; ++a) {
-        d[a] = warp_sum(d[a]);
-        if (lane == 0) dsm[a * rows_per_tile + (j - j_beg)] = d[a];
-      }
+      if (tid < KT) sidx[tid] = tid < k ? st.pend_idx[(size_t)w * kmax + tid] : -1;
     }
     __syncthreads();
+    const T* Np = n_in_smem ? Ns : (const T*)st.pend_N + (size_t)w * kmax * n;
+    const T* Tw = (const T*)st.Ti + (size_t)w * n * n;
+    const int j_beg = tile * rows_per_tile, j_end = min(n, j_beg + rows_per_tile);
+    for (int j0 = j_beg + warp * RW; j0 < j_end; j0 += nw * RW) {
+      T d[RW][KT];
+#pragma unroll
+      for (int r = 0; r < RW; ++r)
+#pragma unroll
+        for (int a = 0; a < KT; ++a) d[r][a] = S::zero();
+      for (int q = lane; q < nvec; q += 32) {
+        V x[RW];
+#pragma unroll
+        for (int r = 0; r < RW; ++r) {
+          if (j0 + r < j_end) x[r] = ((const V*)(Tw + (size_t)(j0 + r) * n))[q];
+          else { RV::set(x[r], 0, S::zero()); if (VEC == 2) RV::set(x[r], 1, S::zero()); }
+        }
+#pragma unroll
+        for (int a = 0; a < KT; ++a) {
+          if (a < k) {
+            const V nv = ((const V*)(Np + (size_t)a * n))[q];
+#pragma unroll
+            for (int e = 0; e < VEC; ++e)
+#pragma unroll
+              for (int r = 0; r < RW; ++r) d[r][a] = S::fma(RV::get(x[r], e), RV::get(nv, e), d[r][a]);
+          }
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < RW; ++r)
+#pragma unroll
+        for (int a = 0; a < KT; ++a) {
+          T v = warp_sum(d[r][a]);
+          if (j0 + r == sidx[a]) v = S::sub(v, S::one());
+          if (lane == 0 && j0 + r < j_end) dsm[a * rows_per_tile + (j0 + r - j_beg)] = v;
+        }
+    }
+    __syncthreads();
+    // m[b][j] = d[b][j] - sum_s NA[b][s] Bbuf[s][j]: 4 groups of threads split the s range
     const T* NA = (const T*)st.pend_Y + (size_t)w * kmax * cap;
     T* Bb = (T*)st.Bbuf + (size_t)w * cap * n;
-    for (int jj = tid; jj < j_end - j_beg; jj += blockDim.x) {
-      const int j = j_beg + jj;
-      T m[KT];
+    const int nj = j_end - j_beg;
+    const int jj = tid % rows_per_tile, sg = tid / rows_per_tile, nsg = blockDim.x / rows_per_tile;
+    T m[KT];
 #pragma unroll
-      for (int b = 0; b < KT; ++b) {
-        m[b] = b < k ? dsm[b * rows_per_tile + jj] : S::zero();
-        if (j == sidx[b]) m[b] = S::sub(m[b], S::one());
-      }
-      for (int s = 0; s < fill; ++s) {
-        const T bv = Bb[(size_t)s * n + j];
+    for (int b = 0; b < KT; ++b) m[b] = S::zero();
+    if (jj < nj && sg < nsg) {
+      for (int s = sg; s < fill; s += nsg) {
+        const T bv = Bb[(size_t)s * n + j_beg + jj];
 #pragma unroll
         for (int b = 0; b < KT; ++b)
           if (b < k) m[b] = S::fnma(NA[(size_t)b * cap + s], bv, m[b]);
       }
+    }
+    if (sg >= 1 && sg < nsg && jj < nj) {
 #pragma unroll
-      for (int a = 0; a < KT; ++a) {
-        if (a < k) {
-          T acc = S::zero();
+      for (int b = 0; b < KT; ++b) dsm[(sg * KT + b) * rows_per_tile + jj] = m[b];
+    }
+    __syncthreads();
+    if (sg == 0 && jj < nj) {
 #pragma unroll
-          for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], m[b], acc);
-          Bb[(size_t)(fill + a) * n + j] = acc;
-        }
+      for (int b = 0; b < KT; ++b) {
+        T v = S::add(dsm[b * rows_per_tile + jj], m[b]);
+        for (int g = 1; g < nsg; ++g) v = S::add(v, dsm[(g * KT + b) * rows_per_tile + jj]);
+        dsm[b * rows_per_tile + jj] = v;
       }
+    }
+    __syncthreads();
+    for (int q = tid; q < k * nj; q += blockDim.x) {
+      const int a = q / nj, j2 = q % nj;
+      T acc = S::zero();
+#pragma unroll
+      for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], dsm[b * rows_per_tile + j2], acc);
+      Bb[(size_t)(fill + a) * n + j_beg + j2] = acc;
     }
   }
 }
@@ -440,64 +508,6 @@ __global__ void flush_clear_kernel(State st) {
   const int w = st.flist[it];
   st.fill[w] = 0;
   st.nupd[w] = 0;
-}
-
-// ---------------------------------------------------------------- flush (a7), FMA version
-// Ti[j][i] -= sum_s Bbuf[s][j] Abuf[s][i]   (Eq. 12), 64x64 tiles.
-template <typename T>
-__global__ void __launch_bounds__(256) det_flush_kernel(State st, int tiles_1d) {
-  using S = Sc<T>;
-  constexpr int BT = 64, BK = 16;
-  __shared__ T Bs[BK][BT];
-  __shared__ T As[BK][BT];
-  const int n = st.n, cap = st.cap;
-  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-  const int count = st.counters[1];
-  const int tiles = tiles_1d * tiles_1d;
-  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
-    const int w = st.flist[item / tiles];
-    const int tile = item % tiles;
-    const int j0 = (tile / tiles_1d) * BT, i0 = (tile % tiles_1d) * BT;
-    const int fill = st.fill[w];
-    const T* Ab = (const T*)st.Abuf + (size_t)w * cap * n;
-    const T* Bb = (const T*)st.Bbuf + (size_t)w * cap * n;
-    T* Tw = (T*)st.Ti + (size_t)w * n * n;
-    T acc[4][4];
-#pragma unroll
-    for (int a = 0; a < 4; ++a)
-#pragma unroll
-      for (int b = 0; b < 4; ++b) acc[a][b] = S::zero();
-    for (int s0 = 0; s0 < fill; s0 += BK) {
-      __syncthreads();
-      for (int q = tid; q < BK * BT; q += 256) {
-        const int kk = q / BT, c = q % BT;
-        const bool sv = s0 + kk < fill;
-        Bs[kk][c] = (sv && j0 + c < n) ? Bb[(size_t)(s0 + kk) * n + j0 + c] : S::zero();
-        As[kk][c] = (sv && i0 + c < n) ? Ab[(size_t)(s0 + kk) * n + i0 + c] : S::zero();
-      }
-      __syncthreads();
-#pragma unroll
-      for (int kk = 0; kk < BK; ++kk) {
-        T bv[4], av[4];
-#pragma unroll
-        for (int a = 0; a < 4; ++a) { bv[a] = Bs[kk][ty + 16 * a]; av[a] = As[kk][tx + 16 * a]; }
-#pragma unroll
-        for (int a = 0; a < 4; ++a)
-#pragma unroll
-          for (int b = 0; b < 4; ++b) acc[a][b] = S::fma(bv[a], av[b], acc[a][b]);
-      }
-    }
-#pragma unroll
-    for (int a = 0; a < 4; ++a) {
-      const int j = j0 + ty + 16 * a;
-      if (j >= n) continue;
-#pragma unroll
-      for (int b = 0; b < 4; ++b) {
-        const int i = i0 + tx + 16 * b;
-        if (i < n) Tw[(size_t)j * n + i] = S::sub(Tw[(size_t)j * n + i], acc[a][b]);
-      }
-    }
-  }
 }
 
 // ---------------------------------------------------------------- shared helpers
@@ -574,13 +584,28 @@ static int launch_update_kt(const State& st, int k, int num_sms, cudaStream_t s)
 template <typename T, int KT>
 static int launch_append_kt(const State& st, int k, int num_sms, cudaStream_t s) {
   const int n = st.n;
-  int rows_per_tile = 64;
-  if (rows_per_tile > n) rows_per_tile = n;
+  constexpr int VECMAX = sizeof(T) == 8 ? 2 : 1;
+  int nl = 0;
+  {
+    const int groups = (st.cap + 7) / 8;
+    const int grid = persistent_grid(num_sms, 8, (int64_t)st.W * groups);
+    det_prep_kernel<T, KT><<<grid, 256, 0, s>>>(st, k, groups); ++nl;
+  }
+  int rows_per_tile = 64;   // must divide the block size (256)
   const int tiles = (n + rows_per_tile - 1) / rows_per_tile;
-  const size_t smem = (size_t)KT * rows_per_tile * sizeof(T);
-  const int grid = persistent_grid(num_sms, 4, (int64_t)st.W * tiles);
-  det_append_kernel<T, KT><<<grid, 256, smem, s>>>(st, k, tiles, rows_per_tile);
-  return 1;
+  const int n_in_smem = (size_t)k * n * sizeof(T) <= 96 * 1024;
+  const size_t smem = ((n_in_smem ? (size_t)k * n : 0) + 4 * (size_t)KT * rows_per_tile) * sizeof(T);
+  const bool vec = (n % VECMAX) == 0 && VECMAX == 2;
+  auto kern = vec ? det_append_kernel<T, KT, VECMAX, 2> : det_append_kernel<T, KT, 1, 2>;
+  if (smem > 48 * 1024 &&
+      cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return -1;
+  int occ = 1;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, smem);
+  if (occ < 1) return -1;
+  const int grid = persistent_grid(num_sms, occ, (int64_t)st.W * tiles);
+  kern<<<grid, 256, smem, s>>>(st, k, tiles, rows_per_tile, n_in_smem); ++nl;
+  return nl;
 }
 
 template <typename T>
@@ -591,11 +616,9 @@ static int flush_impl(const State& st, bool all, int num_sms, cudaStream_t s, Pr
     reset_counter_kernel<<<1, 1, 0, s>>>(st, 1); ++nl;
     flush_all_select_kernel<<<gw, 256, 0, s>>>(st); ++nl;
   }
-  const int t1 = (st.n + 63) / 64;
-  const int grid = persistent_grid(num_sms, 4, (int64_t)st.W * t1 * t1);
   {
     ProfScope ps(prof, LRUX_PROF_FLUSH, s);
-    det_flush_kernel<T><<<grid, 256, 0, s>>>(st, t1); ++nl;
+    nl += launch_flush_dmma(st, num_sms, s);   // Eq. 12 on the FP64 tensor path
   }
   flush_clear_kernel<<<gw, 256, 0, s>>>(st); ++nl;
   return cudaGetLastError() == cudaSuccess ? nl : -1;
@@ -620,10 +643,8 @@ static int accept_impl(const State& st, int k, const uint8_t* mask, int num_sms,
     if (r < 0) return -1;
     nl += r;
   } else {
-    const int grid = persistent_grid(num_sms, 4, st.W);
     {
       ProfScope ps(prof, LRUX_PROF_APPEND, s);
-      det_prep_kernel<T><<<grid, 256, 0, s>>>(st, k); ++nl;
       switch (kt) {
         case 1: r = launch_append_kt<T, 1>(st, k, num_sms, s); break;
         case 2: r = launch_append_kt<T, 2>(st, k, num_sms, s); break;
@@ -644,12 +665,15 @@ static int accept_impl(const State& st, int k, const uint8_t* mask, int num_sms,
 int launch_det_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
                      void* d_ratio, cudaStream_t s, Prof* prof) {
   ProfScope ps(prof, LRUX_PROF_RATIO, s);
+  const int nt = st.n <= 128 ? 128 : 256;
+  const size_t e = st.dt == LRUX_F64 ? 8 : 16;
+  const size_t smem = (size_t)st.cap * k * e;  // <= 32*8*8*16 = 32 KiB
   if (st.dt == LRUX_F64)
-    det_ratio_kernel<double><<<(unsigned)st.W, 128, 0, s>>>(st, k, d_idx, (const double*)d_rows,
-                                                            (double*)d_ratio);
+    det_ratio_kernel<double><<<(unsigned)st.W, nt, smem, s>>>(st, k, d_idx, (const double*)d_rows,
+                                                              (double*)d_ratio);
   else
-    det_ratio_kernel<cplx><<<(unsigned)st.W, 128, 0, s>>>(st, k, d_idx, (const cplx*)d_rows,
-                                                          (cplx*)d_ratio);
+    det_ratio_kernel<cplx><<<(unsigned)st.W, nt, smem, s>>>(st, k, d_idx, (const cplx*)d_rows,
+                                                            (cplx*)d_ratio);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

@@ -95,6 +95,8 @@ int launch_pf_ratio(const State& st, int k, const int32_t* d_idx, const void* d_
 int launch_pf_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s,
                      Prof* prof);
 int launch_pf_flush(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof);
+// DMMA flush of the delay buffers, det and pf (lrux_flush.cu)
+int launch_flush_dmma(const State& st, int num_sms, cudaStream_t s);
 // shared between det and pf (defined in lrux_det.cu)
 int launch_select(const State& st, const uint8_t* mask, cudaStream_t s);
 int launch_post(const State& st, int ncols, cudaStream_t s);

@@ -358,69 +358,6 @@ __global__ void __launch_bounds__(256) pf_append_kernel(State st, int k) {
   }
 }
 
-// ---------------------------------------------------------------- flush (a7), FMA version
-// Ti[i][j] += sum_s Bbuf[s][i] Abuf[s][j] for j > i, mirrored exactly (Eq. 26).
-template <typename T>
-__global__ void __launch_bounds__(256) pf_flush_kernel(State st, int t1) {
-  using S = Sc<T>;
-  constexpr int BT = 64, BK = 16;
-  __shared__ T Bs[BK][BT];
-  __shared__ T As[BK][BT];
-  const int n = st.n, cap = st.cap;
-  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-  const int count = st.counters[1];
-  const int tiles = t1 * (t1 + 1) / 2;
-  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
-    const int w = st.flist[item / tiles];
-    int rem = item % tiles, I = 0;
-    while (rem >= t1 - I) { rem -= t1 - I; ++I; }
-    const int J = I + rem;
-    const int i0 = I * BT, j0 = J * BT;
-    const int fill = st.fill[w];
-    const T* Ab = (const T*)st.Abuf + (size_t)w * cap * n;
-    const T* Bb = (const T*)st.Bbuf + (size_t)w * cap * n;
-    T* Tw = (T*)st.Ti + (size_t)w * n * n;
-    T acc[4][4];
-#pragma unroll
-    for (int a = 0; a < 4; ++a)
-#pragma unroll
-      for (int b = 0; b < 4; ++b) acc[a][b] = S::zero();
-    for (int s0 = 0; s0 < fill; s0 += BK) {
-      __syncthreads();
-      for (int q = tid; q < BK * BT; q += 256) {
-        const int kk = q / BT, c = q % BT;
-        const bool sv = s0 + kk < fill;
-        Bs[kk][c] = (sv && i0 + c < n) ? Bb[(size_t)(s0 + kk) * n + i0 + c] : S::zero();
-        As[kk][c] = (sv && j0 + c < n) ? Ab[(size_t)(s0 + kk) * n + j0 + c] : S::zero();
-      }
-      __syncthreads();
-#pragma unroll
-      for (int kk = 0; kk < BK; ++kk) {
-        T bv[4], av[4];
-#pragma unroll
-        for (int a = 0; a < 4; ++a) { bv[a] = Bs[kk][ty + 16 * a]; av[a] = As[kk][tx + 16 * a]; }
-#pragma unroll
-        for (int a = 0; a < 4; ++a)
-#pragma unroll
-          for (int b = 0; b < 4; ++b) acc[a][b] = S::fma(bv[a], av[b], acc[a][b]);
-      }
-    }
-#pragma unroll
-    for (int a = 0; a < 4; ++a) {
-      const int i = i0 + ty + 16 * a;
-#pragma unroll
-      for (int b = 0; b < 4; ++b) {
-        const int j = j0 + tx + 16 * b;
-        if (i < n && j < n && j > i) {
-          const T v = S::add(Tw[(size_t)i * n + j], acc[a][b]);
-          Tw[(size_t)i * n + j] = v;
-          Tw[(size_t)j * n + i] = S::neg(v);
-        }
-      }
-    }
-  }
-}
-
 // ---------------------------------------------------------------- launchers
 static inline int round_kt(int k) { return k <= 1 ? 1 : k <= 2 ? 2 : k <= 4 ? 4 : 8; }
 static inline int pgrid(int num_sms, int per_sm, int64_t max_items) {
@@ -471,11 +408,9 @@ template <typename T>
 static int pf_flush_impl(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof) {
   int nl = 0;
   if (all) nl += launch_flush_select_all(st, s);
-  const int t1 = (st.n + 63) / 64;
-  const int grid = pgrid(num_sms, 4, (int64_t)st.W * (t1 * (t1 + 1) / 2));
   {
     ProfScope ps(prof, LRUX_PROF_FLUSH, s);
-    pf_flush_kernel<T><<<grid, 256, 0, s>>>(st, t1); ++nl;
+    nl += launch_flush_dmma(st, num_sms, s);   // Eq. 26 on the FP64 tensor path
   }
   nl += launch_flush_clear(st, s);
   return cudaGetLastError() == cudaSuccess ? nl : -1;
