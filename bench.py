@@ -387,6 +387,35 @@ def roofline_update(wk, run, peak, peak_src):
             "launches": pr["launches"]}
 
 
+def roofline_flush(wk, K, run, hbm_peak, hbm_src, dgemm_tflops):
+    """Roofline of the flush kernel (a7).  Per accepted update (one of the K slots of a
+    flushed buffer): 2 n^2 k flops (x4 complex) and (2 n^2 e)/K + 2 n k e bytes.  Arithmetic
+    intensity Kk/8 flop/B (real), Kk/4 (complex): FP64-tensor-bound when Kk >= 50 (real) /
+    25 (complex), HBM-bound below.  The tensor peak is the cuBLAS FP64
+    GEMM measured in this same run (MEASURED_PEAKS.json carries no FP64 figure)."""
+    fl = run["prof"]["flush"]
+    if K <= 0 or fl["ms"] <= 0 or run["accepted"] == 0:
+        return None
+    cx = wk["cplx"]
+    esz = 16 if cx else 8
+    n, k = wk["n"], wk["k"]
+    flops = 2.0 * n * n * k * (4 if cx else 1) * run["accepted"]
+    byts = (2.0 * n * n * esz / K + 2.0 * n * k * esz) * run["accepted"]
+    tf = flops / (fl["ms"] * 1e-3) / 1e12
+    gbs = byts / (fl["ms"] * 1e-3) / 1e9
+    tensor = K * k >= (25 if cx else 50)
+    out = {"kernel": "flush_dmma_kernel", "Kk": K * k, "tflops": tf, "gbs": gbs,
+           "launches": fl["launches"], "ms": fl["ms"]}
+    if tensor and dgemm_tflops:
+        out.update(bound="tensor", achieved=tf, peak=dgemm_tflops, unit="TFLOP/s",
+                   frac=tf / dgemm_tflops, traffic=None,
+                   peak_source="cuBLAS FP64 GEMM 4096^3 measured in this run (burst)")
+    else:
+        out.update(bound="hbm", achieved=gbs, peak=hbm_peak, unit="GB/s", frac=gbs / hbm_peak,
+                   traffic=None, peak_source=hbm_src)
+    return out
+
+
 def main(argv=None):
     args = parse_args(argv)
     if args.workload not in WORKLOADS:
@@ -431,6 +460,9 @@ def main(argv=None):
     value = W * world * steps / (ms_max * 1e-3)
 
     extras = {}
+    dgemm = dgemm_yardstick(device) if (rank == 0 and (K0 > 0 or not args.no_extras)) else None
+    if dgemm:
+        extras["dgemm_f64_tflops_cublas"] = dgemm
     if not args.no_extras:
         # forced-accept (every proposal applied: what the paper's Fig. 2 times) -> cleanest roofline
         chf = make_chain(wk, K0, seed, orb, occ, unocc, w0, device)
@@ -446,19 +478,11 @@ def main(argv=None):
             chk = make_chain(wk, K, seed, orb, occ, unocc, w0, device)
             rk = timed_run(chk, warmup, steps)
             del chk
-            esz = 16 if wk["cplx"] else 8
-            fl = rk["prof"]["flush"]
             extras["K%d" % K] = {
                 "walker_updates_per_s": W * steps / (rk["ms"] * 1e-3), "ms_per_step": rk["ms"] / steps,
                 "accept_frac": rk["accepted"] / float(W * steps),
                 "prof_ms": {k: v["ms"] for k, v in rk["prof"].items()},
-                # flush: 2 n^2 Kk flops and 2 n^2 e + 2 n Kk e bytes per flushed walker (full buffers)
-                "flush_tflops": (2.0 * wk["n"] ** 2 * wk["k"] * rk["accepted"] / (fl["ms"] * 1e-3) / 1e12
-                                 if fl["ms"] > 0 else None),
-                "flush_gbs": ((2.0 * wk["n"] ** 2 * esz / K + 2.0 * wk["n"] * wk["k"] * esz) * rk["accepted"]
-                              / (fl["ms"] * 1e-3) / 1e9 if fl["ms"] > 0 else None)}
-        if rank == 0:
-            extras["dgemm_f64_tflops_cublas"] = dgemm_yardstick(device)
+                "roofline_flush": roofline_flush(wk, K, rk, peak, peak_src, dgemm)}
 
     # end to end through the C-ABI from host buffers
     e2e_steps = max(1, min(args.e2e_steps, steps))
@@ -469,6 +493,16 @@ def main(argv=None):
     roof = roofline_update(wk, run, peak, peak_src) if K0 == 0 else None
     if roof is None and "forced_accept" in extras and extras["forced_accept"]["roofline"]:
         roof = extras["forced_accept"]["roofline"]
+    roof_append = None
+    if K0 > 0 and run["prof"]["append"]["ms"] > 0:
+        # delayed append (a6): one read-only pass over A0^-1 = n^2 e bytes per accepted walker
+        ap = run["prof"]["append"]
+        gbs = wk["n"] ** 2 * (16.0 if wk["cplx"] else 8.0) * run["accepted"] / (ap["ms"] * 1e-3) / 1e9
+        roof_append = {"bound": "hbm", "kernel": "det_prep_kernel+det_append_kernel", "achieved": gbs,
+                       "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
+                       "peak_source": peak_src}
+        if roof is None:   # the dominant kernel of a delayed configuration
+            roof = roof_append
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
            "warmup": warmup, "ms_per_step": ms_max / steps, "higher_is_better": True,
@@ -486,7 +520,8 @@ def main(argv=None):
            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": ee["h2d"],
                    "d2h_bytes_per_step": ee["d2h"], "steps": e2e_steps,
                    "decision_mismatches_vs_device_chain": ee["mismatch"]},
-           "roofline": roof, "extras": extras}
+           "roofline": roof, "roofline_append": roof_append, "roofline_flush": roofline_flush(wk, K0, run, peak, peak_src, dgemm),
+           "extras": extras}
     if rank == 0:
         if world == 1:
             sec, done, nw = oracle_sample(wk, 2, 20, args.cpu_seconds)

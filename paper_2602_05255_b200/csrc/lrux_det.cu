@@ -13,36 +13,36 @@
 namespace lrux {
 
 // ---------------------------------------------------------------- ratio (a1, a2, a5)
-// One CTA per walker.  Gathers C_eff = A_eff^-1[:,P] (Eq. 14 when the delay buffer
-// holds factors), stashes C_eff and N in the pending area, R = N C_eff, r = det R.
-template <typename T>
+// One CTA per walker.  Each thread owns EPT elements i of the k gathered columns
+// C_eff = A_eff^-1[:,P] and walks the delay buffer ONCE for all of them:
+//   a_tau = A0^-1 v - sum_t a_t (b_t^T v)                       (Eq. 14)
+// (b_t^T v = Bbuf[s][P[a]] is a warp-uniform load).  C_eff and N are stashed for
+// accept; R = N C_eff (Eq. 4 / Eq. 13) is accumulated on the fly when KT <= 4,
+// else from the stash; r = det R by a k x k LU in one thread.
+template <typename T, int KT, int EPT>
 __global__ void __launch_bounds__(256)
 det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __restrict__ rows,
                  T* __restrict__ ratio_out) {
   using S = Sc<T>;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  T* Bp = (T*)smem_raw;  // [fill][k]: b_t^T v = Bbuf[s][P[a]]  (Eq. 14)
+  constexpr bool FLY = KT <= 4;
   __shared__ T Rs[kMaxK * kMaxK];
   __shared__ T Ri[kMaxK * kMaxK];
-  __shared__ int sidx[kMaxK];
-  __shared__ int bad;
+  __shared__ T red[8][FLY ? KT * KT : 1];
   const int w = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
   const int warp = tid >> 5, lane = tid & 31, nw = nt >> 5;
   const int n = st.n, kmax = st.kmax;
   if (w == 0 && tid == 0) st.counters[0] = 0;
-  if (tid == 0) {
-    int b = 0;
-    for (int a = 0; a < k; ++a) {
-      int p = idx[(size_t)w * k + a];
-      sidx[a] = p;
-      if (p < 0 || p >= n) b = 1;
-      for (int c = 0; c < a; ++c)
-        if (sidx[c] == p) b = 1;
-    }
-    bad = b;
+  int P[KT];
+  bool bad = false;
+#pragma unroll
+  for (int a = 0; a < KT; ++a) {
+    P[a] = a < k ? idx[(size_t)w * k + a] : -1 - a;
+    if (a < k && (P[a] < 0 || P[a] >= n)) bad = true;
+#pragma unroll
+    for (int c = 0; c < a; ++c)
+      if (a < k && P[c] == P[a]) bad = true;
   }
-  __syncthreads();
-  if (bad) {
+  if (bad) {   // uniform over the CTA
     if (tid == 0) {
       ratio_out[w] = S::nan();
       ((T*)st.pend_ratio)[w] = S::nan();
@@ -57,35 +57,78 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
   const T* Bb = st.cap ? (const T*)st.Bbuf + (size_t)w * st.cap * n : nullptr;
   T* pC = (T*)st.pend_C + (size_t)w * kmax * n;
   T* pN = (T*)st.pend_N + (size_t)w * kmax * n;
-  for (int q = tid; q < fill * k; q += nt) Bp[q] = Bb[(size_t)(q / k) * n + sidx[q % k]];
-  __syncthreads();
-  // one pass over Abuf for all k columns: a_tau = A0^-1 v - sum_t a_t (b_t^T v)   (Eq. 14)
-  for (int i = tid; i < n; i += nt) {
-    T c[kMaxK];
+  T racc[KT][KT];   // unused (and removed by the compiler) when !FLY
 #pragma unroll
-    for (int a = 0; a < kMaxK; ++a)
-      if (a < k) c[a] = Tw[(size_t)sidx[a] * n + i];
+  for (int b = 0; b < KT; ++b)
+#pragma unroll
+    for (int a = 0; a < KT; ++a) racc[b][a] = S::zero();
+  for (int i0 = 0; i0 < n; i0 += nt * EPT) {
+    T c[KT][EPT];
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+      const int i = i0 + tid + nt * e;
+#pragma unroll
+      for (int a = 0; a < KT; ++a)
+        c[a][e] = (a < k && i < n) ? Tw[(size_t)P[a] * n + i] : S::zero();
+    }
 #pragma unroll 4
     for (int s = 0; s < fill; ++s) {
-      const T av = Ab[(size_t)s * n + i];
+      T av[EPT], bp[KT];
 #pragma unroll
-      for (int a = 0; a < kMaxK; ++a)
-        if (a < k) c[a] = S::fnma(Bp[s * k + a], av, c[a]);
+      for (int e = 0; e < EPT; ++e) {
+        const int i = i0 + tid + nt * e;
+        av[e] = i < n ? Ab[(size_t)s * n + i] : S::zero();
+      }
+#pragma unroll
+      for (int a = 0; a < KT; ++a) bp[a] = a < k ? Bb[(size_t)s * n + P[a]] : S::zero();
+#pragma unroll
+      for (int a = 0; a < KT; ++a)
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) c[a][e] = S::fnma(bp[a], av[e], c[a][e]);
     }
 #pragma unroll
-    for (int a = 0; a < kMaxK; ++a)
-      if (a < k) {
-        pC[(size_t)a * n + i] = c[a];
-        pN[(size_t)a * n + i] = rows[((size_t)w * k + a) * n + i];
+    for (int e = 0; e < EPT; ++e) {
+      const int i = i0 + tid + nt * e;
+      if (i < n) {
+#pragma unroll
+        for (int b = 0; b < KT; ++b) {
+          if (b < k) {
+            const T x = rows[((size_t)w * k + b) * n + i];
+            pN[(size_t)b * n + i] = x;
+            pC[(size_t)b * n + i] = c[b][e];
+            if constexpr (FLY) {
+#pragma unroll
+              for (int a = 0; a < KT; ++a)
+                racc[b][a] = S::fma(x, c[a][e], racc[b][a]);
+            }
+          }
+        }
       }
+    }
   }
-  __syncthreads();
-  for (int pr = warp; pr < k * k; pr += nw) {
-    const int a = pr / k, b = pr % k;
-    T acc = S::zero();
-    for (int i = lane; i < n; i += 32) acc = S::fma(pN[(size_t)a * n + i], pC[(size_t)b * n + i], acc);
-    acc = warp_sum(acc);
-    if (lane == 0) Rs[a * kMaxK + b] = acc;
+  if constexpr (FLY) {
+#pragma unroll
+    for (int b = 0; b < KT; ++b)
+#pragma unroll
+      for (int a = 0; a < KT; ++a) {
+        const T v = warp_sum(racc[b][a]);
+        if (lane == 0) red[warp][b * KT + a] = v;
+      }
+    __syncthreads();
+    if (tid < KT * KT) {
+      T v = red[0][tid];
+      for (int q = 1; q < nw; ++q) v = S::add(v, red[q][tid]);
+      Rs[(tid / KT) * kMaxK + (tid % KT)] = v;
+    }
+  } else {
+    __syncthreads();   // stash visible to the whole CTA
+    for (int pr = warp; pr < k * k; pr += nw) {
+      const int a = pr / k, b = pr % k;
+      T acc = S::zero();
+      for (int i = lane; i < n; i += 32) acc = S::fma(pN[(size_t)a * n + i], pC[(size_t)b * n + i], acc);
+      acc = warp_sum(acc);
+      if (lane == 0) Rs[a * kMaxK + b] = acc;
+    }
   }
   __syncthreads();
   if (tid == 0) {
@@ -96,7 +139,7 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
     st.pend_ok[w] = ok ? 1 : 0;
     T* pR = (T*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
     for (int a = 0; a < k; ++a) {
-      st.pend_idx[(size_t)w * kmax + a] = sidx[a];
+      st.pend_idx[(size_t)w * kmax + a] = P[a];
       for (int b = 0; b < k; ++b) pR[a * st.kc + b] = Ri[a * kMaxK + b];
     }
   }
@@ -414,21 +457,33 @@ det_append_kernel(State st, int k, int tiles, int rows_per_tile, int n_in_smem) 
       for (int r = 0; r < RW; ++r)
 #pragma unroll
         for (int a = 0; a < KT; ++a) d[r][a] = S::zero();
-      for (int q = lane; q < nvec; q += 32) {
-        V x[RW];
+      constexpr int U = 4;   // 16-byte loads in flight per thread = U * RW
+      for (int q0 = lane; q0 < nvec; q0 += 32 * U) {
+        V x[U][RW];
 #pragma unroll
-        for (int r = 0; r < RW; ++r) {
-          if (j0 + r < j_end) x[r] = ((const V*)(Tw + (size_t)(j0 + r) * n))[q];
-          else { RV::set(x[r], 0, S::zero()); if (VEC == 2) RV::set(x[r], 1, S::zero()); }
+        for (int u = 0; u < U; ++u) {
+          const int q = q0 + 32 * u;
+#pragma unroll
+          for (int r = 0; r < RW; ++r) {
+            if (q < nvec && j0 + r < j_end) x[u][r] = ((const V*)(Tw + (size_t)(j0 + r) * n))[q];
+            else { RV::set(x[u][r], 0, S::zero()); if (VEC == 2) RV::set(x[u][r], 1, S::zero()); }
+          }
         }
 #pragma unroll
-        for (int a = 0; a < KT; ++a) {
-          if (a < k) {
-            const V nv = ((const V*)(Np + (size_t)a * n))[q];
+        for (int u = 0; u < U; ++u) {
+          const int q = q0 + 32 * u;
+          if (q < nvec) {
 #pragma unroll
-            for (int e = 0; e < VEC; ++e)
+            for (int a = 0; a < KT; ++a) {
+              if (a < k) {
+                const V nv = ((const V*)(Np + (size_t)a * n))[q];
 #pragma unroll
-              for (int r = 0; r < RW; ++r) d[r][a] = S::fma(RV::get(x[r], e), RV::get(nv, e), d[r][a]);
+                for (int e = 0; e < VEC; ++e)
+#pragma unroll
+                  for (int r = 0; r < RW; ++r)
+                    d[r][a] = S::fma(RV::get(x[u][r], e), RV::get(nv, e), d[r][a]);
+              }
+            }
           }
         }
       }
@@ -662,18 +717,42 @@ static int accept_impl(const State& st, int k, const uint8_t* mask, int num_sms,
   return cudaGetLastError() == cudaSuccess ? nl : -1;
 }
 
+template <typename T, int KT>
+static void launch_ratio_kt(const State& st, int k, const int32_t* d_idx, const void* d_rows,
+                            void* d_ratio, cudaStream_t s) {
+  // threads x elements per thread so that one sweep covers a row when registers allow
+  const int n = st.n;
+  constexpr bool CX = sizeof(T) == 16;
+  constexpr int EMAX = CX ? (KT >= 8 ? 1 : KT == 4 ? 2 : 4) : (KT >= 8 ? 2 : 4);
+  const unsigned W = (unsigned)st.W;
+  const int nt = n <= 256 ? 128 : 256;
+  int ept = (n + nt - 1) / nt;
+  ept = ept >= 4 ? 4 : ept >= 2 ? 2 : 1;
+  if (ept > EMAX) ept = EMAX;
+  if (ept == 1)
+    det_ratio_kernel<T, KT, 1><<<W, nt, 0, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
+  else if (ept == 2)
+    det_ratio_kernel<T, KT, (EMAX >= 2 ? 2 : 1)><<<W, nt, 0, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
+  else
+    det_ratio_kernel<T, KT, EMAX><<<W, nt, 0, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
+}
+
+template <typename T>
+static void launch_ratio_t(const State& st, int k, const int32_t* d_idx, const void* d_rows,
+                           void* d_ratio, cudaStream_t s) {
+  switch (round_kt(k)) {
+    case 1: launch_ratio_kt<T, 1>(st, k, d_idx, d_rows, d_ratio, s); break;
+    case 2: launch_ratio_kt<T, 2>(st, k, d_idx, d_rows, d_ratio, s); break;
+    case 4: launch_ratio_kt<T, 4>(st, k, d_idx, d_rows, d_ratio, s); break;
+    default: launch_ratio_kt<T, 8>(st, k, d_idx, d_rows, d_ratio, s); break;
+  }
+}
+
 int launch_det_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
                      void* d_ratio, cudaStream_t s, Prof* prof) {
   ProfScope ps(prof, LRUX_PROF_RATIO, s);
-  const int nt = st.n <= 128 ? 128 : 256;
-  const size_t e = st.dt == LRUX_F64 ? 8 : 16;
-  const size_t smem = (size_t)st.cap * k * e;  // <= 32*8*8*16 = 32 KiB
-  if (st.dt == LRUX_F64)
-    det_ratio_kernel<double><<<(unsigned)st.W, nt, smem, s>>>(st, k, d_idx, (const double*)d_rows,
-                                                              (double*)d_ratio);
-  else
-    det_ratio_kernel<cplx><<<(unsigned)st.W, nt, smem, s>>>(st, k, d_idx, (const cplx*)d_rows,
-                                                            (cplx*)d_ratio);
+  if (st.dt == LRUX_F64) launch_ratio_t<double>(st, k, d_idx, d_rows, d_ratio, s);
+  else launch_ratio_t<cplx>(st, k, d_idx, d_rows, d_ratio, s);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

@@ -78,6 +78,23 @@ __global__ void __launch_bounds__(256) flush_dmma_kernel(State st, int t1) {
       for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
         for (int nt = 0; nt < 4; ++nt) acc[p][mt][nt][0] = acc[p][mt][nt][1] = 0.0;
+    // real case: issue the loads of the output tile now, consume them in the epilogue
+    // (hides one global-memory latency per work item; the HBM-bound regime, Kk <~ 50)
+    double tv[CX ? 1 : 2][CX ? 1 : 4][2];
+    if (!CX) {
+#pragma unroll
+      for (int mt = 0; mt < 2; ++mt) {
+        const int row = r0 + wr * 16 + mt * 8 + lm;
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const int col = c0 + wc * 32 + nt * 8 + 2 * lk + e;
+            const bool need = row < n && col < n && (!SKEW || col > row);
+            tv[CX ? 0 : mt][CX ? 0 : nt][e] = need ? ((const double*)Tw)[(size_t)row * n + col] : 0.0;
+          }
+      }
+    }
 
     for (int s0 = 0; s0 < fill; s0 += KC) {
       __syncthreads();
@@ -130,14 +147,17 @@ __global__ void __launch_bounds__(256) flush_dmma_kernel(State st, int t1) {
           T a;
           if (!CX) a = sc_from(acc[0][mt][nt][e], 0.0, T{});
           else a = sc_from(acc[0][mt][nt][e], acc[NP - 1][mt][nt][e], T{});
+          T old;
+          if (!CX) old = sc_from(tv[CX ? 0 : mt][CX ? 0 : nt][e], 0.0, T{});
+          else if (!SKEW || col > row) old = Tw[(size_t)row * n + col];
           if (SKEW) {
             if (col > row) {
-              const T v = S::add(Tw[(size_t)row * n + col], a);
+              const T v = S::add(old, a);
               Tw[(size_t)row * n + col] = v;
               Tw[(size_t)col * n + row] = S::neg(v);
             }
           } else {
-            Tw[(size_t)row * n + col] = S::sub(Tw[(size_t)row * n + col], a);
+            Tw[(size_t)row * n + col] = S::sub(old, a);
           }
         }
       }
