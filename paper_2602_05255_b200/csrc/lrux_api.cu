@@ -33,6 +33,11 @@ size_t state_layout(State* st, void* base, int64_t W, int32_t n, int32_t kmax, i
   s.pend_Rinv = take((size_t)W * kc * kc * e);
   s.pend_C = take((size_t)W * kmax * n * e);
   s.pend_N = take((size_t)W * kmax * n * e);
+  if (kind == KIND_DET) {
+    const size_t nsplit = ((size_t)n + kRatioSlice - 1) / kRatioSlice;
+    s.pend_Rpart = take((size_t)W * nsplit * kmax * kmax * e);
+    s.pend_cnt = (int32_t*)take((size_t)W * 4);
+  }
   if (kind == KIND_PF) {
     s.pend_Y = take((size_t)W * kmax * n * e);
     s.pend_AN = cap ? take((size_t)W * kmax * cap * e) : nullptr;
@@ -55,9 +60,11 @@ static lrux_status_t check_dims(int64_t W, int32_t n, int32_t kmax, int32_t K, i
   if (kind == KIND_PF && (n % 2 != 0)) return LRUX_EINVAL;
   if (kmax > n) return LRUX_EINVAL;
   // the delayed ratio stages K*kmax*kmax coefficients in shared memory (48 KiB static limit)
-  if ((size_t)K * kmax * kmax * (kind == KIND_PF ? 4 : 1) * (dt == LRUX_C128 ? 16 : 8) > 48 * 1024)
+  const size_t kt = kmax <= 1 ? 1 : kmax <= 2 ? 2 : kmax <= 4 ? 4 : 8;   // kernels' template rank
+  if ((size_t)K * kmax * kt * (kind == KIND_PF ? 4 : 1) * (dt == LRUX_C128 ? 16 : 8) > 48 * 1024)
     return LRUX_EUNSUPPORTED;
   if (W > (int64_t)2000000000) return LRUX_EINVAL;
+  if (n > kRatioSlice * kRatioSplitMax) return LRUX_EUNSUPPORTED;
   return LRUX_OK;
 }
 

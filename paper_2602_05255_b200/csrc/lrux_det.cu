@@ -13,25 +13,33 @@
 namespace lrux {
 
 // ---------------------------------------------------------------- ratio (a1, a2, a5)
-// One CTA per walker.  Each thread owns EPT elements i of the k gathered columns
-// C_eff = A_eff^-1[:,P] and walks the delay buffer ONCE for all of them:
+// Grid (W, nsplit): CTA (w, sp) owns the column slice [sp*256, sp*256+256) of walker w.
+// Each thread owns EPT elements i of the k gathered columns C_eff = A_eff^-1[:,P] and
+// walks the delay buffer ONCE for all of them:
 //   a_tau = A0^-1 v - sum_t a_t (b_t^T v)                       (Eq. 14)
 // (b_t^T v = Bbuf[s][P[a]] is a warp-uniform load).  C_eff and N are stashed for
-// accept; R = N C_eff (Eq. 4 / Eq. 13) is accumulated on the fly when KT <= 4,
-// else from the stash; r = det R by a k x k LU in one thread.
+// accept.  R = N C_eff (Eq. 4 / Eq. 13): every slice writes its partial k x k sum
+// (KT <= 4: accumulated on the fly), and the slice that finishes last adds the partials
+// in slice order (deterministic) -- or, for KT = 8, forms R from the complete stash --
+// and evaluates r = det R by a k x k LU in one thread.
 template <typename T, int KT, int EPT>
 __global__ void __launch_bounds__(256)
 det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __restrict__ rows,
                  T* __restrict__ ratio_out) {
   using S = Sc<T>;
   constexpr bool FLY = KT <= 4;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* Bp = (T*)smem_raw;  // [fill][KT]: b_t^T v = Bbuf[s][P[a]]
   __shared__ T Rs[kMaxK * kMaxK];
   __shared__ T Ri[kMaxK * kMaxK];
   __shared__ T red[8][FLY ? KT * KT : 1];
-  const int w = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
+  __shared__ int sP[KT];
+  __shared__ int is_last;
+  const int w = blockIdx.x, sp = blockIdx.y, nsplit = gridDim.y;
+  const int tid = threadIdx.x, nt = blockDim.x;
   const int warp = tid >> 5, lane = tid & 31, nw = nt >> 5;
   const int n = st.n, kmax = st.kmax;
-  if (w == 0 && tid == 0) st.counters[0] = 0;
+  if (w == 0 && sp == 0 && tid == 0) st.counters[0] = 0;
   int P[KT];
   bool bad = false;
 #pragma unroll
@@ -42,8 +50,8 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
     for (int c = 0; c < a; ++c)
       if (a < k && P[c] == P[a]) bad = true;
   }
-  if (bad) {   // uniform over the CTA
-    if (tid == 0) {
+  if (bad) {   // uniform over the walker's CTAs
+    if (sp == 0 && tid == 0) {
       ratio_out[w] = S::nan();
       ((T*)st.pend_ratio)[w] = S::nan();
       st.pend_ok[w] = 0;
@@ -62,7 +70,17 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
   for (int b = 0; b < KT; ++b)
 #pragma unroll
     for (int a = 0; a < KT; ++a) racc[b][a] = S::zero();
-  for (int i0 = 0; i0 < n; i0 += nt * EPT) {
+  if (fill > 0) {
+    if (tid == 0) {
+#pragma unroll
+      for (int a = 0; a < KT; ++a) sP[a] = a < k ? P[a] : P[0];
+    }
+    __syncthreads();
+    for (int q = tid; q < fill * KT; q += nt) Bp[q] = Bb[(size_t)(q / KT) * n + sP[q % KT]];
+    __syncthreads();
+  }
+  {
+    const int i0 = sp * kRatioSlice;
     T c[KT][EPT];
 #pragma unroll
     for (int e = 0; e < EPT; ++e) {
@@ -71,20 +89,20 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
       for (int a = 0; a < KT; ++a)
         c[a][e] = (a < k && i < n) ? Tw[(size_t)P[a] * n + i] : S::zero();
     }
-#pragma unroll 4
+#pragma unroll 8
     for (int s = 0; s < fill; ++s) {
-      T av[EPT], bp[KT];
+      T av[EPT];
 #pragma unroll
       for (int e = 0; e < EPT; ++e) {
         const int i = i0 + tid + nt * e;
         av[e] = i < n ? Ab[(size_t)s * n + i] : S::zero();
       }
 #pragma unroll
-      for (int a = 0; a < KT; ++a) bp[a] = a < k ? Bb[(size_t)s * n + P[a]] : S::zero();
+      for (int a = 0; a < KT; ++a) {
+        const T bp = Bp[s * KT + a];
 #pragma unroll
-      for (int a = 0; a < KT; ++a)
-#pragma unroll
-        for (int e = 0; e < EPT; ++e) c[a][e] = S::fnma(bp[a], av[e], c[a][e]);
+        for (int e = 0; e < EPT; ++e) c[a][e] = S::fnma(bp, av[e], c[a][e]);
+      }
     }
 #pragma unroll
     for (int e = 0; e < EPT; ++e) {
@@ -98,14 +116,14 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
             pC[(size_t)b * n + i] = c[b][e];
             if constexpr (FLY) {
 #pragma unroll
-              for (int a = 0; a < KT; ++a)
-                racc[b][a] = S::fma(x, c[a][e], racc[b][a]);
+              for (int a = 0; a < KT; ++a) racc[b][a] = S::fma(x, c[a][e], racc[b][a]);
             }
           }
         }
       }
     }
   }
+  T* part = (T*)st.pend_Rpart + ((size_t)w * nsplit + sp) * kmax * kmax;
   if constexpr (FLY) {
 #pragma unroll
     for (int b = 0; b < KT; ++b)
@@ -118,16 +136,55 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
     if (tid < KT * KT) {
       T v = red[0][tid];
       for (int q = 1; q < nw; ++q) v = S::add(v, red[q][tid]);
-      Rs[(tid / KT) * kMaxK + (tid % KT)] = v;
+      if (nsplit == 1) Rs[(tid / KT) * kMaxK + (tid % KT)] = v;
+      else if (tid / KT < k && tid % KT < k) part[(tid / KT) * kmax + (tid % KT)] = v;
     }
-  } else {
-    __syncthreads();   // stash visible to the whole CTA
-    for (int pr = warp; pr < k * k; pr += nw) {
-      const int a = pr / k, b = pr % k;
-      T acc = S::zero();
-      for (int i = lane; i < n; i += 32) acc = S::fma(pN[(size_t)a * n + i], pC[(size_t)b * n + i], acc);
-      acc = warp_sum(acc);
-      if (lane == 0) Rs[a * kMaxK + b] = acc;
+  }
+  if (nsplit > 1 || !FLY) {
+    // make this slice's stash / partial visible, then find out whether we are last
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+      const int done = nsplit > 1 ? atomicAdd(&st.pend_cnt[w], 1) : 0;
+      is_last = done == nsplit - 1;
+      if (is_last && nsplit > 1) st.pend_cnt[w] = 0;
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    if constexpr (FLY) {
+      if (tid < KT * KT && tid / KT < k && tid % KT < k) {
+        const T* p0 = (const T*)st.pend_Rpart + (size_t)w * nsplit * kmax * kmax +
+                      (tid / KT) * kmax + (tid % KT);
+        T v = S::zero();
+        for (int q = 0; q < nsplit; ++q) {
+          const double2* src = (const double2*)(p0 + (size_t)q * kmax * kmax);
+          T x;
+          if constexpr (sizeof(T) == 16) { const double2 t = __ldcg(src); x = sc_from(t.x, t.y, T{}); }
+          else x = sc_from(__ldcg((const double*)src), 0.0, T{});
+          v = S::add(v, x);
+        }
+        Rs[(tid / KT) * kMaxK + (tid % KT)] = v;
+      }
+    } else {
+      for (int pr = warp; pr < k * k; pr += nw) {
+        const int a = pr / k, b = pr % k;
+        T acc = S::zero();
+        for (int i = lane; i < n; i += 32) {
+          T x, y;
+          if constexpr (sizeof(T) == 16) {
+            const double2 tx = __ldcg((const double2*)(pN + (size_t)a * n + i));
+            const double2 ty = __ldcg((const double2*)(pC + (size_t)b * n + i));
+            x = sc_from(tx.x, tx.y, T{}); y = sc_from(ty.x, ty.y, T{});
+          } else {
+            x = sc_from(__ldcg((const double*)(pN + (size_t)a * n + i)), 0.0, T{});
+            y = sc_from(__ldcg((const double*)(pC + (size_t)b * n + i)), 0.0, T{});
+          }
+          acc = S::fma(x, y, acc);
+        }
+        acc = warp_sum(acc);
+        if (lane == 0) Rs[a * kMaxK + b] = acc;
+      }
     }
   }
   __syncthreads();
@@ -395,6 +452,7 @@ __global__ void __launch_bounds__(256) det_prep_kernel(State st, int k, int grou
     T acc[KT];
 #pragma unroll
     for (int b = 0; b < KT; ++b) acc[b] = S::zero();
+#pragma unroll 4
     for (int i = lane; i < n; i += 32) {
       const T x = Ab[(size_t)s * n + i];
 #pragma unroll
@@ -506,6 +564,7 @@ det_append_kernel(State st, int k, int tiles, int rows_per_tile, int n_in_smem) 
 #pragma unroll
     for (int b = 0; b < KT; ++b) m[b] = S::zero();
     if (jj < nj && sg < nsg) {
+#pragma unroll 8
       for (int s = sg; s < fill; s += nsg) {
         const T bv = Bb[(size_t)s * n + j_beg + jj];
 #pragma unroll
@@ -646,7 +705,7 @@ static int launch_append_kt(const State& st, int k, int num_sms, cudaStream_t s)
     const int grid = persistent_grid(num_sms, 8, (int64_t)st.W * groups);
     det_prep_kernel<T, KT><<<grid, 256, 0, s>>>(st, k, groups); ++nl;
   }
-  int rows_per_tile = 64;   // must divide the block size (256)
+  const int rows_per_tile = n >= 1024 ? 128 : 64;   // must divide the block size (256)
   const int tiles = (n + rows_per_tile - 1) / rows_per_tile;
   const int n_in_smem = (size_t)k * n * sizeof(T) <= 96 * 1024;
   const size_t smem = ((n_in_smem ? (size_t)k * n : 0) + 4 * (size_t)KT * rows_per_tile) * sizeof(T);
@@ -720,21 +779,18 @@ static int accept_impl(const State& st, int k, const uint8_t* mask, int num_sms,
 template <typename T, int KT>
 static void launch_ratio_kt(const State& st, int k, const int32_t* d_idx, const void* d_rows,
                             void* d_ratio, cudaStream_t s) {
-  // threads x elements per thread so that one sweep covers a row when registers allow
+  // one CTA per 256-column slice: 128 threads x 2 elements (n <= 256: a single slice,
+  // 1 element per thread when n <= 128), else 256 threads x 1 element
   const int n = st.n;
-  constexpr bool CX = sizeof(T) == 16;
-  constexpr int EMAX = CX ? (KT >= 8 ? 1 : KT == 4 ? 2 : 4) : (KT >= 8 ? 2 : 4);
-  const unsigned W = (unsigned)st.W;
-  const int nt = n <= 256 ? 128 : 256;
-  int ept = (n + nt - 1) / nt;
-  ept = ept >= 4 ? 4 : ept >= 2 ? 2 : 1;
-  if (ept > EMAX) ept = EMAX;
-  if (ept == 1)
-    det_ratio_kernel<T, KT, 1><<<W, nt, 0, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
-  else if (ept == 2)
-    det_ratio_kernel<T, KT, (EMAX >= 2 ? 2 : 1)><<<W, nt, 0, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
+  const int nsplit = (n + kRatioSlice - 1) / kRatioSlice;
+  const dim3 grid((unsigned)st.W, (unsigned)nsplit);
+  const size_t sm = (size_t)st.cap * KT * sizeof(T);   // <= 48 KiB (checked at init)
+  if (n <= 128)
+    det_ratio_kernel<T, KT, 1><<<grid, 128, sm, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
+  else if (n <= 256)
+    det_ratio_kernel<T, KT, 2><<<grid, 128, sm, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
   else
-    det_ratio_kernel<T, KT, EMAX><<<W, nt, 0, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
+    det_ratio_kernel<T, KT, 1><<<grid, 256, sm, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
 }
 
 template <typename T>

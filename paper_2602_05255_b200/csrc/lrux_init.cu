@@ -275,6 +275,7 @@ static int init_impl(const State& st, const void* d_A0, cudaStream_t s) {
   cudaMemsetAsync(st.nupd, 0, W * 4, s);
   cudaMemsetAsync(st.pend_ok, 0, W, s);
   cudaMemsetAsync(st.counters, 0, 32, s);
+  if (st.pend_cnt) cudaMemsetAsync(st.pend_cnt, 0, W * 4, s);
   const size_t smem_gj = 2 * (size_t)n * sizeof(T) + (size_t)n * 4;
   const size_t smem_pr = 2 * (size_t)n * sizeof(T);
   if (cudaFuncSetAttribute(gj_inverse_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,

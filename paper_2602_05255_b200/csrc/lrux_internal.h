@@ -11,6 +11,8 @@
 namespace lrux {
 
 enum Kind { KIND_DET = 0, KIND_PF = 1 };
+constexpr int kRatioSlice = 256;       // columns of A^-1[:,P] handled by one CTA of the det ratio
+constexpr int kRatioSplitMax = 64;     // => n <= 16384
 
 // Views into the caller-owned d_state buffer (all device pointers, 256 B aligned).
 // Element type is double (LRUX_F64) or interleaved complex (LRUX_C128); sizes
@@ -34,6 +36,8 @@ struct State {
   void* pend_N;      // [W][kmax][n]  new rows
   void* pend_Y;      // pf: [W][kmax][n]  A^-1 N ; det delayed: [W][kmax][cap] N * Abuf^T
   void* pend_AN;     // pf delayed: [W][kmax][cap]  N * Abuf^T
+  void* pend_Rpart;  // det: [W][kRatioSplitMax][kmax*kmax] partial R of each column slice
+  int32_t* pend_cnt; // det: [W] slices of the current ratio call that have finished
   void* Abuf;        // [W][cap][n]  det: a_t (Eq. 10);  pf: a'_t (Eq. 25)
   void* Bbuf;        // [W][cap][n]  det: b_t (Eq. 11);  pf: a'_t R_t^-1
   int32_t* list;     // [W] accepted walkers (compacted)
