@@ -416,11 +416,31 @@ def roofline_flush(wk, K, run, hbm_peak, hbm_src, dgemm_tflops):
     return out
 
 
+def parse_workload(name):
+    """Named workload, or a point of the configs[4] sweep written as
+    `det,n=1024,k=4,K=8[,W=2048][,cplx]` / `pf,n=512,k=1,K=0`.  Without W the walker
+    count is sized so that inverses + orbital matrices + init scratch fit ~100 GB
+    (configs[4] sizes W for 120 GB of inverses alone)."""
+    if name in WORKLOADS:
+        return dict(WORKLOADS[name], name=name)
+    parts = name.split(",")
+    if parts[0] not in ("det", "pf"):
+        raise SystemExit("unknown workload %r" % name)
+    kv = dict(p.split("=") for p in parts[1:] if "=" in p)
+    cplx = "cplx" in parts
+    n, k, K = int(kv["n"]), int(kv.get("k", 1)), int(kv.get("K", 0))
+    esz = 16 if cplx else 8
+    # per walker: inverse n^2 + A0 scratch n^2 + orbitals (det: 2 n^2, pf: 4 n^2) + buffers
+    per = n * n * esz * (2 + (2 if parts[0] == "det" else 4)) + 2 * K * k * (1 if parts[0] == "det" else 2) * n * esz
+    W = int(kv["W"]) if "W" in kv else max(1, int(100e9 // per))
+    return dict(kind=parts[0], cplx=cplx, W=W, n=n, M=2 * n, k=k, Ks=(K,), cfg=5, name=name,
+                desc="configs[4] sweep point: %s %s, n=%d, M=%d, k=%d, K=%d, %d walkers, Metropolis"
+                     % (parts[0], "c128" if cplx else "f64", n, 2 * n, k, K, W))
+
+
 def main(argv=None):
     args = parse_args(argv)
-    if args.workload not in WORKLOADS:
-        raise SystemExit("unknown workload %r" % args.workload)
-    wk = dict(WORKLOADS[args.workload], name=args.workload)
+    wk = parse_workload(args.workload)
     if args.walkers:
         wk["W"] = args.walkers
     if args.delay >= 0:

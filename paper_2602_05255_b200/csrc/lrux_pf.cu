@@ -13,6 +13,7 @@
 // the stored inverse stays exactly skew.
 #include "lrux_common.cuh"
 #include "lrux_internal.h"
+#include "lrux_tma.cuh"
 
 namespace lrux {
 
@@ -321,6 +322,174 @@ __global__ void __launch_bounds__(256) pf_update_kernel(State st, int k, int t1)
   }
 }
 
+// ---------------------------------------------------------------- streaming update (a4)
+// Large walkers: work item = (accepted walker, tile of 64 rows).  Y' and g = Y' R'^-1
+// (2k x n each) are staged in shared memory; each warp streams whole rows of Ti with
+// coalesced loads and stores.  As in the resident kernel every element is produced by
+// its own thread: below the diagonal the thread recomputes the mirrored upper value
+// from -Ti[r][c] with the same operands in the same order and stores its negative
+// (exact skewness, no transposed access).
+template <typename T>
+__global__ void __launch_bounds__(256)
+pf_update_stream_kernel(State st, int k, int tiles, int rows_per_tile) {
+  using S = Sc<T>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int n = st.n, kmax = st.kmax, m = 2 * k;
+  T* yv = (T*)smem_raw;          // [m][n]
+  T* gv = yv + (size_t)m * n;    // [m][n]
+  __shared__ T Ri[kMaxC * kMaxC];
+  __shared__ int P[kMaxK];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
+  const int count = st.counters[0];
+  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
+    const int w = st.list[item / tiles];
+    const int tile = item % tiles;
+    const T* pC = (const T*)st.pend_C + (size_t)w * kmax * n;
+    const T* pY = (const T*)st.pend_Y + (size_t)w * kmax * n;
+    T* Tw = (T*)st.Ti + (size_t)w * n * n;
+    __syncthreads();
+    for (int q = tid; q < m * m; q += 256)
+      Ri[(q / m) * kMaxC + (q % m)] =
+          ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + (q / m) * st.kc + (q % m)];
+    if (tid < k) P[tid] = st.pend_idx[(size_t)w * kmax + tid];
+    __syncthreads();
+    for (int i = tid; i < n; i += 256) {
+      T yp[kMaxC];
+      for (int alpha = 0; alpha < m; ++alpha) {
+        yp[alpha] = yprime(pY, pC, P, k, n, alpha, i);
+        yv[(size_t)alpha * n + i] = yp[alpha];
+      }
+      for (int beta = 0; beta < m; ++beta) {
+        T g = S::zero();
+        for (int alpha = 0; alpha < m; ++alpha) g = S::fma(yp[alpha], Ri[alpha * kMaxC + beta], g);
+        gv[(size_t)beta * n + i] = g;
+      }
+    }
+    __syncthreads();
+    const int r_end = min(n, (tile + 1) * rows_per_tile);
+    for (int r = tile * rows_per_tile + warp; r < r_end; r += nw) {
+      T* row = Tw + (size_t)r * n;
+#pragma unroll 4
+      for (int c = lane; c < n; c += 32) {
+        const bool up = r < c;
+        const int i = up ? r : c, j = up ? c : r;
+        const T x = row[c];
+        T v = up ? x : S::neg(x);
+        for (int beta = 0; beta < m; ++beta)
+          v = S::fma(gv[(size_t)beta * n + i], yv[(size_t)beta * n + j], v);
+        row[c] = (r == c) ? S::zero() : (up ? v : S::neg(v));
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------- resident update (a4)
+// Small walkers (n^2 e <= ~190 KB: n <= 152 fp64, config C3's n = 128): the whole inverse
+// of an accepted walker is brought into shared memory by ONE bulk asynchronous copy
+// (TMA), Y = A^-1 N (k = 1; for k >= 2 the ratio already left it in pend_Y), g = Y' R'^-1
+// and the rank-2k update are done on chip, and the matrix goes back with one bulk
+// store: HBM traffic = read n^2 e + write n^2 e, the compulsory minimum (SURVEY.md
+// §7 H3).  Every element is updated by its own thread with no transposed access:
+// for r > c the thread recomputes the upper value v(c,r) from -Ti[r][c] (the matrix
+// is exactly skew on entry) with the same operands in the same order and stores -v,
+// so the result is exactly skew again.
+template <typename T>
+__global__ void __launch_bounds__(512) pf_resident_update_kernel(State st, int k, int need_y) {
+  using S = Sc<T>;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int n = st.n, kmax = st.kmax, m = 2 * k;
+  T* Ts = (T*)smem_raw;                 // [n][n]
+  T* yv = Ts + (size_t)n * n;           // [m][n]  Y'
+  T* gv = yv + (size_t)m * n;           // [m][n]  Y' R'^-1
+  T* nv = gv + (size_t)m * n;           // [n]     new row (k = 1)
+  __shared__ T Ri[kMaxC * kMaxC];
+  __shared__ int P[kMaxK];
+  __shared__ __align__(8) uint64_t bar;
+  const int tid = threadIdx.x, nt = blockDim.x, warp = tid >> 5, lane = tid & 31, nw = nt >> 5;
+  const int count = st.counters[0];
+  const uint32_t bytes = (uint32_t)((size_t)n * n * sizeof(T));
+  if (tid == 0) {
+    tma::mbar_init(&bar, 1);
+    tma::fence_barrier_init();
+  }
+  __syncthreads();
+  uint32_t phase = 0;
+  for (int it = blockIdx.x; it < count; it += gridDim.x) {
+    const int w = st.list[it];
+    T* Tw = (T*)st.Ti + (size_t)w * n * n;
+    if (tid == 0) {
+      tma::mbar_arrive_expect_tx(&bar, bytes);
+      tma::load(Ts, Tw, bytes, &bar);
+    }
+    const T* pC = (const T*)st.pend_C + (size_t)w * kmax * n;
+    const T* pY = (const T*)st.pend_Y + (size_t)w * kmax * n;
+    const T* pN = (const T*)st.pend_N + (size_t)w * kmax * n;
+    for (int q = tid; q < m * m; q += nt)
+      Ri[(q / m) * kMaxC + (q % m)] =
+          ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + (q / m) * st.kc + (q % m)];
+    if (tid < k) P[tid] = st.pend_idx[(size_t)w * kmax + tid];
+    __syncthreads();
+    for (int q = tid; q < k * n; q += nt) {
+      const int a = q / n, i = q % n;
+      yv[(size_t)(k + a) * n + i] = pC[q];
+      if (need_y) nv[q] = pN[q];   // k == 1
+      else yv[q] = (i == P[a]) ? S::add(pY[q], S::one()) : pY[q];
+    }
+    __syncthreads();
+    tma::mbar_wait(&bar, phase);
+    phase ^= 1;
+    if (need_y) {
+      for (int i = warp; i < n; i += nw) {
+        T acc = S::zero();
+        for (int j = lane; j < n; j += 32) acc = S::fma(Ts[(size_t)i * n + j], nv[j], acc);
+        acc = warp_sum(acc);
+        if (lane == 0) yv[i] = (i == P[0]) ? S::add(acc, S::one()) : acc;
+      }
+      __syncthreads();
+    }
+    for (int q = tid; q < m * n; q += nt) {
+      const int beta = q / n, i = q % n;
+      T g = S::zero();
+      for (int alpha = 0; alpha < m; ++alpha)
+        g = S::fma(yv[(size_t)alpha * n + i], Ri[alpha * kMaxC + beta], g);
+      gv[q] = g;
+    }
+    __syncthreads();
+    // one warp per row, lanes over columns; row-dependent factors hoisted
+    for (int r = warp; r < n; r += nw) {
+      T* row = Ts + (size_t)r * n;
+      if (m == 2) {
+        const T g0r = gv[r], g1r = gv[n + r], y0r = yv[r], y1r = yv[n + r];
+        for (int c = lane; c < n; c += 32) {
+          const bool up = r < c;
+          const T x = row[c];
+          T v = up ? x : S::neg(x);
+          v = S::fma(up ? g0r : gv[c], up ? yv[c] : y0r, v);
+          v = S::fma(up ? g1r : gv[n + c], up ? yv[n + c] : y1r, v);
+          row[c] = (r == c) ? S::zero() : (up ? v : S::neg(v));
+        }
+      } else {
+        for (int c = lane; c < n; c += 32) {
+          const bool up = r < c;
+          const int i = up ? r : c, j = up ? c : r;
+          const T x = row[c];
+          T v = up ? x : S::neg(x);
+          for (int beta = 0; beta < m; ++beta) v = S::fma(gv[beta * n + i], yv[beta * n + j], v);
+          row[c] = (r == c) ? S::zero() : (up ? v : S::neg(v));
+        }
+      }
+    }
+    tma::fence_proxy_async();
+    __syncthreads();
+    if (tid == 0) {
+      tma::store(Tw, Ts, bytes);
+      tma::store_commit();
+      tma::store_wait_read<0>();   // Ts may be overwritten by the next walker's load
+    }
+    __syncthreads();
+  }
+}
+
 // ---------------------------------------------------------------- delayed append (a6)
 // Abuf[fill+alpha][:] = Y'[alpha][:]  (a'_tau, Eq. 28), Bbuf[fill+beta][:] = (a'_tau R'^-1)[:, beta].
 template <typename T>
@@ -420,12 +589,38 @@ template <typename T>
 static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_sms, cudaStream_t s,
                           Prof* prof) {
   int nl = launch_select(st, mask, s);
+  {
+    // whole-walker residency on chip when the inverse fits in shared memory
+    const int n = st.n;
+    const size_t sm = ((size_t)n * n + (size_t)(4 * k + 1) * n) * sizeof(T);
+    if (st.K == 0 && sm <= 200 * 1024) {
+      auto kern = pf_resident_update_kernel<T>;
+      if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess)
+        return -1;
+      ProfScope ps(prof, LRUX_PROF_UPDATE, s);
+      kern<<<pgrid(num_sms, 1, st.W), 512, sm, s>>>(st, k, k == 1 ? 1 : 0); ++nl;
+      return cudaGetLastError() == cudaSuccess ? nl : -1;
+    }
+  }
   if (k == 1) nl += launch_y<T>(st, k, 1, num_sms, s, prof);  // Y only for accepted walkers
   if (st.K == 0) {
-    const int t1 = (st.n + 31) / 32;
-    const int grid = pgrid(num_sms, 4, (int64_t)st.W * (t1 * (t1 + 1) / 2));
     ProfScope ps(prof, LRUX_PROF_UPDATE, s);
-    pf_update_kernel<T><<<grid, 256, 0, s>>>(st, k, t1); ++nl;
+    const size_t sm = 4 * (size_t)k * st.n * sizeof(T);   // Y' and g
+    if (sm <= 160 * 1024) {
+      auto kern = pf_update_stream_kernel<T>;
+      if (sm > 48 * 1024 &&
+          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess)
+        return -1;
+      const int rpt = 64, tiles = (st.n + rpt - 1) / rpt;
+      int occ = 1;
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, sm);
+      if (occ < 1) return -1;
+      kern<<<pgrid(num_sms, occ, (int64_t)st.W * tiles), 256, sm, s>>>(st, k, tiles, rpt); ++nl;
+    } else {
+      const int t1 = (st.n + 31) / 32;
+      const int grid = pgrid(num_sms, 4, (int64_t)st.W * (t1 * (t1 + 1) / 2));
+      pf_update_kernel<T><<<grid, 256, 0, s>>>(st, k, t1); ++nl;
+    }
   } else {
     {
       ProfScope ps(prof, LRUX_PROF_APPEND, s);

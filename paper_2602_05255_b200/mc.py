@@ -27,12 +27,16 @@ class Chain:
         self.W, self.n = self.occ.shape
         self.M = self.orb.shape[1]
         W, n = self.W, self.n
-        ar = torch.arange(W, device=dev)[:, None]
-        occl = self.occ.long()
-        if kind == "det":
-            A0 = self.orb[ar, occl]                                   # [W][n][n]
-        else:
-            A0 = self.orb[ar[:, :, None], occl[:, :, None], occl[:, None, :]]
+        A0 = torch.empty((W, n, n), dtype=dt, device=dev)
+        step = max(1, (1 << 26) // (n * n))        # bound the temporaries of the index gather
+        for c0 in range(0, W, step):
+            c1 = min(W, c0 + step)
+            ar = torch.arange(c0, c1, device=dev)[:, None]
+            occl = self.occ[c0:c1].long()
+            if kind == "det":
+                A0[c0:c1] = self.orb[ar, occl]                        # Phi[w][occ,:]
+            else:
+                A0[c0:c1] = self.orb[ar[:, :, None], occl[:, :, None], occl[:, None, :]]
         cls = lrux.DetWalkers if kind == "det" else lrux.PfWalkers
         self.walkers = cls(A0, kmax=self.k if kmax is None else kmax, K=self.K)
         del A0

@@ -83,6 +83,12 @@ def test_pf_config3_shape_reduced():
     _run("pf", wl.BASE_SEED + 3, 24, 128, 256, 1, 0, 80, walkers=[0, 7, 15, 23])
 
 
+@pytest.mark.parametrize("k", [1, 2])
+def test_pf_large_n_streaming_path(k):
+    """n=200: the inverse (320 KB) does not fit in shared memory -> tiled update kernels."""
+    _run("pf", 99 + k, 3, 200, 400, k, 0, 12, walkers=[0, 2], scratch_every=3)
+
+
 def test_det_config4_shape_reduced():
     """configs[3] shape reduced: complex128, k=4, delay K=32, n=256."""
     _run("det", wl.BASE_SEED + 4, 6, 256, 512, 4, 32, 80, cplx=True, walkers=[0, 5], scratch_every=5)
