@@ -44,6 +44,8 @@ struct Sc<double> {
   static __device__ __forceinline__ double inv(double a) { return 1.0 / a; }
   static __device__ __forceinline__ double div(double a, double b) { return a / b; }
   static __device__ __forceinline__ double scale(double a, double s) { return a * s; }
+  // a / |a| given |a|: exactly +-1 for real data
+  static __device__ __forceinline__ double unit(double a, double) { return copysign(1.0, a); }
   static __device__ __forceinline__ bool is_zero(double a) { return a == 0.0; }
   static __device__ __forceinline__ bool finite(double a) { return isfinite(a); }
   static __device__ __forceinline__ double nan() { return __longlong_as_double(0x7ff8000000000000LL); }
@@ -87,6 +89,9 @@ struct Sc<cplx> {
   }
   static __device__ __forceinline__ cplx div(cplx a, cplx b) { return mul(a, inv(b)); }
   static __device__ __forceinline__ cplx scale(cplx a, double s) { return cplx{a.re * s, a.im * s}; }
+  static __device__ __forceinline__ cplx unit(cplx a, double abs_a) {
+    return cplx{a.re / abs_a, a.im / abs_a};
+  }
   static __device__ __forceinline__ bool is_zero(cplx a) { return a.re == 0.0 && a.im == 0.0; }
   static __device__ __forceinline__ bool finite(cplx a) { return isfinite(a.re) && isfinite(a.im); }
   static __device__ __forceinline__ cplx nan() {

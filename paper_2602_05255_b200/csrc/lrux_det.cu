@@ -7,6 +7,8 @@
 //   A'^-1 = A^-1 - C R^-1 Wm                                  (Eq. 5)
 // State Ti = A^-T row-major, so C[:,a] is the contiguous row P[a] of Ti and column
 // j of Wm depends only on row j of Ti: the update is a single pass over Ti.
+#include <stdlib.h>
+
 #include "lrux_common.cuh"
 #include "lrux_internal.h"
 
@@ -224,7 +226,7 @@ __global__ void select_kernel(State st, const uint8_t* __restrict__ mask) {
   const double ar = S::abs(r);
   st.logabs[w] += log(ar);
   T* ph = (T*)st.phase;
-  ph[w] = S::mul(ph[w], S::scale(r, 1.0 / ar));
+  ph[w] = S::mul(ph[w], S::unit(r, ar));
 }
 template __global__ void select_kernel<double>(State, const uint8_t*);
 template __global__ void select_kernel<cplx>(State, const uint8_t*);
@@ -677,6 +679,16 @@ template <typename T, int KT>
 static int launch_update_kt(const State& st, int k, int num_sms, cudaStream_t s) {
   const int n = st.n;
   constexpr int VECMAX = sizeof(T) == 8 ? 2 : 1;
+  {
+    // rows of >= 8 KB: TMA-staged kernel (lrux_det_tma.cu).  LRUX_UPDATE_PATH=reg|tma
+    // overrides the choice (tuning / A-B measurements only).
+    static const char* path = getenv("LRUX_UPDATE_PATH");
+    const bool force_tma = path && path[0] == 't', force_reg = path && path[0] == 'r';
+    if (!force_reg && (force_tma || (size_t)n * sizeof(T) >= 8 * 1024)) {
+      const int r = launch_det_update_tma(st, k, num_sms, s);
+      if (r != 0) return r;
+    }
+  }
   const size_t smem = 2 * (size_t)k * n * sizeof(T);
   const bool vec_ok = (n % VECMAX) == 0;
   const int nvec = n / VECMAX;

@@ -136,7 +136,7 @@ gj_inverse_kernel(T* __restrict__ Mall, int n, T* __restrict__ phase_out,
     const T dinv = S::inv(d);
     if (tid == 0) {
       double ad = S::abs(d);
-      T u = S::scale(d, 1.0 / ad);
+      T u = S::unit(d, ad);
       phase = S::mul(phase, u);
       if (p != c) phase = S::neg(phase);
       logabs += log(ad);
@@ -232,7 +232,7 @@ parlett_reid_kernel(T* __restrict__ Mall, int n, T* __restrict__ phase_out,
     const T ainv = S::inv(a);
     {
       double ad = S::abs(a);
-      phase = S::mul(phase, S::scale(a, 1.0 / ad));
+      phase = S::mul(phase, S::unit(a, ad));
       logabs += log(ad);
     }
     for (int c = j + 2 + tid; c < n; c += nt) {

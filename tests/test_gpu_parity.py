@@ -83,6 +83,47 @@ def test_pf_config3_shape_reduced():
     _run("pf", wl.BASE_SEED + 3, 24, 128, 256, 1, 0, 80, walkers=[0, 7, 15, 23])
 
 
+@pytest.mark.parametrize("n,k,cplx,steps", [
+    (1024, 4, False, 10),     # rows of 8 KB: RC=4 rows per bulk copy, 2 vectors per lane
+    (1024, 8, False, 8),      # k=8: 32 partial sums per warp
+    (1100, 1, False, 10),     # ragged: 550 vectors per row, 4-row chunks with a 3-row tail
+    (512, 2, True, 10),       # complex128, 8 KB rows
+    (2048, 2, False, 4),      # 16 KB rows: RC=2, 4 vectors per lane
+])
+def test_det_tma_update_path(n, k, cplx, steps):
+    """Immediate update through the TMA-staged kernel (lrux_det_tma.cu)."""
+    _run("det", 500 + n + k, 2, n, 2 * n, k, 0, steps, cplx, walkers=[1],
+         scratch_every=0 if n >= 2048 else steps - 1)
+
+
+def test_det_tma_update_n4096_properties():
+    """n=4096 (32 KB rows, one row per bulk copy): the oracle is too slow here, so check
+    what holds at any size: A_T A_T^-1 = 1 and the tracked amplitude against a library
+    slogdet of A_T."""
+    from paper_2602_05255_b200 import mc
+
+    n, M, W, k = 4096, 8192, 2, 2
+    seed = 4242
+    Phi = wl.orbital_matrices_torch(seed, 0, W, M, n, 1.0 / n, "cuda")
+    occ, unocc = wl.initial_occupations(seed, W, M, n)
+    ch = mc.Chain("det", Phi, torch.as_tensor(occ, device="cuda"), torch.as_tensor(unocc, device="cuda"),
+                  k=k, K=0, seed=seed)
+    for t in range(8):
+        ch.step(t, forced=(t % 2 == 0))
+    torch.cuda.synchronize()
+    assert not ch.walkers.info.any()
+    assert int(ch.naccept.item()) >= 4 * W
+    ph, la = ch.walkers.get_amplitude()
+    inv = ch.walkers.get_inverse()
+    for w in range(W):
+        A = Phi[w][ch.occ[w].long()]
+        resid = (A @ inv[w] - torch.eye(n, dtype=A.dtype, device="cuda")).abs().max().item()
+        assert resid < 1e-9, resid
+        sign, logabs = torch.linalg.slogdet(A)
+        assert abs(la[w].item() - logabs.item()) < 1e-8 * max(1.0, abs(logabs.item()))
+        assert ph[w].item() == sign.item()
+
+
 @pytest.mark.parametrize("k", [1, 2])
 def test_pf_large_n_streaming_path(k):
     """n=200: the inverse (320 KB) does not fit in shared memory -> tiled update kernels."""
