@@ -120,6 +120,18 @@ lrux_status_t lrux_pf_get_amplitude(lrux_handle_t h, void* d_phase, double* d_lo
                                     void* stream);
 lrux_status_t lrux_pf_get_inverse(lrux_handle_t h, void* d_out, void* stream);
 
+/* ---------------------------------------------------------------- attach (checkpoint / resume)
+ * The walker state lives entirely in the caller's d_state buffer (plus d_info), so a
+ * byte copy of that buffer taken while no proposal is pending is a checkpoint.
+ * lrux_*_attach builds a handle over such a buffer WITHOUT running the O(n^3)
+ * initialisation: same (W, n, kmax, K, dt) as the lrux_*_init that produced it, buffer
+ * 256-byte aligned.  Launches nothing; d_info is used as is (not zeroed). */
+lrux_status_t lrux_det_attach(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, int32_t K,
+                              lrux_dtype_t dt, void* d_state, size_t state_bytes,
+                              int32_t* d_info);
+lrux_status_t lrux_pf_attach(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, int32_t K,
+                             lrux_dtype_t dt, void* d_state, size_t state_bytes, int32_t* d_info);
+
 /* ---------------------------------------------------------------- profiling
  * Device time per kernel class, taken with CUDA events the library records on the
  * caller's stream directly around its own launches (bench.py's roofline figures:

@@ -77,10 +77,11 @@ static lrux_status_t state_bytes(int64_t W, int32_t n, int32_t kmax, int32_t K, 
   return LRUX_OK;
 }
 
+// d_A0 == nullptr with attach == true: build the handle only (lrux_*_attach)
 static lrux_status_t init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, int32_t K,
                           lrux_dtype_t dt, const void* d_A0, void* d_state, size_t sb,
-                          int32_t* d_info, void* stream, int kind) {
-  if (!h || !d_A0 || !d_state || !d_info) return LRUX_EINVAL;
+                          int32_t* d_info, void* stream, int kind, bool attach = false) {
+  if (!h || (!d_A0 && !attach) || !d_state || !d_info) return LRUX_EINVAL;
   lrux_status_t s = check_dims(W, n, kmax, K, dt, kind);
   if (s != LRUX_OK) return s;
   if (((uintptr_t)d_state & 255) != 0) return LRUX_EINVAL;
@@ -97,8 +98,9 @@ static lrux_status_t init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, 
   hh->pending_k = 0;
   hh->launches = 0;
   hh->num_sms = sms;
-  int nl = kind == KIND_DET ? launch_det_init(hh->st, d_A0, (cudaStream_t)stream)
-                            : launch_pf_init(hh->st, d_A0, (cudaStream_t)stream);
+  int nl = attach ? 0
+           : kind == KIND_DET ? launch_det_init(hh->st, d_A0, (cudaStream_t)stream)
+                              : launch_pf_init(hh->st, d_A0, (cudaStream_t)stream);
   if (nl < 0) {
     delete hh;
     return LRUX_ECUDA;
@@ -143,6 +145,15 @@ lrux_status_t lrux_pf_init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax,
                            lrux_dtype_t dt, const void* d_A0, void* d_state, size_t state_bytes,
                            int32_t* d_info, void* stream) {
   return init(h, W, n, kmax, K, dt, d_A0, d_state, state_bytes, d_info, stream, KIND_PF);
+}
+
+lrux_status_t lrux_det_attach(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, int32_t K,
+                              lrux_dtype_t dt, void* d_state, size_t state_bytes, int32_t* d_info) {
+  return init(h, W, n, kmax, K, dt, nullptr, d_state, state_bytes, d_info, nullptr, KIND_DET, true);
+}
+lrux_status_t lrux_pf_attach(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, int32_t K,
+                             lrux_dtype_t dt, void* d_state, size_t state_bytes, int32_t* d_info) {
+  return init(h, W, n, kmax, K, dt, nullptr, d_state, state_bytes, d_info, nullptr, KIND_PF, true);
 }
 
 lrux_status_t lrux_det_ratio(lrux_handle_t h, int32_t k, const int32_t* d_idx, const void* d_rows,

@@ -27,6 +27,8 @@ SIGNATURES = {
     "lrux_pf_state_bytes": [_i64, _i32, _i32, _i32, C.c_int, C.POINTER(_sz)],
     "lrux_det_init": [C.POINTER(_vp), _i64, _i32, _i32, _i32, C.c_int, _vp, _vp, _sz, _vp, _vp],
     "lrux_pf_init": [C.POINTER(_vp), _i64, _i32, _i32, _i32, C.c_int, _vp, _vp, _sz, _vp, _vp],
+    "lrux_det_attach": [C.POINTER(_vp), _i64, _i32, _i32, _i32, C.c_int, _vp, _sz, _vp],
+    "lrux_pf_attach": [C.POINTER(_vp), _i64, _i32, _i32, _i32, C.c_int, _vp, _sz, _vp],
     "lrux_det_ratio": [_vp, _i32, _vp, _vp, _vp, _vp],
     "lrux_pf_ratio": [_vp, _i32, _vp, _vp, _vp, _vp],
     "lrux_det_accept": [_vp, _vp, _vp],
@@ -126,6 +128,26 @@ class _Walkers:
         _check(fn(C.byref(self._h), self.W, self.n, self.kmax, self.K, _dt(self.dtype), _ptr(A0),
                   C.c_void_p(self._state_ptr), nbytes, _ptr(self.info), _stream(stream)))
         self._lib = lib
+
+    def clone(self):
+        """Independent copy of these walkers: byte copy of the state buffer + lrux_*_attach
+        (no re-initialisation).  No proposal may be pending."""
+        new = object.__new__(type(self))
+        for a in ("W", "n", "kmax", "K", "dtype", "device", "_lib"):
+            setattr(new, a, getattr(self, a))
+        nbytes = state_bytes(self.kind, self.W, self.n, self.kmax, self.K, self.dtype)
+        new.state = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        off = (-new.state.data_ptr()) % 256
+        new._state_ptr = new.state.data_ptr() + off
+        src_off = self._state_ptr - self.state.data_ptr()
+        new.state[off:off + nbytes].copy_(self.state[src_off:src_off + nbytes])
+        new.info = self.info.clone()
+        new.ratio = torch.empty(self.W, dtype=self.dtype, device=self.device)
+        new._h = C.c_void_p()
+        fn = getattr(self._lib, "lrux_%s_attach" % self.kind)
+        _check(fn(C.byref(new._h), self.W, self.n, self.kmax, self.K, _dt(self.dtype),
+                  C.c_void_p(new._state_ptr), nbytes, _ptr(new.info)))
+        return new
 
     def _fn(self, name):
         return getattr(self._lib, "lrux_%s_%s" % (self.kind, name))

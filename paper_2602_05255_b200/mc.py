@@ -17,7 +17,7 @@ class Chain:
     occ [W][n], unocc [W][M-n] int32 device tensors are updated in place.
     """
 
-    def __init__(self, kind, orbitals, occ, unocc, k, K=0, seed=0, w0=0, kmax=None):
+    def __init__(self, kind, orbitals, occ, unocc, k, K=0, seed=0, w0=0, kmax=None, walkers=None):
         assert kind in ("det", "pf")
         self.kind, self.k, self.K, self.seed, self.w0 = kind, int(k), int(K), int(seed), int(w0)
         self.orb = orbitals.contiguous()
@@ -27,6 +27,10 @@ class Chain:
         self.W, self.n = self.occ.shape
         self.M = self.orb.shape[1]
         W, n = self.W, self.n
+        if walkers is not None:       # already initialised (e.g. a clone of the step-0 state)
+            self.walkers = walkers
+            self._buffers(W, n, dt, dev)
+            return
         A0 = torch.empty((W, n, n), dtype=dt, device=dev)
         step = max(1, (1 << 26) // (n * n))        # bound the temporaries of the index gather
         for c0 in range(0, W, step):
@@ -40,6 +44,9 @@ class Chain:
         cls = lrux.DetWalkers if kind == "det" else lrux.PfWalkers
         self.walkers = cls(A0, kmax=self.k if kmax is None else kmax, K=self.K)
         del A0
+        self._buffers(W, n, dt, dev)
+
+    def _buffers(self, W, n, dt, dev):
         self.idx = torch.zeros((W, self.k), dtype=torch.int32, device=dev)
         self.upos = torch.zeros((W, self.k), dtype=torch.int32, device=dev)
         self.rows = torch.zeros((W, self.k, n), dtype=dt, device=dev)

@@ -135,6 +135,32 @@ def test_det_config4_shape_reduced():
     _run("det", wl.BASE_SEED + 4, 6, 256, 512, 4, 32, 80, cplx=True, walkers=[0, 5], scratch_every=5)
 
 
+def test_attach_resumes_from_a_state_copy():
+    """lrux_*_attach: a byte copy of the state buffer is a checkpoint; a chain resumed
+    from it reproduces the original chain bit for bit (det with a half-full delay
+    buffer, and Pfaffian)."""
+    from paper_2602_05255_b200 import mc
+
+    for kind, n, M, k, K in (("det", 48, 96, 2, 5), ("pf", 40, 80, 1, 0)):
+        seed = 31 + n
+        orb, occ, unocc = pu.make_inputs(kind, seed, 5, n, M)
+        dev = "cuda"
+        a = mc.Chain(kind, torch.as_tensor(orb, device=dev), torch.as_tensor(occ, device=dev),
+                     torch.as_tensor(unocc, device=dev), k=k, K=K, seed=seed)
+        for t in range(7):
+            a.step(t)
+        b = mc.Chain(kind, a.orb, a.occ.clone(), a.unocc.clone(), k=k, K=K, seed=seed,
+                     walkers=a.walkers.clone())
+        for t in range(7, 20):
+            a.step(t)
+            b.step(t)
+            assert torch.equal(a.ratio, b.ratio) and torch.equal(a.mask, b.mask)
+        assert torch.equal(a.walkers.get_inverse(), b.walkers.get_inverse())
+        pa, la = a.walkers.get_amplitude()
+        pb, lb = b.walkers.get_amplitude()
+        assert torch.equal(pa, pb) and torch.equal(la, lb)
+
+
 # ---------------------------------------------------------------- error paths
 def test_errors_and_info_bits():
     dev = "cuda"
