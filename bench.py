@@ -85,6 +85,8 @@ class ClockSampler:
         self.index, self.proc, self.lines = index, None, []
 
     def start(self):
+        """Launch nvidia-smi and wait (<= 3 s) for its first sample, so that the sampler
+        is already running when the timed region begins."""
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS,
@@ -92,24 +94,36 @@ class ClockSampler:
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
+            t0 = time.perf_counter()
+            while not self.lines and time.perf_counter() - t0 < 3.0:
+                time.sleep(0.01)
         except Exception:
             self.proc = None
 
     def _read(self):
         for line in self.proc.stdout:
-            self.lines.append(line.strip())
+            self.lines.append((time.perf_counter(), line.strip()))
+
+    def mark_begin(self):
+        self.t_begin = time.perf_counter()
 
     def stop(self):
+        t_end = time.perf_counter()
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.03)          # let a sample that straddles the end arrive
         self.proc.terminate()
         try:
             self.proc.wait(timeout=5)
         except Exception:
             self.proc.kill()
+        t_begin = getattr(self, "t_begin", 0.0)
+        inside = [ln for (t, ln) in self.lines if t_begin <= t <= t_end + 0.03]
+        if not inside:            # timed region shorter than one sampling period: nearest samples
+            inside = [ln for (_, ln) in self.lines[-2:]]
         sm, smax, reasons, power = [], [], set(), []
         names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
-        for ln in self.lines:
+        for ln in inside:
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 7:
                 continue
@@ -187,6 +201,7 @@ def timed_run(ch, warmup, steps, forced=False, sampler=None):
         sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     if sampler:
+        sampler.mark_begin()
         torch.cuda.profiler.start()   # ncu --profile-from-start off sees the timed region only
     e0.record()
     for t in range(steps):

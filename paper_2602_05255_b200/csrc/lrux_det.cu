@@ -682,7 +682,7 @@ static int launch_update_kt(const State& st, int k, int num_sms, cudaStream_t s)
   {
     // rows of >= 8 KB: TMA-staged kernel (lrux_det_tma.cu).  LRUX_UPDATE_PATH=reg|tma
     // overrides the choice (tuning / A-B measurements only).
-    static const char* path = getenv("LRUX_UPDATE_PATH");
+    const char* path = getenv("LRUX_UPDATE_PATH");
     const bool force_tma = path && path[0] == 't', force_reg = path && path[0] == 'r';
     if (!force_reg && (force_tma || (size_t)n * sizeof(T) >= 8 * 1024)) {
       const int r = launch_det_update_tma(st, k, num_sms, s);
@@ -716,6 +716,17 @@ static int launch_append_kt(const State& st, int k, int num_sms, cudaStream_t s)
     const int groups = (st.cap + 7) / 8;
     const int grid = persistent_grid(num_sms, 8, (int64_t)st.W * groups);
     det_prep_kernel<T, KT><<<grid, 256, 0, s>>>(st, k, groups); ++nl;
+  }
+  {
+    // rows of >= 8 KB: the TMA-staged pass (lrux_det_tma.cu) + finish kernel
+    // (measured on B200: the register-row append below is still faster at configs[3],
+    // 0.60 vs 0.45 of HBM peak, so the TMA pass is opt-in for the delayed path)
+    const char* path = getenv("LRUX_UPDATE_PATH");
+    const bool force_tma = path && path[0] == 't';
+    if (force_tma) {
+      const int r = launch_det_append_tma(st, k, num_sms, s);
+      if (r != 0) return r < 0 ? -1 : nl + r;
+    }
   }
   const int rows_per_tile = n >= 1024 ? 128 : 64;   // must divide the block size (256)
   const int tiles = (n + rows_per_tile - 1) / rows_per_tile;

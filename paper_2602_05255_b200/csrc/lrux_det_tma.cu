@@ -15,6 +15,8 @@
 // slice (rows from shared memory, its slices of N and C cached in registers), the
 // partial sums meet in shared memory, g = R^-1 d, then the same lanes apply the rank-k
 // update to their columns in place and the chunk goes back to HBM.
+#include <stdlib.h>
+
 #include "lrux_common.cuh"
 #include "lrux_internal.h"
 #include "lrux_tma.cuh"
@@ -77,28 +79,33 @@ struct Vec16<cplx> {
 __device__ __forceinline__ void to_doubles(double x, double* o) { o[0] = x; }
 __device__ __forceinline__ void to_doubles(cplx x, double* o) { o[0] = x.re; o[1] = x.im; }
 
-// RC rows per chunk (one bulk copy), TV 16-byte vectors of every row per lane.  All 8
-// warps split the columns of a chunk: lane owns the vectors q = warp*32 + lane + 256 t,
+// RC rows per chunk (one bulk copy), TV 16-byte vectors of every row per lane.  All NW
+// warps split the columns of a chunk: lane owns the vectors q = warp*32 + lane + 32 NW t,
 // t < TV, of EVERY row -- so its slices of N and C (k x TV vectors each) stay in
 // registers for as long as the CTA works on one walker, and shared memory carries only
 // the streamed rows.
-template <typename T, int KT, int RC, int TV>
-__global__ void __launch_bounds__(256, 1)
+//
+// APPEND = true is the delayed-update variant (row a6): the same streamed pass, read
+// only -- it leaves D[a][j] = N_a . Ti[j][:] - [j == P[a]]  (= u^T A0^-1, Eq. 15) in the
+// pending area (pend_C, free once det_prep_kernel has copied a_tau into the buffer) for
+// det_append_finish_kernel; nothing is written back to A0^-1.
+template <typename T, int KT, int RC, int TV, bool APPEND, int NW>
+__global__ void __launch_bounds__(NW * 32, 1)
 det_update_tma_kernel(State st, int k, int NS) {
   using S = Sc<T>;
   using V = Vec16<T>;
   constexpr int VEC = V::N;
   constexpr int ND = sizeof(T) / 8;          // doubles per element
   constexpr int NV = RC * KT * ND;           // values reduced per warp and chunk (<= 32)
-  constexpr int NW = 8;
   static_assert(NV <= 32, "too many partial sums per warp");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int n = st.n, kmax = st.kmax;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const size_t chunk_elems = (size_t)RC * n;
   T* stage_buf = (T*)smem_raw;                                   // [NS][RC][n]
-  double* dpart = (double*)(stage_buf + (size_t)NS * chunk_elems);   // [NW][NV]
-  T* gsm = (T*)(dpart + NW * NV);                                // [RC][KT]
+  double* dpart0 = (double*)(stage_buf + (size_t)NS * chunk_elems);  // [2][NW][NV]
+  double* dsum0 = dpart0 + 2 * NW * NV;                          // [2][NV]
+  T* gsm = (T*)(dsum0 + 2 * NV);                                 // [RC][KT]
   uint64_t* full = (uint64_t*)(gsm + RC * KT);                   // [NS]
   __shared__ T Ri[KT * KT];
   __shared__ int sidx[KT];
@@ -146,10 +153,10 @@ det_update_tma_kernel(State st, int k, int NS) {
       for (int a = 0; a < KT; ++a)
 #pragma unroll
         for (int t = 0; t < TV; ++t) {
-          const int q = warp * 32 + lane + 256 * t;
+          const int q = warp * 32 + lane + 32 * NW * t;
           const bool ok = a < k && q < nvec;
           nreg[a][t] = ok ? gN[(size_t)a * nvec + q] : make_double2(0.0, 0.0);
-          creg[a][t] = ok ? gC[(size_t)a * nvec + q] : make_double2(0.0, 0.0);
+          if (!APPEND) creg[a][t] = ok ? gC[(size_t)a * nvec + q] : make_double2(0.0, 0.0);
         }
       if (tid < KT * KT) {
         const int a = tid / KT, b = tid % KT;
@@ -161,9 +168,11 @@ det_update_tma_kernel(State st, int k, int NS) {
       __syncthreads();
     }
     if (tid == 0 && li + NS - 2 < my) {
-      tma::store_wait_read<1>();   // the stage consumed two chunks ago has been read out
+      if (!APPEND) tma::store_wait_read<1>();   // the stage consumed two chunks ago has been read out
       issue(li + NS - 2);
     }
+    double* dpart = dpart0 + (li & 1) * NW * NV;   // double-buffered by chunk parity
+    double* dsum = dsum0 + (li & 1) * NV;
     tma::mbar_wait(&full[stg], (uint32_t)((li / NS) & 1));
     T* xs = stage_buf + (size_t)stg * chunk_elems;
 
@@ -175,7 +184,7 @@ det_update_tma_kernel(State st, int k, int NS) {
       for (int a = 0; a < KT; ++a) d[r][a] = S::zero();
 #pragma unroll
     for (int t = 0; t < TV; ++t) {
-      const int q = warp * 32 + lane + 256 * t;
+      const int q = warp * 32 + lane + 32 * NW * t;
       if (q < nvec) {
 #pragma unroll
         for (int r = 0; r < RC; ++r) {
@@ -198,25 +207,35 @@ det_update_tma_kernel(State st, int k, int NS) {
       if (multi_writer<NV>(lane)) dpart[warp * NV + multi_index<NV>(lane)] = v[0];
     }
     __syncthreads();
-    // ---- g[r][a] = sum_b Ri[a][b] (d[r][b] - [j0 + r == P[b]])
+    // ---- cross-warp sum of the partials: one thread per value, then (a second short
+    // phase) g[r][a] = sum_b Ri[a][b] (d[r][b] - [j0 + r == P[b]])
+    if (tid < NV) {
+      double v = 0.0;
+#pragma unroll
+      for (int c = 0; c < NW; ++c) v += dpart[c * NV + tid];
+      dsum[tid] = v;
+    }
+    __syncthreads();
     if (tid < RC * KT) {
       const int r = tid / KT, a = tid % KT;
-      T acc = S::zero();
-#pragma unroll
-      for (int b = 0; b < KT; ++b) {
-        double re = 0.0, im = 0.0;
-#pragma unroll
-        for (int c = 0; c < NW; ++c) {
-          const double* p = dpart + c * NV + (r * KT + b) * ND;
-          re += p[0];
-          if (ND == 2) im += p[ND - 1];
+      if constexpr (APPEND) {
+        if (a < k && r < rows) {
+          T db = sc_from(dsum[(r * KT + a) * ND], dsum[(r * KT + a) * ND + ND - 1], T{});
+          if (j0 + r == sidx[a]) db = S::sub(db, S::one());
+          ((T*)st.pend_C)[((size_t)w * kmax + a) * n + j0 + r] = db;
         }
-        T db = sc_from(re, im, T{});
-        if (j0 + r == sidx[b]) db = S::sub(db, S::one());
-        acc = S::fma(Ri[a * KT + b], db, acc);
+      } else {
+        T acc = S::zero();
+#pragma unroll
+        for (int b = 0; b < KT; ++b) {
+          T db = sc_from(dsum[(r * KT + b) * ND], dsum[(r * KT + b) * ND + ND - 1], T{});
+          if (j0 + r == sidx[b]) db = S::sub(db, S::one());
+          acc = S::fma(Ri[a * KT + b], db, acc);
+        }
+        gsm[r * KT + a] = acc;
       }
-      gsm[r * KT + a] = acc;
     }
+    if constexpr (APPEND) continue;   // dsum / dpart are double-buffered by chunk parity
     __syncthreads();
     // ---- x[r][i] -= sum_a g[r][a] C[a][i] on this lane's columns, in place
     {
@@ -227,7 +246,7 @@ det_update_tma_kernel(State st, int k, int NS) {
         for (int a = 0; a < KT; ++a) g[r][a] = gsm[r * KT + a];
 #pragma unroll
       for (int t = 0; t < TV; ++t) {
-        const int q = warp * 32 + lane + 256 * t;
+        const int q = warp * 32 + lane + 32 * NW * t;
         if (q < nvec) {
 #pragma unroll
           for (int r = 0; r < RC; ++r) {
@@ -249,66 +268,139 @@ det_update_tma_kernel(State st, int k, int NS) {
       tma::store_commit();
     }
   }
-  if (tid == 0) tma::store_wait_all<0>();
+  if (!APPEND && tid == 0) tma::store_wait_all<0>();
 }
 
-template <typename T, int KT, int RC, int TV>
+// b_tau^T = R^-1 (D - (N Abuf) Bbuf^T) -> Bbuf[fill .. fill+k)   (Eq. 15, PAPER.md:194;
+// DESIGN.md reading 5b).  Work item = (accepted walker, 256 columns); thread per column.
+template <typename T, int KT>
+__global__ void __launch_bounds__(256) det_append_finish_kernel(State st, int k, int chunks) {
+  using S = Sc<T>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* NAs = (T*)smem_raw;   // [fill][KT]
+  __shared__ T Ri[KT * KT];
+  const int n = st.n, kmax = st.kmax, cap = st.cap;
+  const int tid = threadIdx.x;
+  const int count = st.counters[0];
+  for (int item = blockIdx.x; item < count * chunks; item += gridDim.x) {
+    const int w = st.list[item / chunks];
+    const int j = (item % chunks) * 256 + tid;
+    const int fill = st.fill[w];
+    __syncthreads();
+    const T* NA = (const T*)st.pend_Y + (size_t)w * kmax * cap;
+    for (int q = tid; q < fill * KT; q += 256)
+      NAs[q] = (q % KT) < k ? NA[(size_t)(q % KT) * cap + q / KT] : S::zero();
+    if (tid < KT * KT) {
+      const int a = tid / KT, b = tid % KT;
+      Ri[tid] = (a < k && b < k) ? ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + a * st.kc + b]
+                                 : S::zero();
+    }
+    __syncthreads();
+    if (j >= n) continue;
+    const T* D = (const T*)st.pend_C + (size_t)w * kmax * n;
+    T* Bb = (T*)st.Bbuf + (size_t)w * cap * n;
+    T m[KT];
+#pragma unroll
+    for (int b = 0; b < KT; ++b) m[b] = b < k ? D[(size_t)b * n + j] : S::zero();
+#pragma unroll 8
+    for (int s = 0; s < fill; ++s) {
+      const T bv = Bb[(size_t)s * n + j];
+#pragma unroll
+      for (int b = 0; b < KT; ++b) m[b] = S::fnma(NAs[s * KT + b], bv, m[b]);
+    }
+#pragma unroll
+    for (int a = 0; a < KT; ++a) {
+      if (a < k) {
+        T acc = S::zero();
+#pragma unroll
+        for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], m[b], acc);
+        Bb[(size_t)(fill + a) * n + j] = acc;
+      }
+    }
+  }
+}
+
+template <typename T, int KT, int RC, int TV, bool APPEND, int NW>
 static int launch_tma_inst(const State& st, int k, int num_sms, cudaStream_t s) {
   constexpr int ND = sizeof(T) / 8;
-  if constexpr (RC * KT * ND > 32 || KT * TV > 16) {
+  if constexpr (RC * KT * ND > 32 || KT * TV > (APPEND ? 16 : NW == 16 ? 8 : 16)) {
     return 0;   // too many partial sums / cached registers for this instance
   } else {
     const size_t row = (size_t)st.n * sizeof(T);
-    const size_t fixed = 8 * (size_t)(RC * KT * ND) * 8 + (size_t)RC * KT * sizeof(T) + 64 + 256;
+    const size_t fixed = 2 * (NW + 1) * (size_t)(RC * KT * ND) * 8 + (size_t)RC * KT * sizeof(T) + 64 + 256;
     int NS = (int)((220 * 1024 - fixed) / ((size_t)RC * row));
     if (NS > 8) NS = 8;
     if (NS < 3) return 0;
     const size_t smem = (size_t)NS * RC * row + fixed;
-    auto kern = det_update_tma_kernel<T, KT, RC, TV>;
+    auto kern = det_update_tma_kernel<T, KT, RC, TV, APPEND, NW>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
       return -1;
-    kern<<<num_sms, 256, smem, s>>>(st, k, NS);
-    return 1;
+    kern<<<num_sms, NW * 32, smem, s>>>(st, k, NS);
+    if (!APPEND) return 1;
+    const int chunks = (st.n + 255) / 256;
+    int64_t grid = (int64_t)num_sms * 8;
+    if (grid > st.W * chunks) grid = st.W * chunks;
+    det_append_finish_kernel<T, KT><<<(unsigned)grid, 256, (size_t)st.cap * KT * sizeof(T), s>>>(st, k, chunks);
+    return 2;
   }
 }
 
 // Returns the number of launches (1), 0 when this shape is not eligible (caller falls
 // back to the register-row / generic kernels), -1 on a CUDA error.
-template <typename T, int KT>
+template <typename T, int KT, bool APPEND>
 static int launch_update_tma_kt(const State& st, int k, int num_sms, cudaStream_t s) {
   const size_t row = (size_t)st.n * sizeof(T);
   if (row % 16 != 0) return 0;
   const int nvec = (int)(row / 16);
-  const int tv = (nvec + 255) / 256;            // vectors per lane
   // rows per chunk: ~32 KB per bulk copy
   const int rc = row >= 32 * 1024 ? 1 : row >= 16 * 1024 ? 2 : 4;
-#define LRUX_TMA_CASE(RC_, TV_) \
-  if (rc == RC_ && tv <= TV_) return launch_tma_inst<T, KT, RC_, TV_>(st, k, num_sms, s)
-  LRUX_TMA_CASE(4, 1);
-  LRUX_TMA_CASE(4, 2);
-  LRUX_TMA_CASE(4, 4);
-  LRUX_TMA_CASE(2, 2);
-  LRUX_TMA_CASE(2, 4);
-  LRUX_TMA_CASE(1, 4);
-  LRUX_TMA_CASE(1, 8);
+  // 16 warps when a lane would otherwise own >= 2 vectors of a row: more warps to cover
+  // the FP64 / shared-memory latency of the per-chunk arithmetic
+  const int tv8 = (nvec + 255) / 256, tv16 = (nvec + 511) / 512;
+#define LRUX_TMA_CASE(RC_, TV_, NW_)                                                       \
+  if (rc == RC_ && (NW_ == 16 ? tv16 : tv8) <= TV_) {                                      \
+    const int r_ = launch_tma_inst<T, KT, RC_, TV_, APPEND, NW_>(st, k, num_sms, s);       \
+    if (r_ != 0) return r_;                                                                \
+  }
+  const char* warps_env = getenv("LRUX_TMA_WARPS");   // A-B measurements only
+  if (tv8 >= 2 && KT <= 2 && !(warps_env && warps_env[0] == '8')) {
+    LRUX_TMA_CASE(4, 1, 16)
+    LRUX_TMA_CASE(4, 2, 16)
+    LRUX_TMA_CASE(2, 2, 16)
+    LRUX_TMA_CASE(1, 2, 16)
+    LRUX_TMA_CASE(1, 4, 16)
+  }
+  LRUX_TMA_CASE(4, 1, 8)
+  LRUX_TMA_CASE(4, 2, 8)
+  LRUX_TMA_CASE(4, 4, 8)
+  LRUX_TMA_CASE(2, 2, 8)
+  LRUX_TMA_CASE(2, 4, 8)
+  LRUX_TMA_CASE(1, 4, 8)
+  LRUX_TMA_CASE(1, 8, 8)
 #undef LRUX_TMA_CASE
   return 0;
 }
 
-template <typename T>
+template <typename T, bool APPEND>
 static int launch_update_tma_t(const State& st, int k, int num_sms, cudaStream_t s) {
   const int kt = k <= 1 ? 1 : k <= 2 ? 2 : k <= 4 ? 4 : 8;
   switch (kt) {
-    case 1: return launch_update_tma_kt<T, 1>(st, k, num_sms, s);
-    case 2: return launch_update_tma_kt<T, 2>(st, k, num_sms, s);
-    case 4: return launch_update_tma_kt<T, 4>(st, k, num_sms, s);
-    default: return launch_update_tma_kt<T, 8>(st, k, num_sms, s);
+    case 1: return launch_update_tma_kt<T, 1, APPEND>(st, k, num_sms, s);
+    case 2: return launch_update_tma_kt<T, 2, APPEND>(st, k, num_sms, s);
+    case 4: return launch_update_tma_kt<T, 4, APPEND>(st, k, num_sms, s);
+    default: return launch_update_tma_kt<T, 8, APPEND>(st, k, num_sms, s);
   }
 }
 
 int launch_det_update_tma(const State& st, int k, int num_sms, cudaStream_t s) {
-  return st.dt == LRUX_F64 ? launch_update_tma_t<double>(st, k, num_sms, s)
-                           : launch_update_tma_t<cplx>(st, k, num_sms, s);
+  return st.dt == LRUX_F64 ? launch_update_tma_t<double, false>(st, k, num_sms, s)
+                           : launch_update_tma_t<cplx, false>(st, k, num_sms, s);
+}
+
+// delayed append through the same pass (after det_prep_kernel): 2 launches, 0 = not eligible
+int launch_det_append_tma(const State& st, int k, int num_sms, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? launch_update_tma_t<double, true>(st, k, num_sms, s)
+                           : launch_update_tma_t<cplx, true>(st, k, num_sms, s);
 }
 
 }  // namespace lrux

@@ -83,17 +83,32 @@ def test_pf_config3_shape_reduced():
     _run("pf", wl.BASE_SEED + 3, 24, 128, 256, 1, 0, 80, walkers=[0, 7, 15, 23])
 
 
-@pytest.mark.parametrize("n,k,cplx,steps", [
-    (1024, 4, False, 10),     # rows of 8 KB: RC=4 rows per bulk copy, 2 vectors per lane
-    (1024, 8, False, 8),      # k=8: 32 partial sums per warp
-    (1100, 1, False, 10),     # ragged: 550 vectors per row, 4-row chunks with a 3-row tail
-    (512, 2, True, 10),       # complex128, 8 KB rows
-    (2048, 2, False, 4),      # 16 KB rows: RC=2, 4 vectors per lane
+@pytest.mark.parametrize("n,k,K,cplx,steps", [
+    (1024, 4, 0, False, 10),     # rows of 8 KB: RC=4 rows per bulk copy, 2 vectors per lane
+    (1024, 8, 0, False, 8),      # k=8: 32 partial sums per warp
+    (1100, 1, 0, False, 10),     # ragged: 550 vectors per row, 4-row chunks with a 3-row tail
+    (512, 2, 0, True, 10),       # complex128, 8 KB rows
+    (2048, 2, 0, False, 4),      # 16 KB rows: RC=2, 4 vectors per lane
+    (1024, 2, 3, False, 14),     # delayed append through the same pass + finish kernel
+    (512, 4, 2, True, 12),       # complex128 delayed (configs[3] shape at n=512)
 ])
-def test_det_tma_update_path(n, k, cplx, steps):
-    """Immediate update through the TMA-staged kernel (lrux_det_tma.cu)."""
-    _run("det", 500 + n + k, 2, n, 2 * n, k, 0, steps, cplx, walkers=[1],
-         scratch_every=0 if n >= 2048 else steps - 1)
+def test_det_tma_update_path(n, k, K, cplx, steps):
+    """Immediate update / delayed append through the TMA-staged kernel (lrux_det_tma.cu).
+    The delayed variant is opt-in (LRUX_UPDATE_PATH=tma), see launch_append_kt."""
+    import os
+
+    old = os.environ.get("LRUX_UPDATE_PATH")
+    if K > 0:
+        os.environ["LRUX_UPDATE_PATH"] = "tma"
+    try:
+        _run("det", 500 + n + k, 2, n, 2 * n, k, K, steps, cplx, walkers=[1],
+             scratch_every=0 if n >= 2048 else steps - 1)
+    finally:
+        if K > 0:
+            if old is None:
+                del os.environ["LRUX_UPDATE_PATH"]
+            else:
+                os.environ["LRUX_UPDATE_PATH"] = old
 
 
 def test_det_tma_update_n4096_properties():
