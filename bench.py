@@ -33,7 +33,7 @@ WORKLOADS = {
     # BASELINE.json configs[1]: the configuration the metric is quoted on
     "c2": dict(kind="det", cplx=False, W=4096, n=256, M=512, k=2, Ks=(0, 16), cfg=2,
                desc="configs[1]: det f64, 4096 walkers, n=256, M=512, k=2, Metropolis; K=0 vs K=16"),
-    "c3": dict(kind="pf", cplx=False, W=1024, n=128, M=256, k=1, Ks=(0,), cfg=3,
+    "c3": dict(kind="pf", cplx=False, W=1024, n=128, M=256, k=1, Ks=(0, 4), cfg=3,
                desc="configs[2]: pf f64, 1024 walkers, n=128, M=256, k=1, Metropolis"),
     "c4": dict(kind="det", cplx=True, W=512, n=1024, M=2048, k=4, Ks=(32,), cfg=4,
                desc="configs[3]: det c128, 512 walkers, n=1024, M=2048, k=4, K=32, Metropolis"),
@@ -408,7 +408,12 @@ def roofline_update(wk, run, peak, peak_src):
         return None
     byts = 2.0 * wk["n"] ** 2 * esz * run["accepted"]
     ach = byts / (pr["ms"] * 1e-3) / 1e9
-    kern = "%s_update_kernel" % wk["kind"]
+    rowb = wk["n"] * esz
+    if wk["kind"] == "det":
+        kern = "det_update_tma_kernel" if (rowb >= 8192 and rowb % 16 == 0) else "det_update_kernel"
+    else:
+        resident = (wk["n"] ** 2 + (4 * wk["k"] + 1) * wk["n"]) * esz <= 200 * 1024
+        kern = "pf_resident_update_kernel" if resident else "pf_update_stream_kernel"
     tpw = ncu_traffic_per_walker(kern, wk.get("name", ""))
     traffic = tpw * run["accepted"] / pr["launches"] if tpw else None
     return {"bound": "hbm", "kernel": kern, "achieved": ach, "peak": peak,
