@@ -138,22 +138,69 @@ pf_y_kernel(State st, int k, int tiles, int rows_per_tile, int use_list) {
     const T* Tw = (const T*)st.Ti + (size_t)w * n * n;
     const int i_beg = tile * rows_per_tile, i_end = min(n, i_beg + rows_per_tile);
     __syncthreads();
-    for (int i = i_beg + warp; i < i_end; i += nw) {
-      const T* row = Tw + (size_t)i * n;
-      T d[KT];
+    // two rows per warp pass, 16-byte loads, 8 loads in flight per thread
+    constexpr int RW = 2, U = 4;
+    constexpr int VE = sizeof(T) == 8 ? 2 : 1;     // elements per 16-byte vector
+    const bool vec = (n % VE) == 0;
+    for (int i0 = i_beg + warp * RW; i0 < i_end; i0 += nw * RW) {
+      T d[RW][KT];
 #pragma unroll
-      for (int a = 0; a < KT; ++a) d[a] = S::zero();
-      for (int j = lane; j < n; j += 32) {
-        const T x = row[j];
+      for (int r = 0; r < RW; ++r)
 #pragma unroll
-        for (int a = 0; a < KT; ++a)
-          if (a < k) d[a] = S::fma(x, gN[(size_t)a * n + j], d[a]);
+        for (int a = 0; a < KT; ++a) d[r][a] = S::zero();
+      if (vec) {
+        const int nvec = n / VE;
+        for (int q0 = lane; q0 < nvec; q0 += 32 * U) {
+          double2 x[U][RW];
+#pragma unroll
+          for (int u = 0; u < U; ++u)
+#pragma unroll
+            for (int r = 0; r < RW; ++r)
+              x[u][r] = (q0 + 32 * u < nvec && i0 + r < i_end)
+                            ? ((const double2*)(Tw + (size_t)(i0 + r) * n))[q0 + 32 * u]
+                            : make_double2(0.0, 0.0);
+#pragma unroll
+          for (int u = 0; u < U; ++u) {
+            const int q = q0 + 32 * u;
+            if (q < nvec) {
+#pragma unroll
+              for (int a = 0; a < KT; ++a) {
+                if (a < k) {
+                  const double2 nv = ((const double2*)(gN + (size_t)a * n))[q];
+#pragma unroll
+                  for (int r = 0; r < RW; ++r) {
+                    if constexpr (VE == 2) {
+                      d[r][a] = S::fma(sc_from(x[u][r].x, 0.0, T{}), sc_from(nv.x, 0.0, T{}), d[r][a]);
+                      d[r][a] = S::fma(sc_from(x[u][r].y, 0.0, T{}), sc_from(nv.y, 0.0, T{}), d[r][a]);
+                    } else {
+                      d[r][a] = S::fma(sc_from(x[u][r].x, x[u][r].y, T{}), sc_from(nv.x, nv.y, T{}), d[r][a]);
+                    }
+                  }
+                }
+              }
+            }
+          }
+        }
+      } else {
+        for (int j = lane; j < n; j += 32) {
+#pragma unroll
+          for (int r = 0; r < RW; ++r) {
+            if (i0 + r < i_end) {
+              const T x = Tw[(size_t)(i0 + r) * n + j];
+#pragma unroll
+              for (int a = 0; a < KT; ++a)
+                if (a < k) d[r][a] = S::fma(x, gN[(size_t)a * n + j], d[r][a]);
+            }
+          }
+        }
       }
 #pragma unroll
-      for (int a = 0; a < KT; ++a) {
-        d[a] = warp_sum(d[a]);
-        if (lane == 0) dsm[a * rows_per_tile + (i - i_beg)] = d[a];
-      }
+      for (int r = 0; r < RW; ++r)
+#pragma unroll
+        for (int a = 0; a < KT; ++a) {
+          const T v = warp_sum(d[r][a]);
+          if (lane == 0 && i0 + r < i_end) dsm[a * rows_per_tile + (i0 + r - i_beg)] = v;
+        }
     }
     __syncthreads();
     const T* AN = cap ? (const T*)st.pend_AN + (size_t)w * kmax * cap : nullptr;

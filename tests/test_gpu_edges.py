@@ -1,0 +1,128 @@
+"""Edge cases of the CUDA path against the oracle's plain definitions: degenerate sizes,
+nothing accepted, variable k under one handle, a second ratio replacing the pending one,
+explicit flush, get_inverse with a half-full delay buffer."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import lrux_oracle as orc
+from paper_2602_05255_b200 import lrux
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def _t(x, dtype=None):
+    return torch.as_tensor(np.ascontiguousarray(x), device=DEV, dtype=dtype)
+
+
+def _replace_rows(A, idx, rows):
+    B = A.copy()
+    B[idx, :] = rows
+    return B
+
+
+@pytest.mark.parametrize("n,k", [(1, 1), (2, 2), (8, 8), (3, 1)])
+def test_det_degenerate_sizes(n, k):
+    """n = 1, k = n (every row replaced at once), odd n."""
+    rng = np.random.default_rng(n * 10 + k)
+    W = 3
+    A = rng.standard_normal((W, n, n)) + 2 * np.eye(n)
+    wk = lrux.DetWalkers(_t(A), kmax=k)
+    idx = np.stack([rng.permutation(n)[:k] for _ in range(W)]).astype(np.int32)
+    rows = rng.standard_normal((W, k, n))
+    r = wk.ratio_(_t(idx), _t(rows)).cpu().numpy()
+    wk.accept(torch.ones(W, dtype=torch.uint8, device=DEV))
+    inv = wk.get_inverse().cpu().numpy()
+    ph, la = wk.get_amplitude()
+    for w in range(W):
+        B = _replace_rows(A[w], idx[w], rows[w])
+        assert r[w] == pytest.approx(orc.det(B) / orc.det(A[w]), rel=1e-10)
+        assert np.abs(B @ inv[w] - np.eye(n)).max() < 1e-9
+        sph, sla = orc.slogdet(B)
+        assert la[w].item() == pytest.approx(sla, abs=1e-10 * max(1, abs(sla)))
+        assert ph[w].item() == sph
+
+
+@pytest.mark.parametrize("K", [0, 3])
+def test_nothing_accepted_and_single_walker(K):
+    """mask = 0 everywhere (empty work lists in every accept kernel), W = 1."""
+    rng = np.random.default_rng(5)
+    n, k = 20, 2
+    A = rng.standard_normal((1, n, n))
+    wk = lrux.DetWalkers(_t(A), kmax=k, K=K)
+    before = wk.get_inverse().cpu().numpy()
+    for _ in range(4):
+        idx = rng.permutation(n)[:k].astype(np.int32)[None]
+        wk.ratio_(_t(idx), _t(rng.standard_normal((1, k, n))))
+        wk.accept(torch.zeros(1, dtype=torch.uint8, device=DEV))
+    wk.flush()
+    assert np.array_equal(wk.get_inverse().cpu().numpy(), before)
+    assert wk.info.cpu().tolist() == [0]
+
+
+def test_variable_k_second_ratio_and_explicit_flush():
+    """One handle (kmax = 4, K = 3): proposals of k = 1, 4, 2, 3 rows; a second ratio
+    before accept replaces the pending proposal; get_inverse folds a half-full buffer;
+    every ratio and the final inverse against the oracle's plain definitions."""
+    rng = np.random.default_rng(9)
+    W, n, kmax = 4, 24, 4
+    A = rng.standard_normal((W, n, n))
+    cur = A.copy()
+    wk = lrux.DetWalkers(_t(A), kmax=kmax, K=3)
+    logabs = np.array([orc.slogdet(A[w])[1] for w in range(W)])
+    for step, k in enumerate([1, 4, 2, 3, 1, 2]):
+        # a throw-away proposal first: must leave no trace
+        idx0 = np.stack([rng.permutation(n)[:k] for _ in range(W)]).astype(np.int32)
+        wk.ratio_(_t(idx0), _t(rng.standard_normal((W, k, n))))
+        idx = np.stack([rng.permutation(n)[:k] for _ in range(W)]).astype(np.int32)
+        rows = rng.standard_normal((W, k, n))
+        r = wk.ratio_(_t(idx), _t(rows)).cpu().numpy()
+        mask = (rng.random(W) < 0.7).astype(np.uint8)
+        wk.accept(_t(mask))
+        for w in range(W):
+            B = _replace_rows(cur[w], idx[w], rows[w])
+            assert r[w] == pytest.approx(orc.det(B) / orc.det(cur[w]), rel=1e-9)
+            if mask[w]:
+                cur[w] = B
+                logabs[w] += np.log(abs(r[w]))
+        if step == 3:
+            wk.flush()                      # explicit flush in the middle
+    inv = wk.get_inverse().cpu().numpy()     # implies flush of whatever is buffered
+    _, la = wk.get_amplitude()
+    for w in range(W):
+        assert np.abs(cur[w] @ inv[w] - np.eye(n)).max() < 1e-9
+        assert la[w].item() == pytest.approx(orc.slogdet(cur[w])[1], abs=1e-9)
+    assert not wk.info.cpu().numpy().any()
+
+
+def test_pf_degenerate_and_k_equals_half_n():
+    """Pfaffian: n = 2 (k = 1 replaces the only pair), n = 8 with k = 4."""
+    rng = np.random.default_rng(21)
+    for n, k in ((2, 1), (8, 4), (6, 2)):
+        W, M = 3, 2 * n + 2
+        g = rng.standard_normal((W, M, M))
+        F = np.triu(g, 1) - np.triu(g, 1).transpose(0, 2, 1)
+        occ = np.stack([rng.permutation(M)[:n] for _ in range(W)])
+        A = np.stack([F[w][np.ix_(occ[w], occ[w])] for w in range(W)])
+        wk = lrux.PfWalkers(_t(A), kmax=k)
+        idx = np.stack([rng.permutation(n)[:k] for _ in range(W)]).astype(np.int32)
+        newocc = occ.copy()
+        for w in range(W):
+            free = [o for o in range(M) if o not in occ[w]]
+            newocc[w, idx[w]] = rng.permutation(free)[:k]
+        B = np.stack([F[w][np.ix_(newocc[w], newocc[w])] for w in range(W)])
+        rows = np.stack([B[w][idx[w], :] for w in range(W)])
+        r = wk.ratio_(_t(idx), _t(rows)).cpu().numpy()
+        wk.accept(torch.ones(W, dtype=torch.uint8, device=DEV))
+        inv = wk.get_inverse().cpu().numpy()
+        for w in range(W):
+            assert r[w] == pytest.approx(orc.pf(B[w]) / orc.pf(A[w]), rel=1e-9)
+            assert np.abs(B[w] @ inv[w] - np.eye(n)).max() < 1e-8
+            assert np.array_equal(inv[w], -inv[w].T)
+
+
+def test_delay_depth_limit_is_reported():
+    with pytest.raises(lrux.LruxError) as e:
+        lrux.DetWalkers(torch.eye(16, dtype=torch.complex128, device=DEV)[None], kmax=8, K=64)
+    assert e.value.status == lrux.EUNSUPPORTED
