@@ -443,6 +443,7 @@ pf_update_stream_kernel(State st, int k, int tiles, int rows_per_tile) {
 template <typename T>
 __global__ void __launch_bounds__(512) pf_resident_update_kernel(State st, int k, int need_y) {
   using S = Sc<T>;
+  constexpr int NCH = 4;                // row chunks per walker, one bulk copy + mbarrier each
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int n = st.n, kmax = st.kmax, m = 2 * k;
   T* Ts = (T*)smem_raw;                 // [n][n]
@@ -451,23 +452,29 @@ __global__ void __launch_bounds__(512) pf_resident_update_kernel(State st, int k
   T* nv = gv + (size_t)m * n;           // [n]     new row (k = 1)
   __shared__ T Ri[kMaxC * kMaxC];
   __shared__ int P[kMaxK];
-  __shared__ __align__(8) uint64_t bar;
+  __shared__ __align__(8) uint64_t bar[NCH];
   const int tid = threadIdx.x, nt = blockDim.x, warp = tid >> 5, lane = tid & 31, nw = nt >> 5;
   const int count = st.counters[0];
-  const uint32_t bytes = (uint32_t)((size_t)n * n * sizeof(T));
+  const int rpc = (n + NCH - 1) / NCH;  // rows per chunk
   if (tid == 0) {
-    tma::mbar_init(&bar, 1);
+    for (int c = 0; c < NCH; ++c) tma::mbar_init(&bar[c], 1);
     tma::fence_barrier_init();
   }
   __syncthreads();
+  auto load_chunk = [&](int w, int c) {   // thread 0 only
+    const int r0 = c * rpc, rows = min(rpc, n - r0);
+    if (rows <= 0) return;
+    const uint32_t bytes = (uint32_t)((size_t)rows * n * sizeof(T));
+    tma::mbar_arrive_expect_tx(&bar[c], bytes);
+    tma::load(Ts + (size_t)r0 * n, (const T*)st.Ti + (size_t)w * n * n + (size_t)r0 * n, bytes, &bar[c]);
+  };
+  if (tid == 0 && (int)blockIdx.x < count)
+    for (int c = 0; c < NCH; ++c) load_chunk(st.list[blockIdx.x], c);
   uint32_t phase = 0;
   for (int it = blockIdx.x; it < count; it += gridDim.x) {
     const int w = st.list[it];
+    const int w_next = it + (int)gridDim.x < count ? st.list[it + gridDim.x] : -1;
     T* Tw = (T*)st.Ti + (size_t)w * n * n;
-    if (tid == 0) {
-      tma::mbar_arrive_expect_tx(&bar, bytes);
-      tma::load(Ts, Tw, bytes, &bar);
-    }
     const T* pC = (const T*)st.pend_C + (size_t)w * kmax * n;
     const T* pY = (const T*)st.pend_Y + (size_t)w * kmax * n;
     const T* pN = (const T*)st.pend_N + (size_t)w * kmax * n;
@@ -483,17 +490,22 @@ __global__ void __launch_bounds__(512) pf_resident_update_kernel(State st, int k
       else yv[q] = (i == P[a]) ? S::add(pY[q], S::one()) : pY[q];
     }
     __syncthreads();
-    tma::mbar_wait(&bar, phase);
-    phase ^= 1;
-    if (need_y) {
-      for (int i = warp; i < n; i += nw) {
-        T acc = S::zero();
-        for (int j = lane; j < n; j += 32) acc = S::fma(Ts[(size_t)i * n + j], nv[j], acc);
-        acc = warp_sum(acc);
-        if (lane == 0) yv[i] = (i == P[0]) ? S::add(acc, S::one()) : acc;
+    // ---- Y = A^-1 N row by row, chunk by chunk as the bulk copies land (k = 1)
+    for (int c = 0; c < NCH; ++c) {
+      const int r0 = c * rpc, r1 = min(n, r0 + rpc);
+      if (r0 >= n) break;
+      tma::mbar_wait(&bar[c], phase);
+      if (need_y) {
+        for (int i = r0 + warp; i < r1; i += nw) {
+          T acc = S::zero();
+          for (int j = lane; j < n; j += 32) acc = S::fma(Ts[(size_t)i * n + j], nv[j], acc);
+          acc = warp_sum(acc);
+          if (lane == 0) yv[i] = (i == P[0]) ? S::add(acc, S::one()) : acc;
+        }
       }
-      __syncthreads();
     }
+    phase ^= 1;
+    __syncthreads();
     for (int q = tid; q < m * n; q += nt) {
       const int beta = q / n, i = q % n;
       T g = S::zero();
@@ -502,39 +514,51 @@ __global__ void __launch_bounds__(512) pf_resident_update_kernel(State st, int k
       gv[q] = g;
     }
     __syncthreads();
-    // one warp per row, lanes over columns; row-dependent factors hoisted
-    for (int r = warp; r < n; r += nw) {
-      T* row = Ts + (size_t)r * n;
-      if (m == 2) {
-        const T g0r = gv[r], g1r = gv[n + r], y0r = yv[r], y1r = yv[n + r];
-        for (int c = lane; c < n; c += 32) {
-          const bool up = r < c;
-          const T x = row[c];
-          T v = up ? x : S::neg(x);
-          v = S::fma(up ? g0r : gv[c], up ? yv[c] : y0r, v);
-          v = S::fma(up ? g1r : gv[n + c], up ? yv[n + c] : y1r, v);
-          row[c] = (r == c) ? S::zero() : (up ? v : S::neg(v));
+    // ---- rank-2k update chunk by chunk; each finished chunk is stored at once and its
+    // shared memory refilled with the same chunk of this CTA's next walker
+    for (int c = 0; c < NCH; ++c) {
+      const int r0 = c * rpc, r1 = min(n, r0 + rpc);
+      if (r0 >= n) break;
+      for (int r = r0 + warp; r < r1; r += nw) {
+        T* row = Ts + (size_t)r * n;
+        if (m == 2) {
+          const T g0r = gv[r], g1r = gv[n + r], y0r = yv[r], y1r = yv[n + r];
+          for (int cc = lane; cc < n; cc += 32) {
+            const bool up = r < cc;
+            const T x = row[cc];
+            T v = up ? x : S::neg(x);
+            v = S::fma(up ? g0r : gv[cc], up ? yv[cc] : y0r, v);
+            v = S::fma(up ? g1r : gv[n + cc], up ? yv[n + cc] : y1r, v);
+            row[cc] = (r == cc) ? S::zero() : (up ? v : S::neg(v));
+          }
+        } else {
+          for (int cc = lane; cc < n; cc += 32) {
+            const bool up = r < cc;
+            const int i = up ? r : cc, j = up ? cc : r;
+            const T x = row[cc];
+            T v = up ? x : S::neg(x);
+            for (int beta = 0; beta < m; ++beta) v = S::fma(gv[beta * n + i], yv[beta * n + j], v);
+            row[cc] = (r == cc) ? S::zero() : (up ? v : S::neg(v));
+          }
         }
-      } else {
-        for (int c = lane; c < n; c += 32) {
-          const bool up = r < c;
-          const int i = up ? r : c, j = up ? c : r;
-          const T x = row[c];
-          T v = up ? x : S::neg(x);
-          for (int beta = 0; beta < m; ++beta) v = S::fma(gv[beta * n + i], yv[beta * n + j], v);
-          row[c] = (r == c) ? S::zero() : (up ? v : S::neg(v));
+      }
+      tma::fence_proxy_async();
+      __syncthreads();
+      if (tid == 0) {
+        tma::store(Tw + (size_t)r0 * n, Ts + (size_t)r0 * n, (uint32_t)((size_t)(r1 - r0) * n * sizeof(T)));
+        tma::store_commit();
+        if (w_next >= 0 && c >= 1) {
+          tma::store_wait_read<1>();   // the previous chunk has left shared memory
+          load_chunk(w_next, c - 1);
         }
       }
     }
-    tma::fence_proxy_async();
-    __syncthreads();
-    if (tid == 0) {
-      tma::store(Tw, Ts, bytes);
-      tma::store_commit();
-      tma::store_wait_read<0>();   // Ts may be overwritten by the next walker's load
+    if (tid == 0 && w_next >= 0) {
+      tma::store_wait_read<0>();
+      load_chunk(w_next, (min(n, NCH * rpc) - 1) / rpc);   // last non-empty chunk
     }
-    __syncthreads();
   }
+  if (tid == 0) tma::store_wait_all<0>();
 }
 
 // ---------------------------------------------------------------- delayed append (a6)
