@@ -521,6 +521,44 @@ __global__ void __launch_bounds__(512) pf_resident_update_kernel(State st, int k
       if (r0 >= n) break;
       for (int r = r0 + warp; r < r1; r += nw) {
         T* row = Ts + (size_t)r * n;
+        if constexpr (sizeof(T) == 8) {
+          if (m == 2) {
+            // fp64, k = 1 (Eq. 22): pairs of columns; a pair entirely below / above the
+            // diagonal needs no per-element selection
+            const double g0r = gv[r], g1r = gv[n + r], y0r = yv[r], y1r = yv[n + r];
+            const double2* g0 = (const double2*)gv;
+            const double2* g1 = (const double2*)(gv + n);
+            const double2* y0 = (const double2*)yv;
+            const double2* y1 = (const double2*)(yv + n);
+            double2* row2 = (double2*)row;
+            for (int q = lane; q < n / 2; q += 32) {
+              const int c0 = 2 * q;
+              double2 x = row2[q];
+              if (c0 + 1 < r) {          // both below the diagonal: mirrored value, negated
+                const double2 a = g0[q], b = g1[q];
+                x.x = -fma(b.x, y1r, fma(a.x, y0r, -x.x));
+                x.y = -fma(b.y, y1r, fma(a.y, y0r, -x.y));
+              } else if (c0 > r) {       // both above
+                const double2 a = y0[q], b = y1[q];
+                x.x = fma(g1r, b.x, fma(g0r, a.x, x.x));
+                x.y = fma(g1r, b.y, fma(g0r, a.y, x.y));
+              } else {                   // the pair that holds the diagonal element
+                double e[2] = {x.x, x.y};
+#pragma unroll
+                for (int t = 0; t < 2; ++t) {
+                  const int cc = c0 + t;
+                  if (cc == r) e[t] = 0.0;
+                  else if (cc < r) e[t] = -fma(gv[n + cc], y1r, fma(gv[cc], y0r, -e[t]));
+                  else e[t] = fma(g1r, yv[n + cc], fma(g0r, yv[cc], e[t]));
+                }
+                x.x = e[0];
+                x.y = e[1];
+              }
+              row2[q] = x;
+            }
+            continue;
+          }
+        }
         if (m == 2) {
           const T g0r = gv[r], g1r = gv[n + r], y0r = yv[r], y1r = yv[n + r];
           for (int cc = lane; cc < n; cc += 32) {
