@@ -194,6 +194,7 @@ def timed_run(ch, warmup, steps, forced=False, sampler=None):
     torch.cuda.synchronize()
     acc0 = int(ch.naccept.item())
     l0 = ch.launches()
+    f0 = ch.walkers.flush_count() if ch.K > 0 else (0, 0)
     ch.walkers.profile_enable(True)
     for c in range(5):
         ch.walkers.profile_read(c)
@@ -221,7 +222,9 @@ def timed_run(ch, warmup, steps, forced=False, sampler=None):
         t_ms, cnt = ch.walkers.profile_read(c)
         prof[name] = {"ms": t_ms, "launches": cnt}
     ch.walkers.profile_enable(False)
+    f1 = ch.walkers.flush_count() if ch.K > 0 else (0, 0)
     return {"ms": ms, "accepted": int(ch.naccept.item()) - acc0, "launches": ch.launches() - l0,
+            "flushes": f1[0] - f0[0], "flush_cols": f1[1] - f0[1],
             "prof": prof, "clocks": clocks}
 
 
@@ -429,15 +432,21 @@ def roofline_flush(wk, K, run, hbm_peak, hbm_src, dgemm_tflops):
     25 (complex), HBM-bound below.  The tensor peak is the cuBLAS FP64
     GEMM measured in this same run (MEASURED_PEAKS.json carries no FP64 figure)."""
     fl = run["prof"]["flush"]
-    if K <= 0 or fl["ms"] <= 0 or run["accepted"] == 0:
+    if K <= 0 or fl["ms"] <= 0 or run.get("flush_cols", 0) <= 0:
         return None
     cx = wk["cplx"]
     esz = 16 if cx else 8
     n, k = wk["n"], wk["k"]
-    flops = 2.0 * n * n * k * (4 if cx else 1) * run["accepted"]
-    byts = (2.0 * n * n * esz / K + 2.0 * n * k * esz) * run["accepted"]
+    pf = wk["kind"] == "pf"
+    # exact counts from the library (lrux_get_flush_count): buffer columns folded and walker
+    # flushes inside the timed region.  det: 2 n^2 flops per column (x4 complex); pf: the upper
+    # triangle only, n^2 per column.  Bytes: 2 n^2 e per flushed walker + 2 n e per column.
+    cols, nfl = run["flush_cols"], run["flushes"]
+    flops = (1.0 if pf else 2.0) * n * n * cols * (4 if cx else 1)
+    byts = 2.0 * n * n * esz * nfl + 2.0 * n * esz * cols
     tf = flops / (fl["ms"] * 1e-3) / 1e12
     gbs = byts / (fl["ms"] * 1e-3) / 1e9
+    k = (2 * k) if pf else k      # inner dimension per update
     tensor = K * k >= (25 if cx else 50)
     out = {"kernel": "flush_dmma_kernel", "Kk": K * k, "tflops": tf, "gbs": gbs,
            "launches": fl["launches"], "ms": fl["ms"]}
@@ -549,11 +558,15 @@ def main(argv=None):
     if roof is None and "forced_accept" in extras and extras["forced_accept"]["roofline"]:
         roof = extras["forced_accept"]["roofline"]
     roof_append = None
-    if K0 > 0 and run["prof"]["append"]["ms"] > 0:
+    if K0 > 0 and run["prof"]["append"]["ms"] > 0 and not (wk["kind"] == "pf" and wk["k"] > 1):
         # delayed append (a6): one read-only pass over A0^-1 = n^2 e bytes per accepted walker
-        ap = run["prof"]["append"]
+        # (det: prep + append kernels; pf, k = 1: the Y pass + append kernel)
+        ap_ms = run["prof"]["append"]["ms"] + (run["prof"]["ypass"]["ms"] if wk["kind"] == "pf" else 0.0)
+        ap = {"ms": ap_ms}
         gbs = wk["n"] ** 2 * (16.0 if wk["cplx"] else 8.0) * run["accepted"] / (ap["ms"] * 1e-3) / 1e9
-        roof_append = {"bound": "hbm", "kernel": "det_prep_kernel+det_append_kernel", "achieved": gbs,
+        roof_append = {"bound": "hbm",
+                       "kernel": ("det_prep_kernel+det_append_kernel" if wk["kind"] == "det"
+                                  else "pf_y_kernel+pf_append_kernel"), "achieved": gbs,
                        "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
                        "peak_source": peak_src}
         if roof is None:   # the dominant kernel of a delayed configuration

@@ -151,6 +151,12 @@ lrux_status_t lrux_profile_enable(lrux_handle_t h, int32_t on);
 lrux_status_t lrux_profile_read(lrux_handle_t h, int32_t cls, double* ms_total,
                                 int64_t* launches);
 
+/* Running totals of the delay-buffer folds since init (or since the state the handle
+ * was attached to was initialised): d_out[0] = walker flushes, d_out[1] = buffer columns
+ * folded (k per determinant update, 2k per Pfaffian update).  d_out is DEVICE memory,
+ * 2 x int64; stream-ordered copy.  bench.py uses it to count the flush flops exactly. */
+lrux_status_t lrux_get_flush_count(lrux_handle_t h, int64_t* d_out, void* stream);
+
 /* ---------------------------------------------------------------- common */
 /* Number of kernel launches the library has enqueued through this handle so far
  * (host counter; bench.py reports it as gpu_launches). */

@@ -47,9 +47,14 @@ size_t state_layout(State* st, void* base, int64_t W, int32_t n, int32_t kmax, i
   }
   s.Abuf = cap ? take((size_t)W * cap * n * e) : nullptr;
   s.Bbuf = cap ? take((size_t)W * cap * n * e) : nullptr;
+  if (n >= kBlockedInitMin) {
+    s.init_A = take((size_t)W * 32 * n * e);
+    s.init_B = take((size_t)W * 32 * n * e);
+    s.init_piv = (int32_t*)take((size_t)W * n * 4);
+  }
   s.list = (int32_t*)take((size_t)W * 4);
   s.flist = (int32_t*)take((size_t)W * 4);
-  s.counters = (int32_t*)take(8 * 4);
+  s.counters = (int32_t*)take(8 * 4);   // [0] accepted, [1] to flush, [4..7] two uint64 flush totals
   if (st) *st = s;
   return off;
 }
@@ -99,8 +104,8 @@ static lrux_status_t init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, 
   hh->launches = 0;
   hh->num_sms = sms;
   int nl = attach ? 0
-           : kind == KIND_DET ? launch_det_init(hh->st, d_A0, (cudaStream_t)stream)
-                              : launch_pf_init(hh->st, d_A0, (cudaStream_t)stream);
+           : kind == KIND_DET ? launch_det_init(hh->st, d_A0, sms, (cudaStream_t)stream)
+                              : launch_pf_init(hh->st, d_A0, sms, (cudaStream_t)stream);
   if (nl < 0) {
     delete hh;
     return LRUX_ECUDA;
@@ -230,6 +235,14 @@ lrux_status_t lrux_pf_get_inverse(lrux_handle_t h, void* d_out, void* stream) {
   if (!d_out) return LRUX_EINVAL;
   if (h->st.K > 0) LRUX_COUNT(h, launch_pf_flush(h->st, true, h->num_sms, (cudaStream_t)stream, &h->prof));
   LRUX_COUNT(h, launch_get_inverse(h->st, d_out, (cudaStream_t)stream));
+  return LRUX_OK;
+}
+
+lrux_status_t lrux_get_flush_count(lrux_handle_t h, int64_t* d_out, void* stream) {
+  if (!h || !d_out) return LRUX_EINVAL;
+  if (cudaMemcpyAsync(d_out, h->st.counters + 4, 16, cudaMemcpyDeviceToDevice,
+                      (cudaStream_t)stream) != cudaSuccess)
+    return LRUX_ECUDA;
   return LRUX_OK;
 }
 

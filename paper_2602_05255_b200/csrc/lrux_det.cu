@@ -622,6 +622,10 @@ __global__ void flush_clear_kernel(State st) {
   const int it = blockIdx.x * blockDim.x + threadIdx.x;
   if (it >= st.counters[1]) return;
   const int w = st.flist[it];
+  // running totals for lrux_*_get_flush_count: [walker flushes, buffer columns folded]
+  unsigned long long* tot = (unsigned long long*)(st.counters + 4);
+  atomicAdd(&tot[0], 1ULL);
+  atomicAdd(&tot[1], (unsigned long long)st.fill[w]);
   st.fill[w] = 0;
   st.nupd[w] = 0;
 }
@@ -661,7 +665,8 @@ static int launch_update_reg(const State& st, int k, int num_sms, cudaStream_t s
   const int n = st.n;
   const size_t smem = 2 * (size_t)k * n * sizeof(T);
   auto kern = det_update_kernel<T, KT, VEC, CH, RW>;
-  if (smem > 48 * 1024 &&
+  if (smem > 40 * 1024 &&   // static shared memory counts towards the 48 KiB default
+
       cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return -1;
   int rows_per_tile = 64;
@@ -734,7 +739,8 @@ static int launch_append_kt(const State& st, int k, int num_sms, cudaStream_t s)
   const size_t smem = ((n_in_smem ? (size_t)k * n : 0) + 4 * (size_t)KT * rows_per_tile) * sizeof(T);
   const bool vec = (n % VECMAX) == 0 && VECMAX == 2;
   auto kern = vec ? det_append_kernel<T, KT, VECMAX, 2> : det_append_kernel<T, KT, 1, 2>;
-  if (smem > 48 * 1024 &&
+  if (smem > 40 * 1024 &&   // static shared memory counts towards the 48 KiB default
+
       cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return -1;
   int occ = 1;

@@ -266,7 +266,7 @@ parlett_reid_kernel(T* __restrict__ Mall, int n, T* __restrict__ phase_out,
 
 // ---------------------------------------------------------------- launchers
 template <typename T>
-static int init_impl(const State& st, const void* d_A0, cudaStream_t s) {
+static int init_impl(const State& st, const void* d_A0, int num_sms, cudaStream_t s) {
   const int n = st.n;
   const size_t W = (size_t)st.W;
   int nl = 0;
@@ -282,8 +282,13 @@ static int init_impl(const State& st, const void* d_A0, cudaStream_t s) {
                            (int)smem_gj) != cudaSuccess) return -1;
   if (st.kind == KIND_DET) {
     launch_copy<T>(d_A0, st.Ti, st.W, n, /*transpose=*/true, /*skew=*/false, s); ++nl;
-    gj_inverse_kernel<T><<<(unsigned)W, 256, smem_gj, s>>>((T*)st.Ti, n, (T*)st.phase, st.logabs,
-                                                           st.info, true); ++nl;
+    const int rb = n >= kBlockedInitMin ? launch_gj_blocked(st, true, num_sms, s) : 0;
+    if (rb < 0) return -1;
+    if (rb > 0) nl += rb;
+    else {
+      gj_inverse_kernel<T><<<(unsigned)W, 256, smem_gj, s>>>((T*)st.Ti, n, (T*)st.phase, st.logabs,
+                                                             st.info, true); ++nl;
+    }
   } else {
     if (cudaFuncSetAttribute(parlett_reid_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)smem_pr) != cudaSuccess) return -1;
@@ -291,19 +296,26 @@ static int init_impl(const State& st, const void* d_A0, cudaStream_t s) {
     parlett_reid_kernel<T><<<(unsigned)W, 256, smem_pr, s>>>((T*)st.Ti, n, (T*)st.phase, st.logabs,
                                                              st.info); ++nl;
     launch_copy<T>(d_A0, st.Ti, st.W, n, false, true, s); ++nl;
-    gj_inverse_kernel<T><<<(unsigned)W, 256, smem_gj, s>>>((T*)st.Ti, n, (T*)st.phase, st.logabs,
-                                                           st.info, false); ++nl;
+    const int rb = n >= kBlockedInitMin ? launch_gj_blocked(st, false, num_sms, s) : 0;
+    if (rb < 0) return -1;
+    if (rb > 0) nl += rb;
+    else {
+      gj_inverse_kernel<T><<<(unsigned)W, 256, smem_gj, s>>>((T*)st.Ti, n, (T*)st.phase, st.logabs,
+                                                             st.info, false); ++nl;
+    }
     dim3 grid((n + 31) / 32, (n + 7) / 8, (unsigned)W), block(32, 8);
     skew_project_kernel<T><<<grid, block, 0, s>>>((T*)st.Ti, n); ++nl;
   }
   return cudaGetLastError() == cudaSuccess ? nl : -1;
 }
 
-int launch_det_init(const State& st, const void* d_A0, cudaStream_t s) {
-  return st.dt == LRUX_F64 ? init_impl<double>(st, d_A0, s) : init_impl<cplx>(st, d_A0, s);
+int launch_det_init(const State& st, const void* d_A0, int num_sms, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? init_impl<double>(st, d_A0, num_sms, s)
+                           : init_impl<cplx>(st, d_A0, num_sms, s);
 }
-int launch_pf_init(const State& st, const void* d_A0, cudaStream_t s) {
-  return st.dt == LRUX_F64 ? init_impl<double>(st, d_A0, s) : init_impl<cplx>(st, d_A0, s);
+int launch_pf_init(const State& st, const void* d_A0, int num_sms, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? init_impl<double>(st, d_A0, num_sms, s)
+                           : init_impl<cplx>(st, d_A0, num_sms, s);
 }
 
 int launch_get_amplitude(const State& st, void* d_phase, double* d_logabs, cudaStream_t s) {

@@ -13,6 +13,7 @@ namespace lrux {
 enum Kind { KIND_DET = 0, KIND_PF = 1 };
 constexpr int kRatioSlice = 256;       // columns of A^-1[:,P] handled by one CTA of the det ratio
 constexpr int kRatioSplitMax = 64;     // => n <= 16384
+constexpr int kBlockedInitMin = 768;   // blocked (panel + DMMA) initialisation from this n on
 
 // Views into the caller-owned d_state buffer (all device pointers, 256 B aligned).
 // Element type is double (LRUX_F64) or interleaved complex (LRUX_C128); sizes
@@ -38,6 +39,9 @@ struct State {
   void* pend_AN;     // pf delayed: [W][kmax][cap]  N * Abuf^T
   void* pend_Rpart;  // det: [W][kRatioSplitMax][kmax*kmax] partial R of each column slice
   int32_t* pend_cnt; // det: [W] slices of the current ratio call that have finished
+  void* init_A;      // n >= kBlockedInitMin: [W][32][n] scratch of the blocked initialisation
+  void* init_B;      //                       [W][32][n]
+  int32_t* init_piv; //                       [W][n] pivot rows
   void* Abuf;        // [W][cap][n]  det: a_t (Eq. 10);  pf: a'_t (Eq. 25)
   void* Bbuf;        // [W][cap][n]  det: b_t (Eq. 11);  pf: a'_t R_t^-1
   int32_t* list;     // [W] accepted walkers (compacted)
@@ -87,8 +91,10 @@ size_t state_layout(State* st, void* base, int64_t W, int32_t n, int32_t kmax, i
                     int32_t dt, int32_t kind);
 
 // launchers (each returns the number of kernels it enqueued, or -1 on a CUDA error)
-int launch_det_init(const State& st, const void* d_A0, cudaStream_t s);
-int launch_pf_init(const State& st, const void* d_A0, cudaStream_t s);
+int launch_det_init(const State& st, const void* d_A0, int num_sms, cudaStream_t s);
+int launch_pf_init(const State& st, const void* d_A0, int num_sms, cudaStream_t s);
+// blocked in-place inverse of st.Ti (lrux_init_blocked.cu); 0 = not applicable
+int launch_gj_blocked(const State& st, bool write_amp, int num_sms, cudaStream_t s);
 int launch_det_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
                      void* d_ratio, cudaStream_t s, Prof* prof);
 int launch_det_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s,

@@ -717,7 +717,7 @@ static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_s
     const size_t sm = 4 * (size_t)k * st.n * sizeof(T);   // Y' and g
     if (sm <= 160 * 1024) {
       auto kern = pf_update_stream_kernel<T>;
-      if (sm > 48 * 1024 &&
+      if (sm > 40 * 1024 &&
           cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess)
         return -1;
       const int rpt = 64, tiles = (st.n + rpt - 1) / rpt;

@@ -39,6 +39,7 @@ SIGNATURES = {
     "lrux_pf_get_amplitude": [_vp, _vp, _vp, _vp],
     "lrux_det_get_inverse": [_vp, _vp, _vp],
     "lrux_pf_get_inverse": [_vp, _vp, _vp],
+    "lrux_get_flush_count": [_vp, _vp, _vp],
     "lrux_launch_count": [_vp, C.POINTER(_i64)],
     "lrux_profile_enable": [_vp, _i32],
     "lrux_profile_read": [_vp, _i32, C.POINTER(C.c_double), C.POINTER(_i64)],
@@ -176,6 +177,12 @@ class _Walkers:
         out = torch.empty((self.W, self.n, self.n), dtype=self.dtype, device=self.device)
         _check(self._fn("get_inverse")(self._h, _ptr(out), _stream(stream)))
         return out
+
+    def flush_count(self, stream=None):
+        """(walker flushes, buffer columns folded) since init; synchronises."""
+        out = torch.zeros(2, dtype=torch.int64, device=self.device)
+        _check(self._lib.lrux_get_flush_count(self._h, _ptr(out), _stream(stream)))
+        return tuple(int(x) for x in out.cpu())
 
     def launch_count(self):
         c = _i64(0)

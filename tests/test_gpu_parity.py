@@ -210,6 +210,41 @@ def test_errors_and_info_bits():
         lrux.PfWalkers(torch.zeros((2, 5, 5), dtype=torch.float64, device=dev))
 
 
+@pytest.mark.parametrize("kind,n,cplx", [("det", 800, False), ("det", 1000, False),
+                                          ("det", 800, True), ("pf", 1000, False)])
+def test_blocked_init(kind, n, cplx):
+    """Step a0 through the blocked (panel + DMMA) Gauss-Jordan path (n >= 768), including a
+    ragged last panel (1000 = 31*32 + 8), a walker that needs row exchanges in every panel
+    and a singular walker."""
+    from oracle import lrux_oracle as orc
+
+    rng = np.random.default_rng(n + cplx)
+    W = 3
+    A = rng.standard_normal((W, n, n))
+    if cplx:
+        A = A + 1j * rng.standard_normal((W, n, n))
+    if kind == "pf":
+        A = np.triu(A, 1) - np.triu(A, 1).transpose(0, 2, 1)
+    else:
+        A[1] = A[1][rng.permutation(n)] * 1e-3       # pivots far from the diagonal, small scale
+        A[2, 5] = 0.0                                 # a zero row: exactly singular
+    wk = (lrux.DetWalkers if kind == "det" else lrux.PfWalkers)(torch.as_tensor(A, device="cuda"), kmax=1)
+    ph, la = wk.get_amplitude()
+    inv = wk.get_inverse().cpu().numpy()
+    info = wk.info.cpu().numpy()
+    good = [0, 1] if kind == "det" else [0, 1, 2]
+    if kind == "det":
+        assert info[2] & 1 and np.isneginf(la[2].item())
+    for w in good:
+        assert info[w] == 0
+        oph, ola = orc.slogdet(A[w]) if kind == "det" else orc.slogpf(A[w])
+        assert abs(ph[w].item() - oph) < 1e-9
+        assert abs(la[w].item() - ola) <= 1e-10 * max(1.0, abs(ola))
+        assert np.abs(inv[w] @ A[w] - np.eye(n)).max() < 1e-7
+        if kind == "pf":
+            assert np.array_equal(inv[w], -inv[w].T)
+
+
 def test_init_amplitude_and_inverse():
     """Step a0 alone: A^-1 and (phase, log|det|), (phase, log|pf|) vs the oracle."""
     from oracle import lrux_oracle as orc
