@@ -21,15 +21,15 @@ namespace lrux {
 //   a_tau = A0^-1 v - sum_t a_t (b_t^T v)                       (Eq. 14)
 // (b_t^T v = Bbuf[s][P[a]] is a warp-uniform load).  C_eff and N are stashed for
 // accept.  R = N C_eff (Eq. 4 / Eq. 13): every slice writes its partial k x k sum
-// (KT <= 4: accumulated on the fly), and the slice that finishes last adds the partials
-// in slice order (deterministic) -- or, for KT = 8, forms R from the complete stash --
+// (accumulated on the fly), and the slice that finishes last adds the partials in slice
+// order (deterministic) -- or, for complex128 with KT = 8, forms R from the complete stash --
 // and evaluates r = det R by a k x k LU in one thread.
 template <typename T, int KT, int EPT>
 __global__ void __launch_bounds__(256)
 det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __restrict__ rows,
                  T* __restrict__ ratio_out) {
   using S = Sc<T>;
-  constexpr bool FLY = KT <= 4;
+  constexpr bool FLY = KT <= 4 || sizeof(T) == 8;   // k x k accumulators in registers
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* Bp = (T*)smem_raw;  // [fill][KT]: b_t^T v = Bbuf[s][P[a]]
   __shared__ T Rs[kMaxK * kMaxK];
