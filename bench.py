@@ -257,20 +257,38 @@ def e2e_run(wk, seed, orb, occ, unocc, w0, device, warmup, steps):
     del rec
     xi = np.stack([wl.to_uniform(wl.rnd64(seed, np.arange(w0, w0 + W, dtype=np.uint64),
                                           wl.STREAM_ACCEPT, np.uint64(t))) for t in range(T)])
-    idx_d, rows_d, mask_d = A0_chain.idx, A0_chain.rows, A0_chain.mask
+    mask_d = A0_chain.mask
+    # two sets of device input buffers: the upload of step t+1 (copy stream) overlaps the
+    # host decision and the accept of step t (compute stream)
+    idx_d = [A0_chain.idx, torch.empty_like(A0_chain.idx)]
+    rows_d = [A0_chain.rows, torch.empty_like(A0_chain.rows)]
     ratio_h = torch.empty(W, dtype=dt).pin_memory()
     mask_h = torch.empty(W, dtype=torch.uint8).pin_memory()
+    main = torch.cuda.current_stream()
+    cs = torch.cuda.Stream()
+    copied = [torch.cuda.Event(), torch.cuda.Event()]
+
+    def upload(t):
+        b = t & 1
+        with torch.cuda.stream(cs):
+            idx_d[b].copy_(idx_h[t], non_blocking=True)
+            rows_d[b].copy_(rows_h[t], non_blocking=True)
+            copied[b].record(cs)
+
     mism = 0
     t_start = 0.0
+    upload(0)
     for t in range(T):
         if t == warmup:
             torch.cuda.synchronize()
             t_start = time.perf_counter()
-        idx_d.copy_(idx_h[t], non_blocking=True)
-        rows_d.copy_(rows_h[t], non_blocking=True)
-        wkr.ratio_(idx_d, rows_d)
+        b = t & 1
+        main.wait_event(copied[b])
+        wkr.ratio_(idx_d[b], rows_d[b])           # copies what accept needs into the state
         ratio_h.copy_(wkr.ratio, non_blocking=True)
-        torch.cuda.synchronize()
+        if t + 1 < T:
+            upload(t + 1)                         # buffer 1-b: its ratio finished last step
+        main.synchronize()
         r = ratio_h.numpy()
         a2 = r.real ** 2 + r.imag ** 2 if wk["cplx"] else r * r
         m = (xi[t] < np.minimum(1.0, a2))
