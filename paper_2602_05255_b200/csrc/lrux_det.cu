@@ -394,36 +394,58 @@ det_update_stream_kernel(State st, int k, int tiles, int rows_per_tile) {
     const T* gC = (const T*)st.pend_C + (size_t)w * kmax * n;
     T* Tw = (T*)st.Ti + (size_t)w * n * n;
     const int j_end = min(n, (tile + 1) * rows_per_tile);
-    for (int j = tile * rows_per_tile + warp; j < j_end; j += nw) {
-      T* row = Tw + (size_t)j * n;
-      T d[KT];
+    // RW rows per warp pass: every N / C element fetched from L1/L2 serves RW rows
+    constexpr int RW = 4;
+    for (int j0 = tile * rows_per_tile + warp * RW; j0 < j_end; j0 += nw * RW) {
+      T d[RW][KT];
 #pragma unroll
-      for (int a = 0; a < KT; ++a) d[a] = S::zero();
+      for (int r = 0; r < RW; ++r)
+#pragma unroll
+        for (int a = 0; a < KT; ++a) d[r][a] = S::zero();
       for (int i = lane; i < n; i += 32) {
-        const T x = row[i];
+        T x[RW];
 #pragma unroll
-        for (int a = 0; a < KT; ++a)
-          if (a < k) d[a] = S::fma(x, gN[(size_t)a * n + i], d[a]);
+        for (int r = 0; r < RW; ++r) x[r] = j0 + r < j_end ? Tw[(size_t)(j0 + r) * n + i] : S::zero();
+#pragma unroll
+        for (int a = 0; a < KT; ++a) {
+          if (a < k) {
+            const T nv = gN[(size_t)a * n + i];
+#pragma unroll
+            for (int r = 0; r < RW; ++r) d[r][a] = S::fma(x[r], nv, d[r][a]);
+          }
+        }
       }
-      T g[KT];
+      T g[RW][KT];
 #pragma unroll
-      for (int a = 0; a < KT; ++a) {
-        d[a] = warp_sum(d[a]);
-        if (j == sidx[a]) d[a] = S::sub(d[a], S::one());
-      }
+      for (int r = 0; r < RW; ++r) {
 #pragma unroll
-      for (int a = 0; a < KT; ++a) {
-        T acc = S::zero();
+        for (int a = 0; a < KT; ++a) {
+          d[r][a] = warp_sum(d[r][a]);
+          if (j0 + r == sidx[a]) d[r][a] = S::sub(d[r][a], S::one());
+        }
 #pragma unroll
-        for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], d[b], acc);
-        g[a] = acc;
+        for (int a = 0; a < KT; ++a) {
+          T acc = S::zero();
+#pragma unroll
+          for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], d[r][b], acc);
+          g[r][a] = acc;
+        }
       }
       for (int i = lane; i < n; i += 32) {
-        T x = row[i];
+        T x[RW];
 #pragma unroll
-        for (int a = 0; a < KT; ++a)
-          if (a < k) x = S::fnma(g[a], gC[(size_t)a * n + i], x);
-        row[i] = x;
+        for (int r = 0; r < RW; ++r) x[r] = j0 + r < j_end ? Tw[(size_t)(j0 + r) * n + i] : S::zero();
+#pragma unroll
+        for (int a = 0; a < KT; ++a) {
+          if (a < k) {
+            const T cv = gC[(size_t)a * n + i];
+#pragma unroll
+            for (int r = 0; r < RW; ++r) x[r] = S::fnma(g[r][a], cv, x[r]);
+          }
+        }
+#pragma unroll
+        for (int r = 0; r < RW; ++r)
+          if (j0 + r < j_end) Tw[(size_t)(j0 + r) * n + i] = x[r];
       }
     }
   }

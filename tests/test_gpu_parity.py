@@ -57,9 +57,11 @@ def test_det_config2_shape_reduced():
         _run("det", wl.BASE_SEED + 2, 40, 256, 512, 2, K, 60, walkers=[0, 13, 27, 39])
 
 
-def test_det_large_n_stream_path():
-    """n=1100 > register-row limit: generic streaming update kernel."""
-    _run("det", 77, 3, 1100, 2200, 1, 0, 12, walkers=[0, 2], scratch_every=4)
+@pytest.mark.parametrize("n,k", [(1101, 2), (1100, 1)])
+def test_det_large_n_stream_path(n, k):
+    """Large rows: n=1101 (odd: rows not 16-byte aligned) takes the generic streaming
+    update kernel, n=1100 the TMA-staged one with a ragged chunk tail."""
+    _run("det", 77, 3, n, 2 * n, k, 0, 12, walkers=[0, 2], scratch_every=4)
 
 
 @pytest.mark.parametrize("n,M,k,K,cplx", [
