@@ -451,6 +451,60 @@ det_update_stream_kernel(State st, int k, int tiles, int rows_per_tile) {
   }
 }
 
+// ---------------------------------------------------------------- rank split (a3, large k n)
+// A rank-k row replacement is the rank-c replacement of its first c rows followed by
+// the rank-(k-c) replacement of the rest in the once-updated matrix.  With
+// R^-1 = [[X11, X12], [X21, X22]] (c | k-c blocks) everything the two steps need follows
+// from the stash without touching A^-1:
+//   first step :  C1, N1, P1,  R11^-1 = X11 - X12 X22^-1 X21
+//   second step:  C2' = A1^-1[:,P2] = C2 + C1 X12 X22^-1,  N2, P2,  (Schur complement)^-1 = X22
+// This kernel rewrites pend_Rinv[0:c,0:c] and pend_C[c:k] in place (per accepted walker);
+// the second step then runs on pointer-shifted views of the same pending area, and may
+// be split again.  Used when no TMA-staged instance exists for the full k (registers).
+template <typename T>
+__global__ void __launch_bounds__(256) det_split_prep_kernel(State st, int c, int k) {
+  using S = Sc<T>;
+  __shared__ T X22[kMaxK * kMaxK], Z[kMaxK * kMaxK], Q[kMaxK * kMaxK];
+  const int n = st.n, kmax = st.kmax, kc = st.kc, m = k - c;
+  const int tid = threadIdx.x;
+  const int count = st.counters[0];
+  for (int it = blockIdx.x; it < count; it += gridDim.x) {
+    const int w = st.list[it];
+    T* Ri = (T*)st.pend_Rinv + (size_t)w * kc * kc;
+    __syncthreads();
+    if (tid < m * m) X22[(tid / m) * kMaxK + tid % m] = Ri[(c + tid / m) * kc + c + tid % m];
+    __syncthreads();
+    if (tid == 0) {
+      bool ok;
+      small_det_inv(X22, Z, m, kMaxK, &ok);   // Z = X22^-1 (X22 is destroyed)
+    }
+    __syncthreads();
+    if (tid < c * m) {   // Q = X12 Z   (c x m)
+      const int a = tid / m, b = tid % m;
+      T acc = S::zero();
+      for (int q = 0; q < m; ++q) acc = S::fma(Ri[a * kc + c + q], Z[q * kMaxK + b], acc);
+      Q[a * kMaxK + b] = acc;
+    }
+    __syncthreads();
+    if (tid < c * c) {   // R11^-1 = X11 - Q X21 (each thread rewrites only its own X11 entry)
+      const int a = tid / c, b = tid % c;
+      T acc = Ri[a * kc + b];
+      for (int q = 0; q < m; ++q) acc = S::fnma(Q[a * kMaxK + q], Ri[(c + q) * kc + b], acc);
+      Ri[a * kc + b] = acc;
+    }
+    T* pC = (T*)st.pend_C + (size_t)w * kmax * n;
+    for (int i = tid; i < n; i += 256) {
+      T c1[kMaxK];
+      for (int a = 0; a < c; ++a) c1[a] = pC[(size_t)a * n + i];
+      for (int b = 0; b < m; ++b) {
+        T v = pC[(size_t)(c + b) * n + i];
+        for (int a = 0; a < c; ++a) v = S::fma(c1[a], Q[a * kMaxK + b], v);
+        pC[(size_t)(c + b) * n + i] = v;
+      }
+    }
+  }
+}
+
 // ---------------------------------------------------------------- delayed append (a6)
 // prep: work item = (accepted walker, group of 8 buffer rows).  Each warp reads one
 // row a_s of Abuf once and forms NA[b][s] = N_b . a_s for all b (-> pend_Y); group 0
@@ -714,6 +768,32 @@ static int launch_update_kt(const State& st, int k, int num_sms, cudaStream_t s)
     if (!force_reg && (force_tma || (size_t)n * sizeof(T) >= 8 * 1024)) {
       const int r = launch_det_update_tma(st, k, num_sms, s);
       if (r != 0) return r;
+      // no instance for the full rank (register budget): peel off chunks of the largest
+      // rank that has one; each chunk is one full pass over A^-1
+      int c = 0;
+      for (int cand = 4; cand >= 1; cand >>= 1)
+        if (cand < k && launch_det_update_tma_ok(st, cand)) { c = cand; break; }
+      if (c > 0) {
+        int nl = 0, rem = k;
+        State v = st;   // view of the pending area, shifted past the chunks already applied
+        const size_t e = sizeof(T);
+        while (rem > 0) {
+          const int cur = rem > c ? c : rem;
+          if (rem > cur) {
+            det_split_prep_kernel<T><<<persistent_grid(num_sms, 4, st.W), 256, 0, s>>>(v, cur, rem);
+            ++nl;
+          }
+          const int r2 = launch_det_update_tma(v, cur, num_sms, s);
+          if (r2 <= 0) return -1;
+          nl += r2;
+          v.pend_idx += cur;
+          v.pend_N = (char*)v.pend_N + (size_t)cur * n * e;
+          v.pend_C = (char*)v.pend_C + (size_t)cur * n * e;
+          v.pend_Rinv = (char*)v.pend_Rinv + ((size_t)cur * st.kc + cur) * e;
+          rem -= cur;
+        }
+        return nl;
+      }
     }
   }
   const size_t smem = 2 * (size_t)k * n * sizeof(T);

@@ -332,6 +332,7 @@ static int launch_tma_inst(const State& st, int k, int num_sms, cudaStream_t s) 
     if (NS > 8) NS = 8;
     if (NS < 3) return 0;
     const size_t smem = (size_t)NS * RC * row + fixed;
+    if (num_sms <= 0) return 1;   // eligibility probe (launch_det_update_tma_ok)
     auto kern = det_update_tma_kernel<T, KT, RC, TV, APPEND, NW>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
       return -1;
@@ -395,6 +396,11 @@ static int launch_update_tma_t(const State& st, int k, int num_sms, cudaStream_t
 int launch_det_update_tma(const State& st, int k, int num_sms, cudaStream_t s) {
   return st.dt == LRUX_F64 ? launch_update_tma_t<double, false>(st, k, num_sms, s)
                            : launch_update_tma_t<cplx, false>(st, k, num_sms, s);
+}
+
+// true when a rank-k immediate update of this shape has a TMA-staged instance
+bool launch_det_update_tma_ok(const State& st, int k) {
+  return launch_det_update_tma(st, k, 0, nullptr) == 1;
 }
 
 // delayed append through the same pass (after det_prep_kernel): 2 launches, 0 = not eligible

@@ -109,6 +109,7 @@ int launch_pf_flush(const State& st, bool all, int num_sms, cudaStream_t s, Prof
 // 0 = shape not eligible, -1 = CUDA error
 int launch_det_update_tma(const State& st, int k, int num_sms, cudaStream_t s);
 int launch_det_append_tma(const State& st, int k, int num_sms, cudaStream_t s);
+bool launch_det_update_tma_ok(const State& st, int k);
 // DMMA flush of the delay buffers, det and pf (lrux_flush.cu)
 int launch_flush_dmma(const State& st, int num_sms, cudaStream_t s);
 // shared between det and pf (defined in lrux_det.cu)

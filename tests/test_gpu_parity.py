@@ -91,6 +91,8 @@ def test_pf_config3_shape_reduced():
     (1100, 1, 0, False, 10),     # ragged: 550 vectors per row, 4-row chunks with a 3-row tail
     (512, 2, 0, True, 10),       # complex128, 8 KB rows
     (2048, 2, 0, False, 4),      # 16 KB rows: RC=2, 4 vectors per lane
+    (1100, 8, 0, False, 8),      # no rank-8 instance at this n: split into two rank-4 passes
+    (1100, 7, 0, False, 8),      # 4 + 3
     (1024, 2, 3, False, 14),     # delayed append through the same pass + finish kernel
     (512, 4, 2, True, 12),       # complex128 delayed (configs[3] shape at n=512)
 ])
