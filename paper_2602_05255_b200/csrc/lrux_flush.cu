@@ -96,17 +96,32 @@ __global__ void __launch_bounds__(256) flush_dmma_kernel(State st, int t1) {
       }
     }
 
-    for (int s0 = 0; s0 < fill; s0 += KC) {
-      __syncthreads();
-      for (int q = tid; q < KC * BT; q += 256) {
+    // register double buffering: the global loads of panel chunk s0+KC are in flight
+    // while the DMMAs of chunk s0 run
+    constexpr int EPT = KC * BT / 256;   // staged elements per thread and panel
+    T rb[EPT], ra[EPT];
+    auto fetch = [&](int s0) {
+#pragma unroll
+      for (int u = 0; u < EPT; ++u) {
+        const int q = tid + 256 * u;
         const int kk = q / BT, c = q % BT;
         const bool sv = s0 + kk < fill;
-        const T bv = (sv && r0 + c < n) ? Bb[(size_t)(s0 + kk) * n + r0 + c] : S::zero();
-        const T av = (sv && c0 + c < n) ? Ab[(size_t)(s0 + kk) * n + c0 + c] : S::zero();
-        split_store(&Bs[0][kk][0], &Bs[NP - 1][kk][0], c, bv);
-        split_store(&As[0][kk][0], &As[NP - 1][kk][0], c, av);
+        rb[u] = (sv && r0 + c < n) ? Bb[(size_t)(s0 + kk) * n + r0 + c] : S::zero();
+        ra[u] = (sv && c0 + c < n) ? Ab[(size_t)(s0 + kk) * n + c0 + c] : S::zero();
+      }
+    };
+    fetch(0);
+    for (int s0 = 0; s0 < fill; s0 += KC) {
+      __syncthreads();
+#pragma unroll
+      for (int u = 0; u < EPT; ++u) {
+        const int q = tid + 256 * u;
+        const int kk = q / BT, c = q % BT;
+        split_store(&Bs[0][kk][0], &Bs[NP - 1][kk][0], c, rb[u]);
+        split_store(&As[0][kk][0], &As[NP - 1][kk][0], c, ra[u]);
       }
       __syncthreads();
+      if (s0 + KC < fill) fetch(s0 + KC);
       const int kend = min(KC, (fill - s0 + 3) & ~3);
       for (int k4 = 0; k4 < kend; k4 += 4) {
         double bf[NP][2], af[NP][4];
