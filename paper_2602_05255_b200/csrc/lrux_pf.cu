@@ -376,7 +376,7 @@ __global__ void __launch_bounds__(256) pf_update_kernel(State st, int k, int t1)
 // its own thread: below the diagonal the thread recomputes the mirrored upper value
 // from -Ti[r][c] with the same operands in the same order and stores its negative
 // (exact skewness, no transposed access).
-template <typename T>
+template <typename T, int MT>   // MT >= 2k: size of the per-row factor arrays
 __global__ void __launch_bounds__(256)
 pf_update_stream_kernel(State st, int k, int tiles, int rows_per_tile) {
   using S = Sc<T>;
@@ -416,15 +416,29 @@ pf_update_stream_kernel(State st, int k, int tiles, int rows_per_tile) {
     const int r_end = min(n, (tile + 1) * rows_per_tile);
     for (int r = tile * rows_per_tile + warp; r < r_end; r += nw) {
       T* row = Tw + (size_t)r * n;
-#pragma unroll 4
-      for (int c = lane; c < n; c += 32) {
-        const bool up = r < c;
-        const int i = up ? r : c, j = up ? c : r;
-        const T x = row[c];
-        T v = up ? x : S::neg(x);
-        for (int beta = 0; beta < m; ++beta)
-          v = S::fma(gv[(size_t)beta * n + i], yv[(size_t)beta * n + j], v);
-        row[c] = (r == c) ? S::zero() : (up ? v : S::neg(v));
+      // the row's own factors live in registers; one shared-memory operand per FMA
+      T gr[MT], yr[MT];
+#pragma unroll
+      for (int beta = 0; beta < MT; ++beta) {
+        gr[beta] = beta < m ? gv[(size_t)beta * n + r] : S::zero();
+        yr[beta] = beta < m ? yv[(size_t)beta * n + r] : S::zero();
+      }
+#pragma unroll 2
+      for (int c = lane; c < r; c += 32) {          // below the diagonal: -v(c, r)
+        T v = S::neg(row[c]);
+#pragma unroll
+        for (int beta = 0; beta < MT; ++beta)
+          if (beta < m) v = S::fma(gv[(size_t)beta * n + c], yr[beta], v);
+        row[c] = S::neg(v);
+      }
+      if (lane == 0) row[r] = S::zero();
+#pragma unroll 2
+      for (int c = r + 1 + lane; c < n; c += 32) {   // above: v(r, c)
+        T v = row[c];
+#pragma unroll
+        for (int beta = 0; beta < MT; ++beta)
+          if (beta < m) v = S::fma(gr[beta], yv[(size_t)beta * n + c], v);
+        row[c] = v;
       }
     }
   }
@@ -716,7 +730,8 @@ static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_s
     ProfScope ps(prof, LRUX_PROF_UPDATE, s);
     const size_t sm = 4 * (size_t)k * st.n * sizeof(T);   // Y' and g
     if (sm <= 160 * 1024) {
-      auto kern = pf_update_stream_kernel<T>;
+      auto kern = k <= 1 ? pf_update_stream_kernel<T, 2> : k <= 2 ? pf_update_stream_kernel<T, 4>
+                : k <= 4 ? pf_update_stream_kernel<T, 8> : pf_update_stream_kernel<T, 16>;
       if (sm > 40 * 1024 &&
           cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess)
         return -1;
