@@ -428,6 +428,24 @@ def ncu_traffic_per_walker(kernel, workload):
     return best
 
 
+def pf_update_kernel_name(n, k, esz):
+    """Mirror of the dispatch in csrc/lrux_pf.cu:pf_accept_impl (K = 0): which kernel
+    applies the immediate Pfaffian update for this shape."""
+    k1 = esz == 8 and k == 1 and n <= 512
+    lg = 5
+    while (1 << lg) < n // 2:
+        lg += 1
+    for cl in (4, 8):
+        rpc = (n + cl - 1) // cl
+        smc = (rpc * n * 8 + ((256 >> lg) + 2 * cl) * (n // 2) * 16 + n * 40) if k1 \
+            else (rpc * n + (6 * k + 1) * n) * esz
+        if smc <= (56 if cl == 4 else 100) * 1024:
+            return "pf_cluster_k1_kernel" if k1 else "pf_cluster_update_kernel"
+    if (n * n + (4 * k + 1) * n) * esz <= 200 * 1024:
+        return "pf_resident_update_kernel"
+    return "pf_update_stream_kernel"
+
+
 def roofline_update(wk, run, peak, peak_src):
     """HBM roofline of the immediate Woodbury update kernel:
     algorithmic bytes = 2 n^2 e per accepted walker (read once + write once)."""
@@ -441,8 +459,7 @@ def roofline_update(wk, run, peak, peak_src):
     if wk["kind"] == "det":
         kern = "det_update_tma_kernel" if (rowb >= 8192 and rowb % 16 == 0) else "det_update_kernel"
     else:
-        resident = (wk["n"] ** 2 + (4 * wk["k"] + 1) * wk["n"]) * esz <= 200 * 1024
-        kern = "pf_resident_update_kernel" if resident else "pf_update_stream_kernel"
+        kern = pf_update_kernel_name(wk["n"], wk["k"], esz)
     tpw = ncu_traffic_per_walker(kern, wk.get("name", ""))
     traffic = tpw * run["accepted"] / pr["launches"] if tpw else None
     return {"bound": "hbm", "kernel": kern, "achieved": ach, "peak": peak,

@@ -14,6 +14,9 @@
 #include "lrux_common.cuh"
 #include "lrux_internal.h"
 #include "lrux_tma.cuh"
+#include <cooperative_groups.h>
+#include <cstdlib>
+#include <cstring>
 
 namespace lrux {
 
@@ -444,6 +447,74 @@ pf_update_stream_kernel(State st, int k, int tiles, int rows_per_tile) {
   }
 }
 
+// One row of the on-chip rank-2k update (Eq. 21; k = 1: Eq. 22), done by one warp.  Every
+// element is produced by its own lane: for r > c the mirrored upper value v(c,r) is
+// recomputed from -row[c] with the same operands in the same order and stored negated,
+// so the matrix stays exactly skew with no transposed access.
+template <typename T>
+__device__ __forceinline__ void pf_row_update(T* row, int r, int n, int m, const T* yv, const T* gv,
+                                              int lane) {
+  using S = Sc<T>;
+  if constexpr (sizeof(T) == 8) {
+    if (m == 2) {
+      // fp64, k = 1 (Eq. 22): pairs of columns; a pair entirely below / above the
+      // diagonal needs no per-element selection
+      const double g0r = gv[r], g1r = gv[n + r], y0r = yv[r], y1r = yv[n + r];
+      const double2* g0 = (const double2*)gv;
+      const double2* g1 = (const double2*)(gv + n);
+      const double2* y0 = (const double2*)yv;
+      const double2* y1 = (const double2*)(yv + n);
+      double2* row2 = (double2*)row;
+      for (int q = lane; q < n / 2; q += 32) {
+        const int c0 = 2 * q;
+        double2 x = row2[q];
+        if (c0 + 1 < r) {          // both below the diagonal: mirrored value, negated
+          const double2 a = g0[q], b = g1[q];
+          x.x = -fma(b.x, y1r, fma(a.x, y0r, -x.x));
+          x.y = -fma(b.y, y1r, fma(a.y, y0r, -x.y));
+        } else if (c0 > r) {       // both above
+          const double2 a = y0[q], b = y1[q];
+          x.x = fma(g1r, b.x, fma(g0r, a.x, x.x));
+          x.y = fma(g1r, b.y, fma(g0r, a.y, x.y));
+        } else {                   // the pair that holds the diagonal element
+          double e[2] = {x.x, x.y};
+#pragma unroll
+          for (int t = 0; t < 2; ++t) {
+            const int cc = c0 + t;
+            if (cc == r) e[t] = 0.0;
+            else if (cc < r) e[t] = -fma(gv[n + cc], y1r, fma(gv[cc], y0r, -e[t]));
+            else e[t] = fma(g1r, yv[n + cc], fma(g0r, yv[cc], e[t]));
+          }
+          x.x = e[0];
+          x.y = e[1];
+        }
+        row2[q] = x;
+      }
+      return;
+    }
+  }
+  if (m == 2) {
+    const T g0r = gv[r], g1r = gv[n + r], y0r = yv[r], y1r = yv[n + r];
+    for (int cc = lane; cc < n; cc += 32) {
+      const bool up = r < cc;
+      const T x = row[cc];
+      T v = up ? x : S::neg(x);
+      v = S::fma(up ? g0r : gv[cc], up ? yv[cc] : y0r, v);
+      v = S::fma(up ? g1r : gv[n + cc], up ? yv[n + cc] : y1r, v);
+      row[cc] = (r == cc) ? S::zero() : (up ? v : S::neg(v));
+    }
+  } else {
+    for (int cc = lane; cc < n; cc += 32) {
+      const bool up = r < cc;
+      const int i = up ? r : cc, j = up ? cc : r;
+      const T x = row[cc];
+      T v = up ? x : S::neg(x);
+      for (int beta = 0; beta < m; ++beta) v = S::fma(gv[beta * n + i], yv[beta * n + j], v);
+      row[cc] = (r == cc) ? S::zero() : (up ? v : S::neg(v));
+    }
+  }
+}
+
 // ---------------------------------------------------------------- resident update (a4)
 // Small walkers (n^2 e <= ~190 KB: n <= 152 fp64, config C3's n = 128): the whole inverse
 // of an accepted walker is brought into shared memory by ONE bulk asynchronous copy
@@ -534,65 +605,7 @@ __global__ void __launch_bounds__(512) pf_resident_update_kernel(State st, int k
       const int r0 = c * rpc, r1 = min(n, r0 + rpc);
       if (r0 >= n) break;
       for (int r = r0 + warp; r < r1; r += nw) {
-        T* row = Ts + (size_t)r * n;
-        if constexpr (sizeof(T) == 8) {
-          if (m == 2) {
-            // fp64, k = 1 (Eq. 22): pairs of columns; a pair entirely below / above the
-            // diagonal needs no per-element selection
-            const double g0r = gv[r], g1r = gv[n + r], y0r = yv[r], y1r = yv[n + r];
-            const double2* g0 = (const double2*)gv;
-            const double2* g1 = (const double2*)(gv + n);
-            const double2* y0 = (const double2*)yv;
-            const double2* y1 = (const double2*)(yv + n);
-            double2* row2 = (double2*)row;
-            for (int q = lane; q < n / 2; q += 32) {
-              const int c0 = 2 * q;
-              double2 x = row2[q];
-              if (c0 + 1 < r) {          // both below the diagonal: mirrored value, negated
-                const double2 a = g0[q], b = g1[q];
-                x.x = -fma(b.x, y1r, fma(a.x, y0r, -x.x));
-                x.y = -fma(b.y, y1r, fma(a.y, y0r, -x.y));
-              } else if (c0 > r) {       // both above
-                const double2 a = y0[q], b = y1[q];
-                x.x = fma(g1r, b.x, fma(g0r, a.x, x.x));
-                x.y = fma(g1r, b.y, fma(g0r, a.y, x.y));
-              } else {                   // the pair that holds the diagonal element
-                double e[2] = {x.x, x.y};
-#pragma unroll
-                for (int t = 0; t < 2; ++t) {
-                  const int cc = c0 + t;
-                  if (cc == r) e[t] = 0.0;
-                  else if (cc < r) e[t] = -fma(gv[n + cc], y1r, fma(gv[cc], y0r, -e[t]));
-                  else e[t] = fma(g1r, yv[n + cc], fma(g0r, yv[cc], e[t]));
-                }
-                x.x = e[0];
-                x.y = e[1];
-              }
-              row2[q] = x;
-            }
-            continue;
-          }
-        }
-        if (m == 2) {
-          const T g0r = gv[r], g1r = gv[n + r], y0r = yv[r], y1r = yv[n + r];
-          for (int cc = lane; cc < n; cc += 32) {
-            const bool up = r < cc;
-            const T x = row[cc];
-            T v = up ? x : S::neg(x);
-            v = S::fma(up ? g0r : gv[cc], up ? yv[cc] : y0r, v);
-            v = S::fma(up ? g1r : gv[n + cc], up ? yv[n + cc] : y1r, v);
-            row[cc] = (r == cc) ? S::zero() : (up ? v : S::neg(v));
-          }
-        } else {
-          for (int cc = lane; cc < n; cc += 32) {
-            const bool up = r < cc;
-            const int i = up ? r : cc, j = up ? cc : r;
-            const T x = row[cc];
-            T v = up ? x : S::neg(x);
-            for (int beta = 0; beta < m; ++beta) v = S::fma(gv[beta * n + i], yv[beta * n + j], v);
-            row[cc] = (r == cc) ? S::zero() : (up ? v : S::neg(v));
-          }
-        }
+        pf_row_update<T>(Ts + (size_t)r * n, r, n, m, yv, gv, lane);
       }
       tma::fence_proxy_async();
       __syncthreads();
@@ -608,6 +621,252 @@ __global__ void __launch_bounds__(512) pf_resident_update_kernel(State st, int k
     if (tid == 0 && w_next >= 0) {
       tma::store_wait_read<0>();
       load_chunk(w_next, (min(n, NCH * rpc) - 1) / rpc);   // last non-empty chunk
+    }
+  }
+  if (tid == 0) tma::store_wait_all<0>();
+}
+
+// ---------------------------------------------------------------- cluster-resident update (a4)
+// The same on-chip update with a walker's inverse spread over a thread-block CLUSTER:
+// CTA `cr` of CL holds rows [cr*rpc, (cr+1)*rpc) (one bulk copy in, one bulk store out).
+// A 32-row slab of C3 is 32 KB, so several CTAs share an SM and the load of one slab
+// overlaps the arithmetic and the store of others without any in-CTA pipeline, and
+// ~4x more work items than walkers even out the tail of the persistent grid.  The only
+// cross-CTA data is Y = A^-1 N (k = 1): each CTA computes the entries of its own rows
+// and writes them into every peer's shared memory (distributed shared memory), one
+// cluster barrier per walker.  The Y' buffer alternates between two slots so that a
+// peer that is one walker ahead never overwrites what this CTA still reads.
+template <typename T>
+__global__ void __launch_bounds__(256) pf_cluster_update_kernel(State st, int k, int need_y) {
+  using S = Sc<T>;
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int n = st.n, kmax = st.kmax, m = 2 * k;
+  const int CL = (int)cluster.num_blocks(), cr = (int)cluster.block_rank();
+  const int ncl = (int)gridDim.x / CL, cid = (int)blockIdx.x / CL;
+  const int rpc = (n + CL - 1) / CL, r0 = cr * rpc, r1 = min(n, r0 + rpc);
+  const int rows = max(0, r1 - r0);
+  T* Ts = (T*)smem_raw;                  // [rpc][n]  this CTA's rows
+  T* yvb = Ts + (size_t)rpc * n;         // [2][m][n] Y' (two slots)
+  T* gv = yvb + (size_t)2 * m * n;       // [m][n]    Y' R'^-1
+  T* nv = gv + (size_t)m * n;            // [n]       new row (k = 1)
+  __shared__ T Ri[kMaxC * kMaxC];
+  __shared__ int P[kMaxK];
+  __shared__ __align__(8) uint64_t bar;
+  const int tid = threadIdx.x, nt = blockDim.x, warp = tid >> 5, lane = tid & 31, nw = nt >> 5;
+  const int count = st.counters[0];
+  const uint32_t bytes = (uint32_t)((size_t)rows * n * sizeof(T));
+  if (tid == 0) {
+    tma::mbar_init(&bar, 1);
+    tma::fence_barrier_init();
+  }
+  __syncthreads();
+  auto load_rows = [&](int w) {   // thread 0 only
+    if (rows <= 0) return;
+    tma::mbar_arrive_expect_tx(&bar, bytes);
+    tma::load(Ts, (const T*)st.Ti + (size_t)w * n * n + (size_t)r0 * n, bytes, &bar);
+  };
+  if (tid == 0 && cid < count) load_rows(st.list[cid]);
+  uint32_t phase = 0;
+  int slot = 0;
+  for (int it = cid; it < count; it += ncl, slot ^= 1) {
+    const int w = st.list[it];
+    const int w_next = it + ncl < count ? st.list[it + ncl] : -1;
+    T* yv = yvb + (size_t)slot * m * n;
+    const T* pC = (const T*)st.pend_C + (size_t)w * kmax * n;
+    const T* pY = (const T*)st.pend_Y + (size_t)w * kmax * n;
+    const T* pN = (const T*)st.pend_N + (size_t)w * kmax * n;
+    for (int q = tid; q < m * m; q += nt)
+      Ri[(q / m) * kMaxC + (q % m)] =
+          ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + (q / m) * st.kc + (q % m)];
+    if (tid < k) P[tid] = st.pend_idx[(size_t)w * kmax + tid];
+    __syncthreads();
+    for (int q = tid; q < k * n; q += nt) {
+      const int a = q / n, i = q % n;
+      yv[(size_t)(k + a) * n + i] = pC[q];
+      if (need_y) nv[q] = pN[q];   // k == 1
+      else yv[q] = (i == P[a]) ? S::add(pY[q], S::one()) : pY[q];
+    }
+    __syncthreads();
+    if (rows > 0) tma::mbar_wait(&bar, phase);
+    phase ^= 1;
+    if (need_y) {
+      // Y = A^-1 N for the rows held here, broadcast to every CTA of the cluster
+      for (int i = r0 + warp; i < r1; i += nw) {
+        const T* row = Ts + (size_t)(i - r0) * n;
+        T acc = S::zero();
+        for (int j = lane; j < n; j += 32) acc = S::fma(row[j], nv[j], acc);
+        acc = warp_sum(acc);
+        if (i == P[0]) acc = S::add(acc, S::one());
+        if (lane < CL) cluster.map_shared_rank(yv, lane)[i] = acc;
+      }
+      cluster.sync();
+    } else {
+      __syncthreads();
+    }
+    for (int q = tid; q < m * n; q += nt) {
+      const int beta = q / n, i = q % n;
+      T g = S::zero();
+      for (int alpha = 0; alpha < m; ++alpha)
+        g = S::fma(yv[(size_t)alpha * n + i], Ri[alpha * kMaxC + beta], g);
+      gv[q] = g;
+    }
+    __syncthreads();
+    for (int r = r0 + warp; r < r1; r += nw)
+      pf_row_update<T>(Ts + (size_t)(r - r0) * n, r, n, m, yv, gv, lane);
+    tma::fence_proxy_async();
+    __syncthreads();
+    if (tid == 0 && rows > 0) {
+      tma::store((T*)st.Ti + (size_t)w * n * n + (size_t)r0 * n, Ts, bytes);
+      tma::store_commit();
+      if (w_next >= 0) {
+        tma::store_wait_read<0>();   // the slab has left shared memory
+        load_rows(w_next);
+      }
+    }
+  }
+  if (tid == 0) tma::store_wait_all<0>();
+}
+
+// ---------------------------------------------------------------- cluster-resident update, fp64 k = 1
+// Config C3's case (Eq. 22), laid out to minimise issued instructions (the generic kernel
+// above is issue-bound at n = 128, not memory-bound): thread (q, rg) owns the COLUMN PAIR
+// (2q, 2q+1) and every RG-th row of the slab, so that
+//  * Y = A^-1 N needs no warp reduction: by skewness y[c] = -sum_j Ti[j][c] N[j], a running
+//    sum down the thread's own columns; the partial sums of the row groups meet in shared
+//    memory, those of the CL slabs in every peer's shared memory (DSMEM), and every CTA adds
+//    them in the same order (identical Y everywhere: the mirror stays exact);
+//  * the column factors y0,y1,-g0,-g1 of the pair stay in registers for the whole slab, the
+//    row factors come from one 32-byte broadcast load per row;
+//  * below the diagonal -fma(g1c, y1r, fma(g0c, y0r, -x)) is evaluated as
+//    fma(-g1c, y1r, fma(-g0c, y0r, x)): the same value bit for bit (rounding is symmetric
+//    under negation), without the two sign flips.
+__global__ void __launch_bounds__(256, 4) pf_cluster_k1_kernel(State st, int lg_nqp) {
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int n = st.n, kmax = st.kmax, NQ = n >> 1;
+  const int CL = (int)cluster.num_blocks(), cr = (int)cluster.block_rank();
+  const int ncl = (int)gridDim.x / CL, cid = (int)blockIdx.x / CL;
+  const int rpc = (n + CL - 1) / CL, r0 = cr * rpc, r1 = min(n, r0 + rpc);
+  const int rows = max(0, r1 - r0);
+  const int RG = 256 >> lg_nqp;
+  const int tid = threadIdx.x, q = tid & ((1 << lg_nqp) - 1), rg = tid >> lg_nqp;
+  const bool act = q < NQ;
+  double* Ts = (double*)smem_raw;                          // [rpc][n]   this CTA's rows
+  double2* Ts2 = (double2*)Ts;
+  double2* part = (double2*)(Ts + (size_t)rpc * n);        // [RG][NQ]   column sums per row group
+  double2* ysum = part + (size_t)RG * NQ;                  // [2][CL][NQ] column sums per slab (two slots)
+  double2* rowc = ysum + (size_t)2 * CL * NQ;              // [n][2]     {g0,g1},{y0,y1} of row r
+  double* nv = (double*)(rowc + (size_t)2 * n);            // [n]        new row
+  __shared__ __align__(8) uint64_t bar;
+  const int count = st.counters[0];
+  const uint32_t bytes = (uint32_t)((size_t)rows * n * sizeof(double));
+  if (tid == 0) {
+    tma::mbar_init(&bar, 1);
+    tma::fence_barrier_init();
+  }
+  __syncthreads();
+  auto load_rows = [&](int w) {   // thread 0 only
+    if (rows <= 0) return;
+    tma::mbar_arrive_expect_tx(&bar, bytes);
+    tma::load(Ts, (const double*)st.Ti + (size_t)w * n * n + (size_t)r0 * n, bytes, &bar);
+  };
+  if (tid == 0 && cid < count) load_rows(st.list[cid]);
+  uint32_t phase = 0;
+  int slot = 0;
+  for (int it = cid; it < count; it += ncl, slot ^= 1) {
+    const int w = st.list[it];
+    const int w_next = it + ncl < count ? st.list[it + ncl] : -1;
+    const double* pC = (const double*)st.pend_C + (size_t)w * kmax * n;
+    const double* pN = (const double*)st.pend_N + (size_t)w * kmax * n;
+    const double* Rw = (const double*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
+    const double Ri00 = Rw[0], Ri01 = Rw[1], Ri10 = Rw[st.kc], Ri11 = Rw[st.kc + 1];
+    const int p0 = st.pend_idx[(size_t)w * kmax];
+    const double2 y1q = act ? ((const double2*)pC)[q] : make_double2(0.0, 0.0);
+    for (int i = tid; i < n; i += 256) nv[i] = pN[i];
+    __syncthreads();
+    if (rows > 0) tma::mbar_wait(&bar, phase);
+    phase ^= 1;
+    // ---- column sums over the slab's rows
+    if (act) {
+      double2 acc = make_double2(0.0, 0.0);
+      for (int rr = rg; rr < rows; rr += RG) {
+        const double2 x = Ts2[(size_t)rr * NQ + q];
+        const double nr = nv[r0 + rr];
+        acc.x = fma(x.x, nr, acc.x);
+        acc.y = fma(x.y, nr, acc.y);
+      }
+      part[rg * NQ + q] = acc;
+    }
+    __syncthreads();
+    if (act) {
+      double2 sum = part[q];
+      for (int g = 1; g < RG; ++g) {
+        const double2 t = part[g * NQ + q];
+        sum.x += t.x;
+        sum.y += t.y;
+      }
+      for (int p = rg; p < CL; p += RG)
+        cluster.map_shared_rank(ysum, p)[(size_t)(slot * CL + cr) * NQ + q] = sum;
+    }
+    cluster.sync();
+    double2 y0q = make_double2(0.0, 0.0), g0q = y0q, g1q = y0q;
+    if (act) {
+      double2 sum = ysum[(size_t)(slot * CL) * NQ + q];
+      for (int c = 1; c < CL; ++c) {
+        const double2 t = ysum[(size_t)(slot * CL + c) * NQ + q];
+        sum.x += t.x;
+        sum.y += t.y;
+      }
+      y0q.x = (2 * q == p0) ? -sum.x + 1.0 : -sum.x;
+      y0q.y = (2 * q + 1 == p0) ? -sum.y + 1.0 : -sum.y;
+      g0q.x = fma(y1q.x, Ri10, y0q.x * Ri00);
+      g0q.y = fma(y1q.y, Ri10, y0q.y * Ri00);
+      g1q.x = fma(y1q.x, Ri11, y0q.x * Ri01);
+      g1q.y = fma(y1q.y, Ri11, y0q.y * Ri01);
+      if (rg == 0) {
+        rowc[4 * q + 0] = make_double2(g0q.x, g1q.x);
+        rowc[4 * q + 1] = make_double2(y0q.x, y1q.x);
+        rowc[4 * q + 2] = make_double2(g0q.y, g1q.y);
+        rowc[4 * q + 3] = make_double2(y0q.y, y1q.y);
+      }
+    }
+    __syncthreads();
+    // ---- rank-2 update of the slab (Eq. 22)
+    if (act) {
+      const double2 ng0 = make_double2(-g0q.x, -g0q.y), ng1 = make_double2(-g1q.x, -g1q.y);
+      const int c0 = 2 * q;
+      for (int rr = rg; rr < rows; rr += RG) {
+        const int r = r0 + rr;
+        double2 x = Ts2[(size_t)rr * NQ + q];
+        const double2 gr = rowc[2 * r], yr = rowc[2 * r + 1];
+        if (c0 + 1 < r) {            // both below the diagonal
+          x.x = fma(ng1.x, yr.y, fma(ng0.x, yr.x, x.x));
+          x.y = fma(ng1.y, yr.y, fma(ng0.y, yr.x, x.y));
+        } else if (c0 > r) {         // both above
+          x.x = fma(gr.y, y1q.x, fma(gr.x, y0q.x, x.x));
+          x.y = fma(gr.y, y1q.y, fma(gr.x, y0q.y, x.y));
+        } else if (c0 == r) {        // (r,r), (r,r+1)
+          x.x = 0.0;
+          x.y = fma(gr.y, y1q.y, fma(gr.x, y0q.y, x.y));
+        } else {                     // (r,r-1), (r,r)
+          x.x = fma(ng1.x, yr.y, fma(ng0.x, yr.x, x.x));
+          x.y = 0.0;
+        }
+        Ts2[(size_t)rr * NQ + q] = x;
+      }
+    }
+    tma::fence_proxy_async();
+    __syncthreads();
+    if (tid == 0 && rows > 0) {
+      tma::store((double*)st.Ti + (size_t)w * n * n + (size_t)r0 * n, Ts, bytes);
+      tma::store_commit();
+      if (w_next >= 0) {
+        tma::store_wait_read<0>();   // the slab has left shared memory
+        load_rows(w_next);
+      }
     }
   }
   if (tid == 0) tma::store_wait_all<0>();
@@ -715,6 +974,47 @@ static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_s
   {
     // whole-walker residency on chip when the inverse fits in shared memory
     const int n = st.n;
+    // cluster-resident: CL CTAs share a walker; taken when a slab leaves room for >= 2 CTAs per SM
+    if (st.K == 0) {
+      const char* env = getenv("LRUX_PF_PATH");   // A-B measurements only
+      const bool force_cta = env && !strcmp(env, "cta");
+      // fp64 k = 1: the column-pair kernel (n/2 <= 256 threads' worth of column pairs)
+      const bool k1 = sizeof(T) == 8 && k == 1 && n <= 512 && !(env && !strcmp(env, "cluster_generic"));
+      int lg = 5;
+      while ((1 << lg) < n / 2) ++lg;
+      for (int CL = 4; CL <= 8 && !force_cta; CL *= 2) {
+        const int rpc = (n + CL - 1) / CL;
+        const size_t smc = k1 ? (size_t)rpc * n * 8 + (size_t)((256 >> lg) + 2 * CL) * (n / 2) * 16 + (size_t)n * 40
+                              : ((size_t)rpc * n + (size_t)(6 * k + 1) * n) * sizeof(T);
+        if (smc > (CL == 4 ? 56 : 100) * 1024) continue;
+        const void* kern = k1 ? (const void*)pf_cluster_k1_kernel : (const void*)pf_cluster_update_kernel<T>;
+        if (smc > 40 * 1024 &&
+            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smc) != cudaSuccess)
+          return -1;
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = CL;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.blockDim = dim3(256);
+        cfg.dynamicSmemBytes = smc;
+        cfg.stream = s;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        cfg.gridDim = dim3(CL);
+        int ncl = 0;   // co-resident clusters on the whole GPU
+        if (cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg) != cudaSuccess || ncl < 1) { cudaGetLastError(); break; }
+        cfg.gridDim = dim3((unsigned)(CL * (int)std::min<int64_t>(st.W, ncl)));
+        ProfScope ps(prof, LRUX_PROF_UPDATE, s);
+        State stc = st;
+        int a1 = k1 ? lg : k, a2 = k == 1 ? 1 : 0;
+        void* args3[3] = {&stc, &a1, &a2};
+        if (cudaLaunchKernelExC(&cfg, kern, args3) != cudaSuccess) return -1;
+        ++nl;
+        return cudaGetLastError() == cudaSuccess ? nl : -1;
+      }
+    }
     const size_t sm = ((size_t)n * n + (size_t)(4 * k + 1) * n) * sizeof(T);
     if (st.K == 0 && sm <= 200 * 1024) {
       auto kern = pf_resident_update_kernel<T>;
