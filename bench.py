@@ -435,11 +435,13 @@ def pf_update_kernel_name(n, k, esz):
     lg = 5
     while (1 << lg) < n // 2:
         lg += 1
+    if esz == 8 and k == 1 and lg <= 8 and n * n * 8 + (1024 >> lg) * (n // 2) * 16 + n * 40 <= 200 * 1024:
+        return "pf_resident_k1_kernel"
     for cl in (4, 8):
         rpc = (n + cl - 1) // cl
         smc = (rpc * n * 8 + ((256 >> lg) + 2 * cl) * (n // 2) * 16 + n * 40) if k1 \
             else (rpc * n + (6 * k + 1) * n) * esz
-        if smc <= (56 if cl == 4 else 100) * 1024:
+        if smc <= (56 if cl == 4 else 111) * 1024:
             return "pf_cluster_k1_kernel" if k1 else "pf_cluster_update_kernel"
     if (n * n + (4 * k + 1) * n) * esz <= 200 * 1024:
         return "pf_resident_update_kernel"

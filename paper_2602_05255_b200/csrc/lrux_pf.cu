@@ -742,16 +742,22 @@ __global__ void __launch_bounds__(256) pf_cluster_update_kernel(State st, int k,
 //  * below the diagonal -fma(g1c, y1r, fma(g0c, y0r, -x)) is evaluated as
 //    fma(-g1c, y1r, fma(-g0c, y0r, x)): the same value bit for bit (rounding is symmetric
 //    under negation), without the two sign flips.
-__global__ void __launch_bounds__(256, 4) pf_cluster_k1_kernel(State st, int lg_nqp) {
+// LG > 0: n/2 = 2^LG column pairs and exactly RPT rows per thread (loops fully unrolled, RPT
+// independent shared-memory loads in flight); LG = 0: sizes taken at run time.
+template <int LG, int RPT>
+__global__ void __launch_bounds__(256, 4) pf_cluster_k1_kernel(State st, int lg_dyn) {
+  const int lg_nqp = LG > 0 ? LG : lg_dyn;
   namespace cg = cooperative_groups;
   cg::cluster_group cluster = cg::this_cluster();
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  const int n = st.n, kmax = st.kmax, NQ = n >> 1;
+  const int n = LG > 0 ? (2 << LG) : st.n, kmax = st.kmax, NQ = n >> 1;
   const int CL = (int)cluster.num_blocks(), cr = (int)cluster.block_rank();
   const int ncl = (int)gridDim.x / CL, cid = (int)blockIdx.x / CL;
   const int rpc = (n + CL - 1) / CL, r0 = cr * rpc, r1 = min(n, r0 + rpc);
   const int rows = max(0, r1 - r0);
   const int RG = 256 >> lg_nqp;
+  const int rpt = LG > 0 ? RPT                                               // rows of this thread
+                         : (rows > (int)(threadIdx.x >> lg_nqp) ? (rows - 1 - (int)(threadIdx.x >> lg_nqp)) / RG + 1 : 0);
   const int tid = threadIdx.x, q = tid & ((1 << lg_nqp) - 1), rg = tid >> lg_nqp;
   const bool act = q < NQ;
   double* Ts = (double*)smem_raw;                          // [rpc][n]   this CTA's rows
@@ -792,8 +798,10 @@ __global__ void __launch_bounds__(256, 4) pf_cluster_k1_kernel(State st, int lg_
     // ---- column sums over the slab's rows
     if (act) {
       double2 acc = make_double2(0.0, 0.0);
-      for (int rr = rg; rr < rows; rr += RG) {
-        const double2 x = Ts2[(size_t)rr * NQ + q];
+#pragma unroll
+      for (int t = 0; t < (LG > 0 ? RPT : rpt); ++t) {
+        const int rr = rg + RG * t;
+        const double2 x = Ts2[rr * NQ + q];
         const double nr = nv[r0 + rr];
         acc.x = fma(x.x, nr, acc.x);
         acc.y = fma(x.y, nr, acc.y);
@@ -838,9 +846,10 @@ __global__ void __launch_bounds__(256, 4) pf_cluster_k1_kernel(State st, int lg_
     if (act) {
       const double2 ng0 = make_double2(-g0q.x, -g0q.y), ng1 = make_double2(-g1q.x, -g1q.y);
       const int c0 = 2 * q;
-      for (int rr = rg; rr < rows; rr += RG) {
-        const int r = r0 + rr;
-        double2 x = Ts2[(size_t)rr * NQ + q];
+#pragma unroll
+      for (int t = 0; t < (LG > 0 ? RPT : rpt); ++t) {
+        const int rr = rg + RG * t, r = r0 + rr;
+        double2 x = Ts2[rr * NQ + q];
         const double2 gr = rowc[2 * r], yr = rowc[2 * r + 1];
         if (c0 + 1 < r) {            // both below the diagonal
           x.x = fma(ng1.x, yr.y, fma(ng0.x, yr.x, x.x));
@@ -855,7 +864,7 @@ __global__ void __launch_bounds__(256, 4) pf_cluster_k1_kernel(State st, int lg_
           x.x = fma(ng1.x, yr.y, fma(ng0.x, yr.x, x.x));
           x.y = 0.0;
         }
-        Ts2[(size_t)rr * NQ + q] = x;
+        Ts2[rr * NQ + q] = x;
       }
     }
     tma::fence_proxy_async();
@@ -867,6 +876,147 @@ __global__ void __launch_bounds__(256, 4) pf_cluster_k1_kernel(State st, int lg_
         tma::store_wait_read<0>();   // the slab has left shared memory
         load_rows(w_next);
       }
+    }
+  }
+  if (tid == 0) tma::store_wait_all<0>();
+}
+
+// ---------------------------------------------------------------- whole-walker resident update, fp64 k = 1
+// The column-pair scheme of pf_cluster_k1_kernel with the whole inverse of a walker in ONE
+// CTA of 1024 threads (n^2 e <= ~190 KB; C3's n = 128 is the unrolled instance): no cluster
+// barrier and no DSMEM traffic, per-walker fixed costs paid once, and the chunked bulk-copy
+// pipeline of pf_resident_update_kernel (the store of chunk c frees its shared memory for
+// chunk c of the CTA's next walker while chunks c+1.. are still being updated).
+template <int LG>
+__global__ void __launch_bounds__(1024, 1) pf_resident_k1_kernel(State st, int lg_dyn) {
+  constexpr int NCH = 4;                // row chunks per walker, one bulk copy + mbarrier each
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int lg = LG > 0 ? LG : lg_dyn;
+  const int n = LG > 0 ? (2 << LG) : st.n, kmax = st.kmax, NQ = n >> 1;
+  const int RG = 1024 >> lg;
+  const int tid = threadIdx.x, q = tid & ((1 << lg) - 1), rg = tid >> lg;
+  const bool act = q < NQ;
+  const int rpc = (n + NCH - 1) / NCH;  // rows per chunk
+  double* Ts = (double*)smem_raw;                          // [n][n]
+  double2* Ts2 = (double2*)Ts;
+  double2* part = (double2*)(Ts + (size_t)n * n);          // [RG][NQ]  column sums per row group
+  double2* rowc = part + (size_t)RG * NQ;                  // [n][2]    {g0,g1},{y0,y1} of row r
+  double* nv = (double*)(rowc + (size_t)2 * n);            // [n]       new row
+  __shared__ __align__(8) uint64_t bar[NCH];
+  const int count = st.counters[0];
+  if (tid == 0) {
+    for (int c = 0; c < NCH; ++c) tma::mbar_init(&bar[c], 1);
+    tma::fence_barrier_init();
+  }
+  __syncthreads();
+  auto load_chunk = [&](int w, int c) {   // thread 0 only
+    const int r0 = c * rpc, rows = min(rpc, n - r0);
+    if (rows <= 0) return;
+    const uint32_t bytes = (uint32_t)((size_t)rows * n * sizeof(double));
+    tma::mbar_arrive_expect_tx(&bar[c], bytes);
+    tma::load(Ts + (size_t)r0 * n, (const double*)st.Ti + (size_t)w * n * n + (size_t)r0 * n, bytes, &bar[c]);
+  };
+  if (tid == 0 && (int)blockIdx.x < count)
+    for (int c = 0; c < NCH; ++c) load_chunk(st.list[blockIdx.x], c);
+  uint32_t phase = 0;
+  for (int it = blockIdx.x; it < count; it += gridDim.x) {
+    const int w = st.list[it];
+    const int w_next = it + (int)gridDim.x < count ? st.list[it + gridDim.x] : -1;
+    double* Tw = (double*)st.Ti + (size_t)w * n * n;
+    const double* pC = (const double*)st.pend_C + (size_t)w * kmax * n;
+    const double* pN = (const double*)st.pend_N + (size_t)w * kmax * n;
+    const double* Rw = (const double*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
+    const double Ri00 = Rw[0], Ri01 = Rw[1], Ri10 = Rw[st.kc], Ri11 = Rw[st.kc + 1];
+    const int p0 = st.pend_idx[(size_t)w * kmax];
+    const double2 y1q = act ? ((const double2*)pC)[q] : make_double2(0.0, 0.0);
+    for (int i = tid; i < n; i += 1024) nv[i] = pN[i];
+    __syncthreads();
+    // ---- column sums, chunk by chunk as the bulk copies land: y[c] = -sum_j Ti[j][c] N[j]
+    double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) {
+      const int r0 = c * rpc, r1 = min(n, r0 + rpc);
+      if (r0 < n) {
+        tma::mbar_wait(&bar[c], phase);
+        if (act) {
+#pragma unroll 2
+          for (int rr = r0 + rg; rr < r1; rr += RG) {
+            const double2 x = Ts2[rr * NQ + q];
+            const double nr = nv[rr];
+            acc.x = fma(x.x, nr, acc.x);
+            acc.y = fma(x.y, nr, acc.y);
+          }
+        }
+      }
+    }
+    phase ^= 1;
+    if (act) part[rg * NQ + q] = acc;
+    __syncthreads();
+    double2 y0q = make_double2(0.0, 0.0), g0q = y0q, g1q = y0q;
+    if (act) {
+      double2 sum = part[q];
+      for (int g = 1; g < RG; ++g) {
+        const double2 t = part[g * NQ + q];
+        sum.x += t.x;
+        sum.y += t.y;
+      }
+      y0q.x = (2 * q == p0) ? -sum.x + 1.0 : -sum.x;
+      y0q.y = (2 * q + 1 == p0) ? -sum.y + 1.0 : -sum.y;
+      g0q.x = fma(y1q.x, Ri10, y0q.x * Ri00);
+      g0q.y = fma(y1q.y, Ri10, y0q.y * Ri00);
+      g1q.x = fma(y1q.x, Ri11, y0q.x * Ri01);
+      g1q.y = fma(y1q.y, Ri11, y0q.y * Ri01);
+      if (rg == 0) {
+        rowc[4 * q + 0] = make_double2(g0q.x, g1q.x);
+        rowc[4 * q + 1] = make_double2(y0q.x, y1q.x);
+        rowc[4 * q + 2] = make_double2(g0q.y, g1q.y);
+        rowc[4 * q + 3] = make_double2(y0q.y, y1q.y);
+      }
+    }
+    __syncthreads();
+    // ---- rank-2 update (Eq. 22) chunk by chunk; a finished chunk is stored at once and its
+    // shared memory refilled with the same chunk of this CTA's next walker
+    const double2 ng0 = make_double2(-g0q.x, -g0q.y), ng1 = make_double2(-g1q.x, -g1q.y);
+    const int c0 = 2 * q;
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) {
+      const int r0 = c * rpc, r1 = min(n, r0 + rpc);
+      if (r0 >= n) break;
+      if (act) {
+#pragma unroll 2
+        for (int r = r0 + rg; r < r1; r += RG) {
+          double2 x = Ts2[r * NQ + q];
+          const double2 gr = rowc[2 * r], yr = rowc[2 * r + 1];
+          if (c0 + 1 < r) {            // both below the diagonal
+            x.x = fma(ng1.x, yr.y, fma(ng0.x, yr.x, x.x));
+            x.y = fma(ng1.y, yr.y, fma(ng0.y, yr.x, x.y));
+          } else if (c0 > r) {         // both above
+            x.x = fma(gr.y, y1q.x, fma(gr.x, y0q.x, x.x));
+            x.y = fma(gr.y, y1q.y, fma(gr.x, y0q.y, x.y));
+          } else if (c0 == r) {        // (r,r), (r,r+1)
+            x.x = 0.0;
+            x.y = fma(gr.y, y1q.y, fma(gr.x, y0q.y, x.y));
+          } else {                     // (r,r-1), (r,r)
+            x.x = fma(ng1.x, yr.y, fma(ng0.x, yr.x, x.x));
+            x.y = 0.0;
+          }
+          Ts2[r * NQ + q] = x;
+        }
+      }
+      tma::fence_proxy_async();
+      __syncthreads();
+      if (tid == 0) {
+        tma::store(Tw + (size_t)r0 * n, Ts + (size_t)r0 * n, (uint32_t)((size_t)(r1 - r0) * n * sizeof(double)));
+        tma::store_commit();
+        if (w_next >= 0 && c >= 1) {
+          tma::store_wait_read<1>();   // the previous chunk has left shared memory
+          load_chunk(w_next, c - 1);
+        }
+      }
+    }
+    if (tid == 0 && w_next >= 0) {
+      tma::store_wait_read<0>();
+      load_chunk(w_next, (min(n, NCH * rpc) - 1) / rpc);   // last non-empty chunk
     }
   }
   if (tid == 0) tma::store_wait_all<0>();
@@ -978,6 +1128,20 @@ static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_s
     if (st.K == 0) {
       const char* env = getenv("LRUX_PF_PATH");   // A-B measurements only
       const bool force_cta = env && !strcmp(env, "cta");
+      // fp64 k = 1 with the whole inverse in one CTA's shared memory: column-pair kernel, 1024 threads
+      if (sizeof(T) == 8 && k == 1 && !force_cta && !(env && !strncmp(env, "cluster", 7))) {
+        int lg1 = 5;
+        while ((1 << lg1) < n / 2) ++lg1;
+        const size_t sm1 = (size_t)n * n * 8 + (size_t)(1024 >> lg1) * (n / 2) * 16 + (size_t)n * 40;
+        if (lg1 <= 8 && sm1 <= 200 * 1024) {
+          auto kern = ((2 << lg1) == n && lg1 == 6) ? pf_resident_k1_kernel<6> : pf_resident_k1_kernel<0>;
+          if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm1) != cudaSuccess)
+            return -1;
+          ProfScope ps(prof, LRUX_PROF_UPDATE, s);
+          kern<<<pgrid(num_sms, 1, st.W), 1024, sm1, s>>>(st, lg1); ++nl;
+          return cudaGetLastError() == cudaSuccess ? nl : -1;
+        }
+      }
       // fp64 k = 1: the column-pair kernel (n/2 <= 256 threads' worth of column pairs)
       const bool k1 = sizeof(T) == 8 && k == 1 && n <= 512 && !(env && !strcmp(env, "cluster_generic"));
       int lg = 5;
@@ -986,8 +1150,15 @@ static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_s
         const int rpc = (n + CL - 1) / CL;
         const size_t smc = k1 ? (size_t)rpc * n * 8 + (size_t)((256 >> lg) + 2 * CL) * (n / 2) * 16 + (size_t)n * 40
                               : ((size_t)rpc * n + (size_t)(6 * k + 1) * n) * sizeof(T);
-        if (smc > (CL == 4 ? 56 : 100) * 1024) continue;
-        const void* kern = k1 ? (const void*)pf_cluster_k1_kernel : (const void*)pf_cluster_update_kernel<T>;
+        if (smc > (CL == 4 ? 56 : 111) * 1024) continue;
+        // unrolled instance when n/2 is a power of two and the slab splits evenly over the row groups
+        const bool even = k1 && (2 << lg) == n && n % CL == 0 && rpc % (256 >> lg) == 0;
+        const int rpt = even ? rpc / (256 >> lg) : 0;
+        const void* kern = !k1 ? (const void*)pf_cluster_update_kernel<T>
+                         : (lg == 6 && rpt == 8) ? (const void*)pf_cluster_k1_kernel<6, 8>
+                         : (lg == 7 && rpt == 16) ? (const void*)pf_cluster_k1_kernel<7, 16>
+                         : (lg == 5 && rpt == 2) ? (const void*)pf_cluster_k1_kernel<5, 2>
+                         : (const void*)pf_cluster_k1_kernel<0, 0>;
         if (smc > 40 * 1024 &&
             cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smc) != cudaSuccess)
           return -1;
