@@ -883,65 +883,98 @@ __global__ void __launch_bounds__(256, 4) pf_cluster_k1_kernel(State st, int lg_
 
 // ---------------------------------------------------------------- whole-walker resident update, fp64 k = 1
 // The column-pair scheme of pf_cluster_k1_kernel with the whole inverse of a walker in ONE
-// CTA of 1024 threads (n^2 e <= ~190 KB; C3's n = 128 is the unrolled instance): no cluster
-// barrier and no DSMEM traffic, per-walker fixed costs paid once, and the chunked bulk-copy
-// pipeline of pf_resident_update_kernel (the store of chunk c frees its shared memory for
-// chunk c of the CTA's next walker while chunks c+1.. are still being updated).
+// CTA of 1024 threads (C3's n = 128 is the unrolled instance): no cluster barrier, no DSMEM
+// traffic, per-walker fixed costs paid once.  Everything the next walker needs is in flight
+// while the current one is updated:
+//  * the inverse moves in NCH row chunks through NB = NCH+1 rotating shared-memory buffers
+//    (one bulk copy + mbarrier each): chunk c of the next walker lands in the buffer of
+//    chunk c-1 of the current one as soon as that has been stored, chunk 0 in the spare;
+//  * the walker's small operands (new row, gathered column, R'^-1, slot) are staged two-deep
+//    with cp.async, the walker index is read two items ahead;
+//  * the column sums of the 1024/2^LG row groups are combined in two levels (4-way each for
+//    LG = 6) instead of every thread re-adding all of them: the kernel is bound by
+//    shared-memory bandwidth, not by HBM, until these are trimmed.
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(tma::smem_u32(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void* smem_dst, const void* gsrc) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(tma::smem_u32(smem_dst)), "l"(gsrc) : "memory");
+}
+
 template <int LG>
 __global__ void __launch_bounds__(1024, 1) pf_resident_k1_kernel(State st, int lg_dyn) {
-  constexpr int NCH = 4;                // row chunks per walker, one bulk copy + mbarrier each
+  constexpr int NCH = 4, NB = NCH + 1;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int lg = LG > 0 ? LG : lg_dyn;
   const int n = LG > 0 ? (2 << LG) : st.n, kmax = st.kmax, NQ = n >> 1;
-  const int RG = 1024 >> lg;
+  const int RG = 1024 >> lg, R2 = RG >> 2;
   const int tid = threadIdx.x, q = tid & ((1 << lg) - 1), rg = tid >> lg;
   const bool act = q < NQ;
   const int rpc = (n + NCH - 1) / NCH;  // rows per chunk
-  double* Ts = (double*)smem_raw;                          // [n][n]
-  double2* Ts2 = (double2*)Ts;
-  double2* part = (double2*)(Ts + (size_t)n * n);          // [RG][NQ]  column sums per row group
-  double2* rowc = part + (size_t)RG * NQ;                  // [n][2]    {g0,g1},{y0,y1} of row r
-  double* nv = (double*)(rowc + (size_t)2 * n);            // [n]       new row
-  __shared__ __align__(8) uint64_t bar[NCH];
-  const int count = st.counters[0];
+  const int cstride2 = rpc * NQ;        // double2 per chunk buffer
+  const int STG = 2 * n + 6;            // doubles per staging slot: N row, C row, R'^-1 (2x2), slot index
+  double2* Tb2 = (double2*)smem_raw;                       // [NB][rpc][n/2]
+  double2* part = Tb2 + (size_t)NB * cstride2;             // [RG][NQ]   column sums per row group
+  double2* part2 = part + (size_t)RG * NQ;                 // [R2][NQ]   ... per four row groups
+  double2* rowc = part2 + (size_t)R2 * NQ;                 // [n][2]     {g0,g1},{y0,y1} of row r
+  double* stg = (double*)(rowc + (size_t)2 * n);           // [2][STG]
+  __shared__ __align__(8) uint64_t bar[NB];
+  const int count = st.counters[0], grid = (int)gridDim.x;
   if (tid == 0) {
-    for (int c = 0; c < NCH; ++c) tma::mbar_init(&bar[c], 1);
+    for (int c = 0; c < NB; ++c) tma::mbar_init(&bar[c], 1);
     tma::fence_barrier_init();
   }
   __syncthreads();
-  auto load_chunk = [&](int w, int c) {   // thread 0 only
+  auto load_chunk = [&](int w, int c, int g) {   // thread 0 only; g = position in the chunk sequence
     const int r0 = c * rpc, rows = min(rpc, n - r0);
     if (rows <= 0) return;
+    const int b = g % NB;
     const uint32_t bytes = (uint32_t)((size_t)rows * n * sizeof(double));
-    tma::mbar_arrive_expect_tx(&bar[c], bytes);
-    tma::load(Ts + (size_t)r0 * n, (const double*)st.Ti + (size_t)w * n * n + (size_t)r0 * n, bytes, &bar[c]);
+    tma::mbar_arrive_expect_tx(&bar[b], bytes);
+    tma::load(Tb2 + (size_t)b * cstride2, (const double*)st.Ti + (size_t)w * n * n + (size_t)r0 * n, bytes, &bar[b]);
   };
-  if (tid == 0 && (int)blockIdx.x < count)
-    for (int c = 0; c < NCH; ++c) load_chunk(st.list[blockIdx.x], c);
-  uint32_t phase = 0;
-  for (int it = blockIdx.x; it < count; it += gridDim.x) {
-    const int w = st.list[it];
-    const int w_next = it + (int)gridDim.x < count ? st.list[it + gridDim.x] : -1;
-    double* Tw = (double*)st.Ti + (size_t)w * n * n;
-    const double* pC = (const double*)st.pend_C + (size_t)w * kmax * n;
-    const double* pN = (const double*)st.pend_N + (size_t)w * kmax * n;
+  auto stage = [&](int w, int slot) {            // small operands of walker w -> staging slot
+    double* d = stg + slot * STG;
     const double* Rw = (const double*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
-    const double Ri00 = Rw[0], Ri01 = Rw[1], Ri10 = Rw[st.kc], Ri11 = Rw[st.kc + 1];
-    const int p0 = st.pend_idx[(size_t)w * kmax];
-    const double2 y1q = act ? ((const double2*)pC)[q] : make_double2(0.0, 0.0);
-    for (int i = tid; i < n; i += 1024) nv[i] = pN[i];
+    if (tid < NQ) cp_async16(d + 2 * tid, (const double*)st.pend_N + (size_t)w * kmax * n + 2 * tid);
+    else if (tid < 2 * NQ) cp_async16(d + n + 2 * (tid - NQ), (const double*)st.pend_C + (size_t)w * kmax * n + 2 * (tid - NQ));
+    else if (tid == 2 * NQ) cp_async16(d + 2 * n, Rw);
+    else if (tid == 2 * NQ + 1) cp_async16(d + 2 * n + 2, Rw + st.kc);
+    else if (tid == 2 * NQ + 2) cp_async4(d + 2 * n + 4, st.pend_idx + (size_t)w * kmax);
+  };
+  int w = (int)blockIdx.x < count ? st.list[blockIdx.x] : -1;
+  int w1 = (int)blockIdx.x + grid < count ? st.list[blockIdx.x + grid] : -1;
+  if (w >= 0) {
+    if (tid == 0)
+      for (int c = 0; c < NCH; ++c) load_chunk(w, c, c);
+    stage(w, 0);
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  int j = 0;
+  for (int it = blockIdx.x; it < count; it += grid, ++j) {
+    const int w2 = it + 2 * grid < count ? st.list[it + 2 * grid] : -1;   // needed one item from now
+    const int slot = j & 1, g0 = j * NCH;
+    double* Tw = (double*)st.Ti + (size_t)w * n * n;
+    if (w1 >= 0) stage(w1, slot ^ 1);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    asm volatile("cp.async.wait_group 1;" ::: "memory");
     __syncthreads();
+    const double* sd = stg + slot * STG;
+    const double* nv = sd;
+    const double2 y1q = act ? ((const double2*)(sd + n))[q] : make_double2(0.0, 0.0);
     // ---- column sums, chunk by chunk as the bulk copies land: y[c] = -sum_j Ti[j][c] N[j]
     double2 acc = make_double2(0.0, 0.0);
 #pragma unroll
     for (int c = 0; c < NCH; ++c) {
       const int r0 = c * rpc, r1 = min(n, r0 + rpc);
       if (r0 < n) {
-        tma::mbar_wait(&bar[c], phase);
+        const int g = g0 + c, b = g % NB;
+        tma::mbar_wait(&bar[b], (uint32_t)((g / NB) & 1));
         if (act) {
+          const double2* Tc = Tb2 + (size_t)b * cstride2 - (size_t)r0 * NQ;
 #pragma unroll 2
           for (int rr = r0 + rg; rr < r1; rr += RG) {
-            const double2 x = Ts2[rr * NQ + q];
+            const double2 x = Tc[rr * NQ + q];
             const double nr = nv[rr];
             acc.x = fma(x.x, nr, acc.x);
             acc.y = fma(x.y, nr, acc.y);
@@ -949,14 +982,31 @@ __global__ void __launch_bounds__(1024, 1) pf_resident_k1_kernel(State st, int l
         }
       }
     }
-    phase ^= 1;
     if (act) part[rg * NQ + q] = acc;
+    __syncthreads();
+    // the spare buffer (last chunk of the previous walker, stored long ago) takes chunk 0 of the next walker
+    if (tid == 0 && w1 >= 0) {
+      tma::store_wait_read<0>();
+      load_chunk(w1, 0, g0 + NCH);
+    }
+    if (act && rg < R2) {
+      double2 sum = part[(4 * rg) * NQ + q];
+#pragma unroll
+      for (int g = 1; g < 4; ++g) {
+        const double2 t = part[(4 * rg + g) * NQ + q];
+        sum.x += t.x;
+        sum.y += t.y;
+      }
+      part2[rg * NQ + q] = sum;
+    }
     __syncthreads();
     double2 y0q = make_double2(0.0, 0.0), g0q = y0q, g1q = y0q;
     if (act) {
-      double2 sum = part[q];
-      for (int g = 1; g < RG; ++g) {
-        const double2 t = part[g * NQ + q];
+      const double Ri00 = sd[2 * n], Ri01 = sd[2 * n + 1], Ri10 = sd[2 * n + 2], Ri11 = sd[2 * n + 3];
+      const int p0 = *(const int*)(sd + 2 * n + 4);
+      double2 sum = part2[q];
+      for (int g = 1; g < R2; ++g) {
+        const double2 t = part2[g * NQ + q];
         sum.x += t.x;
         sum.y += t.y;
       }
@@ -974,18 +1024,20 @@ __global__ void __launch_bounds__(1024, 1) pf_resident_k1_kernel(State st, int l
       }
     }
     __syncthreads();
-    // ---- rank-2 update (Eq. 22) chunk by chunk; a finished chunk is stored at once and its
-    // shared memory refilled with the same chunk of this CTA's next walker
+    // ---- rank-2 update (Eq. 22) chunk by chunk; a finished chunk is stored at once, and the
+    // buffer of the chunk stored before it is refilled with the next walker's data
     const double2 ng0 = make_double2(-g0q.x, -g0q.y), ng1 = make_double2(-g1q.x, -g1q.y);
     const int c0 = 2 * q;
 #pragma unroll
     for (int c = 0; c < NCH; ++c) {
       const int r0 = c * rpc, r1 = min(n, r0 + rpc);
       if (r0 >= n) break;
+      const int b = (g0 + c) % NB;
+      double2* Tc = Tb2 + (size_t)b * cstride2 - (size_t)r0 * NQ;
       if (act) {
 #pragma unroll 2
         for (int r = r0 + rg; r < r1; r += RG) {
-          double2 x = Ts2[r * NQ + q];
+          double2 x = Tc[r * NQ + q];
           const double2 gr = rowc[2 * r], yr = rowc[2 * r + 1];
           if (c0 + 1 < r) {            // both below the diagonal
             x.x = fma(ng1.x, yr.y, fma(ng0.x, yr.x, x.x));
@@ -1000,25 +1052,24 @@ __global__ void __launch_bounds__(1024, 1) pf_resident_k1_kernel(State st, int l
             x.x = fma(ng1.x, yr.y, fma(ng0.x, yr.x, x.x));
             x.y = 0.0;
           }
-          Ts2[r * NQ + q] = x;
+          Tc[r * NQ + q] = x;
         }
       }
       tma::fence_proxy_async();
       __syncthreads();
       if (tid == 0) {
-        tma::store(Tw + (size_t)r0 * n, Ts + (size_t)r0 * n, (uint32_t)((size_t)(r1 - r0) * n * sizeof(double)));
+        tma::store(Tw + (size_t)r0 * n, Tb2 + (size_t)b * cstride2, (uint32_t)((size_t)(r1 - r0) * n * sizeof(double)));
         tma::store_commit();
-        if (w_next >= 0 && c >= 1) {
-          tma::store_wait_read<1>();   // the previous chunk has left shared memory
-          load_chunk(w_next, c - 1);
+        if (w1 >= 0 && c >= 1) {
+          tma::store_wait_read<1>();   // chunk c-1 has left shared memory: its buffer takes chunk c of the next walker
+          load_chunk(w1, c, g0 + NCH + c);
         }
       }
     }
-    if (tid == 0 && w_next >= 0) {
-      tma::store_wait_read<0>();
-      load_chunk(w_next, (min(n, NCH * rpc) - 1) / rpc);   // last non-empty chunk
-    }
+    w = w1;
+    w1 = w2;
   }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
   if (tid == 0) tma::store_wait_all<0>();
 }
 
@@ -1132,8 +1183,10 @@ static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_s
       if (sizeof(T) == 8 && k == 1 && !force_cta && !(env && !strncmp(env, "cluster", 7))) {
         int lg1 = 5;
         while ((1 << lg1) < n / 2) ++lg1;
-        const size_t sm1 = (size_t)n * n * 8 + (size_t)(1024 >> lg1) * (n / 2) * 16 + (size_t)n * 40;
-        if (lg1 <= 8 && sm1 <= 200 * 1024) {
+        const int rg1 = 1024 >> lg1;
+        const size_t sm1 = (size_t)5 * ((n + 3) / 4) * n * 8 + (size_t)(rg1 + rg1 / 4) * (n / 2) * 16 +
+                           (size_t)n * 32 + (size_t)2 * (2 * n + 6) * 8;
+        if (lg1 <= 7 && sm1 <= 224 * 1024) {
           auto kern = ((2 << lg1) == n && lg1 == 6) ? pf_resident_k1_kernel<6> : pf_resident_k1_kernel<0>;
           if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm1) != cudaSuccess)
             return -1;
