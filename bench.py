@@ -437,7 +437,7 @@ def pf_update_kernel_name(n, k, esz):
         lg += 1
     rg1 = 1024 >> lg
     if esz == 8 and k == 1 and lg <= 7 and (5 * ((n + 3) // 4) * n * 8 + (rg1 + rg1 // 4) * (n // 2) * 16
-                                            + n * 32 + 2 * (2 * n + 6) * 8) <= 224 * 1024:
+                                            + n * 32 + 2 * (2 * n + 6) * 8) <= 226 * 1024:
         return "pf_resident_k1_kernel"
     for cl in (4, 8):
         rpc = (n + cl - 1) // cl

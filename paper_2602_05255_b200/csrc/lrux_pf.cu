@@ -901,9 +901,9 @@ __device__ __forceinline__ void cp_async4(void* smem_dst, const void* gsrc) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(tma::smem_u32(smem_dst)), "l"(gsrc) : "memory");
 }
 
-template <int LG>
+template <int LG, int NB>
 __global__ void __launch_bounds__(1024, 1) pf_resident_k1_kernel(State st, int lg_dyn) {
-  constexpr int NCH = 4, NB = NCH + 1;
+  constexpr int NCH = 4, SP = NB - NCH;   // SP spare buffers: the next walker's loads run SP chunks ahead
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int lg = LG > 0 ? LG : lg_dyn;
   const int n = LG > 0 ? (2 << LG) : st.n, kmax = st.kmax, NQ = n >> 1;
@@ -912,7 +912,7 @@ __global__ void __launch_bounds__(1024, 1) pf_resident_k1_kernel(State st, int l
   const bool act = q < NQ;
   const int rpc = (n + NCH - 1) / NCH;  // rows per chunk
   const int cstride2 = rpc * NQ;        // double2 per chunk buffer
-  const int STG = 2 * n + 6;            // doubles per staging slot: N row, C row, R'^-1 (2x2), slot index
+  const int STG = 2 * n + 6;            // doubles per staging slot: N row, C row, R'^-1 (2x2), {slot index, next walker}
   double2* Tb2 = (double2*)smem_raw;                       // [NB][rpc][n/2]
   double2* part = Tb2 + (size_t)NB * cstride2;             // [RG][NQ]   column sums per row group
   double2* part2 = part + (size_t)RG * NQ;                 // [R2][NQ]   ... per four row groups
@@ -933,7 +933,7 @@ __global__ void __launch_bounds__(1024, 1) pf_resident_k1_kernel(State st, int l
     tma::mbar_arrive_expect_tx(&bar[b], bytes);
     tma::load(Tb2 + (size_t)b * cstride2, (const double*)st.Ti + (size_t)w * n * n + (size_t)r0 * n, bytes, &bar[b]);
   };
-  auto stage = [&](int w, int slot) {            // small operands of walker w -> staging slot
+  auto stage = [&](int w, int slot, const int* next) {   // small operands of walker w -> staging slot
     double* d = stg + slot * STG;
     const double* Rw = (const double*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
     if (tid < NQ) cp_async16(d + 2 * tid, (const double*)st.pend_N + (size_t)w * kmax * n + 2 * tid);
@@ -941,25 +941,27 @@ __global__ void __launch_bounds__(1024, 1) pf_resident_k1_kernel(State st, int l
     else if (tid == 2 * NQ) cp_async16(d + 2 * n, Rw);
     else if (tid == 2 * NQ + 1) cp_async16(d + 2 * n + 2, Rw + st.kc);
     else if (tid == 2 * NQ + 2) cp_async4(d + 2 * n + 4, st.pend_idx + (size_t)w * kmax);
+    else if (tid == 2 * NQ + 3 && next) cp_async4((int*)(d + 2 * n + 4) + 1, next);   // walker after w in this CTA's sequence
   };
   int w = (int)blockIdx.x < count ? st.list[blockIdx.x] : -1;
-  int w1 = (int)blockIdx.x + grid < count ? st.list[blockIdx.x + grid] : -1;
   if (w >= 0) {
     if (tid == 0)
       for (int c = 0; c < NCH; ++c) load_chunk(w, c, c);
-    stage(w, 0);
+    stage(w, 0, (int)blockIdx.x + grid < count ? st.list + blockIdx.x + grid : nullptr);
   }
   asm volatile("cp.async.commit_group;" ::: "memory");
   int j = 0;
   for (int it = blockIdx.x; it < count; it += grid, ++j) {
-    const int w2 = it + 2 * grid < count ? st.list[it + 2 * grid] : -1;   // needed one item from now
     const int slot = j & 1, g0 = j * NCH;
     double* Tw = (double*)st.Ti + (size_t)w * n * n;
-    if (w1 >= 0) stage(w1, slot ^ 1);
-    asm volatile("cp.async.commit_group;" ::: "memory");
-    asm volatile("cp.async.wait_group 1;" ::: "memory");
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
     const double* sd = stg + slot * STG;
+    // the next walker's index arrived with this walker's operands; its operands (and the index after
+    // it) are requested now and have this whole item to land
+    const int w1 = it + grid < count ? *((const int*)(sd + 2 * n + 4) + 1) : -1;
+    if (w1 >= 0) stage(w1, slot ^ 1, it + 2 * grid < count ? st.list + it + 2 * grid : nullptr);
+    asm volatile("cp.async.commit_group;" ::: "memory");
     const double* nv = sd;
     const double2 y1q = act ? ((const double2*)(sd + n))[q] : make_double2(0.0, 0.0);
     // ---- column sums, chunk by chunk as the bulk copies land: y[c] = -sum_j Ti[j][c] N[j]
@@ -984,10 +986,10 @@ __global__ void __launch_bounds__(1024, 1) pf_resident_k1_kernel(State st, int l
     }
     if (act) part[rg * NQ + q] = acc;
     __syncthreads();
-    // the spare buffer (last chunk of the previous walker, stored long ago) takes chunk 0 of the next walker
+    // the spare buffers (last chunks of the previous walker, stored long ago) take the first chunks of the next walker
     if (tid == 0 && w1 >= 0) {
       tma::store_wait_read<0>();
-      load_chunk(w1, 0, g0 + NCH);
+      for (int c = 0; c < SP; ++c) load_chunk(w1, c, g0 + NCH + c);
     }
     if (act && rg < R2) {
       double2 sum = part[(4 * rg) * NQ + q];
@@ -1060,14 +1062,13 @@ __global__ void __launch_bounds__(1024, 1) pf_resident_k1_kernel(State st, int l
       if (tid == 0) {
         tma::store(Tw + (size_t)r0 * n, Tb2 + (size_t)b * cstride2, (uint32_t)((size_t)(r1 - r0) * n * sizeof(double)));
         tma::store_commit();
-        if (w1 >= 0 && c >= 1) {
-          tma::store_wait_read<1>();   // chunk c-1 has left shared memory: its buffer takes chunk c of the next walker
-          load_chunk(w1, c, g0 + NCH + c);
+        if (w1 >= 0 && c >= 1 && c - 1 + SP < NCH) {
+          tma::store_wait_read<1>();   // chunk c-1 has left shared memory: its buffer takes chunk c-1+SP of the next walker
+          load_chunk(w1, c - 1 + SP, g0 + NCH + c - 1 + SP);
         }
       }
     }
     w = w1;
-    w1 = w2;
   }
   asm volatile("cp.async.wait_group 0;" ::: "memory");
   if (tid == 0) tma::store_wait_all<0>();
@@ -1184,10 +1185,15 @@ static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_s
         int lg1 = 5;
         while ((1 << lg1) < n / 2) ++lg1;
         const int rg1 = 1024 >> lg1;
-        const size_t sm1 = (size_t)5 * ((n + 3) / 4) * n * 8 + (size_t)(rg1 + rg1 / 4) * (n / 2) * 16 +
-                           (size_t)n * 32 + (size_t)2 * (2 * n + 6) * 8;
-        if (lg1 <= 7 && sm1 <= 224 * 1024) {
-          auto kern = ((2 << lg1) == n && lg1 == 6) ? pf_resident_k1_kernel<6> : pf_resident_k1_kernel<0>;
+        const size_t smx = (size_t)(rg1 + rg1 / 4) * (n / 2) * 16 + (size_t)n * 32 + (size_t)2 * (2 * n + 6) * 8;
+        const size_t chunk = (size_t)((n + 3) / 4) * n * 8;
+        const bool nb5 = env && !strcmp(env, "nb5");
+        const int nb = (!nb5 && 6 * chunk + smx <= 226 * 1024) ? 6 : 5;   // two spare chunk buffers when they fit
+        const size_t sm1 = nb * chunk + smx;
+        if (lg1 <= 7 && sm1 <= 226 * 1024) {
+          const bool c3 = (2 << lg1) == n && lg1 == 6;
+          auto kern = c3 ? (nb == 6 ? pf_resident_k1_kernel<6, 6> : pf_resident_k1_kernel<6, 5>)
+                         : (nb == 6 ? pf_resident_k1_kernel<0, 6> : pf_resident_k1_kernel<0, 5>);
           if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm1) != cudaSuccess)
             return -1;
           ProfScope ps(prof, LRUX_PROF_UPDATE, s);
