@@ -132,6 +132,25 @@ lrux_status_t lrux_det_attach(lrux_handle_t* h, int64_t W, int32_t n, int32_t km
 lrux_status_t lrux_pf_attach(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, int32_t K,
                              lrux_dtype_t dt, void* d_state, size_t state_bytes, int32_t* d_info);
 
+/* ---------------------------------------------------------------- refresh (accuracy guard)
+ * SURVEY.md §8(f) f3.  The paper only advises double precision against the error that
+ * accumulates in a tracked inverse and is silent on recomputation
+ * (reading 18); plain fp64 Woodbury on the paper's workloads drifts to 1e-9
+ * relative in a ratio after a few hundred accepted updates (reading 14).
+ * lrux_*_refresh rebuilds A^-1 and the amplitude (phase, log abs) of EVERY walker from
+ * scratch from the caller's current matrices, with the kernels of lrux_*_init (step a0),
+ * on the existing handle: d_A is [W][n][n] row-major DEVICE memory, the matrices the
+ * walkers have reached (the library stores no A; Pf: only the strict upper triangle is
+ * read), valid until the work completes on `stream`.  Unflushed delay factors are
+ * discarded (they describe the same A), a pending proposal is dropped, d_info bit 1 is
+ * re-evaluated (set again if a matrix is singular; that walker's state is then
+ * undefined), bits 2 and 4 and the flush totals are kept.  Cost O(n^3) per walker: call
+ * it on a schedule (every few hundred accepted updates), not per step.  Asynchronous,
+ * stream-ordered.  Errors: LRUX_EINVAL (null pointer), LRUX_ESTATE (wrong handle kind),
+ * LRUX_ECUDA. */
+lrux_status_t lrux_det_refresh(lrux_handle_t h, const void* d_A, void* stream);
+lrux_status_t lrux_pf_refresh(lrux_handle_t h, const void* d_A, void* stream);
+
 /* ---------------------------------------------------------------- profiling
  * Device time per kernel class, taken with CUDA events the library records on the
  * caller's stream directly around its own launches (bench.py's roofline figures:

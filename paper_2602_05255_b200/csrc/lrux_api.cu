@@ -238,6 +238,21 @@ lrux_status_t lrux_pf_get_inverse(lrux_handle_t h, void* d_out, void* stream) {
   return LRUX_OK;
 }
 
+static lrux_status_t refresh(lrux_handle_t h, const void* d_A, void* stream) {
+  if (!d_A) return LRUX_EINVAL;
+  LRUX_COUNT(h, launch_refresh(h->st, d_A, h->num_sms, (cudaStream_t)stream));
+  h->pending_k = 0;
+  return LRUX_OK;
+}
+lrux_status_t lrux_det_refresh(lrux_handle_t h, const void* d_A, void* stream) {
+  LRUX_CHECK_HANDLE(h, KIND_DET);
+  return refresh(h, d_A, stream);
+}
+lrux_status_t lrux_pf_refresh(lrux_handle_t h, const void* d_A, void* stream) {
+  LRUX_CHECK_HANDLE(h, KIND_PF);
+  return refresh(h, d_A, stream);
+}
+
 lrux_status_t lrux_get_flush_count(lrux_handle_t h, int64_t* d_out, void* stream) {
   if (!h || !d_out) return LRUX_EINVAL;
   if (cudaMemcpyAsync(d_out, h->st.counters + 4, 16, cudaMemcpyDeviceToDevice,

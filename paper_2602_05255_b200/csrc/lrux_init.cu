@@ -265,16 +265,26 @@ parlett_reid_kernel(T* __restrict__ Mall, int n, T* __restrict__ phase_out,
 }
 
 // ---------------------------------------------------------------- launchers
+// refresh: bit 1 (singular matrix) is re-evaluated, the other sticky bits stay
+__global__ void info_clear_singular_kernel(int32_t* __restrict__ info, int64_t W) {
+  const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (w < W) info[w] &= ~1;
+}
+
 template <typename T>
-static int init_impl(const State& st, const void* d_A0, int num_sms, cudaStream_t s) {
+static int init_impl(const State& st, const void* d_A0, int num_sms, cudaStream_t s, bool refresh = false) {
   const int n = st.n;
   const size_t W = (size_t)st.W;
   int nl = 0;
-  cudaMemsetAsync(st.info, 0, W * 4, s);
+  if (refresh) {
+    info_clear_singular_kernel<<<(unsigned)((W + 255) / 256), 256, 0, s>>>(st.info, (int64_t)W); ++nl;
+  } else {
+    cudaMemsetAsync(st.info, 0, W * 4, s);
+  }
   cudaMemsetAsync(st.fill, 0, W * 4, s);
   cudaMemsetAsync(st.nupd, 0, W * 4, s);
   cudaMemsetAsync(st.pend_ok, 0, W, s);
-  cudaMemsetAsync(st.counters, 0, 32, s);
+  cudaMemsetAsync(st.counters, 0, refresh ? 16 : 32, s);   // a refresh keeps the flush totals
   if (st.pend_cnt) cudaMemsetAsync(st.pend_cnt, 0, W * 4, s);
   const size_t smem_gj = 2 * (size_t)n * sizeof(T) + (size_t)n * 4;
   const size_t smem_pr = 2 * (size_t)n * sizeof(T);
@@ -316,6 +326,11 @@ int launch_det_init(const State& st, const void* d_A0, int num_sms, cudaStream_t
 int launch_pf_init(const State& st, const void* d_A0, int num_sms, cudaStream_t s) {
   return st.dt == LRUX_F64 ? init_impl<double>(st, d_A0, num_sms, s)
                            : init_impl<cplx>(st, d_A0, num_sms, s);
+}
+
+int launch_refresh(const State& st, const void* d_A, int num_sms, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? init_impl<double>(st, d_A, num_sms, s, true)
+                           : init_impl<cplx>(st, d_A, num_sms, s, true);
 }
 
 int launch_get_amplitude(const State& st, void* d_phase, double* d_logabs, cudaStream_t s) {

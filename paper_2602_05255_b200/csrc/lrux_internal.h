@@ -93,6 +93,7 @@ size_t state_layout(State* st, void* base, int64_t W, int32_t n, int32_t kmax, i
 // launchers (each returns the number of kernels it enqueued, or -1 on a CUDA error)
 int launch_det_init(const State& st, const void* d_A0, int num_sms, cudaStream_t s);
 int launch_pf_init(const State& st, const void* d_A0, int num_sms, cudaStream_t s);
+int launch_refresh(const State& st, const void* d_A, int num_sms, cudaStream_t s);
 // blocked in-place inverse of st.Ti (lrux_init_blocked.cu); 0 = not applicable
 int launch_gj_blocked(const State& st, bool write_amp, int num_sms, cudaStream_t s);
 int launch_det_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,

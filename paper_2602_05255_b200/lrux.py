@@ -29,6 +29,8 @@ SIGNATURES = {
     "lrux_pf_init": [C.POINTER(_vp), _i64, _i32, _i32, _i32, C.c_int, _vp, _vp, _sz, _vp, _vp],
     "lrux_det_attach": [C.POINTER(_vp), _i64, _i32, _i32, _i32, C.c_int, _vp, _sz, _vp],
     "lrux_pf_attach": [C.POINTER(_vp), _i64, _i32, _i32, _i32, C.c_int, _vp, _sz, _vp],
+    "lrux_det_refresh": [_vp, _vp, _vp],
+    "lrux_pf_refresh": [_vp, _vp, _vp],
     "lrux_det_ratio": [_vp, _i32, _vp, _vp, _vp, _vp],
     "lrux_pf_ratio": [_vp, _i32, _vp, _vp, _vp, _vp],
     "lrux_det_accept": [_vp, _vp, _vp],
@@ -166,6 +168,14 @@ class _Walkers:
 
     def flush(self, stream=None):
         _check(self._fn("flush")(self._h, _stream(stream)))
+
+    def refresh(self, A, stream=None):
+        """lrux_*_refresh: rebuild A^-1 and the amplitude from the walkers' current matrices
+        A [W][n][n] (the library stores none)."""
+        if not A.is_cuda or tuple(A.shape) != (self.W, self.n, self.n) or A.dtype != self.dtype:
+            raise ValueError("A must be a CUDA tensor [W][n][n] of the walkers' dtype")
+        A = A.contiguous()
+        _check(self._fn("refresh")(self._h, _ptr(A), _stream(stream)))
 
     def get_amplitude(self, stream=None):
         phase = torch.empty(self.W, dtype=self.dtype, device=self.device)

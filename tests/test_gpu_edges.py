@@ -126,3 +126,80 @@ def test_delay_depth_limit_is_reported():
     with pytest.raises(lrux.LruxError) as e:
         lrux.DetWalkers(torch.eye(16, dtype=torch.complex128, device=DEV)[None], kmax=8, K=64)
     assert e.value.status == lrux.EUNSUPPORTED
+
+
+@pytest.mark.parametrize("kind,dtype,K", [("det", np.float64, 0), ("det", np.complex128, 3), ("pf", np.float64, 0),
+                                          ("pf", np.float64, 2)])
+def test_refresh_rebuilds_inverse_and_amplitude(kind, dtype, K):
+    """lrux_*_refresh: after a run of accepted updates — with factors still
+    unflushed when K > 0 — a refresh from the walkers' current matrices gives the from-scratch
+    inverse and amplitude of the oracle, drops the delay factors, and the chain goes on."""
+    rng = np.random.default_rng(77 + K)
+    W, n, k = 3, 24, 2
+    cplx = dtype == np.complex128
+
+    def rnd(*shape):
+        x = rng.standard_normal(shape)
+        return x + 1j * rng.standard_normal(shape) if cplx else x
+
+    def skew(x):
+        return np.triu(x, 1) - np.triu(x, 1).transpose(0, 2, 1)
+
+    A = skew(rnd(W, n, n)) if kind == "pf" else rnd(W, n, n) + 3 * np.eye(n)
+    wk = (lrux.PfWalkers if kind == "pf" else lrux.DetWalkers)(_t(A), kmax=k, K=K)
+    ones = torch.ones(W, dtype=torch.uint8, device=DEV)
+
+    def step(A):
+        idx = np.stack([rng.permutation(n)[:k] for _ in range(W)]).astype(np.int32)
+        B = A.copy()
+        rows = np.empty((W, k, n), dtype=A.dtype)
+        for w in range(W):
+            new = rnd(k, n)
+            if kind == "pf":
+                for a, p in enumerate(idx[w]):
+                    new[a, p] = 0.0
+                for a, p in enumerate(idx[w]):          # crossing entries stay skew
+                    for b, q in enumerate(idx[w]):
+                        if b > a:
+                            new[b, p] = -new[a, q]
+                for a, p in enumerate(idx[w]):
+                    B[w, p, :] = new[a]
+                    B[w, :, p] = -new[a]
+            else:
+                B[w, idx[w], :] = new
+            rows[w] = new
+        r = wk.ratio_(_t(idx), _t(rows)).cpu().numpy()
+        wk.accept(ones)
+        return B, r
+
+    amp = orc.slogpf if kind == "pf" else orc.slogdet
+    for _ in range(5):        # K = 3 / 2: the buffers are partly filled when the refresh comes
+        A, _ = step(A)
+    # poison the tracked state's accuracy claim: refresh must not depend on it
+    wk.refresh(_t(A))
+    inv = wk.get_inverse().cpu().numpy()
+    ph, la = wk.get_amplitude()
+    assert wk.info.cpu().numpy().tolist() == [0] * W
+    for w in range(W):
+        assert np.abs(A[w] @ inv[w] - np.eye(n)).max() < 1e-11
+        p0, l0 = amp(A[w])
+        assert la[w].item() == pytest.approx(l0, abs=1e-11)
+        assert abs(complex(ph[w].item()) - complex(p0)) < 1e-11
+        if kind == "pf":
+            assert np.array_equal(inv[w], -inv[w].T)
+    A_old = A
+    A, r = step(A)            # the chain continues from the refreshed state
+    for w in range(W):
+        p1, l1 = amp(A[w])
+        p0, l0 = amp(A_old[w])
+        assert r[w] == pytest.approx(complex(p1) / complex(p0) * np.exp(l1 - l0), rel=1e-9)
+    # a refresh from a singular matrix raises bit 1 for that walker only
+    S = A.copy()
+    S[1] = 0.0
+    wk.refresh(_t(S))
+    torch.cuda.synchronize()
+    assert wk.info.cpu().numpy().tolist() == [0, 1, 0]
+    wk.refresh(_t(A))         # and a good one clears it again
+    inv = wk.get_inverse().cpu().numpy()
+    assert wk.info.cpu().numpy().tolist() == [0] * W
+    assert np.abs(A[1] @ inv[1] - np.eye(n)).max() < 1e-11
