@@ -435,6 +435,8 @@ def pf_update_kernel_name(n, k, esz):
     lg = 5
     while (1 << lg) < n // 2:
         lg += 1
+    if esz == 8 and k == 1 and n in (64, 128):
+        return "pf_regs_k1_kernel"
     rg1 = 1024 >> lg
     if esz == 8 and k == 1 and lg <= 7 and (5 * ((n + 3) // 4) * n * 8 + (rg1 + rg1 // 4) * (n // 2) * 16
                                             + n * 32 + 2 * (2 * n + 6) * 8) <= 226 * 1024:

@@ -1074,6 +1074,173 @@ __global__ void __launch_bounds__(1024, 1) pf_resident_k1_kernel(State st, int l
   if (tid == 0) tma::store_wait_all<0>();
 }
 
+// ---------------------------------------------------------------- register-resident update, fp64 k = 1
+// pf_resident_k1_kernel is bound by shared-memory bandwidth (every row crosses the LSU pipe
+// three times: column sums, update load, update store, plus the bulk store reading it out
+// again).  Here the inverse of a walker (N = 128: 128 KB = half the register file) is held
+// in REGISTERS between the column sums and the update: 512 threads, lane l of warp rg owns
+// the column pairs {l, l+32, ..} of rows rg, rg+16, ..  Shared memory is only the landing
+// zone of the bulk loads: each row is read from it once, the updated row goes straight from
+// registers to global memory with coalesced 16-byte stores, and the landing zone is free for
+// the NEXT walker's bulk loads as soon as the column sums are done (they then have the whole
+// reduction + update to arrive).  No barrier inside the update, no store staging.
+template <int N>
+__global__ void __launch_bounds__(512, 1) pf_regs_k1_kernel(State st) {
+  constexpr int NQ = N / 2, QL = NQ / 32, RG = 16, RPT = N / RG, NCH = 4, RPC = N / NCH, TPC = RPT / NCH;
+  constexpr int STG = 2 * N + 6;        // doubles per staging slot: N row, C row, R'^-1 (2x2), {slot index, next walker}
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int kmax = st.kmax;
+  const int tid = threadIdx.x, lane = tid & 31, rg = tid >> 5;
+  double2* Ts2 = (double2*)smem_raw;                       // [N][NQ]    landing zone
+  double2* part = Ts2 + (size_t)N * NQ;                    // [RG][NQ]   column sums per row group
+  double2* part2 = part + (size_t)RG * NQ;                 // [4][NQ]    ... per four row groups
+  double2* rowc = part2 + (size_t)4 * NQ;                  // [N][2]     {g0,g1},{y0,y1} of row r
+  double* stg = (double*)(rowc + (size_t)2 * N);           // [2][STG]
+  __shared__ __align__(8) uint64_t bar[NCH];
+  const int count = st.counters[0], grid = (int)gridDim.x;
+  if (tid == 0) {
+    for (int c = 0; c < NCH; ++c) tma::mbar_init(&bar[c], 1);
+    tma::fence_barrier_init();
+  }
+  __syncthreads();
+  auto load_walker = [&](int w) {   // thread 0 only
+    constexpr uint32_t bytes = (uint32_t)(RPC * N * sizeof(double));
+    for (int c = 0; c < NCH; ++c) {
+      tma::mbar_arrive_expect_tx(&bar[c], bytes);
+      tma::load(Ts2 + (size_t)c * RPC * NQ, (const double*)st.Ti + (size_t)w * N * N + (size_t)c * RPC * N, bytes, &bar[c]);
+    }
+  };
+  auto stage = [&](int w, int slot, const int* next) {   // small operands of walker w -> staging slot
+    double* d = stg + slot * STG;
+    const double* Rw = (const double*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
+    if (tid < NQ) cp_async16(d + 2 * tid, (const double*)st.pend_N + (size_t)w * kmax * N + 2 * tid);
+    else if (tid < 2 * NQ) cp_async16(d + N + 2 * (tid - NQ), (const double*)st.pend_C + (size_t)w * kmax * N + 2 * (tid - NQ));
+    else if (tid == 2 * NQ) cp_async16(d + 2 * N, Rw);
+    else if (tid == 2 * NQ + 1) cp_async16(d + 2 * N + 2, Rw + st.kc);
+    else if (tid == 2 * NQ + 2) cp_async4(d + 2 * N + 4, st.pend_idx + (size_t)w * kmax);
+    else if (tid == 2 * NQ + 3 && next) cp_async4((int*)(d + 2 * N + 4) + 1, next);   // walker after w in this CTA's sequence
+  };
+  int w = (int)blockIdx.x < count ? st.list[blockIdx.x] : -1;
+  if (w >= 0) {
+    if (tid == 0) load_walker(w);
+    stage(w, 0, (int)blockIdx.x + grid < count ? st.list + blockIdx.x + grid : nullptr);
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  int j = 0;
+  for (int it = blockIdx.x; it < count; it += grid, ++j) {
+    const int slot = j & 1;
+    double2* Tw2 = (double2*)((double*)st.Ti + (size_t)w * N * N);
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();
+    const double* sd = stg + slot * STG;
+    const int w1 = it + grid < count ? *((const int*)(sd + 2 * N + 4) + 1) : -1;
+    if (w1 >= 0) stage(w1, slot ^ 1, it + 2 * grid < count ? st.list + it + 2 * grid : nullptr);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    double2 y1q[QL];
+#pragma unroll
+    for (int u = 0; u < QL; ++u) y1q[u] = ((const double2*)(sd + N))[lane + 32 * u];
+    // ---- rows -> registers, chunk by chunk as the bulk copies land, with the column sums
+    // y[c] = -sum_j Ti[j][c] N[j] taken on the way
+    double2 x[RPT][QL], acc[QL];
+#pragma unroll
+    for (int u = 0; u < QL; ++u) acc[u] = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) {
+      tma::mbar_wait(&bar[c], (uint32_t)(j & 1));
+#pragma unroll
+      for (int tt = 0; tt < TPC; ++tt) {
+        const int t = c * TPC + tt, r = rg + RG * t;
+        const double nr = sd[r];
+#pragma unroll
+        for (int u = 0; u < QL; ++u) {
+          x[t][u] = Ts2[r * NQ + lane + 32 * u];
+          acc[u].x = fma(x[t][u].x, nr, acc[u].x);
+          acc[u].y = fma(x[t][u].y, nr, acc[u].y);
+        }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < QL; ++u) part[rg * NQ + lane + 32 * u] = acc[u];
+    __syncthreads();
+    // every row is in registers: the landing zone takes the next walker
+    if (tid == 0 && w1 >= 0) load_walker(w1);
+    if (rg < 4) {
+#pragma unroll
+      for (int u = 0; u < QL; ++u) {
+        const int q = lane + 32 * u;
+        double2 sum = part[(4 * rg) * NQ + q];
+#pragma unroll
+        for (int g = 1; g < 4; ++g) {
+          const double2 t = part[(4 * rg + g) * NQ + q];
+          sum.x += t.x;
+          sum.y += t.y;
+        }
+        part2[rg * NQ + q] = sum;
+      }
+    }
+    __syncthreads();
+    double2 y0q[QL], ng0[QL], ng1[QL];
+    {
+      const double Ri00 = sd[2 * N], Ri01 = sd[2 * N + 1], Ri10 = sd[2 * N + 2], Ri11 = sd[2 * N + 3];
+      const int p0 = *(const int*)(sd + 2 * N + 4);
+#pragma unroll
+      for (int u = 0; u < QL; ++u) {
+        const int q = lane + 32 * u;
+        double2 sum = part2[q];
+#pragma unroll
+        for (int g = 1; g < 4; ++g) {
+          const double2 t = part2[g * NQ + q];
+          sum.x += t.x;
+          sum.y += t.y;
+        }
+        y0q[u].x = (2 * q == p0) ? -sum.x + 1.0 : -sum.x;
+        y0q[u].y = (2 * q + 1 == p0) ? -sum.y + 1.0 : -sum.y;
+        double2 g0q, g1q;
+        g0q.x = fma(y1q[u].x, Ri10, y0q[u].x * Ri00);
+        g0q.y = fma(y1q[u].y, Ri10, y0q[u].y * Ri00);
+        g1q.x = fma(y1q[u].x, Ri11, y0q[u].x * Ri01);
+        g1q.y = fma(y1q[u].y, Ri11, y0q[u].y * Ri01);
+        if (rg == 0) {
+          rowc[4 * q + 0] = make_double2(g0q.x, g1q.x);
+          rowc[4 * q + 1] = make_double2(y0q[u].x, y1q[u].x);
+          rowc[4 * q + 2] = make_double2(g0q.y, g1q.y);
+          rowc[4 * q + 3] = make_double2(y0q[u].y, y1q[u].y);
+        }
+        ng0[u] = make_double2(-g0q.x, -g0q.y);
+        ng1[u] = make_double2(-g1q.x, -g1q.y);
+      }
+    }
+    __syncthreads();
+    // ---- rank-2 update (Eq. 22) in registers, rows stored straight to global memory
+#pragma unroll
+    for (int t = 0; t < RPT; ++t) {
+      const int r = rg + RG * t;
+      const double2 gr = rowc[2 * r], yr = rowc[2 * r + 1];
+#pragma unroll
+      for (int u = 0; u < QL; ++u) {
+        const int q = lane + 32 * u, c0 = 2 * q;
+        double2 v = x[t][u];
+        if (c0 + 1 < r) {            // both below the diagonal
+          v.x = fma(ng1[u].x, yr.y, fma(ng0[u].x, yr.x, v.x));
+          v.y = fma(ng1[u].y, yr.y, fma(ng0[u].y, yr.x, v.y));
+        } else if (c0 > r) {         // both above
+          v.x = fma(gr.y, y1q[u].x, fma(gr.x, y0q[u].x, v.x));
+          v.y = fma(gr.y, y1q[u].y, fma(gr.x, y0q[u].y, v.y));
+        } else if (c0 == r) {        // (r,r), (r,r+1)
+          v.x = 0.0;
+          v.y = fma(gr.y, y1q[u].y, fma(gr.x, y0q[u].y, v.y));
+        } else {                     // (r,r-1), (r,r)
+          v.x = fma(ng1[u].x, yr.y, fma(ng0[u].x, yr.x, v.x));
+          v.y = 0.0;
+        }
+        Tw2[r * NQ + q] = v;
+      }
+    }
+    w = w1;
+  }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+}
+
 // ---------------------------------------------------------------- delayed append (a6)
 // Abuf[fill+alpha][:] = Y'[alpha][:]  (a'_tau, Eq. 28), Bbuf[fill+beta][:] = (a'_tau R'^-1)[:, beta].
 template <typename T>
@@ -1182,6 +1349,16 @@ static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_s
       const bool force_cta = env && !strcmp(env, "cta");
       // fp64 k = 1 with the whole inverse in one CTA's shared memory: column-pair kernel, 1024 threads
       if (sizeof(T) == 8 && k == 1 && !force_cta && !(env && !strncmp(env, "cluster", 7))) {
+        if ((n == 128 || n == 64) && !(env && !strncmp(env, "smem", 4)) && !(env && !strcmp(env, "nb5"))) {
+          // the walker's inverse in registers between the column sums and the update
+          const size_t smr = (size_t)n * n * 8 + (size_t)20 * (n / 2) * 16 + (size_t)n * 32 + (size_t)2 * (2 * n + 6) * 8;
+          auto kern = n == 128 ? pf_regs_k1_kernel<128> : pf_regs_k1_kernel<64>;
+          if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smr) != cudaSuccess)
+            return -1;
+          ProfScope ps(prof, LRUX_PROF_UPDATE, s);
+          kern<<<pgrid(num_sms, 1, st.W), 512, smr, s>>>(st); ++nl;
+          return cudaGetLastError() == cudaSuccess ? nl : -1;
+        }
         int lg1 = 5;
         while ((1 << lg1) < n / 2) ++lg1;
         const int rg1 = 1024 >> lg1;
