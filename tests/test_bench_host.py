@@ -34,7 +34,7 @@ def test_roofline_update_counts_algorithmic_bytes():
     assert r["bytes_per_launch"] == pytest.approx(byts / 10)
     big = bench.parse_workload("det,n=2048,k=4,K=0,W=8")
     assert bench.roofline_update(big, run, 6534.1, "m")["kernel"] == "det_update_tma_kernel"
-    assert bench.roofline_update(bench.parse_workload("c3"), run, 1.0, "m")["kernel"] == "pf_resident_update_kernel"
+    assert bench.roofline_update(bench.parse_workload("c3"), run, 1.0, "m")["kernel"] == "pf_regs_k1_kernel"
 
 
 def test_roofline_flush_bound_selection():
