@@ -506,12 +506,16 @@ __global__ void __launch_bounds__(256) det_split_prep_kernel(State st, int c, in
 }
 
 // ---------------------------------------------------------------- delayed append (a6)
-// prep: work item = (accepted walker, group of 8 buffer rows).  Each warp reads one
-// row a_s of Abuf once and forms NA[b][s] = N_b . a_s for all b (-> pend_Y); group 0
-// also copies a_tau = C_eff into Abuf[fill .. fill+k)   (Eq. 14).
+// prep: work item = (accepted walker, group of 8*RW buffer rows).  Each warp reads RW rows
+// a_s of Abuf once and forms NA[b][s] = N_b . a_s for all b (-> pend_Y), so that one
+// load of N from L2 serves RW buffer rows (with one row per warp the kernel moved four
+// times more N than Abuf); group 0 also copies a_tau = C_eff into Abuf[fill .. fill+k)
+// (Eq. 14).
+constexpr int kPrepRows = 4;   // buffer rows per warp
 template <typename T, int KT>
 __global__ void __launch_bounds__(256) det_prep_kernel(State st, int k, int groups) {
   using S = Sc<T>;
+  constexpr int RW = kPrepRows;
   const int n = st.n, kmax = st.kmax, cap = st.cap;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int count = st.counters[0];
@@ -525,24 +529,36 @@ __global__ void __launch_bounds__(256) det_prep_kernel(State st, int k, int grou
       const T* gC = (const T*)st.pend_C + (size_t)w * kmax * n;
       for (int q = tid; q < k * n; q += blockDim.x) Ab[(size_t)fill * n + q] = gC[q];
     }
-    const int s = grp * 8 + warp;
-    if (s >= fill) continue;
-    T acc[KT];
+    const int s0 = (grp * 8 + warp) * RW;
+    if (s0 >= fill) continue;
+    T acc[RW][KT];
 #pragma unroll
-    for (int b = 0; b < KT; ++b) acc[b] = S::zero();
-#pragma unroll 4
+    for (int r = 0; r < RW; ++r)
+#pragma unroll
+      for (int b = 0; b < KT; ++b) acc[r][b] = S::zero();
+#pragma unroll 2
     for (int i = lane; i < n; i += 32) {
-      const T x = Ab[(size_t)s * n + i];
+      T x[RW];
 #pragma unroll
-      for (int b = 0; b < KT; ++b)
-        if (b < k) acc[b] = S::fma(gN[(size_t)b * n + i], x, acc[b]);
+      for (int r = 0; r < RW; ++r) x[r] = s0 + r < fill ? Ab[(size_t)(s0 + r) * n + i] : S::zero();
+#pragma unroll
+      for (int b = 0; b < KT; ++b) {
+        if (b < k) {
+          const T nb = gN[(size_t)b * n + i];
+#pragma unroll
+          for (int r = 0; r < RW; ++r) acc[r][b] = S::fma(nb, x[r], acc[r][b]);
+        }
+      }
     }
     T* NA = (T*)st.pend_Y + (size_t)w * kmax * cap;
 #pragma unroll
-    for (int b = 0; b < KT; ++b) {
-      if (b < k) {
-        const T v = warp_sum(acc[b]);
-        if (lane == 0) NA[(size_t)b * cap + s] = v;
+    for (int r = 0; r < RW; ++r) {
+#pragma unroll
+      for (int b = 0; b < KT; ++b) {
+        if (b < k) {
+          const T v = warp_sum(acc[r][b]);
+          if (lane == 0 && s0 + r < fill) NA[(size_t)b * cap + s0 + r] = v;
+        }
       }
     }
   }
@@ -593,7 +609,7 @@ det_append_kernel(State st, int k, int tiles, int rows_per_tile, int n_in_smem) 
       for (int r = 0; r < RW; ++r)
 #pragma unroll
         for (int a = 0; a < KT; ++a) d[r][a] = S::zero();
-      constexpr int U = 4;   // 16-byte loads in flight per thread = U * RW
+      constexpr int U = sizeof(T) == 16 ? 8 : 4;   // 16-byte loads in flight per thread = U * RW
       for (int q0 = lane; q0 < nvec; q0 += 32 * U) {
         V x[U][RW];
 #pragma unroll
@@ -820,7 +836,7 @@ static int launch_append_kt(const State& st, int k, int num_sms, cudaStream_t s)
   constexpr int VECMAX = sizeof(T) == 8 ? 2 : 1;
   int nl = 0;
   {
-    const int groups = (st.cap + 7) / 8;
+    const int groups = (st.cap + 8 * kPrepRows - 1) / (8 * kPrepRows);
     const int grid = persistent_grid(num_sms, 8, (int64_t)st.W * groups);
     det_prep_kernel<T, KT><<<grid, 256, 0, s>>>(st, k, groups); ++nl;
   }
