@@ -11,6 +11,8 @@
 
 #include "lrux_common.cuh"
 #include "lrux_internal.h"
+#include <cstdlib>
+#include <cstring>
 
 namespace lrux {
 
@@ -564,6 +566,54 @@ __global__ void __launch_bounds__(256) det_prep_kernel(State st, int k, int grou
   }
 }
 
+// Second half of the append for one (walker, row tile): dsm[b][j] holds d = N A0^-1 - I[P,:]
+// on entry; subtract (N Abuf) Bbuf^T, apply R^-1, write Bbuf[fill .. fill+k).
+template <typename T, int KT>
+__device__ __forceinline__ void append_finish(const State& st, int w, int k, int fill, int j_beg, int j_end,
+                                              int rows_per_tile, T* dsm, const T* Ri) {
+  using S = Sc<T>;
+  const int n = st.n, kmax = st.kmax, cap = st.cap, tid = threadIdx.x;
+  __syncthreads();
+  // m[b][j] = d[b][j] - sum_s NA[b][s] Bbuf[s][j]: 4 groups of threads split the s range
+  const T* NA = (const T*)st.pend_Y + (size_t)w * kmax * cap;
+  T* Bb = (T*)st.Bbuf + (size_t)w * cap * n;
+  const int nj = j_end - j_beg;
+  const int jj = tid % rows_per_tile, sg = tid / rows_per_tile, nsg = blockDim.x / rows_per_tile;
+  T m[KT];
+#pragma unroll
+  for (int b = 0; b < KT; ++b) m[b] = S::zero();
+  if (jj < nj && sg < nsg) {
+#pragma unroll 8
+    for (int s = sg; s < fill; s += nsg) {
+      const T bv = Bb[(size_t)s * n + j_beg + jj];
+#pragma unroll
+      for (int b = 0; b < KT; ++b)
+        if (b < k) m[b] = S::fnma(NA[(size_t)b * cap + s], bv, m[b]);
+    }
+  }
+  if (sg >= 1 && sg < nsg && jj < nj) {
+#pragma unroll
+    for (int b = 0; b < KT; ++b) dsm[(sg * KT + b) * rows_per_tile + jj] = m[b];
+  }
+  __syncthreads();
+  if (sg == 0 && jj < nj) {
+#pragma unroll
+    for (int b = 0; b < KT; ++b) {
+      T v = S::add(dsm[b * rows_per_tile + jj], m[b]);
+      for (int g = 1; g < nsg; ++g) v = S::add(v, dsm[(g * KT + b) * rows_per_tile + jj]);
+      dsm[b * rows_per_tile + jj] = v;
+    }
+  }
+  __syncthreads();
+  for (int q = tid; q < k * nj; q += blockDim.x) {
+    const int a = q / nj, j2 = q % nj;
+    T acc = S::zero();
+#pragma unroll
+    for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], dsm[b * rows_per_tile + j2], acc);
+    Bb[(size_t)(fill + a) * n + j_beg + j2] = acc;
+  }
+}
+
 // append: b_tau^T = R^-1 (N A0^-1 - (N Abuf) Bbuf^T - I[P,:])   (Eq. 15 in new-rows form,
 // PAPER.md:194; reading 5b) -> Bbuf[fill .. fill+k).  One read-only pass over
 // Ti: work item = (accepted walker, tile of RPT rows); N staged in shared memory, each
@@ -648,45 +698,108 @@ det_append_kernel(State st, int k, int tiles, int rows_per_tile, int n_in_smem) 
           if (lane == 0 && j0 + r < j_end) dsm[a * rows_per_tile + (j0 + r - j_beg)] = v;
         }
     }
+    append_finish<T, KT>(st, w, k, fill, j_beg, j_end, rows_per_tile, dsm, Ri);
+  }
+}
+
+// The same pass for complex128 with k <= 4 on the FP64 tensor pipe.  The k dot products per
+// row are an (rows x n)(n x k) contraction: per warp, 8 rows x 4 columns of Ti form the A
+// fragment of mma.sync.m8n8k4.f64 straight from the global loads (lane = (row, column): one
+// 16-byte complex element, both halves used), and the 8 real columns [Re N | Im N] the B
+// fragment, so that  A=Re Ti, B=[Re N | Im N]  and  A=Im Ti, B'=[-Im N | Re N]  accumulate
+// [Re W | Im W] in two DMMAs per 8x4 complex elements.  Against the scalar pass: 2 tensor
+// instructions instead of 32 DFMAs + shuffles, 4 accumulator registers per lane instead of
+// 32, which leaves room for 16 loads of 16 bytes in flight per lane.  Measured at C4: 689 us per step for the
+// append class against 697 us for the scalar pass -- the pass is bound by its per-item phases and
+// the walker-count tail, not by issue; 64-row tiles (less tail, twice the per-item work) were slower (762 us).
+__device__ __forceinline__ void dmma884_acc(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(d0), "+d"(d1)
+               : "d"(a), "d"(b));
+}
+
+template <int KT>
+__global__ void __launch_bounds__(256, 2)
+det_append_dmma_kernel(State st, int k, int tiles, int rows_per_tile) {
+  using T = cplx;
+  using S = Sc<T>;
+  constexpr int UN = 8;                          // column steps of 4 per batch of loads: 2 x 8 16-byte loads in flight per lane
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int n = st.n, kmax = st.kmax;
+  T* dsm = (T*)smem_raw;                         // [4][KT][rows_per_tile] partial sums
+  double* Bs = (double*)(dsm + 4 * KT * rows_per_tile);   // [n][8]  Re N (cols 0-3), Im N (cols 4-7)
+  __shared__ T Ri[KT * KT];
+  __shared__ int sidx[KT];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
+  const int r8 = lane >> 2, kk = lane & 3;       // A: (row, column) of the lane; B: (column kk, N-column r8)
+  const int count = st.counters[0];
+  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
+    const int w = st.list[item / tiles];
+    const int tile = item % tiles;
+    const int fill = st.fill[w];
     __syncthreads();
-    // m[b][j] = d[b][j] - sum_s NA[b][s] Bbuf[s][j]: 4 groups of threads split the s range
-    const T* NA = (const T*)st.pend_Y + (size_t)w * kmax * cap;
-    T* Bb = (T*)st.Bbuf + (size_t)w * cap * n;
-    const int nj = j_end - j_beg;
-    const int jj = tid % rows_per_tile, sg = tid / rows_per_tile, nsg = blockDim.x / rows_per_tile;
-    T m[KT];
+    {
+      const T* gN = (const T*)st.pend_N + (size_t)w * kmax * n;
+      for (int q = tid; q < 4 * n; q += blockDim.x) {
+        const int a = q / n, i = q % n;
+        const T v = a < k ? gN[(size_t)a * n + i] : S::zero();
+        Bs[i * 8 + a] = v.re;
+        Bs[i * 8 + 4 + a] = v.im;
+      }
+      if (tid < KT * KT) {
+        const int a = tid / KT, b = tid % KT;
+        Ri[tid] = (a < k && b < k) ? ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + a * st.kc + b]
+                                   : S::zero();
+      }
+      if (tid < KT) sidx[tid] = tid < k ? st.pend_idx[(size_t)w * kmax + tid] : -1;
+    }
+    __syncthreads();
+    const T* Tw = (const T*)st.Ti + (size_t)w * n * n;
+    const int j_beg = tile * rows_per_tile, j_end = min(n, j_beg + rows_per_tile);
+    for (int j0 = j_beg + warp * 16; j0 < j_end; j0 += nw * 16) {
+      double acc[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+      const T* row0 = Tw + (size_t)min(j0 + r8, j_end - 1) * n + kk;        // rows past the tile: clamped, discarded
+      const T* row1 = Tw + (size_t)min(j0 + 8 + r8, j_end - 1) * n + kk;
+      const double* bp = Bs + kk * 8 + r8;
+      const double* bq = Bs + kk * 8 + (r8 ^ 4);
+      const bool lo = r8 < 4;
+      for (int i0 = 0; i0 < n; i0 += 4 * UN) {
+        T x0[UN], x1[UN];
 #pragma unroll
-    for (int b = 0; b < KT; ++b) m[b] = S::zero();
-    if (jj < nj && sg < nsg) {
-#pragma unroll 8
-      for (int s = sg; s < fill; s += nsg) {
-        const T bv = Bb[(size_t)s * n + j_beg + jj];
+        for (int u = 0; u < UN; ++u) {
+          const bool in = i0 + 4 * u < n;
+          x0[u] = in ? row0[i0 + 4 * u] : S::zero();
+          x1[u] = in ? row1[i0 + 4 * u] : S::zero();
+        }
 #pragma unroll
-        for (int b = 0; b < KT; ++b)
-          if (b < k) m[b] = S::fnma(NA[(size_t)b * cap + s], bv, m[b]);
+        for (int u = 0; u < UN; ++u) {
+          if (i0 + 4 * u < n) {
+            const double b = bp[(i0 + 4 * u) * 8];
+            const double b2 = bq[(i0 + 4 * u) * 8];
+            const double bm = lo ? -b2 : b2;          // B' = [-Im N | Re N]
+            dmma884_acc(acc[0][0], acc[0][1], x0[u].re, b);
+            dmma884_acc(acc[0][0], acc[0][1], x0[u].im, bm);
+            dmma884_acc(acc[1][0], acc[1][1], x1[u].re, b);
+            dmma884_acc(acc[1][0], acc[1][1], x1[u].im, bm);
+          }
+        }
+      }
+      // D fragment: row r8, columns 2*kk, 2*kk+1 of [Re W | Im W]
+#pragma unroll
+      for (int mt = 0; mt < 2; ++mt) {
+        const int j = j0 + 8 * mt + r8;
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int col = 2 * kk + e, a = col & 3;
+          if (j < j_end && a < KT) {
+            double v = acc[mt][e];
+            if (col < 4 && j == sidx[a]) v -= 1.0;
+            ((double*)&dsm[a * rows_per_tile + (j - j_beg)])[col >> 2] = v;
+          }
+        }
       }
     }
-    if (sg >= 1 && sg < nsg && jj < nj) {
-#pragma unroll
-      for (int b = 0; b < KT; ++b) dsm[(sg * KT + b) * rows_per_tile + jj] = m[b];
-    }
-    __syncthreads();
-    if (sg == 0 && jj < nj) {
-#pragma unroll
-      for (int b = 0; b < KT; ++b) {
-        T v = S::add(dsm[b * rows_per_tile + jj], m[b]);
-        for (int g = 1; g < nsg; ++g) v = S::add(v, dsm[(g * KT + b) * rows_per_tile + jj]);
-        dsm[b * rows_per_tile + jj] = v;
-      }
-    }
-    __syncthreads();
-    for (int q = tid; q < k * nj; q += blockDim.x) {
-      const int a = q / nj, j2 = q % nj;
-      T acc = S::zero();
-#pragma unroll
-      for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], dsm[b * rows_per_tile + j2], acc);
-      Bb[(size_t)(fill + a) * n + j_beg + j2] = acc;
-    }
+    append_finish<T, KT>(st, w, k, fill, j_beg, j_end, rows_per_tile, dsm, Ri);
   }
 }
 
@@ -855,6 +968,22 @@ static int launch_append_kt(const State& st, int k, int num_sms, cudaStream_t s)
   const int tiles = (n + rows_per_tile - 1) / rows_per_tile;
   const int n_in_smem = (size_t)k * n * sizeof(T) <= 96 * 1024;
   const size_t smem = ((n_in_smem ? (size_t)k * n : 0) + 4 * (size_t)KT * rows_per_tile) * sizeof(T);
+  if constexpr (sizeof(T) == 16 && KT <= 4) {
+    // complex data, k <= 4: the dot products on the FP64 tensor pipe
+    const char* env = getenv("LRUX_APPEND_PATH");   // A-B measurements only
+    const int rpt_d = rows_per_tile, tiles_d = tiles;
+    const size_t smd = (size_t)n * 64 + 4 * (size_t)KT * rpt_d * sizeof(T);
+    if (n % 4 == 0 && rows_per_tile == 128 && smd <= 100 * 1024 && !(env && !strcmp(env, "scalar"))) {
+      auto kd = det_append_dmma_kernel<KT>;
+      if (cudaFuncSetAttribute(kd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smd) != cudaSuccess)
+        return -1;
+      int occd = 1;
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occd, kd, 256, smd);
+      if (occd < 1) return -1;
+      kd<<<persistent_grid(num_sms, occd, (int64_t)st.W * tiles_d), 256, smd, s>>>(st, k, tiles_d, rpt_d); ++nl;
+      return nl;
+    }
+  }
   const bool vec = (n % VECMAX) == 0 && VECMAX == 2;
   auto kern = vec ? det_append_kernel<T, KT, VECMAX, 2> : det_append_kernel<T, KT, 1, 2>;
   if (smem > 40 * 1024 &&   // static shared memory counts towards the 48 KiB default
