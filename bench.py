@@ -428,6 +428,16 @@ def ncu_traffic_per_walker(kernel, workload):
     return best
 
 
+def det_append_kernel_name(wk):
+    """Mirror of csrc/lrux_det.cu:launch_append_kt: complex data with k <= 4 and 128-row tiles
+    (n >= 1024, [Re N | Im N] + the tile's partial sums within 100 KB) take the DMMA pass."""
+    n = wk["n"]
+    kt = 1 if wk["k"] <= 1 else 2 if wk["k"] <= 2 else 4 if wk["k"] <= 4 else 8
+    if wk["cplx"] and kt <= 4 and n >= 1024 and n % 4 == 0 and n * 64 + 4 * kt * 128 * 16 <= 100 * 1024:
+        return "det_append_dmma_kernel"
+    return "det_append_kernel"
+
+
 def pf_update_kernel_name(n, k, esz):
     """Mirror of the dispatch in csrc/lrux_pf.cu:pf_accept_impl (K = 0): which kernel
     applies the immediate Pfaffian update for this shape."""
@@ -614,7 +624,7 @@ def main(argv=None):
         ap = {"ms": ap_ms}
         gbs = wk["n"] ** 2 * (16.0 if wk["cplx"] else 8.0) * run["accepted"] / (ap["ms"] * 1e-3) / 1e9
         roof_append = {"bound": "hbm",
-                       "kernel": ("det_prep_kernel+det_append_kernel" if wk["kind"] == "det"
+                       "kernel": (("det_prep_kernel+" + det_append_kernel_name(wk)) if wk["kind"] == "det"
                                   else "pf_y_kernel+pf_append_kernel"), "achieved": gbs,
                        "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
                        "peak_source": peak_src}
