@@ -67,6 +67,7 @@ def test_det_large_n_stream_path(n, k):
 @pytest.mark.parametrize("n,M,k,K,cplx", [
     (32, 64, 1, 0, False),
     (50, 100, 1, 0, False),
+    (64, 128, 1, 0, False),      # register-resident kernel, n = 64 instance
     (34, 70, 2, 0, False),
     (64, 128, 3, 0, False),
     (40, 80, 4, 0, False),
@@ -143,10 +144,22 @@ def test_det_tma_update_n4096_properties():
         assert ph[w].item() == sign.item()
 
 
-@pytest.mark.parametrize("k", [1, 2])
-def test_pf_large_n_streaming_path(k):
-    """n=200: the inverse (320 KB) does not fit in shared memory -> tiled update kernels."""
-    _run("pf", 99 + k, 3, 200, 400, k, 0, 12, walkers=[0, 2], scratch_every=3)
+@pytest.mark.parametrize("n,k", [(200, 1), (200, 2), (320, 1), (320, 2)])
+def test_pf_large_n_paths(n, k):
+    """n=200: the inverse (320 KB) does not fit in one CTA's shared memory -> 8-CTA cluster
+    kernels (row slabs, Y over DSMEM); n=320: beyond the cluster kernels too -> Y pass +
+    streaming update."""
+    _run("pf", 99 + k, 3, n, 2 * n, k, 0, 10, walkers=[0, 2], scratch_every=3)
+
+
+@pytest.mark.parametrize("path", ["smem", "nb5", "cluster", "cluster_generic", "cta"])
+def test_pf_config3_shape_older_kernels(path, monkeypatch):
+    """The Pfaffian update kernels the register-resident one superseded at n = 128 stay
+    selectable (LRUX_PF_PATH, read at every accept) and must give the same trajectory:
+    shared-memory resident with 6 / 5 chunk buffers, 4-CTA cluster column-pair kernel,
+    generic cluster kernel, single-CTA warp-per-row kernel."""
+    monkeypatch.setenv("LRUX_PF_PATH", path)
+    _run("pf", wl.BASE_SEED + 3, 12, 128, 256, 1, 0, 40, walkers=[0, 5, 11])
 
 
 def test_det_config4_shape_reduced():
