@@ -18,6 +18,10 @@ struct cplx {
 
 __device__ __forceinline__ double sc_from(double re, double, double) { return re; }
 __device__ __forceinline__ cplx sc_from(double re, double im, cplx) { return cplx{re, im}; }
+__device__ __forceinline__ double sc_re(double x) { return x; }
+__device__ __forceinline__ double sc_im(double) { return 0.0; }
+__device__ __forceinline__ double sc_re(cplx x) { return x.re; }
+__device__ __forceinline__ double sc_im(cplx x) { return x.im; }
 
 template <typename T>
 struct Sc;

@@ -227,6 +227,121 @@ pf_y_kernel(State st, int k, int tiles, int rows_per_tile, int use_list) {
   }
 }
 
+// ---------------------------------------------------------------- Y pass by column sums
+// Y = A0^-1 N without a single warp reduction: A0^-1 is exactly skew, so
+// Y[a][c] = -sum_j Ti[j][c] N[a][j] is a running sum DOWN the columns.  Work item = (walker,
+// block of CW 16-byte column vectors); thread (cq, rg) owns one vector of columns and every
+// RG-th row, streams its column slab with U row loads in flight (each warp load is 512
+// contiguous bytes of a row), N[a][j] comes from shared memory as a broadcast.  Row groups
+// (RG > 1 only when the matrix is narrower than the CTA) are combined through shared
+// memory in a fixed order.  The buffer terms of the delayed path are added as in
+// pf_y_kernel.  pf_y_kernel (row dot products, 5 shuffle stages per row and operand) ran
+// at 0.36 of HBM at n = 512.
+template <typename T, int KT>
+__global__ void __launch_bounds__(256)
+pf_y_colsum_kernel(State st, int k, int cblocks, int lg_cw, int use_list) {
+  using S = Sc<T>;
+  constexpr int VE = sizeof(T) == 8 ? 2 : 1;     // elements per 16-byte vector
+  constexpr int U = 8;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int n = st.n, kmax = st.kmax, cap = st.cap, nvec = n / VE;
+  const int CW = 1 << lg_cw, RG = 256 >> lg_cw;
+  T* Ns = (T*)smem_raw;                                   // [k][n]
+  double2* part = (double2*)(Ns + (size_t)k * n);         // [RG][KT][CW]
+  const int tid = threadIdx.x, cq = tid & (CW - 1), rg = tid >> lg_cw;
+  const int count = use_list ? st.counters[0] : (int)st.W;
+  for (int item = blockIdx.x; item < count * cblocks; item += gridDim.x) {
+    const int w = use_list ? st.list[item / cblocks] : item / cblocks;
+    const int cb = item % cblocks;
+    if (st.pend_idx[(size_t)w * kmax] < 0) continue;  // invalid proposal (uniform per CTA)
+    const int fill = cap ? st.fill[w] : 0;
+    const T* gN = (const T*)st.pend_N + (size_t)w * kmax * n;
+    const double2* Tw2 = (const double2*)((const T*)st.Ti + (size_t)w * n * n);
+    __syncthreads();
+    for (int q = tid; q < k * n; q += blockDim.x) Ns[q] = gN[q];
+    __syncthreads();
+    const int q = cb * CW + cq;
+    const bool act = q < nvec;
+    double2 acc[KT];
+#pragma unroll
+    for (int a = 0; a < KT; ++a) acc[a] = make_double2(0.0, 0.0);
+    if (act) {
+      for (int j0 = rg; j0 < n; j0 += RG * U) {
+        double2 x[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const int j = j0 + u * RG;
+          x[u] = j < n ? Tw2[(size_t)j * nvec + q] : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const int j = j0 + u * RG;
+          if (j < n) {
+#pragma unroll
+            for (int a = 0; a < KT; ++a) {
+              if (a < k) {
+                const T nv = Ns[(size_t)a * n + j];
+                if constexpr (VE == 2) {
+                  acc[a].x = fma(x[u].x, sc_re(nv), acc[a].x);
+                  acc[a].y = fma(x[u].y, sc_re(nv), acc[a].y);
+                } else {
+                  const T r = S::fma(sc_from(x[u].x, x[u].y, T{}), nv, sc_from(acc[a].x, acc[a].y, T{}));
+                  acc[a] = make_double2(sc_re(r), sc_im(r));
+                }
+              }
+            }
+          }
+        }
+      }
+    }
+    if (RG > 1) {
+#pragma unroll
+      for (int a = 0; a < KT; ++a)
+        if (a < k) part[((size_t)rg * KT + a) * CW + cq] = acc[a];
+      __syncthreads();
+      if (rg == 0) {
+#pragma unroll
+        for (int a = 0; a < KT; ++a) {
+          if (a < k) {
+            for (int g = 1; g < RG; ++g) {
+              const double2 t = part[((size_t)g * KT + a) * CW + cq];
+              acc[a].x += t.x;
+              acc[a].y += t.y;
+            }
+          }
+        }
+      }
+    }
+    if (rg == 0 && act) {
+      const T* AN = cap ? (const T*)st.pend_AN + (size_t)w * kmax * cap : nullptr;
+      const double2* Bb2 = cap ? (const double2*)((const T*)st.Bbuf + (size_t)w * cap * n) : nullptr;
+      double2* pY2 = (double2*)((T*)st.pend_Y + (size_t)w * kmax * n);
+      double2 y[KT];
+#pragma unroll
+      for (int a = 0; a < KT; ++a) y[a] = make_double2(-acc[a].x, -acc[a].y);
+      for (int sft = 0; sft < fill; ++sft) {
+        const double2 bv = Bb2[(size_t)sft * nvec + q];
+#pragma unroll
+        for (int a = 0; a < KT; ++a) {
+          if (a < k) {
+            const T an = AN[(size_t)a * cap + sft];
+            if constexpr (VE == 2) {
+              y[a].x = fma(bv.x, sc_re(an), y[a].x);
+              y[a].y = fma(bv.y, sc_re(an), y[a].y);
+            } else {
+              const T r = S::fma(sc_from(bv.x, bv.y, T{}), an, sc_from(y[a].x, y[a].y, T{}));
+              y[a] = make_double2(sc_re(r), sc_im(r));
+            }
+          }
+        }
+      }
+#pragma unroll
+      for (int a = 0; a < KT; ++a)
+        if (a < k) pY2[(size_t)a * nvec + q] = y[a];
+    }
+  }
+}
+
 // ---------------------------------------------------------------- core (k >= 2)
 // Builds the exactly skew 2k x 2k core R', r = (-1)^(k(k-1)/2) pf R', R'^-1.
 template <typename T>
@@ -1293,11 +1408,30 @@ static int launch_y(const State& st, int k, int use_list, int num_sms, cudaStrea
   if (st.cap) {
     pf_an_kernel<T><<<pgrid(num_sms, 4, st.W), 256, 0, s>>>(st, k, use_list); ++nl;
   }
+  const int kt = round_kt(k);
+  {
+    // column sums (no warp reductions) whenever N fits in shared memory
+    constexpr int VE = sizeof(T) == 8 ? 2 : 1;
+    const int nvec = st.n / VE;
+    int lg = 5;
+    while ((1 << lg) < nvec && lg < 8) ++lg;
+    const int CW = 1 << lg, RG = 256 >> lg, cblocks = (nvec + CW - 1) / CW;
+    const size_t smy = (size_t)k * st.n * sizeof(T) + (RG > 1 ? (size_t)RG * kt * CW * 16 : 0);
+    const char* env = getenv("LRUX_PF_Y");   // A-B measurements only
+    if (st.n % VE == 0 && smy <= 64 * 1024 && !(env && !strcmp(env, "rows"))) {
+      auto kern = kt == 1 ? pf_y_colsum_kernel<T, 1> : kt == 2 ? pf_y_colsum_kernel<T, 2>
+                : kt == 4 ? pf_y_colsum_kernel<T, 4> : pf_y_colsum_kernel<T, 8>;
+      if (smy > 40 * 1024 &&
+          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smy) != cudaSuccess)
+        return -1;
+      kern<<<pgrid(num_sms, 8, (int64_t)st.W * cblocks), 256, smy, s>>>(st, k, cblocks, lg, use_list);
+      return nl + 1;
+    }
+  }
   int rpt = 64;
   if (rpt > st.n) rpt = st.n;
   const int tiles = (st.n + rpt - 1) / rpt;
   const int grid = pgrid(num_sms, 4, (int64_t)st.W * tiles);
-  const int kt = round_kt(k);
   const size_t smem = (size_t)kt * rpt * sizeof(T);
   switch (kt) {
     case 1: pf_y_kernel<T, 1><<<grid, 256, smem, s>>>(st, k, tiles, rpt, use_list); break;
