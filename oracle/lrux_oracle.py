@@ -458,13 +458,16 @@ def det_trajectory(Phi, occ, unocc, P, J, xi, scratch_every=1, delay=0, on_step=
             else:
                 _, Ainv = det_lru(Ainv, u, v, return_update=True)
             A = A_new
-            s_ph, s_la = slogdet(A)
+            if scratch_every:                # from-scratch amplitude of the current A (checks only)
+                s_ph, s_la = slogdet(A)
             phase = phase * (r / abs(r))
             logabs = logabs + float(np.log(abs(r)))
             for a in range(len(p)):
                 occ[p[a]], unocc[J[t][a]] = unocc[J[t][a]], occ[p[a]]
         if on_step is not None:
             on_step(t)        # timing hook for bench.py; takes no part in the arithmetic
+    if not scratch_every:
+        s_ph, s_la = slogdet(A)              # amplitude of the final A, once
     out.update(A=A, Ainv=carrier.inverse() if carrier else Ainv, occ=occ, unocc=unocc,
                phase=phase, logabs=logabs, scratch_phase=s_ph, scratch_logabs=s_la)
     return out
@@ -513,13 +516,16 @@ def pf_trajectory(F, occ, unocc, P, J, xi, scratch_every=1, delay=0, on_step=Non
             else:
                 _, Ainv = pf_lru(Ainv, u, return_update=True)
             A = A_new
-            s_ph, s_la = slogpf(A)
+            if scratch_every:                # from-scratch amplitude of the current A (checks only)
+                s_ph, s_la = slogpf(A)
             phase = phase * (r / abs(r))
             logabs = logabs + float(np.log(abs(r)))
             for a in range(len(p)):
                 occ[p[a]], unocc[J[t][a]] = unocc[J[t][a]], occ[p[a]]
         if on_step is not None:
             on_step(t)        # timing hook for bench.py; takes no part in the arithmetic
+    if not scratch_every:
+        s_ph, s_la = slogpf(A)               # amplitude of the final A, once
     out.update(A=A, Ainv=carrier.inverse() if carrier else Ainv, occ=occ, unocc=unocc,
                phase=phase, logabs=logabs, scratch_phase=s_ph, scratch_logabs=s_la)
     return out

@@ -5,9 +5,22 @@ import os
 import numpy as np
 import pytest
 
-from oracle import lrux_oracle as orc
+from oracle import c_oracle, lrux_oracle as pyorc
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "pf_closed_forms.txt")
+
+
+class _COracle:
+    """The C oracle, with the helpers it does not restate (brute force, J, one-hot)
+    taken from the numpy one: those are what BOTH implementations are pinned to."""
+
+    def __getattr__(self, name):
+        return getattr(c_oracle, name) if hasattr(c_oracle, name) else getattr(pyorc, name)
+
+
+@pytest.fixture(params=["numpy", "c"])
+def orc(request):
+    return pyorc if request.param == "numpy" else _COracle()
 
 
 def rand(rng, shape, cplx):
@@ -30,19 +43,19 @@ def _golden_rows(tag):
             yield [float(x) for x in line[1:]]
 
 
-def test_pf_closed_form_A2():
+def test_pf_closed_form_A2(orc):
     for a, exp in _golden_rows("A2"):
         assert orc.pf(np.array([[0, a], [-a, 0.0]])) == pytest.approx(exp, rel=1e-15)
 
 
-def test_pf_closed_form_A3():
+def test_pf_closed_form_A3(orc):
     for a, b, c, d, e, f, exp in _golden_rows("A3"):
         A = np.array([[0, a, b, c], [-a, 0, d, e], [-b, -d, 0, f], [-c, -e, -f, 0.0]])
         assert orc.pf(A) == pytest.approx(exp, rel=1e-14, abs=1e-14)
         assert orc.pf_bruteforce(A) == pytest.approx(exp, rel=1e-14, abs=1e-14)
 
 
-def test_pf_skew_eye():
+def test_pf_skew_eye(orc):
     for k, exp in _golden_rows("PFJ"):
         k = int(k)
         assert orc.pf_skew_eye(k) == exp
@@ -54,7 +67,7 @@ def test_pf_skew_eye():
 # ---------------------------------------------------------------- brute force
 @pytest.mark.parametrize("cplx", [False, True])
 @pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 7])
-def test_lu_det_vs_leibniz(n, cplx):
+def test_lu_det_vs_leibniz(orc, n, cplx):
     rng = np.random.default_rng(100 + n)
     for _ in range(3):
         A = rand(rng, (n, n), cplx)
@@ -63,21 +76,21 @@ def test_lu_det_vs_leibniz(n, cplx):
 
 @pytest.mark.parametrize("cplx", [False, True])
 @pytest.mark.parametrize("n", [2, 4, 6, 8])
-def test_parlett_reid_vs_matchings(n, cplx):
+def test_parlett_reid_vs_matchings(orc, n, cplx):
     rng = np.random.default_rng(200 + n)
     for _ in range(3):
         A = rand_skew(rng, n, cplx)
         assert orc.pf(A) == pytest.approx(orc.pf_bruteforce(A), rel=1e-12)
 
 
-def test_pf_pivoting_needed_case():
+def test_pf_pivoting_needed_case(orc):
     # A[0][1] = 0 forces a pivot swap; brute force fixes the sign
     A = np.array([[0, 0, 2, 1], [0, 0, 3, 5], [-2, -3, 0, 7], [-1, -5, -7, 0.0]])
     assert orc.pf(A) == pytest.approx(orc.pf_bruteforce(A), rel=1e-14)
     assert orc.pf(A) == pytest.approx(0 * 7 - 2 * 5 + 1 * 3)
 
 
-def test_pf_odd_and_singular():
+def test_pf_odd_and_singular(orc):
     assert orc.pf(np.zeros((3, 3))) == 0
     assert orc.pf(np.zeros((4, 4))) == 0
     assert orc.det(np.zeros((3, 3))) == 0
@@ -87,7 +100,7 @@ def test_pf_odd_and_singular():
 # ---------------------------------------------------------------- library / textbook
 @pytest.mark.parametrize("cplx", [False, True])
 @pytest.mark.parametrize("n", [3, 17, 64])
-def test_lu_vs_numpy_linalg(n, cplx):
+def test_lu_vs_numpy_linalg(orc, n, cplx):
     rng = np.random.default_rng(300 + n)
     A = rand(rng, (n, n), cplx)
     ph, la = orc.slogdet(A)
@@ -98,7 +111,7 @@ def test_lu_vs_numpy_linalg(n, cplx):
     assert np.allclose(orc.inv(A) @ A, np.eye(n), atol=1e-10)
 
 
-def test_det_triangular_and_product():
+def test_det_triangular_and_product(orc):
     rng = np.random.default_rng(5)
     U = np.triu(rng.standard_normal((6, 6)))
     assert orc.det(U) == pytest.approx(np.prod(np.diag(U)), rel=1e-13)
@@ -112,7 +125,7 @@ def test_det_triangular_and_product():
 
 # ---------------------------------------------------------------- Pfaffian identities A.4-A.9
 @pytest.mark.parametrize("cplx", [False, True])
-def test_pf_identities(cplx):
+def test_pf_identities(orc, cplx):
     rng = np.random.default_rng(7)
     n = 10
     A = rand_skew(rng, n, cplx)
@@ -151,7 +164,7 @@ def test_pf_identities(cplx):
 # ---------------------------------------------------------------- lemma / Woodbury
 @pytest.mark.parametrize("cplx", [False, True])
 @pytest.mark.parametrize("k", [1, 2, 3])
-def test_det_lemma_dense(k, cplx):
+def test_det_lemma_dense(orc, k, cplx):
     """PAPER.md:69-85 recipe: det A * r == det(A + v u^T); Eq. 5 gives the inverse."""
     rng = np.random.default_rng(10 + k)
     n = 6
@@ -169,7 +182,7 @@ def test_det_lemma_dense(k, cplx):
 
 @pytest.mark.parametrize("cplx", [False, True])
 @pytest.mark.parametrize("k", [1, 2])
-def test_pf_lemma_dense(k, cplx):
+def test_pf_lemma_dense(orc, k, cplx):
     """PAPER.md:250-267 recipe: pf A * r == pf(A - u J u^T); Eq. 21 gives the inverse."""
     rng = np.random.default_rng(20 + k)
     n = 8
@@ -195,7 +208,7 @@ def test_pf_lemma_dense(k, cplx):
 
 
 @pytest.mark.parametrize("k", [1, 2, 3])
-def test_pf_update_vectors_reproduce_row_col_replacement(k):
+def test_pf_update_vectors_reproduce_row_col_replacement(orc, k):
     """Reading 5: A - u J u^T must equal A with rows and columns P replaced."""
     rng = np.random.default_rng(30 + k)
     n = 8
@@ -217,3 +230,40 @@ def test_pf_update_vectors_reproduce_row_col_replacement(k):
     Ainv = np.linalg.inv(A)
     Ainv = (Ainv - Ainv.T) / 2
     assert orc.pf_lru(Ainv, u) == pytest.approx(orc.pf_bruteforce(A1) / orc.pf_bruteforce(A), rel=1e-10)
+
+
+# ---------------------------------------------------------------- C oracle == numpy oracle
+@pytest.mark.parametrize("cplx", [False, True])
+def test_c_oracle_agrees_with_numpy_oracle(cplx):
+    """Two independent restatements of the same definitions (different language, different
+    summation order) agree to rounding on every shared function."""
+    rng = np.random.default_rng(77)
+    for n in (1, 2, 5, 12, 40):
+        A = rand(rng, (n, n), cplx)
+        (p1, l1), (p2, l2) = pyorc.slogdet(A), c_oracle.slogdet(A)
+        assert p1 == pytest.approx(p2, abs=1e-11) and l1 == pytest.approx(l2, abs=1e-11)
+        assert np.allclose(pyorc.inv(A), c_oracle.inv(A), rtol=1e-9, atol=1e-11)
+        k = min(3, n)
+        u, v = rand(rng, (n, k), cplx), rand(rng, (n, k), cplx)
+        Ai = np.linalg.inv(A)
+        r1, n1 = pyorc.det_lru(Ai, u, v, True)
+        r2, n2 = c_oracle.det_lru(Ai, u, v, True)
+        assert r1 == pytest.approx(r2, rel=1e-11)
+        assert np.allclose(n1, n2, rtol=1e-9, atol=1e-11)
+    for n in (2, 6, 12, 40):
+        A = rand_skew(rng, n, cplx)
+        (p1, l1), (p2, l2) = pyorc.slogpf(A), c_oracle.slogpf(A)
+        assert p1 == pytest.approx(p2, abs=1e-11) and l1 == pytest.approx(l2, abs=1e-11)
+        k = min(2, n // 2)
+        u = rand(rng, (n, 2 * k), cplx)
+        Ai = np.linalg.inv(A)
+        Ai = (Ai - Ai.T) / 2
+        r1, n1 = pyorc.pf_lru(Ai, u, True)
+        r2, n2 = c_oracle.pf_lru(Ai, u, True)
+        assert r1 == pytest.approx(r2, rel=1e-10)
+        assert np.allclose(n1, n2, rtol=1e-8, atol=1e-10)
+        assert np.array_equal(n2, -n2.T)
+    assert c_oracle.slogdet(np.zeros((3, 3)))[1] == -np.inf
+    assert c_oracle.slogpf(np.zeros((4, 4)))[1] == -np.inf
+    with pytest.raises(np.linalg.LinAlgError):
+        c_oracle.inv(np.zeros((3, 3)))

@@ -5,8 +5,16 @@ ratios (Eq. 3) and A_t A_t^-1 = 1.  CPU only."""
 import numpy as np
 import pytest
 
-from oracle import lrux_oracle as orc
+from oracle import c_oracle, lrux_oracle as pyorc
 from paper_2602_05255_b200 import workload as wl
+
+orc = pyorc     # the carrier objects exist in the numpy oracle only; the C carriers are pinned
+                # through the delayed trajectories below and by C == numpy
+
+
+@pytest.fixture(params=["numpy", "c"])
+def traj(request):
+    return pyorc if request.param == "numpy" else c_oracle
 
 
 def rand(rng, shape, cplx):
@@ -81,10 +89,10 @@ def _config1():
     return Phi, occ, unocc, P[:, 0], J[:, 0], xi[:, 0]
 
 
-def test_det_trajectory_config1():
+def test_det_trajectory_config1(traj):
     """BASELINE.json configs[0]: 200 steps, k=1, n=32."""
     Phi, occ, unocc, P, J, xi = _config1()
-    tr = orc.det_trajectory(Phi, occ, unocc, P, J, xi, scratch_every=1)
+    tr = traj.det_trajectory(Phi, occ, unocc, P, J, xi, scratch_every=1)
     acc = tr["accepted"]
     assert 0.2 < acc.mean() < 0.6          # SURVEY probe: ~0.36
     # lemma == from-scratch ratio at every step (Eq. 2)
@@ -96,20 +104,20 @@ def test_det_trajectory_config1():
     assert np.allclose(tr["A"] @ tr["Ainv"], np.eye(32), atol=1e-9)
     assert sorted(list(tr["occ"]) + list(tr["unocc"])) == list(range(64))
     # delayed path takes the same decisions and ends in the same inverse
-    td = orc.det_trajectory(Phi, occ, unocc, P, J, xi, scratch_every=0, delay=4)
+    td = traj.det_trajectory(Phi, occ, unocc, P, J, xi, scratch_every=0, delay=4)
     assert np.array_equal(td["accepted"], acc)
     np.testing.assert_allclose(td["r_lemma"], tr["r_lemma"], rtol=1e-8)
     assert np.allclose(td["Ainv"], tr["Ainv"], rtol=1e-7, atol=1e-9)
 
 
 @pytest.mark.parametrize("k", [2, 4])
-def test_det_trajectory_complex_k(k):
+def test_det_trajectory_complex_k(traj, k):
     seed = wl.BASE_SEED + 4
     n, M, steps = 16, 32, 60
     Phi = wl.orbital_matrix(seed, 3, M, n, 1.0 / (2 * n), complex_=True)
     occ, unocc = wl.initial_occupation(seed, 3, M, n)
     P, J, xi = wl.proposals(seed, 4, steps, n, M, k, walkers=[3])
-    tr = orc.det_trajectory(Phi, occ, unocc, P[:, 0], J[:, 0], xi[:, 0])
+    tr = traj.det_trajectory(Phi, occ, unocc, P[:, 0], J[:, 0], xi[:, 0])
     assert tr["accepted"].sum() > 3
     np.testing.assert_allclose(tr["r_lemma"], tr["r_scratch"], rtol=1e-7)
     assert tr["phase"] == pytest.approx(tr["scratch_phase"], abs=1e-9)
@@ -118,7 +126,7 @@ def test_det_trajectory_complex_k(k):
 
 
 @pytest.mark.parametrize("k,delay", [(1, 0), (2, 0), (1, 3), (2, 3)])
-def test_pf_trajectory(k, delay):
+def test_pf_trajectory(traj, k, delay):
     """BASELINE.json configs[2] shape at n=16: F skew 32x32, k orbital swaps."""
     seed = wl.BASE_SEED + 3
     n, M, steps = 16, 32, 80
@@ -126,7 +134,7 @@ def test_pf_trajectory(k, delay):
     assert np.array_equal(F, -F.T)
     occ, unocc = wl.initial_occupation(seed, 1, M, n)
     P, J, xi = wl.proposals(seed, 2, steps, n, M, k, walkers=[1])
-    tr = orc.pf_trajectory(F, occ, unocc, P[:, 0], J[:, 0], xi[:, 0], delay=delay)
+    tr = traj.pf_trajectory(F, occ, unocc, P[:, 0], J[:, 0], xi[:, 0], delay=delay)
     assert tr["accepted"].sum() > 5
     np.testing.assert_allclose(tr["r_lemma"], tr["r_scratch"], rtol=1e-7)
     assert tr["phase"] == tr["scratch_phase"]
@@ -143,3 +151,49 @@ def test_metropolis_rule():
     assert not orc.metropolis_accept(float("nan"), 0.0)[0]  # NaN rejects
     assert orc.metropolis_accept(0.3 + 0.4j, 0.2499)[0]
     assert not orc.metropolis_accept(0.3 + 0.4j, 0.2501)[0]
+
+
+@pytest.mark.parametrize("kind,k,delay,cplx", [("det", 2, 0, False), ("det", 3, 5, True), ("det", 1, 4, False),
+                                               ("pf", 1, 0, False), ("pf", 2, 3, False), ("pf", 2, 0, True),
+                                               ("pf", 1, 4, True)])
+def test_c_trajectory_equals_numpy_trajectory(kind, k, delay, cplx):
+    """Same seeded inputs through both restatements: identical decisions, ratios and final
+    state to rounding -- immediate and delayed (carriers, Eq. 10-15 / 25-28) alike."""
+    seed, n, M, steps = 991 + k, 14, 30, 50
+    if kind == "det":
+        orb = wl.orbital_matrix(seed, 2, M, n, 1.0 / n, cplx)
+    else:
+        orb = wl.pairing_matrix(seed, 2, M, 1.0 / n, cplx)
+    occ, unocc = wl.initial_occupation(seed, 2, M, n)
+    P, J, xi = wl.proposals(seed, 3, steps, n, M, k, walkers=[2])
+    a = getattr(pyorc, kind + "_trajectory")(orb, occ, unocc, P[:, 0], J[:, 0], xi[:, 0], scratch_every=3, delay=delay)
+    b = getattr(c_oracle, kind + "_trajectory")(orb, occ, unocc, P[:, 0], J[:, 0], xi[:, 0], scratch_every=3, delay=delay)
+    assert np.array_equal(a["accepted"], b["accepted"]) and a["accepted"].sum() > 3
+    np.testing.assert_allclose(a["r_lemma"], b["r_lemma"], rtol=1e-8)
+    m = ~np.isnan(a["r_scratch"])
+    assert np.array_equal(m, ~np.isnan(b["r_scratch"]))
+    np.testing.assert_allclose(a["r_scratch"][m], b["r_scratch"][m], rtol=1e-9)
+    assert np.array_equal(a["occ"], b["occ"]) and np.array_equal(a["A"], b["A"])
+    assert np.allclose(a["Ainv"], b["Ainv"], rtol=1e-7, atol=1e-9)
+    assert a["logabs"] == pytest.approx(b["logabs"], abs=1e-9)
+    assert a["scratch_logabs"] == pytest.approx(b["scratch_logabs"], abs=1e-10)
+    assert a["phase"] == pytest.approx(b["phase"], abs=1e-9)
+    assert a["init_logabs"] == pytest.approx(b["init_logabs"], abs=1e-11)
+
+
+def test_c_batch_runs_walkers_independently():
+    """orc_batch (OpenMP over walkers) gives each walker exactly its single-walker result,
+    and scratch_every = 0 changes no tracked value (only the from-scratch checks go away)."""
+    seed, W, n, M, k, steps = 555, 5, 12, 24, 2, 30
+    orb = np.stack([wl.orbital_matrix(seed, w, M, n, 1.0 / n) for w in range(W)])
+    occ, unocc = wl.initial_occupations(seed, W, M, n)
+    P, J, xi = wl.proposals(seed, W, steps, n, M, k)
+    res = c_oracle.batch("det", orb, occ, unocc, P, J, xi, scratch_every=1, threads=3)
+    res0 = c_oracle.batch("det", orb, occ, unocc, P, J, xi, scratch_every=0, threads=2)
+    for w in range(W):
+        one = c_oracle.det_trajectory(orb[w], occ[w], unocc[w], P[:, w], J[:, w], xi[:, w])
+        for key in ("r_lemma", "accepted", "occ", "Ainv"):
+            assert np.array_equal(res[w][key], one[key]) and np.array_equal(res0[w][key], one[key])
+        assert res[w]["logabs"] == one["logabs"] == res0[w]["logabs"]
+        assert res0[w]["scratch_logabs"] == one["scratch_logabs"]
+        assert np.isnan(res0[w]["r_scratch"]).all()
