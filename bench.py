@@ -223,9 +223,12 @@ def timed_run(ch, warmup, steps, forced=False, sampler=None):
         prof[name] = {"ms": t_ms, "launches": cnt}
     ch.walkers.profile_enable(False)
     f1 = ch.walkers.flush_count() if ch.K > 0 else (0, 0)
+    kernels = {name: ch.walkers.kernel_name(c) for name, c in
+               (("ratio", lrux.PROF_RATIO), ("update", lrux.PROF_UPDATE), ("append", lrux.PROF_APPEND),
+                ("flush", lrux.PROF_FLUSH), ("ypass", lrux.PROF_YPASS))}
     return {"ms": ms, "accepted": int(ch.naccept.item()) - acc0, "launches": ch.launches() - l0,
             "flushes": f1[0] - f0[0], "flush_cols": f1[1] - f0[1],
-            "prof": prof, "clocks": clocks}
+            "prof": prof, "clocks": clocks, "kernels": kernels}
 
 
 def e2e_run(wk, seed, orb, occ, unocc, w0, device, warmup, steps):
@@ -312,57 +315,43 @@ def e2e_run(wk, seed, orb, occ, unocc, w0, device, warmup, steps):
 
 
 # ---------------------------------------------------------------------------- CPU oracle arm
-def oracle_cores():
-    try:
-        from threadpoolctl import threadpool_info
-
-        nt = [int(p.get("num_threads", 1)) for p in threadpool_info()]
-        return max(nt) if nt else 1
-    except Exception:
-        return 1
-
-
-class _Clock:
-    """Timestamps delivered by the oracle's on_step hook."""
-
-    def __init__(self):
-        self.t = {}
-
-    def __call__(self, step):
-        self.t[step] = time.perf_counter()
-
-
-def oracle_sample(wk, warmup, steps, budget_s, max_walkers=1 << 30):
-    """Time the oracle (as it stands) on walkers 0,1,2,... of the workload, `warmup`
-    untimed + `steps` timed Monte-Carlo steps each, until `budget_s` seconds of timed
-    work are spent.  Returns (timed seconds, walker-steps done, walkers)."""
+def oracle_sample(wk, warmup, steps, budget_s, walkers=0):
+    """Time the oracle AS IT STANDS (oracle/lrux_oracle_c.c: plain loops, no BLAS, gcc -O2) on
+    the host cores: walkers 0..Wc-1 of the workload (Wc = 4 x cores unless given), one OpenMP
+    thread per walker in flight, all cores busy, the oracle's naive path only (lemma ratio +
+    Eq. 5 / Eq. 21 Woodbury update or the delayed carrier; no from-scratch recomputation:
+    scratch_every = 0).  Each walker clocks its own steps >= `warmup` (the O(n^3)
+    initialisation and the warm-up steps are left out); throughput = walker-steps /
+    (sum of those times / threads), i.e. what the box sustains with every core on a walker.
+    A short probe sizes T <= `steps` so that the timed part stays near `budget_s` seconds.
+    Returns (seconds, walker-steps, walkers, threads, T)."""
     import numpy as np
-    from oracle import lrux_oracle as orc
+    from oracle import c_oracle
     from paper_2602_05255_b200 import workload as wl
 
     seed = wl.BASE_SEED + wk["cfg"]
-    n, M, k = wk["n"], wk["M"], wk["k"]
-    T = warmup + steps
-    total, done, nw = 0.0, 0, 0
-    while total < budget_s and nw < max_walkers:
-        w = nw
-        if wk["kind"] == "det":
-            var = 1.0 / (2 * n) if wk["cplx"] else 1.0 / n
-            orb = wl.orbital_matrix(seed, w, M, n, var, wk["cplx"])
-        else:
-            orb = wl.pairing_matrix(seed, w, M, 1.0 / n, wk["cplx"])
-        occ, unocc = wl.initial_occupation(seed, w, M, n)
-        P, J, xi = wl.proposals(seed, w + 1, T, n, M, k, walkers=[w])
-        clk = _Clock()
-        fn = orc.det_trajectory if wk["kind"] == "det" else orc.pf_trajectory
-        t_init = time.perf_counter()
-        fn(orb, occ, unocc, P[:, 0], J[:, 0], xi[:, 0], scratch_every=0, delay=wk["Ks"][0],
-           on_step=clk)
-        t_begin = clk.t[warmup - 1] if warmup > 0 else t_init
-        total += clk.t[T - 1] - t_begin
-        done += steps
-        nw += 1
-    return total, done, nw
+    n, M, k, K = wk["n"], wk["M"], wk["k"], wk["Ks"][0]
+    threads = c_oracle.num_threads()
+    Wc = walkers or min(wk["W"], 4 * threads)
+    used = min(threads, Wc)
+    if wk["kind"] == "det":
+        var = 1.0 / (2 * n) if wk["cplx"] else 1.0 / n
+        orb = np.stack([wl.orbital_matrix(seed, w, M, n, var, wk["cplx"]) for w in range(Wc)])
+    else:
+        orb = np.stack([wl.pairing_matrix(seed, w, M, 1.0 / n, wk["cplx"]) for w in range(Wc)])
+    occ, unocc = wl.initial_occupations(seed, Wc, M, n)
+
+    def run(nw, T):
+        P, J, xi = wl.proposals(seed, nw, warmup + T, n, M, k)
+        res = c_oracle.batch(wk["kind"], orb[:nw], occ[:nw], unocc[:nw], P, J, xi, scratch_every=0, delay=K,
+                             final_scratch=False, want_matrices=False, mark_step=warmup)
+        return sum(r["seconds"] for r in res) / min(used, nw)
+
+    probe = max(1, min(steps, 4))
+    per_step = max(run(used, probe) / probe, 1e-7) * Wc / used       # one step of all Wc walkers
+    T = int(max(1, min(steps, budget_s / per_step)))
+    sec = max(run(Wc, T), 1e-9)
+    return sec, Wc * T, Wc, used, T
 
 
 def reference_arm(args, wk):
@@ -374,14 +363,14 @@ def reference_arm(args, wk):
     if rank != 0:
         return 0
     steps, warmup = args.steps, args.warmup
-    # bounded sample: at most ~cpu-seconds*4 of oracle work in total
-    sec, done, nw = oracle_sample(wk, warmup, steps, args.cpu_seconds * 4, max_walkers=64)
+    # each step of this arm is a bounded sample of the workload's step: Wc walkers instead of W
+    sec, done, nw, cores, T = oracle_sample(wk, warmup, steps, args.cpu_seconds * 2)
     value = done / sec
-    cores = oracle_cores()
-    sample = "%d walker(s) x %d steps of %s, oracle naive path (scratch_every=0)" % (nw, steps, args.workload)
+    sample = ("%d of %d walkers x %d steps of %s (after %d warm-up steps), C oracle naive path, "
+              "one OpenMP thread per walker in flight" % (nw, wk["W"], T, args.workload, max(1, warmup)))
     out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
            "n_gpus": args.gpus, "steps": steps, "warmup": warmup,
-           "ms_per_step": 1e3 * sec / max(1, steps), "higher_is_better": True, "scaling": "weak",
+           "ms_per_step": 1e3 * sec / max(1, T), "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "c128" if wk["cplx"] else "f64", "data": "synthetic",
            "config": {"workload": wk["desc"], "K": wk["Ks"][0], "sample": sample},
            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -414,52 +403,19 @@ def dgemm_yardstick(device, n=4096, reps=5):
 
 
 def ncu_traffic_per_walker(kernel, workload):
-    """DRAM bytes per updated walker from the committed ncu --set full capture
-    (profiles/*_traffic.csv, newest round last); None when there is no capture."""
+    """(DRAM bytes per updated walker, source file) from the newest committed `ncu --set full`
+    capture of this kernel on this workload (profiles/*_traffic.csv); (None, None) when there
+    is none.  NOT measured in the bench run: the bench line says where it comes from."""
     import csv
     import glob
 
-    best = None
+    best = (None, None)
     for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
         for row in csv.DictReader(open(path)):
             if row["kernel"] == kernel and row["workload"] == workload:
                 best = ((float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]))
-                        / float(row["walkers_updated_per_launch"]))
+                        / float(row["walkers_updated_per_launch"]), os.path.relpath(path, ROOT))
     return best
-
-
-def det_append_kernel_name(wk):
-    """Mirror of csrc/lrux_det.cu:launch_append_kt: complex data with k <= 4 and 128-row tiles
-    (n >= 1024, [Re N | Im N] + the tile's partial sums within 100 KB) take the DMMA pass."""
-    n = wk["n"]
-    kt = 1 if wk["k"] <= 1 else 2 if wk["k"] <= 2 else 4 if wk["k"] <= 4 else 8
-    if wk["cplx"] and kt <= 4 and n >= 1024 and n % 4 == 0 and n * 64 + 4 * kt * 128 * 16 <= 100 * 1024:
-        return "det_append_dmma_kernel"
-    return "det_append_kernel"
-
-
-def pf_update_kernel_name(n, k, esz):
-    """Mirror of the dispatch in csrc/lrux_pf.cu:pf_accept_impl (K = 0): which kernel
-    applies the immediate Pfaffian update for this shape."""
-    k1 = esz == 8 and k == 1 and n <= 512
-    lg = 5
-    while (1 << lg) < n // 2:
-        lg += 1
-    if esz == 8 and k == 1 and n in (64, 128):
-        return "pf_regs_k1_kernel"
-    rg1 = 1024 >> lg
-    if esz == 8 and k == 1 and lg <= 7 and (5 * ((n + 3) // 4) * n * 8 + (rg1 + rg1 // 4) * (n // 2) * 16
-                                            + n * 32 + 2 * (2 * n + 6) * 8) <= 226 * 1024:
-        return "pf_resident_k1_kernel"
-    for cl in (4, 8):
-        rpc = (n + cl - 1) // cl
-        smc = (rpc * n * 8 + ((256 >> lg) + 2 * cl) * (n // 2) * 16 + n * 40) if k1 \
-            else (rpc * n + (6 * k + 1) * n) * esz
-        if smc <= (56 if cl == 4 else 111) * 1024:
-            return "pf_cluster_k1_kernel" if k1 else "pf_cluster_update_kernel"
-    if (n * n + (4 * k + 1) * n) * esz <= 200 * 1024:
-        return "pf_resident_update_kernel"
-    return "pf_update_stream_kernel"
 
 
 def roofline_update(wk, run, peak, peak_src):
@@ -471,15 +427,14 @@ def roofline_update(wk, run, peak, peak_src):
         return None
     byts = 2.0 * wk["n"] ** 2 * esz * run["accepted"]
     ach = byts / (pr["ms"] * 1e-3) / 1e9
-    rowb = wk["n"] * esz
-    if wk["kind"] == "det":
-        kern = "det_update_tma_kernel" if (rowb >= 8192 and rowb % 16 == 0) else "det_update_kernel"
-    else:
-        kern = pf_update_kernel_name(wk["n"], wk["k"], esz)
-    tpw = ncu_traffic_per_walker(kern, wk.get("name", ""))
+    kern = run.get("kernels", {}).get("update", "")      # as reported by the library (lrux_kernel_name)
+    tpw, src = ncu_traffic_per_walker(kern, wk.get("name", ""))
     traffic = tpw * run["accepted"] / pr["launches"] if tpw else None
     return {"bound": "hbm", "kernel": kern, "achieved": ach, "peak": peak,
-            "unit": "GB/s", "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
+            "unit": "GB/s", "frac": ach / peak, "traffic": traffic,
+            "traffic_source": ("committed ncu --set full capture %s, scaled to this run's accepted walkers per "
+                               "launch; not measured in this run" % src) if tpw else None,
+            "peak_source": peak_src,
             "bytes_per_launch": byts / pr["launches"], "us_per_launch": 1e3 * pr["ms"] / pr["launches"],
             "launches": pr["launches"]}
 
@@ -507,7 +462,7 @@ def roofline_flush(wk, K, run, hbm_peak, hbm_src, dgemm_tflops):
     gbs = byts / (fl["ms"] * 1e-3) / 1e9
     k = (2 * k) if pf else k      # inner dimension per update
     tensor = K * k >= (25 if cx else 50)
-    out = {"kernel": "flush_dmma_kernel", "Kk": K * k, "tflops": tf, "gbs": gbs,
+    out = {"kernel": run.get("kernels", {}).get("flush", ""), "Kk": K * k, "tflops": tf, "gbs": gbs,
            "launches": fl["launches"], "ms": fl["ms"]}
     if tensor and dgemm_tflops:
         out.update(bound="tensor", achieved=tf, peak=dgemm_tflops, unit="TFLOP/s",
@@ -517,6 +472,53 @@ def roofline_flush(wk, K, run, hbm_peak, hbm_src, dgemm_tflops):
         out.update(bound="hbm", achieved=gbs, peak=hbm_peak, unit="GB/s", frac=gbs / hbm_peak,
                    traffic=None, peak_source=hbm_src)
     return out
+
+
+def roofline_append(wk, run, peak, peak_src):
+    """HBM roofline of the delayed append class (a6): one read-only pass over A0^-1 = n^2 e
+    bytes per accepted walker (det: prep + append kernels; pf, k = 1: the Y pass + append)."""
+    if run["prof"]["append"]["ms"] <= 0 or (wk["kind"] == "pf" and wk["k"] > 1):
+        return None
+    ap_ms = run["prof"]["append"]["ms"] + (run["prof"]["ypass"]["ms"] if wk["kind"] == "pf" else 0.0)
+    gbs = wk["n"] ** 2 * (16.0 if wk["cplx"] else 8.0) * run["accepted"] / (ap_ms * 1e-3) / 1e9
+    kern = run.get("kernels", {}).get("append", "")
+    if wk["kind"] == "pf":
+        kern = run.get("kernels", {}).get("ypass", "") + "+" + kern
+    return {"bound": "hbm", "kernel": kern, "achieved": gbs, "peak": peak, "unit": "GB/s",
+            "frac": gbs / peak, "traffic": None, "peak_source": peak_src, "ms": ap_ms}
+
+
+def c4_leg(device, peak, peak_src, dgemm, rank, w0_of):
+    """The second half of BASELINE.json's metric -- "% FP64 TC peak (flush)" -- needs a
+    configuration whose flush is in the tensor regime: configs[3] (complex128, n = 1024,
+    k = 4, K = 32: K k = 128).  A short leg of it runs inside the default bench so that the
+    driver's record carries it: 160 untimed steps bring the delay buffers to their steady
+    state (a walker folds after 32 accepted updates, acceptance ~0.2), then 50 timed steps."""
+    import torch
+
+    wk = parse_workload("c4")
+    K = wk["Ks"][0]
+    seed, orb, occ, unocc = build_inputs(wk, wk["W"], w0_of(wk["W"]), device)
+    saved, saved_init = dict(_MASTERS), dict(INIT_SECONDS)
+    _MASTERS.clear()
+    ch = make_chain(wk, K, seed, orb, occ, unocc, w0_of(wk["W"]), device)
+    init_s = INIT_SECONDS.get(K)
+    _MASTERS.clear()
+    _MASTERS.update(saved)
+    INIT_SECONDS.clear()
+    INIT_SECONDS.update(saved_init)
+    steps, warm = 50, 160
+    run = timed_run(ch, warm, steps)
+    bad = int((ch.walkers.info != 0).sum().item())
+    del ch, orb
+    torch.cuda.empty_cache()
+    return {"workload": wk["desc"], "steps": steps, "warmup": warm, "init_s": init_s,
+            "walker_updates_per_s": wk["W"] * steps / (run["ms"] * 1e-3), "ms_per_step": run["ms"] / steps,
+            "accept_frac": run["accepted"] / float(wk["W"] * steps), "info_nonzero_walkers": bad,
+            "gpu_launches": run["launches"], "flushes": run["flushes"], "flush_cols": run["flush_cols"],
+            "prof_ms": {k: v["ms"] for k, v in run["prof"].items()},
+            "roofline_flush": roofline_flush(wk, K, run, peak, peak_src, dgemm),
+            "roofline_append": roofline_append(wk, run, peak, peak_src)}
 
 
 def parse_workload(name):
@@ -616,20 +618,23 @@ def main(argv=None):
     roof = roofline_update(wk, run, peak, peak_src) if K0 == 0 else None
     if roof is None and "forced_accept" in extras and extras["forced_accept"]["roofline"]:
         roof = extras["forced_accept"]["roofline"]
-    roof_append = None
-    if K0 > 0 and run["prof"]["append"]["ms"] > 0 and not (wk["kind"] == "pf" and wk["k"] > 1):
-        # delayed append (a6): one read-only pass over A0^-1 = n^2 e bytes per accepted walker
-        # (det: prep + append kernels; pf, k = 1: the Y pass + append kernel)
-        ap_ms = run["prof"]["append"]["ms"] + (run["prof"]["ypass"]["ms"] if wk["kind"] == "pf" else 0.0)
-        ap = {"ms": ap_ms}
-        gbs = wk["n"] ** 2 * (16.0 if wk["cplx"] else 8.0) * run["accepted"] / (ap["ms"] * 1e-3) / 1e9
-        roof_append = {"bound": "hbm",
-                       "kernel": (("det_prep_kernel+" + det_append_kernel_name(wk)) if wk["kind"] == "det"
-                                  else "pf_y_kernel+pf_append_kernel"), "achieved": gbs,
-                       "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
-                       "peak_source": peak_src}
-        if roof is None:   # the dominant kernel of a delayed configuration
-            roof = roof_append
+    roof_append = roofline_append(wk, run, peak, peak_src) if K0 > 0 else None
+    if roof is None and roof_append is not None:   # the dominant kernel of a delayed configuration
+        roof = roof_append
+    roof_flush = roofline_flush(wk, K0, run, peak, peak_src, dgemm)
+
+    # the metric's flush half: a short configs[3] leg whenever the headline workload's own flush
+    # is not in the FP64-tensor regime (single GPU; the default run)
+    if (not args.no_extras and rank == 0 and world == 1 and wk.get("name") != "c4"
+            and not (roof_flush and roof_flush.get("bound") == "tensor")):
+        del orb
+        _MASTERS.clear()
+        torch.cuda.empty_cache()
+        extras["c4"] = c4_leg(device, peak, peak_src, dgemm, rank, lambda Wc: 0)
+        if roof_flush is None and extras["c4"]["roofline_flush"]:
+            roof_flush = dict(extras["c4"]["roofline_flush"], workload="configs[3] leg (extras.c4)")
+        if roof_append is None and extras["c4"]["roofline_append"]:
+            roof_append = dict(extras["c4"]["roofline_append"], workload="configs[3] leg (extras.c4)")
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
            "warmup": warmup, "ms_per_step": ms_max / steps, "higher_is_better": True,
@@ -648,15 +653,16 @@ def main(argv=None):
            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": ee["h2d"],
                    "d2h_bytes_per_step": ee["d2h"], "steps": e2e_steps,
                    "decision_mismatches_vs_device_chain": ee["mismatch"]},
-           "roofline": roof, "roofline_append": roof_append, "roofline_flush": roofline_flush(wk, K0, run, peak, peak_src, dgemm),
-           "extras": extras}
+           "roofline": roof, "roofline_append": roof_append, "roofline_flush": roof_flush,
+           "kernels": run["kernels"], "extras": extras}
     if rank == 0:
         if world == 1:
-            sec, done, nw = oracle_sample(wk, 2, 20, args.cpu_seconds)
+            sec, done, nw, cores, T = oracle_sample(wk, 2, 200, args.cpu_seconds)
             out["cpu_baseline"] = {
-                "value": done / sec, "unit": UNIT, "cores": oracle_cores(), "kind": "oracle",
-                "sample": "%d walker(s) x 20 steps of %s (after 2 warm-up steps), oracle naive path"
-                          % (nw, args.workload)}
+                "value": done / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
+                "sample": "%d of %d walkers x %d steps of %s (after 2 warm-up steps), C oracle (plain loops, "
+                          "no BLAS, gcc -O2) naive path, one OpenMP thread per walker in flight"
+                          % (nw, W, T, args.workload)}
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()

@@ -39,7 +39,10 @@ typedef enum {
   LRUX_EINVAL = 1,      /* bad size / odd n for Pf / k > kmax / null pointer */
   LRUX_ESTATE = 2,      /* accept without a pending ratio; det call on a pf handle */
   LRUX_EWORKSPACE = 3,  /* state_bytes too small */
-  LRUX_EUNSUPPORTED = 4, /* delay depth too large: K*kmax^2*sizeof(elem) (x4 for Pf) > 48 KiB */
+  LRUX_EUNSUPPORTED = 4, /* n beyond the initialisation kernels' shared-memory scratch (det:
+                            n*(sizeof(elem)+4) > 200 KiB, i.e. n > 16384 f64 / 10240 c128; pf:
+                            2*n*sizeof(elem) > 200 KiB), or a determinant delay depth with
+                            K*kmax*kt*sizeof(elem) > 160 KiB (kt = kmax rounded up to 1,2,4,8) */
   LRUX_ECUDA = 5        /* a CUDA launch failed */
 } lrux_status_t;
 
@@ -167,6 +170,11 @@ typedef enum {
   LRUX_PROF_NCLASS = 5
 } lrux_prof_class_t;
 lrux_status_t lrux_profile_enable(lrux_handle_t h, int32_t on);
+/* Name of the kernel most recently enqueued through this handle for class `cls`
+ * (lrux_prof_class_t), "" when none was.  Kernels are selected by shape alone -- (dtype, n,
+ * k, K), never by the environment -- and this is how a test or a report learns which one
+ * a shape takes.  The pointer is to a static string. */
+const char* lrux_kernel_name(lrux_handle_t h, int32_t cls);
 lrux_status_t lrux_profile_read(lrux_handle_t h, int32_t cls, double* ms_total,
                                 int64_t* launches);
 

@@ -21,7 +21,8 @@ _vp, _i32 = C.c_void_p, C.c_int32
 
 
 class _Cfg(C.Structure):
-    _fields_ = [(k, _i32) for k in ("kind", "n", "M", "k", "steps", "scratch_every", "delay", "final_scratch")]
+    _fields_ = [(k, _i32) for k in ("kind", "n", "M", "k", "steps", "scratch_every", "delay", "final_scratch",
+                                    "mark_step")]
 
 
 def lib():
@@ -122,12 +123,14 @@ def pf_update_vectors(A_old_rows, A_new_rows, P, n):
 
 
 def batch(kind, orb, occ, unocc, P, J, xi, scratch_every=1, delay=0, final_scratch=True, threads=0,
-          want_matrices=True):
+          want_matrices=True, mark_step=None):
     """Trajectories of W independent walkers (OpenMP over walkers).
 
     orb [W][M][n] (det) or [W][M][M] (pf); occ [W][n], unocc [W][M-n] int32;
     P, J [steps][W][k] int32 and xi [steps][W] as ``workload.proposals`` returns them.
     Returns a list of W dicts with the keys of ``lrux_oracle.det_trajectory``.
+    ``mark_step`` (timing only): each dict also carries ``seconds`` = the time that walker
+    spent in steps >= mark_step (the O(n^3) initialisation and earlier steps left out).
     """
     orb, s = _prep(orb)
     occ = np.ascontiguousarray(occ, dtype=np.int32)
@@ -148,10 +151,12 @@ def batch(kind, orb, occ, unocc, P, J, xi, scratch_every=1, delay=0, final_scrat
     Ainv = np.zeros((W, n, n), dt) if want_matrices else None
     occ_o, unocc_o = np.zeros_like(occ), np.zeros_like(unocc)
     amp, logs = np.zeros((W, 3), dt), np.zeros((W, 3))
-    cfg = _Cfg(0 if kind == "det" else 1, n, M, k, steps, int(scratch_every), int(delay), int(bool(final_scratch)))
+    dur = np.zeros(W) if mark_step is not None else None
+    cfg = _Cfg(0 if kind == "det" else 1, n, M, k, steps, int(scratch_every), int(delay), int(bool(final_scratch)),
+               int(mark_step or 0))
     getattr(lib(), "orc_batch_" + s)(C.byref(cfg), W, int(threads), _p(orb), _p(occ), _p(unocc), _p(Pw), _p(Jw),
                                      _p(xw), _p(r_lemma), _p(r_scratch), _p(accepted), _p(near), _p(prob),
-                                     _p(A), _p(Ainv), _p(occ_o), _p(unocc_o), _p(amp), _p(logs))
+                                     _p(A), _p(Ainv), _p(occ_o), _p(unocc_o), _p(amp), _p(logs), _p(dur))
     out = []
     for w in range(W):
         out.append(dict(r_lemma=r_lemma[w], r_scratch=r_scratch[w], accepted=accepted[w].astype(bool),
@@ -159,7 +164,8 @@ def batch(kind, orb, occ, unocc, P, J, xi, scratch_every=1, delay=0, final_scrat
                         A=A[w] if want_matrices else None, Ainv=Ainv[w] if want_matrices else None,
                         occ=occ_o[w], unocc=unocc_o[w],
                         phase=dt.type(amp[w, 0]), scratch_phase=dt.type(amp[w, 1]), init_phase=dt.type(amp[w, 2]),
-                        logabs=float(logs[w, 0]), scratch_logabs=float(logs[w, 1]), init_logabs=float(logs[w, 2])))
+                        logabs=float(logs[w, 0]), scratch_logabs=float(logs[w, 1]), init_logabs=float(logs[w, 2]),
+                        seconds=float(dur[w]) if dur is not None else None))
     return out
 
 

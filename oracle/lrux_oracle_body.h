@@ -572,7 +572,8 @@ int FN(orc_trajectory)(const orc_cfg* cfg, const T* orb, const int32_t* occ_in, 
                        T* r_lemma, T* r_scratch, uint8_t* accepted, uint8_t* near_tie, double* prob,
                        T* A_out, T* Ainv_out, int32_t* occ_out, int32_t* unocc_out,
                        T* amp /* [3]: tracked phase, scratch phase, initial phase */,
-                       double* logs /* [3]: tracked, scratch, initial log|.| */) {
+                       double* logs /* [3]: tracked, scratch, initial log|.| */,
+                       double* dur /* seconds spent in steps >= cfg->mark_step, or NULL */) {
   const int kind = cfg->kind, n = cfg->n, M = cfg->M, k = cfg->k, steps = cfg->steps;
   const int m = kind == 0 ? k : 2 * k;
   int32_t* occ = (int32_t*)malloc((size_t)n * sizeof(int32_t));
@@ -607,7 +608,9 @@ int FN(orc_trajectory)(const orc_cfg* cfg, const T* orb, const int32_t* occ_in, 
   const int delayed = cfg->delay > 0;
   if (delayed) FN(carrier_init)(&car, n, cfg->delay, Ainv);
   const int se = cfg->scratch_every;
+  double t_mark = 0.0;
   for (int t = 0; t < steps; ++t) {
+    if (dur && t == cfg->mark_step) t_mark = orc_now();
     const int32_t* p = P + (size_t)t * k;
     const int32_t* jj = J + (size_t)t * k;
     /* proposed matrix A' and the update vectors */
@@ -684,6 +687,7 @@ int FN(orc_trajectory)(const orc_cfg* cfg, const T* orb, const int32_t* occ_in, 
       }
     }
   }
+  if (dur) *dur = (cfg->mark_step < steps) ? orc_now() - t_mark : 0.0;
   if (!se && cfg->final_scratch) {
     if (kind == 0) FN(orc_slogdet)(n, A, &s_ph, &s_la); else FN(orc_slogpf)(n, A, &s_ph, &s_la);
   }
@@ -711,7 +715,8 @@ int FN(orc_trajectory)(const orc_cfg* cfg, const T* orb, const int32_t* occ_in, 
 int FN(orc_batch)(const orc_cfg* cfg, int W, int threads, const T* orb, const int32_t* occ,
                   const int32_t* unocc, const int32_t* P, const int32_t* J, const double* xi,
                   T* r_lemma, T* r_scratch, uint8_t* accepted, uint8_t* near_tie, double* prob,
-                  T* A_out, T* Ainv_out, int32_t* occ_out, int32_t* unocc_out, T* amp, double* logs) {
+                  T* A_out, T* Ainv_out, int32_t* occ_out, int32_t* unocc_out, T* amp, double* logs,
+                  double* dur /* [W] or NULL */) {
   const size_t n = cfg->n, M = cfg->M, k = cfg->k, steps = cfg->steps;
   const size_t orb_sz = cfg->kind == 0 ? M * n : M * M;
   int ok_all = 1;
@@ -725,7 +730,7 @@ int FN(orc_batch)(const orc_cfg* cfg, int W, int threads, const T* orb, const in
         xi + w * steps, r_lemma + w * steps, r_scratch + w * steps, accepted + w * steps,
         near_tie + w * steps, prob + w * steps, A_out ? A_out + w * n * n : NULL,
         Ainv_out ? Ainv_out + w * n * n : NULL, occ_out ? occ_out + w * n : NULL,
-        unocc_out ? unocc_out + w * (M - n) : NULL, amp + w * 3, logs + w * 3);
+        unocc_out ? unocc_out + w * (M - n) : NULL, amp + w * 3, logs + w * 3, dur ? dur + w : NULL);
     ok_all = ok_all && ok;
   }
   return ok_all;

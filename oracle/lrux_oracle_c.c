@@ -20,6 +20,7 @@
  *
  * Build: gcc -O2 -fopenmp -shared -fPIC (oracle/build_oracle.py).
  */
+#define _POSIX_C_SOURCE 199309L
 #include <complex.h>
 #include <math.h>
 #include <stdint.h>
@@ -32,7 +33,15 @@
 /* kind 0 = determinant, 1 = Pfaffian; see orc_trajectory_* in the body */
 typedef struct {
   int32_t kind, n, M, k, steps, scratch_every, delay, final_scratch;
+  int32_t mark_step;   /* timing only: steps >= mark_step are clocked (bench.py's cpu_baseline) */
 } orc_cfg;
+
+#include <time.h>
+static double orc_now(void) {
+  struct timespec ts;
+  clock_gettime(CLOCK_MONOTONIC, &ts);
+  return (double)ts.tv_sec + 1e-9 * (double)ts.tv_nsec;
+}
 
 #define T double
 #define FN(name) name##_d

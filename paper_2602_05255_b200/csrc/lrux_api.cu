@@ -64,12 +64,18 @@ static lrux_status_t check_dims(int64_t W, int32_t n, int32_t kmax, int32_t K, i
   if (dt != LRUX_F64 && dt != LRUX_C128) return LRUX_EINVAL;
   if (kind == KIND_PF && (n % 2 != 0)) return LRUX_EINVAL;
   if (kmax > n) return LRUX_EINVAL;
-  // the delayed ratio stages K*kmax*kmax coefficients in shared memory (48 KiB static limit)
+  // the delayed determinant ratio stages K*kmax coefficients per proposal row in (opt-in)
+  // dynamic shared memory; the Pfaffian path has no such limit
   const size_t kt = kmax <= 1 ? 1 : kmax <= 2 ? 2 : kmax <= 4 ? 4 : 8;   // kernels' template rank
-  if ((size_t)K * kmax * kt * (kind == KIND_PF ? 4 : 1) * (dt == LRUX_C128 ? 16 : 8) > 48 * 1024)
+  if (kind == KIND_DET && (size_t)K * kmax * kt * (dt == LRUX_C128 ? 16 : 8) > kRatioCoefSmemMax)
     return LRUX_EUNSUPPORTED;
   if (W > (int64_t)2000000000) return LRUX_EINVAL;
   if (n > kRatioSlice * kRatioSplitMax) return LRUX_EUNSUPPORTED;
+  // initialisation scratch in one CTA's shared memory: a row + a pivot list (blocked
+  // Gauss-Jordan), two rows (Parlett-Reid)
+  const size_t e = dt == LRUX_C128 ? 16 : 8;
+  if ((size_t)n * (e + 4) > 200 * 1024) return LRUX_EUNSUPPORTED;
+  if (kind == KIND_PF && 2 * (size_t)n * e > 200 * 1024) return LRUX_EUNSUPPORTED;
   return LRUX_OK;
 }
 
@@ -92,9 +98,10 @@ static lrux_status_t init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, 
   if (((uintptr_t)d_state & 255) != 0) return LRUX_EINVAL;
   size_t need = state_layout(nullptr, nullptr, W, n, kmax, K, dt, kind);
   if (sb < need) return LRUX_EWORKSPACE;
-  int dev = 0, sms = 0;
+  int dev = 0, sms = 0, optin = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return LRUX_ECUDA;
-  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
     return LRUX_ECUDA;
   lrux_handle_s* hh = new (std::nothrow) lrux_handle_s();
   if (!hh) return LRUX_EINVAL;
@@ -102,10 +109,11 @@ static lrux_status_t init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, 
   hh->st.info = d_info;
   hh->pending_k = 0;
   hh->launches = 0;
-  hh->num_sms = sms;
+  hh->cx.num_sms = sms;
+  hh->cx.smem_optin = optin;
   int nl = attach ? 0
-           : kind == KIND_DET ? launch_det_init(hh->st, d_A0, sms, (cudaStream_t)stream)
-                              : launch_pf_init(hh->st, d_A0, sms, (cudaStream_t)stream);
+           : kind == KIND_DET ? launch_det_init(hh->st, d_A0, hh->cx, (cudaStream_t)stream)
+                              : launch_pf_init(hh->st, d_A0, hh->cx, (cudaStream_t)stream);
   if (nl < 0) {
     delete hh;
     return LRUX_ECUDA;
@@ -113,6 +121,54 @@ static lrux_status_t init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, 
   hh->launches += nl;
   *h = hh;
   return LRUX_OK;
+}
+
+// ---------------------------------------------------------------- launch context
+int Ctx::configure(const void* fn, int threads, size_t smem) {
+  for (const Cfg& c : cfgs)
+    if (c.fn == fn && c.threads == threads && c.smem == smem && c.cluster == 0) return c.occ;
+  // static shared memory counts towards the 48 KiB default: opt in from 40 KiB on, always
+  // to the device maximum (a kernel attribute is shared by every handle of the process)
+  if (smem > 40 * 1024 &&
+      cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess) {
+    cudaGetLastError();
+    return -1;
+  }
+  int occ = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, smem) != cudaSuccess || occ < 1) {
+    cudaGetLastError();
+    return -1;
+  }
+  cfgs.push_back(Cfg{fn, threads, smem, 0, occ});
+  return occ;
+}
+
+int Ctx::configure_cluster(const void* fn, int threads, size_t smem, int cluster) {
+  for (const Cfg& c : cfgs)
+    if (c.fn == fn && c.threads == threads && c.smem == smem && c.cluster == cluster) return c.occ;
+  int ncl = 0;
+  if (smem > 40 * 1024 &&
+      cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess) {
+    cudaGetLastError();
+  } else {
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = cluster;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.blockDim = dim3(threads);
+    cfg.gridDim = dim3(cluster);
+    cfg.dynamicSmemBytes = smem;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (cudaOccupancyMaxActiveClusters(&ncl, fn, &cfg) != cudaSuccess || ncl < 0) {
+      cudaGetLastError();
+      ncl = 0;
+    }
+  }
+  cfgs.push_back(Cfg{fn, threads, smem, cluster, ncl});
+  return ncl;
 }
 
 }  // namespace lrux
@@ -165,7 +221,7 @@ lrux_status_t lrux_det_ratio(lrux_handle_t h, int32_t k, const int32_t* d_idx, c
                              void* d_ratio, void* stream) {
   LRUX_CHECK_HANDLE(h, KIND_DET);
   if (k < 1 || k > h->st.kmax || !d_idx || !d_rows || !d_ratio) return LRUX_EINVAL;
-  LRUX_COUNT(h, launch_det_ratio(h->st, k, d_idx, d_rows, d_ratio, (cudaStream_t)stream, &h->prof));
+  LRUX_COUNT(h, launch_det_ratio(h->st, k, d_idx, d_rows, d_ratio, h->cx, (cudaStream_t)stream));
   h->pending_k = k;
   return LRUX_OK;
 }
@@ -173,7 +229,7 @@ lrux_status_t lrux_pf_ratio(lrux_handle_t h, int32_t k, const int32_t* d_idx, co
                             void* d_ratio, void* stream) {
   LRUX_CHECK_HANDLE(h, KIND_PF);
   if (k < 1 || k > h->st.kmax || !d_idx || !d_rows || !d_ratio) return LRUX_EINVAL;
-  LRUX_COUNT(h, launch_pf_ratio(h->st, k, d_idx, d_rows, d_ratio, h->num_sms, (cudaStream_t)stream, &h->prof));
+  LRUX_COUNT(h, launch_pf_ratio(h->st, k, d_idx, d_rows, d_ratio, h->cx, (cudaStream_t)stream));
   h->pending_k = k;
   return LRUX_OK;
 }
@@ -182,7 +238,7 @@ lrux_status_t lrux_det_accept(lrux_handle_t h, const uint8_t* d_mask, void* stre
   LRUX_CHECK_HANDLE(h, KIND_DET);
   if (!d_mask) return LRUX_EINVAL;
   if (h->pending_k == 0) return LRUX_ESTATE;
-  LRUX_COUNT(h, launch_det_accept(h->st, h->pending_k, d_mask, h->num_sms, (cudaStream_t)stream, &h->prof));
+  LRUX_COUNT(h, launch_det_accept(h->st, h->pending_k, d_mask, h->cx, (cudaStream_t)stream));
   h->pending_k = 0;
   return LRUX_OK;
 }
@@ -190,7 +246,7 @@ lrux_status_t lrux_pf_accept(lrux_handle_t h, const uint8_t* d_mask, void* strea
   LRUX_CHECK_HANDLE(h, KIND_PF);
   if (!d_mask) return LRUX_EINVAL;
   if (h->pending_k == 0) return LRUX_ESTATE;
-  LRUX_COUNT(h, launch_pf_accept(h->st, h->pending_k, d_mask, h->num_sms, (cudaStream_t)stream, &h->prof));
+  LRUX_COUNT(h, launch_pf_accept(h->st, h->pending_k, d_mask, h->cx, (cudaStream_t)stream));
   h->pending_k = 0;
   return LRUX_OK;
 }
@@ -198,13 +254,13 @@ lrux_status_t lrux_pf_accept(lrux_handle_t h, const uint8_t* d_mask, void* strea
 lrux_status_t lrux_det_flush(lrux_handle_t h, void* stream) {
   LRUX_CHECK_HANDLE(h, KIND_DET);
   if (h->st.K == 0) return LRUX_OK;
-  LRUX_COUNT(h, launch_det_flush(h->st, true, h->num_sms, (cudaStream_t)stream, &h->prof));
+  LRUX_COUNT(h, launch_det_flush(h->st, true, h->cx, (cudaStream_t)stream));
   return LRUX_OK;
 }
 lrux_status_t lrux_pf_flush(lrux_handle_t h, void* stream) {
   LRUX_CHECK_HANDLE(h, KIND_PF);
   if (h->st.K == 0) return LRUX_OK;
-  LRUX_COUNT(h, launch_pf_flush(h->st, true, h->num_sms, (cudaStream_t)stream, &h->prof));
+  LRUX_COUNT(h, launch_pf_flush(h->st, true, h->cx, (cudaStream_t)stream));
   return LRUX_OK;
 }
 
@@ -226,21 +282,21 @@ lrux_status_t lrux_pf_get_amplitude(lrux_handle_t h, void* d_phase, double* d_lo
 lrux_status_t lrux_det_get_inverse(lrux_handle_t h, void* d_out, void* stream) {
   LRUX_CHECK_HANDLE(h, KIND_DET);
   if (!d_out) return LRUX_EINVAL;
-  if (h->st.K > 0) LRUX_COUNT(h, launch_det_flush(h->st, true, h->num_sms, (cudaStream_t)stream, &h->prof));
+  if (h->st.K > 0) LRUX_COUNT(h, launch_det_flush(h->st, true, h->cx, (cudaStream_t)stream));
   LRUX_COUNT(h, launch_get_inverse(h->st, d_out, (cudaStream_t)stream));
   return LRUX_OK;
 }
 lrux_status_t lrux_pf_get_inverse(lrux_handle_t h, void* d_out, void* stream) {
   LRUX_CHECK_HANDLE(h, KIND_PF);
   if (!d_out) return LRUX_EINVAL;
-  if (h->st.K > 0) LRUX_COUNT(h, launch_pf_flush(h->st, true, h->num_sms, (cudaStream_t)stream, &h->prof));
+  if (h->st.K > 0) LRUX_COUNT(h, launch_pf_flush(h->st, true, h->cx, (cudaStream_t)stream));
   LRUX_COUNT(h, launch_get_inverse(h->st, d_out, (cudaStream_t)stream));
   return LRUX_OK;
 }
 
 static lrux_status_t refresh(lrux_handle_t h, const void* d_A, void* stream) {
   if (!d_A) return LRUX_EINVAL;
-  LRUX_COUNT(h, launch_refresh(h->st, d_A, h->num_sms, (cudaStream_t)stream));
+  LRUX_COUNT(h, launch_refresh(h->st, d_A, h->cx, (cudaStream_t)stream));
   h->pending_k = 0;
   return LRUX_OK;
 }
@@ -267,9 +323,14 @@ lrux_status_t lrux_launch_count(lrux_handle_t h, int64_t* count) {
   return LRUX_OK;
 }
 
+const char* lrux_kernel_name(lrux_handle_t h, int32_t cls) {
+  if (!h || cls < 0 || cls >= LRUX_PROF_NCLASS || !h->cx.last[cls]) return "";
+  return h->cx.last[cls];
+}
+
 lrux_status_t lrux_profile_enable(lrux_handle_t h, int32_t on) {
   if (!h) return LRUX_EINVAL;
-  h->prof.on = on != 0;
+  h->cx.prof.on = on != 0;
   return LRUX_OK;
 }
 
@@ -277,15 +338,15 @@ lrux_status_t lrux_profile_read(lrux_handle_t h, int32_t cls, double* ms_total, 
   if (!h || !ms_total || !launches || cls < 0 || cls >= LRUX_PROF_NCLASS) return LRUX_EINVAL;
   double ms = 0.0;
   int64_t cnt = 0;
-  for (auto& r : h->prof.recs[cls]) {
+  for (auto& r : h->cx.prof.recs[cls]) {
     float t = 0.f;
     if (cudaEventSynchronize(r.b) != cudaSuccess || cudaEventElapsedTime(&t, r.a, r.b) != cudaSuccess)
       return LRUX_ECUDA;
     ms += t;
     ++cnt;
-    h->prof.pool.push_back(r);
+    h->cx.prof.pool.push_back(r);
   }
-  h->prof.recs[cls].clear();
+  h->cx.prof.recs[cls].clear();
   *ms_total = ms;
   *launches = cnt;
   return LRUX_OK;
@@ -294,8 +355,8 @@ lrux_status_t lrux_profile_read(lrux_handle_t h, int32_t cls, double* ms_total, 
 lrux_status_t lrux_destroy(lrux_handle_t h) {
   if (!h) return LRUX_EINVAL;
   for (int c = 0; c < LRUX_PROF_NCLASS; ++c)
-    for (auto& r : h->prof.recs[c]) h->prof.pool.push_back(r);
-  for (auto& r : h->prof.pool) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (auto& r : h->cx.prof.recs[c]) h->cx.prof.pool.push_back(r);
+  for (auto& r : h->cx.prof.pool) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   delete h;
   return LRUX_OK;
 }

@@ -7,12 +7,8 @@
 //   A'^-1 = A^-1 - C R^-1 Wm                                  (Eq. 5)
 // State Ti = A^-T row-major, so C[:,a] is the contiguous row P[a] of Ti and column
 // j of Wm depends only on row j of Ti: the update is a single pass over Ti.
-#include <stdlib.h>
-
 #include "lrux_common.cuh"
 #include "lrux_internal.h"
-#include <cstdlib>
-#include <cstring>
 
 namespace lrux {
 
@@ -857,149 +853,115 @@ int launch_flush_clear(const State& st, cudaStream_t s) {
 }
 
 // ---------------------------------------------------------------- launchers
-static inline int round_kt(int k) { return k <= 1 ? 1 : k <= 2 ? 2 : k <= 4 ? 4 : 8; }
-
-static inline int persistent_grid(int num_sms, int ctas_per_sm, int64_t max_items) {
-  int64_t g = (int64_t)num_sms * ctas_per_sm;
-  if (g > max_items) g = max_items;
-  return g < 1 ? 1 : (int)g;
-}
-
+// Every choice below depends on the shape (dtype, n, k, K) only.
 template <typename T, int KT, int VEC, int CH, int RW>
-static int launch_update_reg(const State& st, int k, int num_sms, cudaStream_t s) {
+static int launch_update_reg(const State& st, int k, Ctx& cx, cudaStream_t s) {
   const int n = st.n;
   const size_t smem = 2 * (size_t)k * n * sizeof(T);
   auto kern = det_update_kernel<T, KT, VEC, CH, RW>;
-  if (smem > 40 * 1024 &&   // static shared memory counts towards the 48 KiB default
-
-      cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-    return -1;
+  const int occ = cx.configure((const void*)kern, 256, smem);
+  if (occ < 0) return -1;
   int rows_per_tile = 64;
   if (rows_per_tile > n) rows_per_tile = n;
   const int tiles = (n + rows_per_tile - 1) / rows_per_tile;
-  int occ = 1;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, smem);
-  if (occ < 1) occ = 1;
-  const int grid = persistent_grid(num_sms, occ, (int64_t)st.W * tiles);
+  const int grid = persistent_grid(cx.num_sms, occ, (int64_t)st.W * tiles);
   kern<<<grid, 256, smem, s>>>(st, k, tiles, rows_per_tile);
+  cx.name(LRUX_PROF_UPDATE, "det_update_kernel");
   return 1;
 }
 
 template <typename T, int KT>
-static int launch_update_kt(const State& st, int k, int num_sms, cudaStream_t s) {
+static int launch_update_kt(const State& st, int k, Ctx& cx, cudaStream_t s) {
   const int n = st.n;
   constexpr int VECMAX = sizeof(T) == 8 ? 2 : 1;
-  {
-    // rows of >= 8 KB: TMA-staged kernel (lrux_det_tma.cu).  LRUX_UPDATE_PATH=reg|tma
-    // overrides the choice (tuning / A-B measurements only).
-    const char* path = getenv("LRUX_UPDATE_PATH");
-    const bool force_tma = path && path[0] == 't', force_reg = path && path[0] == 'r';
-    if (!force_reg && (force_tma || (size_t)n * sizeof(T) >= 8 * 1024)) {
-      const int r = launch_det_update_tma(st, k, num_sms, s);
-      if (r != 0) return r;
-      // no instance for the full rank (register budget): peel off chunks of the largest
-      // rank that has one; each chunk is one full pass over A^-1
-      int c = 0;
-      for (int cand = 4; cand >= 1; cand >>= 1)
-        if (cand < k && launch_det_update_tma_ok(st, cand)) { c = cand; break; }
-      if (c > 0) {
-        int nl = 0, rem = k;
-        State v = st;   // view of the pending area, shifted past the chunks already applied
-        const size_t e = sizeof(T);
-        while (rem > 0) {
-          const int cur = rem > c ? c : rem;
-          if (rem > cur) {
-            det_split_prep_kernel<T><<<persistent_grid(num_sms, 4, st.W), 256, 0, s>>>(v, cur, rem);
-            ++nl;
-          }
-          const int r2 = launch_det_update_tma(v, cur, num_sms, s);
-          if (r2 <= 0) return -1;
-          nl += r2;
-          v.pend_idx += cur;
-          v.pend_N = (char*)v.pend_N + (size_t)cur * n * e;
-          v.pend_C = (char*)v.pend_C + (size_t)cur * n * e;
-          v.pend_Rinv = (char*)v.pend_Rinv + ((size_t)cur * st.kc + cur) * e;
-          rem -= cur;
+  if ((size_t)n * sizeof(T) >= 8 * 1024) {
+    // rows of >= 8 KB: TMA-staged kernel (lrux_det_tma.cu)
+    const int r = launch_det_update_tma(st, k, cx, s);
+    if (r != 0) return r;
+    // no instance for the full rank (register budget): peel off chunks of the largest
+    // rank that has one; each chunk is one full pass over A^-1
+    int c = 0;
+    for (int cand = 4; cand >= 1; cand >>= 1)
+      if (cand < k && launch_det_update_tma(st, cand, cx, s, /*probe=*/true) == 1) { c = cand; break; }
+    if (c > 0) {
+      int nl = 0, rem = k;
+      State v = st;   // view of the pending area, shifted past the chunks already applied
+      const size_t e = sizeof(T);
+      while (rem > 0) {
+        const int cur = rem > c ? c : rem;
+        if (rem > cur) {
+          det_split_prep_kernel<T><<<persistent_grid(cx.num_sms, 4, st.W), 256, 0, s>>>(v, cur, rem);
+          ++nl;
         }
-        return nl;
+        const int r2 = launch_det_update_tma(v, cur, cx, s);
+        if (r2 <= 0) return -1;
+        nl += r2;
+        v.pend_idx += cur;
+        v.pend_N = (char*)v.pend_N + (size_t)cur * n * e;
+        v.pend_C = (char*)v.pend_C + (size_t)cur * n * e;
+        v.pend_Rinv = (char*)v.pend_Rinv + ((size_t)cur * st.kc + cur) * e;
+        rem -= cur;
       }
+      return nl;
     }
   }
   const size_t smem = 2 * (size_t)k * n * sizeof(T);
   const bool vec_ok = (n % VECMAX) == 0;
   const int nvec = n / VECMAX;
   if (vec_ok && smem <= 160 * 1024) {
-    if (nvec <= 32 * 1) return launch_update_reg<T, KT, VECMAX, 1, 2>(st, k, num_sms, s);
-    if (nvec <= 32 * 2) return launch_update_reg<T, KT, VECMAX, 2, 2>(st, k, num_sms, s);
-    if (nvec <= 32 * 4) return launch_update_reg<T, KT, VECMAX, 4, 2>(st, k, num_sms, s);
-    if (nvec <= 32 * 8) return launch_update_reg<T, KT, VECMAX, 8, 1>(st, k, num_sms, s);
-    if (nvec <= 32 * 16) return launch_update_reg<T, KT, VECMAX, 16, 1>(st, k, num_sms, s);
+    if (nvec <= 32 * 1) return launch_update_reg<T, KT, VECMAX, 1, 2>(st, k, cx, s);
+    if (nvec <= 32 * 2) return launch_update_reg<T, KT, VECMAX, 2, 2>(st, k, cx, s);
+    if (nvec <= 32 * 4) return launch_update_reg<T, KT, VECMAX, 4, 2>(st, k, cx, s);
+    if (nvec <= 32 * 8) return launch_update_reg<T, KT, VECMAX, 8, 1>(st, k, cx, s);
+    if (nvec <= 32 * 16) return launch_update_reg<T, KT, VECMAX, 16, 1>(st, k, cx, s);
   }
   int rows_per_tile = 64;
   if (rows_per_tile > n) rows_per_tile = n;
   const int tiles = (n + rows_per_tile - 1) / rows_per_tile;
-  const int grid = persistent_grid(num_sms, 4, (int64_t)st.W * tiles);
+  const int grid = persistent_grid(cx.num_sms, 4, (int64_t)st.W * tiles);
   det_update_stream_kernel<T, KT><<<grid, 256, 0, s>>>(st, k, tiles, rows_per_tile);
+  cx.name(LRUX_PROF_UPDATE, "det_update_stream_kernel");
   return 1;
 }
 
 template <typename T, int KT>
-static int launch_append_kt(const State& st, int k, int num_sms, cudaStream_t s) {
+static int launch_append_kt(const State& st, int k, Ctx& cx, cudaStream_t s) {
   const int n = st.n;
   constexpr int VECMAX = sizeof(T) == 8 ? 2 : 1;
   int nl = 0;
   {
     const int groups = (st.cap + 8 * kPrepRows - 1) / (8 * kPrepRows);
-    const int grid = persistent_grid(num_sms, 8, (int64_t)st.W * groups);
+    const int grid = persistent_grid(cx.num_sms, 8, (int64_t)st.W * groups);
     det_prep_kernel<T, KT><<<grid, 256, 0, s>>>(st, k, groups); ++nl;
-  }
-  {
-    // rows of >= 8 KB: the TMA-staged pass (lrux_det_tma.cu) + finish kernel
-    // (measured on B200: the register-row append below is still faster at configs[3],
-    // 0.60 vs 0.45 of HBM peak, so the TMA pass is opt-in for the delayed path)
-    const char* path = getenv("LRUX_UPDATE_PATH");
-    const bool force_tma = path && path[0] == 't';
-    if (force_tma) {
-      const int r = launch_det_append_tma(st, k, num_sms, s);
-      if (r != 0) return r < 0 ? -1 : nl + r;
-    }
   }
   const int rows_per_tile = n >= 1024 ? 128 : 64;   // must divide the block size (256)
   const int tiles = (n + rows_per_tile - 1) / rows_per_tile;
   const int n_in_smem = (size_t)k * n * sizeof(T) <= 96 * 1024;
   const size_t smem = ((n_in_smem ? (size_t)k * n : 0) + 4 * (size_t)KT * rows_per_tile) * sizeof(T);
   if constexpr (sizeof(T) == 16 && KT <= 4) {
-    // complex data, k <= 4: the dot products on the FP64 tensor pipe
-    const char* env = getenv("LRUX_APPEND_PATH");   // A-B measurements only
-    const int rpt_d = rows_per_tile, tiles_d = tiles;
-    const size_t smd = (size_t)n * 64 + 4 * (size_t)KT * rpt_d * sizeof(T);
-    if (n % 4 == 0 && rows_per_tile == 128 && smd <= 100 * 1024 && !(env && !strcmp(env, "scalar"))) {
+    // complex data, k <= 4, 128-row tiles: the dot products on the FP64 tensor pipe
+    const size_t smd = (size_t)n * 64 + 4 * (size_t)KT * rows_per_tile * sizeof(T);
+    if (n % 4 == 0 && rows_per_tile == 128 && smd <= 100 * 1024) {
       auto kd = det_append_dmma_kernel<KT>;
-      if (cudaFuncSetAttribute(kd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smd) != cudaSuccess)
-        return -1;
-      int occd = 1;
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occd, kd, 256, smd);
-      if (occd < 1) return -1;
-      kd<<<persistent_grid(num_sms, occd, (int64_t)st.W * tiles_d), 256, smd, s>>>(st, k, tiles_d, rpt_d); ++nl;
-      return nl;
+      const int occd = cx.configure((const void*)kd, 256, smd);
+      if (occd < 0) return -1;
+      kd<<<persistent_grid(cx.num_sms, occd, (int64_t)st.W * tiles), 256, smd, s>>>(st, k, tiles, rows_per_tile);
+      cx.name(LRUX_PROF_APPEND, "det_prep_kernel+det_append_dmma_kernel");
+      return nl + 1;
     }
   }
   const bool vec = (n % VECMAX) == 0 && VECMAX == 2;
   auto kern = vec ? det_append_kernel<T, KT, VECMAX, 2> : det_append_kernel<T, KT, 1, 2>;
-  if (smem > 40 * 1024 &&   // static shared memory counts towards the 48 KiB default
-
-      cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-    return -1;
-  int occ = 1;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, smem);
-  if (occ < 1) return -1;
-  const int grid = persistent_grid(num_sms, occ, (int64_t)st.W * tiles);
-  kern<<<grid, 256, smem, s>>>(st, k, tiles, rows_per_tile, n_in_smem); ++nl;
-  return nl;
+  const int occ = cx.configure((const void*)kern, 256, smem);
+  if (occ < 0) return -1;
+  const int grid = persistent_grid(cx.num_sms, occ, (int64_t)st.W * tiles);
+  kern<<<grid, 256, smem, s>>>(st, k, tiles, rows_per_tile, n_in_smem);
+  cx.name(LRUX_PROF_APPEND, "det_prep_kernel+det_append_kernel");
+  return nl + 1;
 }
 
 template <typename T>
-static int flush_impl(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof) {
+static int flush_impl(const State& st, bool all, Ctx& cx, cudaStream_t s) {
   int nl = 0;
   const unsigned gw = (unsigned)((st.W + 255) / 256);
   if (all) {
@@ -1007,45 +969,44 @@ static int flush_impl(const State& st, bool all, int num_sms, cudaStream_t s, Pr
     flush_all_select_kernel<<<gw, 256, 0, s>>>(st); ++nl;
   }
   {
-    ProfScope ps(prof, LRUX_PROF_FLUSH, s);
-    nl += launch_flush_dmma(st, num_sms, s);   // Eq. 12 on the FP64 tensor path
+    ProfScope ps(&cx.prof, LRUX_PROF_FLUSH, s);
+    nl += launch_flush_dmma(st, cx, s);   // Eq. 12 on the FP64 tensor path
   }
   flush_clear_kernel<<<gw, 256, 0, s>>>(st); ++nl;
   return cudaGetLastError() == cudaSuccess ? nl : -1;
 }
 
 template <typename T>
-static int accept_impl(const State& st, int k, const uint8_t* mask, int num_sms, cudaStream_t s,
-                       Prof* prof) {
+static int accept_impl(const State& st, int k, const uint8_t* mask, Ctx& cx, cudaStream_t s) {
   int nl = 0;
   const unsigned gw = (unsigned)((st.W + 255) / 256);
   select_kernel<T><<<gw, 256, 0, s>>>(st, mask); ++nl;
   const int kt = round_kt(k);
   int r = 0;
   if (st.K == 0) {
-    ProfScope ps(prof, LRUX_PROF_UPDATE, s);
+    ProfScope ps(&cx.prof, LRUX_PROF_UPDATE, s);
     switch (kt) {
-      case 1: r = launch_update_kt<T, 1>(st, k, num_sms, s); break;
-      case 2: r = launch_update_kt<T, 2>(st, k, num_sms, s); break;
-      case 4: r = launch_update_kt<T, 4>(st, k, num_sms, s); break;
-      default: r = launch_update_kt<T, 8>(st, k, num_sms, s); break;
+      case 1: r = launch_update_kt<T, 1>(st, k, cx, s); break;
+      case 2: r = launch_update_kt<T, 2>(st, k, cx, s); break;
+      case 4: r = launch_update_kt<T, 4>(st, k, cx, s); break;
+      default: r = launch_update_kt<T, 8>(st, k, cx, s); break;
     }
     if (r < 0) return -1;
     nl += r;
   } else {
     {
-      ProfScope ps(prof, LRUX_PROF_APPEND, s);
+      ProfScope ps(&cx.prof, LRUX_PROF_APPEND, s);
       switch (kt) {
-        case 1: r = launch_append_kt<T, 1>(st, k, num_sms, s); break;
-        case 2: r = launch_append_kt<T, 2>(st, k, num_sms, s); break;
-        case 4: r = launch_append_kt<T, 4>(st, k, num_sms, s); break;
-        default: r = launch_append_kt<T, 8>(st, k, num_sms, s); break;
+        case 1: r = launch_append_kt<T, 1>(st, k, cx, s); break;
+        case 2: r = launch_append_kt<T, 2>(st, k, cx, s); break;
+        case 4: r = launch_append_kt<T, 4>(st, k, cx, s); break;
+        default: r = launch_append_kt<T, 8>(st, k, cx, s); break;
       }
     }
     if (r < 0) return -1;
     nl += r;
     post_kernel<<<gw, 256, 0, s>>>(st, k); ++nl;
-    r = flush_impl<T>(st, false, num_sms, s, prof);
+    r = flush_impl<T>(st, false, cx, s);
     if (r < 0) return -1;
     nl += r;
   }
@@ -1053,50 +1014,49 @@ static int accept_impl(const State& st, int k, const uint8_t* mask, int num_sms,
 }
 
 template <typename T, int KT>
-static void launch_ratio_kt(const State& st, int k, const int32_t* d_idx, const void* d_rows,
-                            void* d_ratio, cudaStream_t s) {
+static int launch_ratio_kt(const State& st, int k, const int32_t* d_idx, const void* d_rows,
+                           void* d_ratio, Ctx& cx, cudaStream_t s) {
   // one CTA per 256-column slice: 128 threads x 2 elements (n <= 256: a single slice,
   // 1 element per thread when n <= 128), else 256 threads x 1 element
   const int n = st.n;
   const int nsplit = (n + kRatioSlice - 1) / kRatioSlice;
   const dim3 grid((unsigned)st.W, (unsigned)nsplit);
-  const size_t sm = (size_t)st.cap * KT * sizeof(T);   // <= 48 KiB (checked at init)
-  if (n <= 128)
-    det_ratio_kernel<T, KT, 1><<<grid, 128, sm, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
-  else if (n <= 256)
-    det_ratio_kernel<T, KT, 2><<<grid, 128, sm, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
-  else
-    det_ratio_kernel<T, KT, 1><<<grid, 256, sm, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
+  const size_t sm = (size_t)st.cap * KT * sizeof(T);   // <= kRatioCoefSmemMax (checked at init)
+  auto kern = n <= 128 ? det_ratio_kernel<T, KT, 1> : n <= 256 ? det_ratio_kernel<T, KT, 2>
+                                                               : det_ratio_kernel<T, KT, 1>;
+  const int threads = n <= 256 ? 128 : 256;
+  if (cx.configure((const void*)kern, threads, sm) < 0) return -1;
+  kern<<<grid, threads, sm, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
+  return 1;
 }
 
 template <typename T>
-static void launch_ratio_t(const State& st, int k, const int32_t* d_idx, const void* d_rows,
-                           void* d_ratio, cudaStream_t s) {
+static int launch_ratio_t(const State& st, int k, const int32_t* d_idx, const void* d_rows,
+                          void* d_ratio, Ctx& cx, cudaStream_t s) {
   switch (round_kt(k)) {
-    case 1: launch_ratio_kt<T, 1>(st, k, d_idx, d_rows, d_ratio, s); break;
-    case 2: launch_ratio_kt<T, 2>(st, k, d_idx, d_rows, d_ratio, s); break;
-    case 4: launch_ratio_kt<T, 4>(st, k, d_idx, d_rows, d_ratio, s); break;
-    default: launch_ratio_kt<T, 8>(st, k, d_idx, d_rows, d_ratio, s); break;
+    case 1: return launch_ratio_kt<T, 1>(st, k, d_idx, d_rows, d_ratio, cx, s);
+    case 2: return launch_ratio_kt<T, 2>(st, k, d_idx, d_rows, d_ratio, cx, s);
+    case 4: return launch_ratio_kt<T, 4>(st, k, d_idx, d_rows, d_ratio, cx, s);
+    default: return launch_ratio_kt<T, 8>(st, k, d_idx, d_rows, d_ratio, cx, s);
   }
 }
 
 int launch_det_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
-                     void* d_ratio, cudaStream_t s, Prof* prof) {
-  ProfScope ps(prof, LRUX_PROF_RATIO, s);
-  if (st.dt == LRUX_F64) launch_ratio_t<double>(st, k, d_idx, d_rows, d_ratio, s);
-  else launch_ratio_t<cplx>(st, k, d_idx, d_rows, d_ratio, s);
-  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+                     void* d_ratio, Ctx& cx, cudaStream_t s) {
+  ProfScope ps(&cx.prof, LRUX_PROF_RATIO, s);
+  cx.name(LRUX_PROF_RATIO, "det_ratio_kernel");
+  const int r = st.dt == LRUX_F64 ? launch_ratio_t<double>(st, k, d_idx, d_rows, d_ratio, cx, s)
+                                  : launch_ratio_t<cplx>(st, k, d_idx, d_rows, d_ratio, cx, s);
+  return (r > 0 && cudaGetLastError() == cudaSuccess) ? r : -1;
 }
 
-int launch_det_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s,
-                      Prof* prof) {
-  return st.dt == LRUX_F64 ? accept_impl<double>(st, k, d_mask, num_sms, s, prof)
-                           : accept_impl<cplx>(st, k, d_mask, num_sms, s, prof);
+int launch_det_accept(const State& st, int k, const uint8_t* d_mask, Ctx& cx, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? accept_impl<double>(st, k, d_mask, cx, s)
+                           : accept_impl<cplx>(st, k, d_mask, cx, s);
 }
 
-int launch_det_flush(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof) {
-  return st.dt == LRUX_F64 ? flush_impl<double>(st, all, num_sms, s, prof)
-                           : flush_impl<cplx>(st, all, num_sms, s, prof);
+int launch_det_flush(const State& st, bool all, Ctx& cx, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? flush_impl<double>(st, all, cx, s) : flush_impl<cplx>(st, all, cx, s);
 }
 
 }  // namespace lrux

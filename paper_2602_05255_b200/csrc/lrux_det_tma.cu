@@ -15,8 +15,6 @@
 // slice (rows from shared memory, its slices of N and C cached in registers), the
 // partial sums meet in shared memory, g = R^-1 d, then the same lanes apply the rank-k
 // update to their columns in place and the chunk goes back to HBM.
-#include <stdlib.h>
-
 #include "lrux_common.cuh"
 #include "lrux_internal.h"
 #include "lrux_tma.cuh"
@@ -84,12 +82,7 @@ __device__ __forceinline__ void to_doubles(cplx x, double* o) { o[0] = x.re; o[1
 // t < TV, of EVERY row -- so its slices of N and C (k x TV vectors each) stay in
 // registers for as long as the CTA works on one walker, and shared memory carries only
 // the streamed rows.
-//
-// APPEND = true is the delayed-update variant (row a6): the same streamed pass, read
-// only -- it leaves D[a][j] = N_a . Ti[j][:] - [j == P[a]]  (= u^T A0^-1, Eq. 15) in the
-// pending area (pend_C, free once det_prep_kernel has copied a_tau into the buffer) for
-// det_append_finish_kernel; nothing is written back to A0^-1.
-template <typename T, int KT, int RC, int TV, bool APPEND, int NW>
+template <typename T, int KT, int RC, int TV, int NW>
 __global__ void __launch_bounds__(NW * 32, 1)
 det_update_tma_kernel(State st, int k, int NS) {
   using S = Sc<T>;
@@ -156,7 +149,7 @@ det_update_tma_kernel(State st, int k, int NS) {
           const int q = warp * 32 + lane + 32 * NW * t;
           const bool ok = a < k && q < nvec;
           nreg[a][t] = ok ? gN[(size_t)a * nvec + q] : make_double2(0.0, 0.0);
-          if (!APPEND) creg[a][t] = ok ? gC[(size_t)a * nvec + q] : make_double2(0.0, 0.0);
+          creg[a][t] = ok ? gC[(size_t)a * nvec + q] : make_double2(0.0, 0.0);
         }
       if (tid < KT * KT) {
         const int a = tid / KT, b = tid % KT;
@@ -168,7 +161,7 @@ det_update_tma_kernel(State st, int k, int NS) {
       __syncthreads();
     }
     if (tid == 0 && li + NS - 2 < my) {
-      if (!APPEND) tma::store_wait_read<1>();   // the stage consumed two chunks ago has been read out
+      tma::store_wait_read<1>();   // the stage consumed two chunks ago has been read out
       issue(li + NS - 2);
     }
     double* dpart = dpart0 + (li & 1) * NW * NV;   // double-buffered by chunk parity
@@ -218,24 +211,15 @@ det_update_tma_kernel(State st, int k, int NS) {
     __syncthreads();
     if (tid < RC * KT) {
       const int r = tid / KT, a = tid % KT;
-      if constexpr (APPEND) {
-        if (a < k && r < rows) {
-          T db = sc_from(dsum[(r * KT + a) * ND], dsum[(r * KT + a) * ND + ND - 1], T{});
-          if (j0 + r == sidx[a]) db = S::sub(db, S::one());
-          ((T*)st.pend_C)[((size_t)w * kmax + a) * n + j0 + r] = db;
-        }
-      } else {
-        T acc = S::zero();
+      T acc = S::zero();
 #pragma unroll
-        for (int b = 0; b < KT; ++b) {
-          T db = sc_from(dsum[(r * KT + b) * ND], dsum[(r * KT + b) * ND + ND - 1], T{});
-          if (j0 + r == sidx[b]) db = S::sub(db, S::one());
-          acc = S::fma(Ri[a * KT + b], db, acc);
-        }
-        gsm[r * KT + a] = acc;
+      for (int b = 0; b < KT; ++b) {
+        T db = sc_from(dsum[(r * KT + b) * ND], dsum[(r * KT + b) * ND + ND - 1], T{});
+        if (j0 + r == sidx[b]) db = S::sub(db, S::one());
+        acc = S::fma(Ri[a * KT + b], db, acc);
       }
+      gsm[r * KT + a] = acc;
     }
-    if constexpr (APPEND) continue;   // dsum / dpart are double-buffered by chunk parity
     __syncthreads();
     // ---- x[r][i] -= sum_a g[r][a] C[a][i] on this lane's columns, in place
     {
@@ -268,62 +252,13 @@ det_update_tma_kernel(State st, int k, int NS) {
       tma::store_commit();
     }
   }
-  if (!APPEND && tid == 0) tma::store_wait_all<0>();
+  if (tid == 0) tma::store_wait_all<0>();
 }
 
-// b_tau^T = R^-1 (D - (N Abuf) Bbuf^T) -> Bbuf[fill .. fill+k)   (Eq. 15, PAPER.md:194;
-// DESIGN.md reading 5b).  Work item = (accepted walker, 256 columns); thread per column.
-template <typename T, int KT>
-__global__ void __launch_bounds__(256) det_append_finish_kernel(State st, int k, int chunks) {
-  using S = Sc<T>;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  T* NAs = (T*)smem_raw;   // [fill][KT]
-  __shared__ T Ri[KT * KT];
-  const int n = st.n, kmax = st.kmax, cap = st.cap;
-  const int tid = threadIdx.x;
-  const int count = st.counters[0];
-  for (int item = blockIdx.x; item < count * chunks; item += gridDim.x) {
-    const int w = st.list[item / chunks];
-    const int j = (item % chunks) * 256 + tid;
-    const int fill = st.fill[w];
-    __syncthreads();
-    const T* NA = (const T*)st.pend_Y + (size_t)w * kmax * cap;
-    for (int q = tid; q < fill * KT; q += 256)
-      NAs[q] = (q % KT) < k ? NA[(size_t)(q % KT) * cap + q / KT] : S::zero();
-    if (tid < KT * KT) {
-      const int a = tid / KT, b = tid % KT;
-      Ri[tid] = (a < k && b < k) ? ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + a * st.kc + b]
-                                 : S::zero();
-    }
-    __syncthreads();
-    if (j >= n) continue;
-    const T* D = (const T*)st.pend_C + (size_t)w * kmax * n;
-    T* Bb = (T*)st.Bbuf + (size_t)w * cap * n;
-    T m[KT];
-#pragma unroll
-    for (int b = 0; b < KT; ++b) m[b] = b < k ? D[(size_t)b * n + j] : S::zero();
-#pragma unroll 8
-    for (int s = 0; s < fill; ++s) {
-      const T bv = Bb[(size_t)s * n + j];
-#pragma unroll
-      for (int b = 0; b < KT; ++b) m[b] = S::fnma(NAs[s * KT + b], bv, m[b]);
-    }
-#pragma unroll
-    for (int a = 0; a < KT; ++a) {
-      if (a < k) {
-        T acc = S::zero();
-#pragma unroll
-        for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], m[b], acc);
-        Bb[(size_t)(fill + a) * n + j] = acc;
-      }
-    }
-  }
-}
-
-template <typename T, int KT, int RC, int TV, bool APPEND, int NW>
-static int launch_tma_inst(const State& st, int k, int num_sms, cudaStream_t s) {
+template <typename T, int KT, int RC, int TV, int NW>
+static int launch_tma_inst(const State& st, int k, Ctx& cx, cudaStream_t s, bool probe) {
   constexpr int ND = sizeof(T) / 8;
-  if constexpr (RC * KT * ND > 32 || KT * TV > (APPEND ? 16 : NW == 16 ? 8 : 16)) {
+  if constexpr (RC * KT * ND > 32 || KT * TV > (NW == 16 ? 8 : 16)) {
     return 0;   // too many partial sums / cached registers for this instance
   } else {
     const size_t row = (size_t)st.n * sizeof(T);
@@ -332,24 +267,19 @@ static int launch_tma_inst(const State& st, int k, int num_sms, cudaStream_t s) 
     if (NS > 8) NS = 8;
     if (NS < 3) return 0;
     const size_t smem = (size_t)NS * RC * row + fixed;
-    if (num_sms <= 0) return 1;   // eligibility probe (launch_det_update_tma_ok)
-    auto kern = det_update_tma_kernel<T, KT, RC, TV, APPEND, NW>;
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-      return -1;
-    kern<<<num_sms, NW * 32, smem, s>>>(st, k, NS);
-    if (!APPEND) return 1;
-    const int chunks = (st.n + 255) / 256;
-    int64_t grid = (int64_t)num_sms * 8;
-    if (grid > st.W * chunks) grid = st.W * chunks;
-    det_append_finish_kernel<T, KT><<<(unsigned)grid, 256, (size_t)st.cap * KT * sizeof(T), s>>>(st, k, chunks);
-    return 2;
+    if (probe) return 1;
+    auto kern = det_update_tma_kernel<T, KT, RC, TV, NW>;
+    if (cx.configure((const void*)kern, NW * 32, smem) < 0) return -1;
+    kern<<<cx.num_sms, NW * 32, smem, s>>>(st, k, NS);
+    cx.name(LRUX_PROF_UPDATE, "det_update_tma_kernel");
+    return 1;
   }
 }
 
 // Returns the number of launches (1), 0 when this shape is not eligible (caller falls
 // back to the register-row / generic kernels), -1 on a CUDA error.
-template <typename T, int KT, bool APPEND>
-static int launch_update_tma_kt(const State& st, int k, int num_sms, cudaStream_t s) {
+template <typename T, int KT>
+static int launch_update_tma_kt(const State& st, int k, Ctx& cx, cudaStream_t s, bool probe) {
   const size_t row = (size_t)st.n * sizeof(T);
   if (row % 16 != 0) return 0;
   const int nvec = (int)(row / 16);
@@ -360,11 +290,10 @@ static int launch_update_tma_kt(const State& st, int k, int num_sms, cudaStream_
   const int tv8 = (nvec + 255) / 256, tv16 = (nvec + 511) / 512;
 #define LRUX_TMA_CASE(RC_, TV_, NW_)                                                       \
   if (rc == RC_ && (NW_ == 16 ? tv16 : tv8) <= TV_) {                                      \
-    const int r_ = launch_tma_inst<T, KT, RC_, TV_, APPEND, NW_>(st, k, num_sms, s);       \
+    const int r_ = launch_tma_inst<T, KT, RC_, TV_, NW_>(st, k, cx, s, probe);             \
     if (r_ != 0) return r_;                                                                \
   }
-  const char* warps_env = getenv("LRUX_TMA_WARPS");   // A-B measurements only
-  if (tv8 >= 2 && KT <= 2 && !(warps_env && warps_env[0] == '8')) {
+  if (tv8 >= 2 && KT <= 2) {
     LRUX_TMA_CASE(4, 1, 16)
     LRUX_TMA_CASE(4, 2, 16)
     LRUX_TMA_CASE(2, 2, 16)
@@ -382,31 +311,19 @@ static int launch_update_tma_kt(const State& st, int k, int num_sms, cudaStream_
   return 0;
 }
 
-template <typename T, bool APPEND>
-static int launch_update_tma_t(const State& st, int k, int num_sms, cudaStream_t s) {
-  const int kt = k <= 1 ? 1 : k <= 2 ? 2 : k <= 4 ? 4 : 8;
-  switch (kt) {
-    case 1: return launch_update_tma_kt<T, 1, APPEND>(st, k, num_sms, s);
-    case 2: return launch_update_tma_kt<T, 2, APPEND>(st, k, num_sms, s);
-    case 4: return launch_update_tma_kt<T, 4, APPEND>(st, k, num_sms, s);
-    default: return launch_update_tma_kt<T, 8, APPEND>(st, k, num_sms, s);
+template <typename T>
+static int launch_update_tma_t(const State& st, int k, Ctx& cx, cudaStream_t s, bool probe) {
+  switch (round_kt(k)) {
+    case 1: return launch_update_tma_kt<T, 1>(st, k, cx, s, probe);
+    case 2: return launch_update_tma_kt<T, 2>(st, k, cx, s, probe);
+    case 4: return launch_update_tma_kt<T, 4>(st, k, cx, s, probe);
+    default: return launch_update_tma_kt<T, 8>(st, k, cx, s, probe);
   }
 }
 
-int launch_det_update_tma(const State& st, int k, int num_sms, cudaStream_t s) {
-  return st.dt == LRUX_F64 ? launch_update_tma_t<double, false>(st, k, num_sms, s)
-                           : launch_update_tma_t<cplx, false>(st, k, num_sms, s);
-}
-
-// true when a rank-k immediate update of this shape has a TMA-staged instance
-bool launch_det_update_tma_ok(const State& st, int k) {
-  return launch_det_update_tma(st, k, 0, nullptr) == 1;
-}
-
-// delayed append through the same pass (after det_prep_kernel): 2 launches, 0 = not eligible
-int launch_det_append_tma(const State& st, int k, int num_sms, cudaStream_t s) {
-  return st.dt == LRUX_F64 ? launch_update_tma_t<double, true>(st, k, num_sms, s)
-                           : launch_update_tma_t<cplx, true>(st, k, num_sms, s);
+int launch_det_update_tma(const State& st, int k, Ctx& cx, cudaStream_t s, bool probe) {
+  return st.dt == LRUX_F64 ? launch_update_tma_t<double>(st, k, cx, s, probe)
+                           : launch_update_tma_t<cplx>(st, k, cx, s, probe);
 }
 
 }  // namespace lrux

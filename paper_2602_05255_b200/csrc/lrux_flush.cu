@@ -181,24 +181,24 @@ __global__ void __launch_bounds__(256) flush_dmma_kernel(State st, int t1) {
 }
 
 template <typename T, bool SKEW>
-static int launch_flush_t(const State& st, int num_sms, cudaStream_t s) {
+static int launch_flush_t(const State& st, Ctx& cx, cudaStream_t s) {
   const int t1 = (st.n + 63) / 64;
   const int64_t tiles = SKEW ? (int64_t)t1 * (t1 + 1) / 2 : (int64_t)t1 * t1;
-  int occ = 1;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, flush_dmma_kernel<T, SKEW>, 256, 0);
-  if (occ < 1) occ = 1;
-  int64_t grid = (int64_t)num_sms * occ;
+  const int occ = cx.configure((const void*)flush_dmma_kernel<T, SKEW>, 256, 0);
+  if (occ < 0) return -1;
+  cx.name(LRUX_PROF_FLUSH, "flush_dmma_kernel");
+  int64_t grid = (int64_t)cx.num_sms * occ;
   if (grid > st.W * tiles) grid = st.W * tiles;
   flush_dmma_kernel<T, SKEW><<<(unsigned)grid, 256, 0, s>>>(st, t1);
   return 1;
 }
 
-int launch_flush_dmma(const State& st, int num_sms, cudaStream_t s) {
+int launch_flush_dmma(const State& st, Ctx& cx, cudaStream_t s) {
   if (st.kind == KIND_PF)
-    return st.dt == LRUX_F64 ? launch_flush_t<double, true>(st, num_sms, s)
-                             : launch_flush_t<cplx, true>(st, num_sms, s);
-  return st.dt == LRUX_F64 ? launch_flush_t<double, false>(st, num_sms, s)
-                           : launch_flush_t<cplx, false>(st, num_sms, s);
+    return st.dt == LRUX_F64 ? launch_flush_t<double, true>(st, cx, s)
+                             : launch_flush_t<cplx, true>(st, cx, s);
+  return st.dt == LRUX_F64 ? launch_flush_t<double, false>(st, cx, s)
+                           : launch_flush_t<cplx, false>(st, cx, s);
 }
 
 }  // namespace lrux

@@ -272,7 +272,7 @@ __global__ void info_clear_singular_kernel(int32_t* __restrict__ info, int64_t W
 }
 
 template <typename T>
-static int init_impl(const State& st, const void* d_A0, int num_sms, cudaStream_t s, bool refresh = false) {
+static int init_impl(const State& st, const void* d_A0, Ctx& cx, cudaStream_t s, bool refresh = false) {
   const int n = st.n;
   const size_t W = (size_t)st.W;
   int nl = 0;
@@ -288,11 +288,11 @@ static int init_impl(const State& st, const void* d_A0, int num_sms, cudaStream_
   if (st.pend_cnt) cudaMemsetAsync(st.pend_cnt, 0, W * 4, s);
   const size_t smem_gj = 2 * (size_t)n * sizeof(T) + (size_t)n * 4;
   const size_t smem_pr = 2 * (size_t)n * sizeof(T);
-  if (cudaFuncSetAttribute(gj_inverse_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)smem_gj) != cudaSuccess) return -1;
+  const bool blocked = n >= kBlockedInitMin;   // the unblocked kernels are configured only where they run
+  if (!blocked && cx.configure((const void*)gj_inverse_kernel<T>, 256, smem_gj) < 0) return -1;
   if (st.kind == KIND_DET) {
     launch_copy<T>(d_A0, st.Ti, st.W, n, /*transpose=*/true, /*skew=*/false, s); ++nl;
-    const int rb = n >= kBlockedInitMin ? launch_gj_blocked(st, true, num_sms, s) : 0;
+    const int rb = blocked ? launch_gj_blocked(st, true, cx, s) : 0;
     if (rb < 0) return -1;
     if (rb > 0) nl += rb;
     else {
@@ -300,13 +300,12 @@ static int init_impl(const State& st, const void* d_A0, int num_sms, cudaStream_
                                                              st.info, true); ++nl;
     }
   } else {
-    if (cudaFuncSetAttribute(parlett_reid_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)smem_pr) != cudaSuccess) return -1;
+    if (cx.configure((const void*)parlett_reid_kernel<T>, 256, smem_pr) < 0) return -1;
     launch_copy<T>(d_A0, st.Ti, st.W, n, false, /*skew=*/true, s); ++nl;
     parlett_reid_kernel<T><<<(unsigned)W, 256, smem_pr, s>>>((T*)st.Ti, n, (T*)st.phase, st.logabs,
                                                              st.info); ++nl;
     launch_copy<T>(d_A0, st.Ti, st.W, n, false, true, s); ++nl;
-    const int rb = n >= kBlockedInitMin ? launch_gj_blocked(st, false, num_sms, s) : 0;
+    const int rb = blocked ? launch_gj_blocked(st, false, cx, s) : 0;
     if (rb < 0) return -1;
     if (rb > 0) nl += rb;
     else {
@@ -319,18 +318,16 @@ static int init_impl(const State& st, const void* d_A0, int num_sms, cudaStream_
   return cudaGetLastError() == cudaSuccess ? nl : -1;
 }
 
-int launch_det_init(const State& st, const void* d_A0, int num_sms, cudaStream_t s) {
-  return st.dt == LRUX_F64 ? init_impl<double>(st, d_A0, num_sms, s)
-                           : init_impl<cplx>(st, d_A0, num_sms, s);
+int launch_det_init(const State& st, const void* d_A0, Ctx& cx, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? init_impl<double>(st, d_A0, cx, s) : init_impl<cplx>(st, d_A0, cx, s);
 }
-int launch_pf_init(const State& st, const void* d_A0, int num_sms, cudaStream_t s) {
-  return st.dt == LRUX_F64 ? init_impl<double>(st, d_A0, num_sms, s)
-                           : init_impl<cplx>(st, d_A0, num_sms, s);
+int launch_pf_init(const State& st, const void* d_A0, Ctx& cx, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? init_impl<double>(st, d_A0, cx, s) : init_impl<cplx>(st, d_A0, cx, s);
 }
 
-int launch_refresh(const State& st, const void* d_A, int num_sms, cudaStream_t s) {
-  return st.dt == LRUX_F64 ? init_impl<double>(st, d_A, num_sms, s, true)
-                           : init_impl<cplx>(st, d_A, num_sms, s, true);
+int launch_refresh(const State& st, const void* d_A, Ctx& cx, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? init_impl<double>(st, d_A, cx, s, true)
+                           : init_impl<cplx>(st, d_A, cx, s, true);
 }
 
 int launch_get_amplitude(const State& st, void* d_phase, double* d_logabs, cudaStream_t s) {

@@ -195,7 +195,7 @@ __global__ void clear_fill_kernel(State st) {
 }
 
 template <typename T>
-static int gj_blocked_t(const State& st, bool write_amp, int num_sms, cudaStream_t s) {
+static int gj_blocked_t(const State& st, bool write_amp, Ctx& cx, cudaStream_t s) {
   const int n = st.n;
   State st2 = st;          // the flush kernel sees the init scratch as a 32-deep delay buffer
   st2.Abuf = st.init_A;
@@ -208,13 +208,10 @@ static int gj_blocked_t(const State& st, bool write_amp, int num_sms, cudaStream
     gj_panel_kernel<T><<<(unsigned)st.W, 256, 0, s>>>((T*)st.Ti, n, c0, st.init_piv, (T*)st.phase,
                                                       st.logabs, st.info, write_amp ? 1 : 0);
     gj_block_apply_kernel<T><<<gcol, 256, 0, s>>>(st2, c0);
-    nl += 2 + launch_flush_dmma(st2, num_sms, s);
+    nl += 2 + launch_flush_dmma(st2, cx, s);
   }
   const size_t sm = (size_t)n * (sizeof(T) + 4);
-  if (sm > 48 * 1024 &&
-      cudaFuncSetAttribute(gj_unpermute_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)sm) != cudaSuccess)
-    return -1;
+  if (cx.configure((const void*)gj_unpermute_kernel<T>, 256, sm) < 0) return -1;
   gj_unpermute_kernel<T><<<dim3((unsigned)st.W, 8), 256, sm, s>>>(st2);
   clear_fill_kernel<<<(unsigned)((st.W + 255) / 256), 256, 0, s>>>(st2);
   nl += 2;
@@ -222,10 +219,13 @@ static int gj_blocked_t(const State& st, bool write_amp, int num_sms, cudaStream
 }
 
 // In-place inverse of st.Ti (already loaded) for n >= kBlockedInitMin; 0 = not applicable.
-int launch_gj_blocked(const State& st, bool write_amp, int num_sms, cudaStream_t s) {
+int launch_gj_blocked(const State& st, bool write_amp, Ctx& cx, cudaStream_t s) {
   if (!st.init_A || !st.init_B || !st.init_piv) return 0;
-  return st.dt == LRUX_F64 ? gj_blocked_t<double>(st, write_amp, num_sms, s)
-                           : gj_blocked_t<cplx>(st, write_amp, num_sms, s);
+  const char* keep = cx.last[LRUX_PROF_FLUSH];   // the trailing updates borrow the flush kernel
+  const int r = st.dt == LRUX_F64 ? gj_blocked_t<double>(st, write_amp, cx, s)
+                                  : gj_blocked_t<cplx>(st, write_amp, cx, s);
+  cx.last[LRUX_PROF_FLUSH] = keep;
+  return r;
 }
 
 }  // namespace lrux

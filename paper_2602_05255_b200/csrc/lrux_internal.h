@@ -14,6 +14,7 @@ enum Kind { KIND_DET = 0, KIND_PF = 1 };
 constexpr int kRatioSlice = 256;       // columns of A^-1[:,P] handled by one CTA of the det ratio
 constexpr int kRatioSplitMax = 64;     // => n <= 16384
 constexpr int kBlockedInitMin = 768;   // blocked (panel + DMMA) initialisation from this n on
+constexpr size_t kRatioCoefSmemMax = 160 * 1024;   // det delayed ratio: K*kmax*KT coefficients staged per CTA
 
 // Views into the caller-owned d_state buffer (all device pointers, 256 B aligned).
 // Element type is double (LRUX_F64) or interleaved complex (LRUX_C128); sizes
@@ -75,14 +76,34 @@ struct ProfScope {
   }
 };
 
+// Per-handle launch context (host only): what a launcher needs besides the state views.
+// Kernel attributes and occupancy are queried ONCE per (kernel, block size, shared memory)
+// and cached here, so that the per-step calls enqueue launches and do nothing else on
+// the host; `last[cls]` names the kernel most recently enqueued for each class
+// (lrux_kernel_name: kernels are selected by shape only, this is how tests and bench.py
+// learn which one a shape takes).
+struct Ctx {
+  int num_sms = 0;
+  int smem_optin = 0;                     // cudaDevAttrMaxSharedMemoryPerBlockOptin
+  Prof prof;
+  const char* last[LRUX_PROF_NCLASS] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  struct Cfg { const void* fn; int threads; size_t smem; int cluster; int occ; };
+  std::vector<Cfg> cfgs;
+  // Resident CTAs per SM of `fn` at this block size / dynamic shared memory (>= 1), or
+  // -1 on a CUDA error.  Opts the kernel into large dynamic shared memory when needed.
+  int configure(const void* fn, int threads, size_t smem);
+  // Co-resident clusters of `cluster` CTAs on the whole GPU (0: not launchable), cached.
+  int configure_cluster(const void* fn, int threads, size_t smem, int cluster);
+  void name(int cls, const char* kernel) { last[cls] = kernel; }
+};
+
 }  // namespace lrux
 
 struct lrux_handle_s {
   lrux::State st;
-  lrux::Prof prof;
+  lrux::Ctx cx;
   int32_t pending_k;  // 0 = nothing pending
   int64_t launches;
-  int32_t num_sms;
 };
 
 namespace lrux {
@@ -90,29 +111,32 @@ namespace lrux {
 size_t state_layout(State* st, void* base, int64_t W, int32_t n, int32_t kmax, int32_t K,
                     int32_t dt, int32_t kind);
 
+static inline int persistent_grid(int num_sms, int ctas_per_sm, int64_t max_items) {
+  int64_t g = (int64_t)num_sms * ctas_per_sm;
+  if (g > max_items) g = max_items;
+  return g < 1 ? 1 : (int)g;
+}
+static inline int round_kt(int k) { return k <= 1 ? 1 : k <= 2 ? 2 : k <= 4 ? 4 : 8; }
+
 // launchers (each returns the number of kernels it enqueued, or -1 on a CUDA error)
-int launch_det_init(const State& st, const void* d_A0, int num_sms, cudaStream_t s);
-int launch_pf_init(const State& st, const void* d_A0, int num_sms, cudaStream_t s);
-int launch_refresh(const State& st, const void* d_A, int num_sms, cudaStream_t s);
+int launch_det_init(const State& st, const void* d_A0, Ctx& cx, cudaStream_t s);
+int launch_pf_init(const State& st, const void* d_A0, Ctx& cx, cudaStream_t s);
+int launch_refresh(const State& st, const void* d_A, Ctx& cx, cudaStream_t s);
 // blocked in-place inverse of st.Ti (lrux_init_blocked.cu); 0 = not applicable
-int launch_gj_blocked(const State& st, bool write_amp, int num_sms, cudaStream_t s);
+int launch_gj_blocked(const State& st, bool write_amp, Ctx& cx, cudaStream_t s);
 int launch_det_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
-                     void* d_ratio, cudaStream_t s, Prof* prof);
-int launch_det_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s,
-                      Prof* prof);
-int launch_det_flush(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof);
+                     void* d_ratio, Ctx& cx, cudaStream_t s);
+int launch_det_accept(const State& st, int k, const uint8_t* d_mask, Ctx& cx, cudaStream_t s);
+int launch_det_flush(const State& st, bool all, Ctx& cx, cudaStream_t s);
 int launch_pf_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
-                    void* d_ratio, int num_sms, cudaStream_t s, Prof* prof);
-int launch_pf_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s,
-                     Prof* prof);
-int launch_pf_flush(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof);
+                    void* d_ratio, Ctx& cx, cudaStream_t s);
+int launch_pf_accept(const State& st, int k, const uint8_t* d_mask, Ctx& cx, cudaStream_t s);
+int launch_pf_flush(const State& st, bool all, Ctx& cx, cudaStream_t s);
 // TMA-staged immediate det update for large rows (lrux_det_tma.cu): 1 = launched,
-// 0 = shape not eligible, -1 = CUDA error
-int launch_det_update_tma(const State& st, int k, int num_sms, cudaStream_t s);
-int launch_det_append_tma(const State& st, int k, int num_sms, cudaStream_t s);
-bool launch_det_update_tma_ok(const State& st, int k);
+// 0 = shape not eligible, -1 = CUDA error.  probe = true: eligibility only, nothing launched.
+int launch_det_update_tma(const State& st, int k, Ctx& cx, cudaStream_t s, bool probe = false);
 // DMMA flush of the delay buffers, det and pf (lrux_flush.cu)
-int launch_flush_dmma(const State& st, int num_sms, cudaStream_t s);
+int launch_flush_dmma(const State& st, Ctx& cx, cudaStream_t s);
 // shared between det and pf (defined in lrux_det.cu)
 int launch_select(const State& st, const uint8_t* mask, cudaStream_t s);
 int launch_post(const State& st, int ncols, cudaStream_t s);

@@ -15,8 +15,7 @@
 #include "lrux_internal.h"
 #include "lrux_tma.cuh"
 #include <cooperative_groups.h>
-#include <cstdlib>
-#include <cstring>
+#include <algorithm>
 
 namespace lrux {
 
@@ -628,117 +627,6 @@ __device__ __forceinline__ void pf_row_update(T* row, int r, int n, int m, const
       row[cc] = (r == cc) ? S::zero() : (up ? v : S::neg(v));
     }
   }
-}
-
-// ---------------------------------------------------------------- resident update (a4)
-// Small walkers (n^2 e <= ~190 KB: n <= 152 fp64, config C3's n = 128): the whole inverse
-// of an accepted walker is brought into shared memory by ONE bulk asynchronous copy
-// (TMA), Y = A^-1 N (k = 1; for k >= 2 the ratio already left it in pend_Y), g = Y' R'^-1
-// and the rank-2k update are done on chip, and the matrix goes back with one bulk
-// store: HBM traffic = read n^2 e + write n^2 e, the compulsory minimum (SURVEY.md
-// §7 H3).  Every element is updated by its own thread with no transposed access:
-// for r > c the thread recomputes the upper value v(c,r) from -Ti[r][c] (the matrix
-// is exactly skew on entry) with the same operands in the same order and stores -v,
-// so the result is exactly skew again.
-template <typename T>
-__global__ void __launch_bounds__(512) pf_resident_update_kernel(State st, int k, int need_y) {
-  using S = Sc<T>;
-  constexpr int NCH = 4;                // row chunks per walker, one bulk copy + mbarrier each
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  const int n = st.n, kmax = st.kmax, m = 2 * k;
-  T* Ts = (T*)smem_raw;                 // [n][n]
-  T* yv = Ts + (size_t)n * n;           // [m][n]  Y'
-  T* gv = yv + (size_t)m * n;           // [m][n]  Y' R'^-1
-  T* nv = gv + (size_t)m * n;           // [n]     new row (k = 1)
-  __shared__ T Ri[kMaxC * kMaxC];
-  __shared__ int P[kMaxK];
-  __shared__ __align__(8) uint64_t bar[NCH];
-  const int tid = threadIdx.x, nt = blockDim.x, warp = tid >> 5, lane = tid & 31, nw = nt >> 5;
-  const int count = st.counters[0];
-  const int rpc = (n + NCH - 1) / NCH;  // rows per chunk
-  if (tid == 0) {
-    for (int c = 0; c < NCH; ++c) tma::mbar_init(&bar[c], 1);
-    tma::fence_barrier_init();
-  }
-  __syncthreads();
-  auto load_chunk = [&](int w, int c) {   // thread 0 only
-    const int r0 = c * rpc, rows = min(rpc, n - r0);
-    if (rows <= 0) return;
-    const uint32_t bytes = (uint32_t)((size_t)rows * n * sizeof(T));
-    tma::mbar_arrive_expect_tx(&bar[c], bytes);
-    tma::load(Ts + (size_t)r0 * n, (const T*)st.Ti + (size_t)w * n * n + (size_t)r0 * n, bytes, &bar[c]);
-  };
-  if (tid == 0 && (int)blockIdx.x < count)
-    for (int c = 0; c < NCH; ++c) load_chunk(st.list[blockIdx.x], c);
-  uint32_t phase = 0;
-  for (int it = blockIdx.x; it < count; it += gridDim.x) {
-    const int w = st.list[it];
-    const int w_next = it + (int)gridDim.x < count ? st.list[it + gridDim.x] : -1;
-    T* Tw = (T*)st.Ti + (size_t)w * n * n;
-    const T* pC = (const T*)st.pend_C + (size_t)w * kmax * n;
-    const T* pY = (const T*)st.pend_Y + (size_t)w * kmax * n;
-    const T* pN = (const T*)st.pend_N + (size_t)w * kmax * n;
-    for (int q = tid; q < m * m; q += nt)
-      Ri[(q / m) * kMaxC + (q % m)] =
-          ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + (q / m) * st.kc + (q % m)];
-    if (tid < k) P[tid] = st.pend_idx[(size_t)w * kmax + tid];
-    __syncthreads();
-    for (int q = tid; q < k * n; q += nt) {
-      const int a = q / n, i = q % n;
-      yv[(size_t)(k + a) * n + i] = pC[q];
-      if (need_y) nv[q] = pN[q];   // k == 1
-      else yv[q] = (i == P[a]) ? S::add(pY[q], S::one()) : pY[q];
-    }
-    __syncthreads();
-    // ---- Y = A^-1 N row by row, chunk by chunk as the bulk copies land (k = 1)
-    for (int c = 0; c < NCH; ++c) {
-      const int r0 = c * rpc, r1 = min(n, r0 + rpc);
-      if (r0 >= n) break;
-      tma::mbar_wait(&bar[c], phase);
-      if (need_y) {
-        for (int i = r0 + warp; i < r1; i += nw) {
-          T acc = S::zero();
-          for (int j = lane; j < n; j += 32) acc = S::fma(Ts[(size_t)i * n + j], nv[j], acc);
-          acc = warp_sum(acc);
-          if (lane == 0) yv[i] = (i == P[0]) ? S::add(acc, S::one()) : acc;
-        }
-      }
-    }
-    phase ^= 1;
-    __syncthreads();
-    for (int q = tid; q < m * n; q += nt) {
-      const int beta = q / n, i = q % n;
-      T g = S::zero();
-      for (int alpha = 0; alpha < m; ++alpha)
-        g = S::fma(yv[(size_t)alpha * n + i], Ri[alpha * kMaxC + beta], g);
-      gv[q] = g;
-    }
-    __syncthreads();
-    // ---- rank-2k update chunk by chunk; each finished chunk is stored at once and its
-    // shared memory refilled with the same chunk of this CTA's next walker
-    for (int c = 0; c < NCH; ++c) {
-      const int r0 = c * rpc, r1 = min(n, r0 + rpc);
-      if (r0 >= n) break;
-      for (int r = r0 + warp; r < r1; r += nw) {
-        pf_row_update<T>(Ts + (size_t)r * n, r, n, m, yv, gv, lane);
-      }
-      tma::fence_proxy_async();
-      __syncthreads();
-      if (tid == 0) {
-        tma::store(Tw + (size_t)r0 * n, Ts + (size_t)r0 * n, (uint32_t)((size_t)(r1 - r0) * n * sizeof(T)));
-        tma::store_commit();
-        if (w_next >= 0 && c >= 1) {
-          tma::store_wait_read<1>();   // the previous chunk has left shared memory
-          load_chunk(w_next, c - 1);
-        }
-      }
-    }
-    if (tid == 0 && w_next >= 0) {
-      tma::store_wait_read<0>();
-      load_chunk(w_next, (min(n, NCH * rpc) - 1) / rpc);   // last non-empty chunk
-    }
-  }
-  if (tid == 0) tma::store_wait_all<0>();
 }
 
 // ---------------------------------------------------------------- cluster-resident update (a4)
@@ -1394,19 +1282,13 @@ __global__ void __launch_bounds__(256) pf_append_kernel(State st, int k) {
 }
 
 // ---------------------------------------------------------------- launchers
-static inline int round_kt(int k) { return k <= 1 ? 1 : k <= 2 ? 2 : k <= 4 ? 4 : 8; }
-static inline int pgrid(int num_sms, int per_sm, int64_t max_items) {
-  int64_t g = (int64_t)num_sms * per_sm;
-  if (g > max_items) g = max_items;
-  return g < 1 ? 1 : (int)g;
-}
-
+// Every choice below depends on the shape (dtype, n, k, K) only.
 template <typename T>
-static int launch_y(const State& st, int k, int use_list, int num_sms, cudaStream_t s, Prof* prof) {
-  ProfScope ps(prof, LRUX_PROF_YPASS, s);
+static int launch_y(const State& st, int k, int use_list, Ctx& cx, cudaStream_t s) {
+  ProfScope ps(&cx.prof, LRUX_PROF_YPASS, s);
   int nl = 0;
   if (st.cap) {
-    pf_an_kernel<T><<<pgrid(num_sms, 4, st.W), 256, 0, s>>>(st, k, use_list); ++nl;
+    pf_an_kernel<T><<<persistent_grid(cx.num_sms, 4, st.W), 256, 0, s>>>(st, k, use_list); ++nl;
   }
   const int kt = round_kt(k);
   {
@@ -1417,21 +1299,19 @@ static int launch_y(const State& st, int k, int use_list, int num_sms, cudaStrea
     while ((1 << lg) < nvec && lg < 8) ++lg;
     const int CW = 1 << lg, RG = 256 >> lg, cblocks = (nvec + CW - 1) / CW;
     const size_t smy = (size_t)k * st.n * sizeof(T) + (RG > 1 ? (size_t)RG * kt * CW * 16 : 0);
-    const char* env = getenv("LRUX_PF_Y");   // A-B measurements only
-    if (st.n % VE == 0 && smy <= 64 * 1024 && !(env && !strcmp(env, "rows"))) {
+    if (st.n % VE == 0 && smy <= 64 * 1024) {
       auto kern = kt == 1 ? pf_y_colsum_kernel<T, 1> : kt == 2 ? pf_y_colsum_kernel<T, 2>
                 : kt == 4 ? pf_y_colsum_kernel<T, 4> : pf_y_colsum_kernel<T, 8>;
-      if (smy > 40 * 1024 &&
-          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smy) != cudaSuccess)
-        return -1;
-      kern<<<pgrid(num_sms, 8, (int64_t)st.W * cblocks), 256, smy, s>>>(st, k, cblocks, lg, use_list);
+      if (cx.configure((const void*)kern, 256, smy) < 0) return -1;
+      kern<<<persistent_grid(cx.num_sms, 8, (int64_t)st.W * cblocks), 256, smy, s>>>(st, k, cblocks, lg, use_list);
+      cx.name(LRUX_PROF_YPASS, "pf_y_colsum_kernel");
       return nl + 1;
     }
   }
   int rpt = 64;
   if (rpt > st.n) rpt = st.n;
   const int tiles = (st.n + rpt - 1) / rpt;
-  const int grid = pgrid(num_sms, 4, (int64_t)st.W * tiles);
+  const int grid = persistent_grid(cx.num_sms, 4, (int64_t)st.W * tiles);
   const size_t smem = (size_t)kt * rpt * sizeof(T);
   switch (kt) {
     case 1: pf_y_kernel<T, 1><<<grid, 256, smem, s>>>(st, k, tiles, rpt, use_list); break;
@@ -1439,160 +1319,160 @@ static int launch_y(const State& st, int k, int use_list, int num_sms, cudaStrea
     case 4: pf_y_kernel<T, 4><<<grid, 256, smem, s>>>(st, k, tiles, rpt, use_list); break;
     default: pf_y_kernel<T, 8><<<grid, 256, smem, s>>>(st, k, tiles, rpt, use_list); break;
   }
+  cx.name(LRUX_PROF_YPASS, "pf_y_kernel");
   return nl + 1;
 }
 
 template <typename T>
 static int pf_ratio_impl(const State& st, int k, const int32_t* idx, const void* rows, void* ratio,
-                         int num_sms, cudaStream_t s, Prof* prof) {
+                         Ctx& cx, cudaStream_t s) {
   int nl = 0;
   {
-    ProfScope ps(prof, LRUX_PROF_RATIO, s);
+    ProfScope ps(&cx.prof, LRUX_PROF_RATIO, s);
     pf_gather_kernel<T><<<(unsigned)st.W, 128, 0, s>>>(st, k, idx, (const T*)rows, (T*)ratio); ++nl;
+    cx.name(LRUX_PROF_RATIO, "pf_gather_kernel");
   }
   if (k > 1) {
-    nl += launch_y<T>(st, k, 0, num_sms, s, prof);
-    ProfScope ps(prof, LRUX_PROF_RATIO, s);
+    const int r = launch_y<T>(st, k, 0, cx, s);
+    if (r < 0) return -1;
+    nl += r;
+    ProfScope ps(&cx.prof, LRUX_PROF_RATIO, s);
     pf_core_kernel<T><<<(unsigned)st.W, 128, 0, s>>>(st, k, (T*)ratio); ++nl;
+    cx.name(LRUX_PROF_RATIO, "pf_gather_kernel+pf_core_kernel");
   }
   return cudaGetLastError() == cudaSuccess ? nl : -1;
 }
 
 template <typename T>
-static int pf_flush_impl(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof) {
+static int pf_flush_impl(const State& st, bool all, Ctx& cx, cudaStream_t s) {
   int nl = 0;
   if (all) nl += launch_flush_select_all(st, s);
   {
-    ProfScope ps(prof, LRUX_PROF_FLUSH, s);
-    nl += launch_flush_dmma(st, num_sms, s);   // Eq. 26 on the FP64 tensor path
+    ProfScope ps(&cx.prof, LRUX_PROF_FLUSH, s);
+    const int r = launch_flush_dmma(st, cx, s);   // Eq. 26 on the FP64 tensor path
+    if (r < 0) return -1;
+    nl += r;
   }
   nl += launch_flush_clear(st, s);
   return cudaGetLastError() == cudaSuccess ? nl : -1;
 }
 
+// Immediate update (K = 0) with the walker resident on chip.  Returns the number of
+// launches, 0 when no resident kernel fits this shape, -1 on a CUDA error.
 template <typename T>
-static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_sms, cudaStream_t s,
-                          Prof* prof) {
-  int nl = launch_select(st, mask, s);
-  {
-    // whole-walker residency on chip when the inverse fits in shared memory
-    const int n = st.n;
-    // cluster-resident: CL CTAs share a walker; taken when a slab leaves room for >= 2 CTAs per SM
-    if (st.K == 0) {
-      const char* env = getenv("LRUX_PF_PATH");   // A-B measurements only
-      const bool force_cta = env && !strcmp(env, "cta");
-      // fp64 k = 1 with the whole inverse in one CTA's shared memory: column-pair kernel, 1024 threads
-      if (sizeof(T) == 8 && k == 1 && !force_cta && !(env && !strncmp(env, "cluster", 7))) {
-        if ((n == 128 || n == 64) && !(env && !strncmp(env, "smem", 4)) && !(env && !strcmp(env, "nb5"))) {
-          // the walker's inverse in registers between the column sums and the update
-          const size_t smr = (size_t)n * n * 8 + (size_t)20 * (n / 2) * 16 + (size_t)n * 32 + (size_t)2 * (2 * n + 6) * 8;
-          auto kern = n == 128 ? pf_regs_k1_kernel<128> : pf_regs_k1_kernel<64>;
-          if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smr) != cudaSuccess)
-            return -1;
-          ProfScope ps(prof, LRUX_PROF_UPDATE, s);
-          kern<<<pgrid(num_sms, 1, st.W), 512, smr, s>>>(st); ++nl;
-          return cudaGetLastError() == cudaSuccess ? nl : -1;
-        }
-        int lg1 = 5;
-        while ((1 << lg1) < n / 2) ++lg1;
-        const int rg1 = 1024 >> lg1;
-        const size_t smx = (size_t)(rg1 + rg1 / 4) * (n / 2) * 16 + (size_t)n * 32 + (size_t)2 * (2 * n + 6) * 8;
-        const size_t chunk = (size_t)((n + 3) / 4) * n * 8;
-        const bool nb5 = env && !strcmp(env, "nb5");
-        const int nb = (!nb5 && 6 * chunk + smx <= 226 * 1024) ? 6 : 5;   // two spare chunk buffers when they fit
-        const size_t sm1 = nb * chunk + smx;
-        if (lg1 <= 7 && sm1 <= 226 * 1024) {
-          const bool c3 = (2 << lg1) == n && lg1 == 6;
-          auto kern = c3 ? (nb == 6 ? pf_resident_k1_kernel<6, 6> : pf_resident_k1_kernel<6, 5>)
-                         : (nb == 6 ? pf_resident_k1_kernel<0, 6> : pf_resident_k1_kernel<0, 5>);
-          if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm1) != cudaSuccess)
-            return -1;
-          ProfScope ps(prof, LRUX_PROF_UPDATE, s);
-          kern<<<pgrid(num_sms, 1, st.W), 1024, sm1, s>>>(st, lg1); ++nl;
-          return cudaGetLastError() == cudaSuccess ? nl : -1;
-        }
-      }
-      // fp64 k = 1: the column-pair kernel (n/2 <= 256 threads' worth of column pairs)
-      const bool k1 = sizeof(T) == 8 && k == 1 && n <= 512 && !(env && !strcmp(env, "cluster_generic"));
-      int lg = 5;
-      while ((1 << lg) < n / 2) ++lg;
-      for (int CL = 4; CL <= 8 && !force_cta; CL *= 2) {
-        const int rpc = (n + CL - 1) / CL;
-        const size_t smc = k1 ? (size_t)rpc * n * 8 + (size_t)((256 >> lg) + 2 * CL) * (n / 2) * 16 + (size_t)n * 40
-                              : ((size_t)rpc * n + (size_t)(6 * k + 1) * n) * sizeof(T);
-        if (smc > (CL == 4 ? 56 : 111) * 1024) continue;
-        // unrolled instance when n/2 is a power of two and the slab splits evenly over the row groups
-        const bool even = k1 && (2 << lg) == n && n % CL == 0 && rpc % (256 >> lg) == 0;
-        const int rpt = even ? rpc / (256 >> lg) : 0;
-        const void* kern = !k1 ? (const void*)pf_cluster_update_kernel<T>
-                         : (lg == 6 && rpt == 8) ? (const void*)pf_cluster_k1_kernel<6, 8>
-                         : (lg == 7 && rpt == 16) ? (const void*)pf_cluster_k1_kernel<7, 16>
-                         : (lg == 5 && rpt == 2) ? (const void*)pf_cluster_k1_kernel<5, 2>
-                         : (const void*)pf_cluster_k1_kernel<0, 0>;
-        if (smc > 40 * 1024 &&
-            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smc) != cudaSuccess)
-          return -1;
-        cudaLaunchConfig_t cfg = {};
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = CL;
-        attr[0].val.clusterDim.y = 1;
-        attr[0].val.clusterDim.z = 1;
-        cfg.blockDim = dim3(256);
-        cfg.dynamicSmemBytes = smc;
-        cfg.stream = s;
-        cfg.attrs = attr;
-        cfg.numAttrs = 1;
-        cfg.gridDim = dim3(CL);
-        int ncl = 0;   // co-resident clusters on the whole GPU
-        if (cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg) != cudaSuccess || ncl < 1) { cudaGetLastError(); break; }
-        cfg.gridDim = dim3((unsigned)(CL * (int)std::min<int64_t>(st.W, ncl)));
-        ProfScope ps(prof, LRUX_PROF_UPDATE, s);
-        State stc = st;
-        int a1 = k1 ? lg : k, a2 = k == 1 ? 1 : 0;
-        void* args3[3] = {&stc, &a1, &a2};
-        if (cudaLaunchKernelExC(&cfg, kern, args3) != cudaSuccess) return -1;
-        ++nl;
-        return cudaGetLastError() == cudaSuccess ? nl : -1;
-      }
+static int launch_pf_resident(const State& st, int k, Ctx& cx, cudaStream_t s) {
+  const int n = st.n;
+  if (sizeof(T) == 8 && k == 1) {
+    if (n == 128 || n == 64) {
+      // the walker's inverse in registers between the column sums and the update
+      const size_t smr = (size_t)n * n * 8 + (size_t)20 * (n / 2) * 16 + (size_t)n * 32 + (size_t)2 * (2 * n + 6) * 8;
+      auto kern = n == 128 ? pf_regs_k1_kernel<128> : pf_regs_k1_kernel<64>;
+      if (cx.configure((const void*)kern, 512, smr) < 0) return -1;
+      ProfScope ps(&cx.prof, LRUX_PROF_UPDATE, s);
+      kern<<<persistent_grid(cx.num_sms, 1, st.W), 512, smr, s>>>(st);
+      cx.name(LRUX_PROF_UPDATE, "pf_regs_k1_kernel");
+      return 1;
     }
-    const size_t sm = ((size_t)n * n + (size_t)(4 * k + 1) * n) * sizeof(T);
-    if (st.K == 0 && sm <= 200 * 1024) {
-      auto kern = pf_resident_update_kernel<T>;
-      if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess)
-        return -1;
-      ProfScope ps(prof, LRUX_PROF_UPDATE, s);
-      kern<<<pgrid(num_sms, 1, st.W), 512, sm, s>>>(st, k, k == 1 ? 1 : 0); ++nl;
-      return cudaGetLastError() == cudaSuccess ? nl : -1;
+    // the whole inverse in one CTA's shared memory: column-pair kernel, 1024 threads
+    int lg1 = 5;
+    while ((1 << lg1) < n / 2) ++lg1;
+    const int rg1 = 1024 >> lg1;
+    const size_t smx = (size_t)(rg1 + rg1 / 4) * (n / 2) * 16 + (size_t)n * 32 + (size_t)2 * (2 * n + 6) * 8;
+    const size_t chunk = (size_t)((n + 3) / 4) * n * 8;
+    const int nb = (6 * chunk + smx <= 226 * 1024) ? 6 : 5;   // two spare chunk buffers when they fit
+    const size_t sm1 = nb * chunk + smx;
+    if (lg1 <= 7 && sm1 <= 226 * 1024) {
+      const bool c3 = (2 << lg1) == n && lg1 == 6;
+      auto kern = c3 ? (nb == 6 ? pf_resident_k1_kernel<6, 6> : pf_resident_k1_kernel<6, 5>)
+                     : (nb == 6 ? pf_resident_k1_kernel<0, 6> : pf_resident_k1_kernel<0, 5>);
+      if (cx.configure((const void*)kern, 1024, sm1) < 0) return -1;
+      ProfScope ps(&cx.prof, LRUX_PROF_UPDATE, s);
+      kern<<<persistent_grid(cx.num_sms, 1, st.W), 1024, sm1, s>>>(st, lg1);
+      cx.name(LRUX_PROF_UPDATE, "pf_resident_k1_kernel");
+      return 1;
     }
   }
-  if (k == 1) nl += launch_y<T>(st, k, 1, num_sms, s, prof);  // Y only for accepted walkers
+  // cluster-resident: CL CTAs share a walker; taken when a slab leaves room for >= 2 CTAs per SM.
+  // fp64 k = 1: the column-pair kernel (n/2 <= 256 threads' worth of column pairs)
+  const bool k1 = sizeof(T) == 8 && k == 1 && n <= 512;
+  int lg = 5;
+  while ((1 << lg) < n / 2) ++lg;
+  for (int CL = 4; CL <= 8; CL *= 2) {
+    const int rpc = (n + CL - 1) / CL;
+    const size_t smc = k1 ? (size_t)rpc * n * 8 + (size_t)((256 >> lg) + 2 * CL) * (n / 2) * 16 + (size_t)n * 40
+                          : ((size_t)rpc * n + (size_t)(6 * k + 1) * n) * sizeof(T);
+    if (smc > (size_t)(CL == 4 ? 56 : 111) * 1024) continue;
+    // unrolled instance when n/2 is a power of two and the slab splits evenly over the row groups
+    const bool even = k1 && (2 << lg) == n && n % CL == 0 && rpc % (256 >> lg) == 0;
+    const int rpt = even ? rpc / (256 >> lg) : 0;
+    const void* kern = !k1 ? (const void*)pf_cluster_update_kernel<T>
+                     : (lg == 6 && rpt == 8) ? (const void*)pf_cluster_k1_kernel<6, 8>
+                     : (lg == 7 && rpt == 16) ? (const void*)pf_cluster_k1_kernel<7, 16>
+                     : (lg == 5 && rpt == 2) ? (const void*)pf_cluster_k1_kernel<5, 2>
+                     : (const void*)pf_cluster_k1_kernel<0, 0>;
+    const int ncl = cx.configure_cluster(kern, 256, smc, CL);   // co-resident clusters on the whole GPU
+    if (ncl < 1) return 0;
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CL;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.blockDim = dim3(256);
+    cfg.dynamicSmemBytes = smc;
+    cfg.stream = s;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cfg.gridDim = dim3((unsigned)(CL * (int)std::min<int64_t>(st.W, ncl)));
+    ProfScope ps(&cx.prof, LRUX_PROF_UPDATE, s);
+    State stc = st;
+    int a1 = k1 ? lg : k, a2 = k == 1 ? 1 : 0;
+    void* args3[3] = {&stc, &a1, &a2};
+    if (cudaLaunchKernelExC(&cfg, kern, args3) != cudaSuccess) return -1;
+    cx.name(LRUX_PROF_UPDATE, k1 ? "pf_cluster_k1_kernel" : "pf_cluster_update_kernel");
+    return 1;
+  }
+  return 0;
+}
+
+template <typename T>
+static int pf_accept_impl(const State& st, int k, const uint8_t* mask, Ctx& cx, cudaStream_t s) {
+  int nl = launch_select(st, mask, s);
   if (st.K == 0) {
-    ProfScope ps(prof, LRUX_PROF_UPDATE, s);
+    const int r = launch_pf_resident<T>(st, k, cx, s);
+    if (r < 0) return -1;
+    if (r > 0) return cudaGetLastError() == cudaSuccess ? nl + r : -1;
+  }
+  if (k == 1) {   // Y only for accepted walkers
+    const int r = launch_y<T>(st, k, 1, cx, s);
+    if (r < 0) return -1;
+    nl += r;
+  }
+  if (st.K == 0) {
+    ProfScope ps(&cx.prof, LRUX_PROF_UPDATE, s);
     const size_t sm = 4 * (size_t)k * st.n * sizeof(T);   // Y' and g
     if (sm <= 160 * 1024) {
       auto kern = k <= 1 ? pf_update_stream_kernel<T, 2> : k <= 2 ? pf_update_stream_kernel<T, 4>
                 : k <= 4 ? pf_update_stream_kernel<T, 8> : pf_update_stream_kernel<T, 16>;
-      if (sm > 40 * 1024 &&
-          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess)
-        return -1;
+      const int occ = cx.configure((const void*)kern, 256, sm);
+      if (occ < 0) return -1;
       const int rpt = 64, tiles = (st.n + rpt - 1) / rpt;
-      int occ = 1;
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 256, sm);
-      if (occ < 1) return -1;
-      kern<<<pgrid(num_sms, occ, (int64_t)st.W * tiles), 256, sm, s>>>(st, k, tiles, rpt); ++nl;
+      kern<<<persistent_grid(cx.num_sms, occ, (int64_t)st.W * tiles), 256, sm, s>>>(st, k, tiles, rpt); ++nl;
+      cx.name(LRUX_PROF_UPDATE, "pf_update_stream_kernel");
     } else {
       const int t1 = (st.n + 31) / 32;
-      const int grid = pgrid(num_sms, 4, (int64_t)st.W * (t1 * (t1 + 1) / 2));
+      const int grid = persistent_grid(cx.num_sms, 4, (int64_t)st.W * (t1 * (t1 + 1) / 2));
       pf_update_kernel<T><<<grid, 256, 0, s>>>(st, k, t1); ++nl;
+      cx.name(LRUX_PROF_UPDATE, "pf_update_kernel");
     }
   } else {
     {
-      ProfScope ps(prof, LRUX_PROF_APPEND, s);
-      pf_append_kernel<T><<<pgrid(num_sms, 4, st.W), 256, 0, s>>>(st, k); ++nl;
+      ProfScope ps(&cx.prof, LRUX_PROF_APPEND, s);
+      pf_append_kernel<T><<<persistent_grid(cx.num_sms, 4, st.W), 256, 0, s>>>(st, k); ++nl;
+      cx.name(LRUX_PROF_APPEND, "pf_append_kernel");
     }
     nl += launch_post(st, 2 * k, s);
-    int r = pf_flush_impl<T>(st, false, num_sms, s, prof);
+    int r = pf_flush_impl<T>(st, false, cx, s);
     if (r < 0) return -1;
     nl += r;
   }
@@ -1600,18 +1480,16 @@ static int pf_accept_impl(const State& st, int k, const uint8_t* mask, int num_s
 }
 
 int launch_pf_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows, void* d_ratio,
-                    int num_sms, cudaStream_t s, Prof* prof) {
-  return st.dt == LRUX_F64 ? pf_ratio_impl<double>(st, k, d_idx, d_rows, d_ratio, num_sms, s, prof)
-                           : pf_ratio_impl<cplx>(st, k, d_idx, d_rows, d_ratio, num_sms, s, prof);
+                    Ctx& cx, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? pf_ratio_impl<double>(st, k, d_idx, d_rows, d_ratio, cx, s)
+                           : pf_ratio_impl<cplx>(st, k, d_idx, d_rows, d_ratio, cx, s);
 }
-int launch_pf_accept(const State& st, int k, const uint8_t* d_mask, int num_sms, cudaStream_t s,
-                     Prof* prof) {
-  return st.dt == LRUX_F64 ? pf_accept_impl<double>(st, k, d_mask, num_sms, s, prof)
-                           : pf_accept_impl<cplx>(st, k, d_mask, num_sms, s, prof);
+int launch_pf_accept(const State& st, int k, const uint8_t* d_mask, Ctx& cx, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? pf_accept_impl<double>(st, k, d_mask, cx, s)
+                           : pf_accept_impl<cplx>(st, k, d_mask, cx, s);
 }
-int launch_pf_flush(const State& st, bool all, int num_sms, cudaStream_t s, Prof* prof) {
-  return st.dt == LRUX_F64 ? pf_flush_impl<double>(st, all, num_sms, s, prof)
-                           : pf_flush_impl<cplx>(st, all, num_sms, s, prof);
+int launch_pf_flush(const State& st, bool all, Ctx& cx, cudaStream_t s) {
+  return st.dt == LRUX_F64 ? pf_flush_impl<double>(st, all, cx, s) : pf_flush_impl<cplx>(st, all, cx, s);
 }
 
 }  // namespace lrux

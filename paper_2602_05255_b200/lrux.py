@@ -43,6 +43,7 @@ SIGNATURES = {
     "lrux_pf_get_inverse": [_vp, _vp, _vp],
     "lrux_get_flush_count": [_vp, _vp, _vp],
     "lrux_launch_count": [_vp, C.POINTER(_i64)],
+    "lrux_kernel_name": [_vp, _i32],
     "lrux_profile_enable": [_vp, _i32],
     "lrux_profile_read": [_vp, _i32, C.POINTER(C.c_double), C.POINTER(_i64)],
     "lrux_destroy": [_vp],
@@ -51,7 +52,7 @@ SIGNATURES = {
     "lruxh_pf_propose": [_u64, _i64, _i64, _i64, _i32, _i32, _i32, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
     "lruxh_decide": [_u64, _i64, _i64, _i64, _i32, _i32, _i32, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
 }
-_RESTYPE = {"lrux_status_string": C.c_char_p}
+_RESTYPE = {"lrux_status_string": C.c_char_p, "lrux_kernel_name": C.c_char_p}
 
 _lib = None
 
@@ -198,6 +199,10 @@ class _Walkers:
         c = _i64(0)
         _check(self._lib.lrux_launch_count(self._h, C.byref(c)))
         return c.value
+
+    def kernel_name(self, cls):
+        """Kernel most recently enqueued for class ``cls`` (PROF_*); "" when none."""
+        return self._lib.lrux_kernel_name(self._h, cls).decode()
 
     def profile_enable(self, on=True):
         _check(self._lib.lrux_profile_enable(self._h, 1 if on else 0))

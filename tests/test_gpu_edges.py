@@ -123,9 +123,12 @@ def test_pf_degenerate_and_k_equals_half_n():
 
 
 def test_delay_depth_limit_is_reported():
+    """K*kmax*kt*sizeof(elem) > 160 KiB of staged coefficients: rejected at init, not at the
+    first ratio call."""
     with pytest.raises(lrux.LruxError) as e:
-        lrux.DetWalkers(torch.eye(16, dtype=torch.complex128, device=DEV)[None], kmax=8, K=64)
+        lrux.DetWalkers(torch.eye(16, dtype=torch.complex128, device=DEV)[None], kmax=8, K=200)
     assert e.value.status == lrux.EUNSUPPORTED
+    lrux.DetWalkers(torch.eye(16, dtype=torch.complex128, device=DEV)[None], kmax=8, K=64)   # 64 KiB: fine
 
 
 @pytest.mark.parametrize("kind,dtype,K", [("det", np.float64, 0), ("det", np.complex128, 3), ("pf", np.float64, 0),

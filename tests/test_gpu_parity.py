@@ -13,17 +13,27 @@ import parity_util as pu
 pytestmark = pytest.mark.gpu
 
 
-def _run(kind, seed, W, n, M, k, K, steps, cplx=False, walkers=None, scratch_every=1):
+def _run(kind, seed, W, n, M, k, K, steps, cplx=False, walkers=None, scratch_every=1, forced=False,
+         refresh_every=0, strict=False, pure_floor=None, acc_range=(0.05, 0.8), kernel=None, kmax=None):
     orb, occ, unocc = pu.make_inputs(kind, seed, W, n, M, cplx)
-    rec = pu.run_gpu_chain(kind, orb, occ, unocc, k, K, seed, steps)
+    rec = pu.run_gpu_chain(kind, orb, occ, unocc, k, K, seed, steps, forced=forced,
+                           refresh_every=refresh_every, kmax=kmax)
     assert not rec["info"].any(), rec["info"]
     walkers = list(range(W)) if walkers is None else walkers
-    oracle = pu.run_oracle(kind, orb, occ, unocc, k, seed, steps, walkers, scratch_every)
-    stats = pu.compare(kind, rec, oracle)
+    oracle = pu.run_oracle(kind, orb, occ, unocc, k, seed, steps, walkers, scratch_every, forced=forced)
+    label = "%s %s n=%d k=%d K=%d%s%s" % (kind, "c128" if cplx else "f64", n, k, K,
+                                         " forced" if forced else "", " refresh/%d" % refresh_every if refresh_every else "")
+    stats = pu.compare(kind, rec, oracle, strict=strict, pure_floor=pure_floor, label=label)
     assert stats["dropped"] == 0
     acc = rec["mask"].mean()
-    assert 0.05 < acc < 0.8, acc
+    if forced:
+        assert acc == 1.0
+    else:
+        assert acc_range[0] < acc < acc_range[1], acc
     assert rec["naccept"] == rec["mask"].sum()
+    if kernel:       # the kernel this shape is meant to reach (selected by shape alone)
+        for cls, name in kernel.items():
+            assert name in rec["kernels"][cls], rec["kernels"]
     return stats
 
 
@@ -98,22 +108,12 @@ def test_pf_config3_shape_reduced():
     (512, 4, 2, True, 12),       # complex128 delayed (configs[3] shape at n=512)
 ])
 def test_det_tma_update_path(n, k, K, cplx, steps):
-    """Immediate update / delayed append through the TMA-staged kernel (lrux_det_tma.cu).
-    The delayed variant is opt-in (LRUX_UPDATE_PATH=tma), see launch_append_kt."""
-    import os
-
-    old = os.environ.get("LRUX_UPDATE_PATH")
-    if K > 0:
-        os.environ["LRUX_UPDATE_PATH"] = "tma"
-    try:
-        _run("det", 500 + n + k, 2, n, 2 * n, k, K, steps, cplx, walkers=[1],
-             scratch_every=0 if n >= 2048 else steps - 1)
-    finally:
-        if K > 0:
-            if old is None:
-                del os.environ["LRUX_UPDATE_PATH"]
-            else:
-                os.environ["LRUX_UPDATE_PATH"] = old
+    """Immediate update through the TMA-staged kernel (rows >= 8 KB, lrux_det_tma.cu); the
+    K > 0 rows take the register-row append (real data) / the DMMA append (complex, n >= 1024)
+    at the same sizes."""
+    _run("det", 500 + n + k, 2, n, 2 * n, k, K, steps, cplx, walkers=[1],
+         scratch_every=steps - 1, acc_range=(0.0, 1.0),
+         kernel={"update": "det_update_tma_kernel"} if K == 0 else {"append": "det_append"})
 
 
 def test_det_tma_update_n4096_properties():
@@ -152,19 +152,95 @@ def test_pf_large_n_paths(n, k):
     _run("pf", 99 + k, 3, n, 2 * n, k, 0, 10, walkers=[0, 2], scratch_every=3)
 
 
-@pytest.mark.parametrize("path", ["smem", "nb5", "cluster", "cluster_generic", "cta"])
-def test_pf_config3_shape_older_kernels(path, monkeypatch):
-    """The Pfaffian update kernels the register-resident one superseded at n = 128 stay
-    selectable (LRUX_PF_PATH, read at every accept) and must give the same trajectory:
-    shared-memory resident with 6 / 5 chunk buffers, 4-CTA cluster column-pair kernel,
-    generic cluster kernel, single-CTA warp-per-row kernel."""
-    monkeypatch.setenv("LRUX_PF_PATH", path)
-    _run("pf", wl.BASE_SEED + 3, 12, 128, 256, 1, 0, 40, walkers=[0, 5, 11])
+@pytest.mark.parametrize("n,k,cplx,name", [
+    (64, 1, False, "pf_regs_k1_kernel"),          # walker in registers
+    (100, 1, False, "pf_resident_k1_kernel"),     # whole walker in one CTA's shared memory, 6 chunk buffers
+    (140, 1, False, "pf_resident_k1_kernel"),     # ... 5 chunk buffers
+    (200, 1, False, "pf_cluster_k1_kernel"),      # 8-CTA cluster, run-time sizes
+    (256, 1, False, "pf_cluster_k1_kernel"),      # 8-CTA cluster, unrolled instance
+    (128, 2, False, "pf_cluster_update_kernel"),  # generic cluster kernel, 4-CTA
+    (96, 1, True, "pf_cluster_update_kernel"),    # complex
+    (320, 1, False, "pf_update_stream_kernel"),   # Y pass + streaming update
+    (320, 2, True, "pf_update_stream_kernel"),
+])
+def test_pf_update_kernel_by_shape(n, k, cplx, name):
+    """Every immediate Pfaffian update kernel, reached by its SHAPE (there is no environment
+    switch): same trajectory as the oracle."""
+    _run("pf", 171 + n + k, 4, n, 2 * n, k, 0, 24, cplx, walkers=[0, 3], scratch_every=4,
+         kernel={"update": name})
+
+
+def test_pf_update_tile_kernel_large_k():
+    """4k n e > 160 KB (here fp64, n = 1024, k = 8): Y' and g no longer fit in shared memory ->
+    the 32x32-tile kernel.  Forced accept (k = 8 proposals are rarely accepted)."""
+    _run("pf", 1812, 2, 1024, 2048, 8, 0, 5, walkers=[1], scratch_every=4, forced=True,
+         kernel={"update": "pf_update_kernel"})
+
+
+@pytest.mark.parametrize("kind,n,k,K,cplx", [
+    ("det", 192, 8, 8, False),     # K k = 64: two 32-row chunks of the real flush loop
+    ("det", 192, 8, 16, False),    # 128
+    ("det", 192, 8, 32, False),    # 256
+    ("det", 96, 4, 16, True),      # complex, K k = 64: four 16-row chunks
+    ("pf", 64, 2, 16, False),      # skew, 2 K k = 64
+    ("pf", 96, 4, 12, False),      # skew, 96 columns
+    ("pf", 48, 2, 16, True),       # skew complex, 64 columns: four chunks
+    ("pf", 64, 8, 4, False),       # k = 8: 16 x 16 core, 64 columns
+])
+def test_flush_multichunk(kind, n, k, K, cplx):
+    """The flush (Eq. 12 / Eq. 26) through MORE THAN ONE K-chunk of its staging loop in every
+    instantiation (real / complex, det / skew), with every proposal applied so that the
+    buffers fill to their full depth: K + 3 steps = one automatic full-depth flush plus the
+    part-filled fold of get_inverse.  The flushed inverse is compared element by element."""
+    st = _run(kind, 900 + n + K, 3, n, 2 * n, k, K, K + 3, cplx, forced=True,
+              kernel={"flush": "flush_dmma_kernel"})
+    assert st["max_inv_rel"] < 1e-9
+
+
+@pytest.mark.parametrize("n,k,K", [(512, 4, 8), (512, 8, 32), (1024, 4, 32), (1024, 8, 8)])
+def test_det_real_append_large_n(n, k, K):
+    """Real-valued delayed append (det_prep_kernel + det_append_kernel) at the sizes of the
+    configs[4] sweep; forced accept so that buffers fill and flush."""
+    _run("det", 40 + n + k + K, 3, n, 2 * n, k, K, min(K, 10) + 3, walkers=[0, 2], scratch_every=6,
+         forced=True, kernel={"append": "det_append_kernel"})
+
+
+@pytest.mark.parametrize("n,k,K,cplx", [(128, 1, 4, False), (512, 2, 8, False), (512, 1, 4, False),
+                                        (128, 2, 4, True), (64, 8, 0, False), (64, 8, 2, False)])
+def test_pf_delayed_and_k8(n, k, K, cplx):
+    """Pfaffian delayed kernels (pf_an / pf_y_colsum / pf_append / skew flush) above n = 50,
+    and k = 8 (16 x 16 skew core), immediate and delayed."""
+    _run("pf", 70 + n + k + K, 3, n, 2 * n, k, K, 20, cplx, walkers=[0, 2], scratch_every=5, forced=(k == 8))
+
+
+@pytest.mark.parametrize("kind,n,k,K", [("det", 64, 2, 0), ("det", 64, 2, 4), ("pf", 64, 1, 0), ("pf", 50, 2, 3)])
+def test_forced_accept_chain(kind, n, k, K):
+    """Forced-accept mode (what every ncu capture and the Fig. 2-style runs use) against the
+    oracle with every proposal applied."""
+    _run(kind, 300 + n + K, 4, n, 2 * n, k, K, 40, forced=True)
+
+
+@pytest.mark.parametrize("kind,n,k,K", [("det", 64, 2, 0), ("det", 96, 4, 0), ("pf", 64, 1, 0), ("det", 64, 2, 8)])
+def test_refresh_restores_bare_tolerance(kind, n, k, K):
+    """lrux_*_refresh every 16 steps (<= 16 accepted updates between rebuilds): every ratio of
+    a 400-step chain within the BARE 1e-10 of the from-scratch value, log-amplitude likewise --
+    the accuracy guard does what it is for."""
+    st = _run(kind, 77 + n + k, 6, n, 2 * n, k, K, 400, refresh_every=16, strict=True)
+    assert st["pure_frac"] == 1.0
 
 
 def test_det_config4_shape_reduced():
     """configs[3] shape reduced: complex128, k=4, delay K=32, n=256."""
     _run("det", wl.BASE_SEED + 4, 6, 256, 512, 4, 32, 80, cplx=True, walkers=[0, 5], scratch_every=5)
+
+
+@pytest.mark.parametrize("kmax,K,cplx", [(8, 32, False), (8, 96, False), (8, 48, True)])
+def test_large_delay_coefficient_staging(kmax, K, cplx):
+    """Delay shapes whose ratio kernel stages > 40 KB of coefficients (opt-in dynamic shared
+    memory): f64 kmax=8 K=96 (48 KB) and c128 kmax=8 K=48 used to pass init and then fail
+    every ratio call; pf kmax=8 K=32 used to be rejected outright."""
+    _run("det", 5 + K, 2, 64, 128, 2, K, 12, cplx, kmax=kmax)
+    _run("pf", 6 + K, 2, 64, 128, 2, min(K, 32), 12, cplx, kmax=kmax)
 
 
 def test_attach_resumes_from_a_state_copy():
