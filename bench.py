@@ -610,10 +610,13 @@ def main(argv=None):
                 "roofline_flush": roofline_flush(wk, K, rk, peak, peak_src, dgemm)}
 
     # end to end through the C-ABI from host buffers
-    e2e_steps = max(1, min(args.e2e_steps, steps))
-    ee = e2e_run(wk, seed, orb, occ, unocc, w0, device, 3, e2e_steps)
-    ee_sec, = shard.reduce_scalars([ee["sec"]], "max", device)
-    e2e_value = W * world * e2e_steps / ee_sec
+    e2e_steps = min(args.e2e_steps, steps)
+    if e2e_steps > 0:
+        ee = e2e_run(wk, seed, orb, occ, unocc, w0, device, 3, e2e_steps)
+        ee_sec, = shard.reduce_scalars([ee["sec"]], "max", device)
+        e2e_value = W * world * e2e_steps / ee_sec
+    else:       # sweep runs (--e2e-steps 0): device-timed figures only
+        ee, e2e_value = {"h2d": None, "d2h": None, "mismatch": None}, None
 
     roof = roofline_update(wk, run, peak, peak_src) if K0 == 0 else None
     if roof is None and "forced_accept" in extras and extras["forced_accept"]["roofline"]:
@@ -656,7 +659,7 @@ def main(argv=None):
            "roofline": roof, "roofline_append": roof_append, "roofline_flush": roof_flush,
            "kernels": run["kernels"], "extras": extras}
     if rank == 0:
-        if world == 1:
+        if world == 1 and args.cpu_seconds > 0:
             sec, done, nw, cores, T = oracle_sample(wk, 2, 200, args.cpu_seconds)
             out["cpu_baseline"] = {
                 "value": done / sec, "unit": UNIT, "cores": cores, "kind": "oracle",

@@ -31,6 +31,7 @@ extern "C" {
 #endif
 
 #define LRUX_MAX_K 8 /* largest kmax accepted by *_init */
+#define LRUX_MAX_K_GENERAL 8 /* largest rank of lrux_det_ratio_general */
 
 typedef struct lrux_handle_s* lrux_handle_t; /* small HOST object */
 typedef enum { LRUX_F64 = 0, LRUX_C128 = 1 } lrux_dtype_t;
@@ -78,6 +79,26 @@ lrux_status_t lrux_det_init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax
 lrux_status_t lrux_det_ratio(lrux_handle_t h, int32_t k, const int32_t* d_idx /*[W][k]*/,
                              const void* d_rows /*[W][k][n]*/, void* d_ratio /*[W]*/,
                              void* stream);
+
+/* General rank-k update A'_w = A_w + v_w u_w^T (Eq. 2) with each n x k factor in
+ * the paper's tuple form (Eq. 6-9): its first kd columns DENSE, the remaining
+ * k - kd columns ONE-HOT e_idx -- so a row replacement is (u dense, v one-hot: Eq. 6, 8), a
+ * column replacement (u one-hot, v dense: Eq. 7), a simultaneous row + column replacement the
+ * mixed tuples of Eq. 9, and kd = k on both sides the fully dense update of Eq. 2-5.  NOTE
+ * the dense columns are the UPDATE (A' - A), as in the paper's statement, not the new rows
+ * lrux_det_ratio takes.
+ *   d_u_dense [W][u_kd][n]  column a of u_w as a contiguous vector     d_u_idx [W][k-u_kd]
+ *   d_v_dense [W][v_kd][n]                                             d_v_idx [W][k-v_kd]
+ * (a pointer may be NULL when its count is 0).  Writes r_w = det(1 + u^T A^-1 v) (Eq. 3-4) to
+ * d_ratio[w] and leaves the proposal pending for lrux_det_accept, which applies Eq. 5.  One-hot
+ * columns cost O(n) gathers; every dense column makes the ratio itself an
+ * O(n^2) pass over the inverse.  On a handle with K > 0 the delay buffers are folded first
+ * (the proposal is evaluated against, and applied at once to, the folded inverse).  1 <= k <=
+ * min(kmax, LRUX_MAX_K_GENERAL); an index outside [0,n) sets info bit 2 (ratio NaN).
+ * LRUX_EUNSUPPORTED when v_kd * n * sizeof(elem) > 200 KiB. */
+lrux_status_t lrux_det_ratio_general(lrux_handle_t h, int32_t k, int32_t u_kd, const void* d_u_dense,
+                                     const int32_t* d_u_idx, int32_t v_kd, const void* d_v_dense,
+                                     const int32_t* d_v_idx, void* d_ratio, void* stream);
 
 /* Apply the pending proposal where d_mask[w] != 0: Woodbury update of the stored
  * inverse (Eq. 5) when K == 0, else append (a_t, b_t) to the delay

@@ -13,12 +13,12 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "lib", "liblrux.so")
-SOURCES = ["lrux_api.cu", "lrux_init.cu", "lrux_init_blocked.cu", "lrux_det.cu", "lrux_det_tma.cu", "lrux_pf.cu", "lrux_flush.cu", "lrux_harness.cu"]
+SOURCES = ["lrux_api.cu", "lrux_init.cu", "lrux_init_blocked.cu", "lrux_det.cu", "lrux_det_tma.cu", "lrux_det_dmma.cu", "lrux_pf.cu", "lrux_flush.cu", "lrux_general.cu", "lrux_harness.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-I" + os.path.join(ROOT, "include"), "-I" + CSRC, "-Xcompiler", "-fPIC",
-]
+] + os.environ.get("LRUX_NVCC_EXTRA", "").split()   # build-time only (A-B builds with -D...); nothing is read at run time
 
 
 def _deps_mtime():

@@ -124,16 +124,27 @@ static lrux_status_t init(lrux_handle_t* h, int64_t W, int32_t n, int32_t kmax, 
 }
 
 // ---------------------------------------------------------------- launch context
+// Static shared memory counts towards the 48 KiB default: opt in from 40 KiB of dynamic
+// shared memory on, always to the most this kernel can have (device opt-in maximum minus its
+// static part) -- a kernel attribute is shared by every handle of the process, so it must
+// never be lowered to what one handle happens to need.
+bool Ctx::optin(const void* fn, size_t smem) {
+  if (smem <= 40 * 1024) return true;
+  cudaFuncAttributes fa;
+  if (cudaFuncGetAttributes(&fa, fn) != cudaSuccess) { cudaGetLastError(); return false; }
+  const int most = smem_optin - (int)fa.sharedSizeBytes;
+  if ((int)smem > most ||
+      cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, most) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return true;
+}
+
 int Ctx::configure(const void* fn, int threads, size_t smem) {
   for (const Cfg& c : cfgs)
     if (c.fn == fn && c.threads == threads && c.smem == smem && c.cluster == 0) return c.occ;
-  // static shared memory counts towards the 48 KiB default: opt in from 40 KiB on, always
-  // to the device maximum (a kernel attribute is shared by every handle of the process)
-  if (smem > 40 * 1024 &&
-      cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess) {
-    cudaGetLastError();
-    return -1;
-  }
+  if (!optin(fn, smem)) return -1;
   int occ = 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, smem) != cudaSuccess || occ < 1) {
     cudaGetLastError();
@@ -147,10 +158,7 @@ int Ctx::configure_cluster(const void* fn, int threads, size_t smem, int cluster
   for (const Cfg& c : cfgs)
     if (c.fn == fn && c.threads == threads && c.smem == smem && c.cluster == cluster) return c.occ;
   int ncl = 0;
-  if (smem > 40 * 1024 &&
-      cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess) {
-    cudaGetLastError();
-  } else {
+  if (optin(fn, smem)) {
     cudaLaunchConfig_t cfg = {};
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -223,6 +231,26 @@ lrux_status_t lrux_det_ratio(lrux_handle_t h, int32_t k, const int32_t* d_idx, c
   if (k < 1 || k > h->st.kmax || !d_idx || !d_rows || !d_ratio) return LRUX_EINVAL;
   LRUX_COUNT(h, launch_det_ratio(h->st, k, d_idx, d_rows, d_ratio, h->cx, (cudaStream_t)stream));
   h->pending_k = k;
+  h->pending_general = false;
+  return LRUX_OK;
+}
+lrux_status_t lrux_det_ratio_general(lrux_handle_t h, int32_t k, int32_t u_kd, const void* d_u_dense,
+                                     const int32_t* d_u_idx, int32_t v_kd, const void* d_v_dense,
+                                     const int32_t* d_v_idx, void* d_ratio, void* stream) {
+  LRUX_CHECK_HANDLE(h, KIND_DET);
+  if (k < 1 || k > h->st.kmax || k > LRUX_MAX_K_GENERAL || u_kd < 0 || u_kd > k || v_kd < 0 || v_kd > k || !d_ratio)
+    return LRUX_EINVAL;
+  if ((u_kd > 0 && !d_u_dense) || (u_kd < k && !d_u_idx) || (v_kd > 0 && !d_v_dense) || (v_kd < k && !d_v_idx))
+    return LRUX_EINVAL;
+  // the proposal is evaluated against, and applied to, the folded inverse
+  if (h->st.K > 0) LRUX_COUNT(h, launch_det_flush(h->st, true, h->cx, (cudaStream_t)stream));
+  const int nl = launch_det_ratio_general(h->st, k, u_kd, d_u_dense, d_u_idx, v_kd, d_v_dense, d_v_idx, d_ratio,
+                                          h->cx, (cudaStream_t)stream);
+  if (nl == -2) return LRUX_EUNSUPPORTED;
+  if (nl < 0) return LRUX_ECUDA;
+  h->launches += nl;
+  h->pending_k = k;
+  h->pending_general = true;
   return LRUX_OK;
 }
 lrux_status_t lrux_pf_ratio(lrux_handle_t h, int32_t k, const int32_t* d_idx, const void* d_rows,
@@ -238,8 +266,12 @@ lrux_status_t lrux_det_accept(lrux_handle_t h, const uint8_t* d_mask, void* stre
   LRUX_CHECK_HANDLE(h, KIND_DET);
   if (!d_mask) return LRUX_EINVAL;
   if (h->pending_k == 0) return LRUX_ESTATE;
-  LRUX_COUNT(h, launch_det_accept(h->st, h->pending_k, d_mask, h->cx, (cudaStream_t)stream));
+  if (h->pending_general)
+    LRUX_COUNT(h, launch_det_accept_general(h->st, h->pending_k, d_mask, h->cx, (cudaStream_t)stream));
+  else
+    LRUX_COUNT(h, launch_det_accept(h->st, h->pending_k, d_mask, h->cx, (cudaStream_t)stream));
   h->pending_k = 0;
+  h->pending_general = false;
   return LRUX_OK;
 }
 lrux_status_t lrux_pf_accept(lrux_handle_t h, const uint8_t* d_mask, void* stream) {

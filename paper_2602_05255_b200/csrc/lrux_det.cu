@@ -10,6 +10,11 @@
 #include "lrux_common.cuh"
 #include "lrux_internal.h"
 
+// smallest template rank (1, 2, 4, 8) from which real-valued updates take the DMMA kernel
+#ifndef LRUX_DMMA_MIN_KT
+#define LRUX_DMMA_MIN_KT 4
+#endif
+
 namespace lrux {
 
 // ---------------------------------------------------------------- ratio (a1, a2, a5)
@@ -874,6 +879,17 @@ template <typename T, int KT>
 static int launch_update_kt(const State& st, int k, Ctx& cx, cudaStream_t s) {
   const int n = st.n;
   constexpr int VECMAX = sizeof(T) == 8 ? 2 : 1;
+  if constexpr (sizeof(T) == 8 && KT >= LRUX_DMMA_MIN_KT) {
+    // real data, k >= 3: 8-row strips on the FP64 tensor pipe (lrux_det_dmma.cu) -- the scalar
+    // kernels below are bound by their operand traffic from k = 4 on.  Measured exception
+    // (profiles/r02_sweep.md): k = 3, 4 at 1024 < n <= 2048, where the strips are split over a
+    // 2-CTA cluster (0.73 of HBM) and the TMA-staged kernel still has a rank-4 instance (0.81-0.84).
+    const bool tma_better = KT == 4 && n > 1024 && n <= 2048 && launch_det_update_tma(st, k, cx, s, true) == 1;
+    if (!tma_better) {
+      const int r = launch_det_update_dmma(st, k, cx, s);
+      if (r != 0) return r;
+    }
+  }
   if ((size_t)n * sizeof(T) >= 8 * 1024) {
     // rows of >= 8 KB: TMA-staged kernel (lrux_det_tma.cu)
     const int r = launch_det_update_tma(st, k, cx, s);

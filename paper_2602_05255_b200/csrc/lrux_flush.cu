@@ -5,13 +5,26 @@
 //         Ti[j][i] = -Ti[i][j] exactly
 // i.e. out[r][c] (-/+)= sum_s Bbuf[s][r] Abuf[s][c]: an (n x fill)(fill x n) contraction
 // per flushed walker.  sm_100a has no tcgen05 kind for f64; the FP64 tensor path is the
-// warp-level DMMA (mma.sync.m8n8k4.f64), fed from shared memory.
+// warp-level DMMA (mma.sync.m8n8k4.f64 -> SASS DMMA.8x8x4), fed from shared memory.
 //
-// Work item = (walker on the flush list, 64x64 output tile); persistent grid.  8 warps
-// as 4 (rows) x 2 (cols), warp tile 16 x 32 = 2 x 4 MMA tiles.  The two buffer panels
-// are staged s-major in shared memory (row stride 72 doubles: the 32 fragment loads
-// of a warp then hit 32 distinct doubles).  complex128 is split into planar re/im
-// planes while staging, so one complex MMA = 4 real DMMAs.
+// Work item = (walker on the flush list, output tile); persistent grid, one CTA of 8
+// warps per SM.  float64: 128 x 128 tiles, warp tile 32 x 64 (4 x 8 MMA tiles, 12 fragment
+// loads per 32 DMMAs); complex128: 64 x 128 tiles, warp tile 16 x 64, one complex MMA = 4
+// real DMMAs on (re, im) pairs read with ONE 16-byte fragment load each -- the buffers stay
+// interleaved, nothing is de-interleaved while staging.
+//
+// Both buffer panels move global -> shared with 16-byte cp.async (LDGSTS) through a ring of
+// NS stages of KC buffer rows; the ring runs ACROSS work items (the first chunks of a
+// CTA's next tile are in flight while it finishes the current one), which is what the
+// HBM-bound regime (K k <= 32: one or two chunks per tile) needs.  Rows past `fill` and
+// columns past n are zero-filled by the copy itself.  Row strides of the staged panels
+// are chosen so that the four buffer rows a fragment load touches fall into disjoint bank
+// groups (stride = 4 mod 16 doubles, 2 mod 8 complex elements): no bank conflicts.
+//
+// The accumulators START as the output tile (loaded while the first chunk lands) and
+// the MMAs run with the negated (det) B-side fragment, so the epilogue is a plain store
+// and needs no second set of registers.  Pf: tiles that hold an element above the
+// diagonal only; each result is also written, negated, at its mirror position.
 #include "lrux_common.cuh"
 #include "lrux_internal.h"
 
@@ -22,175 +35,269 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
                : "+d"(d0), "+d"(d1)
                : "d"(a), "d"(b));
 }
+// 16-byte (or 8-byte) asynchronous copy global -> shared; src_bytes = 0 zero-fills
+__device__ __forceinline__ void cp_async_16(void* smem_dst, const void* gsrc, int src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)),
+               "l"(gsrc), "r"(src_bytes)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async_8(void* smem_dst, const void* gsrc, int src_bytes) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)),
+               "l"(gsrc), "r"(src_bytes)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
 
 template <typename T>
 struct FlushCfg;
 template <>
-struct FlushCfg<double> {
-  static constexpr int NP = 1, KC = 32;
+struct FlushCfg<double> {   // 128 x 128, warps 4 x 2, warp tile 32 x 64
+  static constexpr int BM = 128, BN = 128, MT = 4, NT = 8, KC = 16, NS = 4, LDB = 132, LDA = 132;
 };
 template <>
-struct FlushCfg<cplx> {
-  static constexpr int NP = 2, KC = 16;
+struct FlushCfg<cplx> {     // 64 x 128, warps 4 x 2, warp tile 16 x 64
+  static constexpr int BM = 64, BN = 128, MT = 2, NT = 8, KC = 8, NS = 4, LDB = 66, LDA = 130;
 };
 
-__device__ __forceinline__ void split_store(double* p0, double*, int off, double v) { p0[off] = v; }
-__device__ __forceinline__ void split_store(double* p0, double* p1, int off, cplx v) {
-  p0[off] = v.re;
-  p1[off] = v.im;
-}
+struct FlushItem {
+  int w, r0, c0, fill, nch;
+};
 
-template <typename T, bool SKEW>
-__global__ void __launch_bounds__(256) flush_dmma_kernel(State st, int t1) {
+// V16: rows of the buffers are 16-byte aligned (always for complex; real: n even)
+template <typename T, bool SKEW, bool V16>
+__global__ void __launch_bounds__(256, 1) flush_dmma_kernel(State st, int tr, int tc, int tiles) {
   using S = Sc<T>;
-  constexpr int BT = 64, LD = 72;
-  constexpr int NP = FlushCfg<T>::NP, KC = FlushCfg<T>::KC;
-  constexpr bool CX = NP == 2;
-  __shared__ __align__(16) double Bs[NP][KC][LD];
-  __shared__ __align__(16) double As[NP][KC][LD];
+  using Cfg = FlushCfg<T>;
+  constexpr int BM = Cfg::BM, BN = Cfg::BN, MT = Cfg::MT, NT = Cfg::NT, KC = Cfg::KC, NS = Cfg::NS;
+  constexpr int LDB = Cfg::LDB, LDA = Cfg::LDA;
+  constexpr bool CX = sizeof(T) == 16;
+  constexpr int STAGE = KC * (LDB + LDA);          // elements of T per stage
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  T* ring = (T*)smem_raw;                          // [NS][ Bs[KC][LDB] | As[KC][LDA] ]
   const int n = st.n, cap = st.cap;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int wr = warp >> 1, wc = warp & 1;   // warp position in the 4 x 2 grid
-  const int lm = lane >> 2, lk = lane & 3;   // fragment row / k index
+  const int wr = warp >> 1, wc = warp & 1;         // warp position in the 4 x 2 grid
+  const int lm = lane >> 2, lk = lane & 3;         // fragment row / k index
   const int count = st.counters[1];
-  const int tiles = SKEW ? t1 * (t1 + 1) / 2 : t1 * t1;
-  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
-    const int w = st.flist[item / tiles];
-    int R, Cc;
-    if (SKEW) {
-      int rem = item % tiles;
-      R = 0;
-      while (rem >= t1 - R) { rem -= t1 - R; ++R; }
-      Cc = R + rem;
-    } else {
-      R = (item % tiles) / t1;
-      Cc = (item % tiles) % t1;
-    }
-    const int r0 = R * BT, c0 = Cc * BT;
-    const int fill = st.fill[w];
-    const T* Ab = (const T*)st.Abuf + (size_t)w * cap * n;
-    const T* Bb = (const T*)st.Bbuf + (size_t)w * cap * n;
-    T* Tw = (T*)st.Ti + (size_t)w * n * n;
-    double acc[NP][2][4][2];
-#pragma unroll
-    for (int p = 0; p < NP; ++p)
-#pragma unroll
-      for (int mt = 0; mt < 2; ++mt)
-#pragma unroll
-        for (int nt = 0; nt < 4; ++nt) acc[p][mt][nt][0] = acc[p][mt][nt][1] = 0.0;
-    // real case: issue the loads of the output tile now, consume them in the epilogue
-    // (hides one global-memory latency per work item; the HBM-bound regime, Kk <~ 50)
-    double tv[CX ? 1 : 2][CX ? 1 : 4][2];
-    if (!CX) {
-#pragma unroll
-      for (int mt = 0; mt < 2; ++mt) {
-        const int row = r0 + wr * 16 + mt * 8 + lm;
-#pragma unroll
-        for (int nt = 0; nt < 4; ++nt)
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            const int col = c0 + wc * 32 + nt * 8 + 2 * lk + e;
-            const bool need = row < n && col < n && (!SKEW || col > row);
-            tv[CX ? 0 : mt][CX ? 0 : nt][e] = need ? ((const double*)Tw)[(size_t)row * n + col] : 0.0;
-          }
-      }
-    }
+  const int64_t total = (int64_t)count * tiles;
+  const int G = (int)gridDim.x;
+  const int my_items = (int)((total - blockIdx.x + G - 1) / G);   // items blockIdx.x, +G, ...
+  if (total <= (int64_t)blockIdx.x) return;
 
-    // register double buffering: the global loads of panel chunk s0+KC are in flight
-    // while the DMMAs of chunk s0 run
-    constexpr int EPT = KC * BT / 256;   // staged elements per thread and panel
-    T rb[EPT], ra[EPT];
-    auto fetch = [&](int s0) {
-#pragma unroll
-      for (int u = 0; u < EPT; ++u) {
-        const int q = tid + 256 * u;
-        const int kk = q / BT, c = q % BT;
-        const bool sv = s0 + kk < fill;
-        rb[u] = (sv && r0 + c < n) ? Bb[(size_t)(s0 + kk) * n + r0 + c] : S::zero();
-        ra[u] = (sv && c0 + c < n) ? Ab[(size_t)(s0 + kk) * n + c0 + c] : S::zero();
+  auto decode = [&](int i) {
+    FlushItem it;
+    const int64_t item = (int64_t)blockIdx.x + (int64_t)i * G;
+    it.w = st.flist[item / tiles];
+    int t = (int)(item % tiles), R, Cc;
+    if (SKEW) {
+      // row tile R needs the column tiles Cc >= (R * BM) / BN (an element with col > row)
+      R = 0;
+      while (true) {
+        const int first_c = (R * BM) / BN;
+        if (t < tc - first_c) { Cc = first_c + t; break; }
+        t -= tc - first_c;
+        ++R;
       }
-    };
-    fetch(0);
-    for (int s0 = 0; s0 < fill; s0 += KC) {
-      __syncthreads();
+    } else {
+      R = t / tc;
+      Cc = t % tc;
+    }
+    it.r0 = R * BM;
+    it.c0 = Cc * BN;
+    it.fill = st.fill[it.w];
+    it.nch = max(1, (it.fill + KC - 1) / KC);
+    return it;
+  };
+
+  // ---- producer: one chunk = KC rows of both panels into one stage
+  auto issue = [&](const FlushItem& it, int ch, int stage) {
+    const T* Ab = (const T*)st.Abuf + (size_t)it.w * cap * n;
+    const T* Bb = (const T*)st.Bbuf + (size_t)it.w * cap * n;
+    T* Bs = ring + (size_t)stage * STAGE;
+    T* As = Bs + KC * LDB;
+    const int s0 = ch * KC;
+    constexpr int EPV = V16 ? (CX ? 1 : 2) : 1;            // elements per copy
+    constexpr int VB = BM / EPV, VA = BN / EPV;            // copies per row
 #pragma unroll
-      for (int u = 0; u < EPT; ++u) {
-        const int q = tid + 256 * u;
-        const int kk = q / BT, c = q % BT;
-        split_store(&Bs[0][kk][0], &Bs[NP - 1][kk][0], c, rb[u]);
-        split_store(&As[0][kk][0], &As[NP - 1][kk][0], c, ra[u]);
+    for (int u = 0; u < (KC * VB + 255) / 256; ++u) {
+      const int qd = tid + 256 * u;
+      if (qd < KC * VB) {
+        const int kk = qd / VB, c = (qd % VB) * EPV;
+        const bool ok = s0 + kk < it.fill && it.r0 + c < n;
+        const T* src = Bb + (size_t)(ok ? s0 + kk : 0) * n + (ok ? it.r0 + c : 0);
+        if (V16) cp_async_16(Bs + kk * LDB + c, src, ok ? 16 : 0);
+        else cp_async_8(Bs + kk * LDB + c, src, ok ? 8 : 0);
       }
-      __syncthreads();
-      if (s0 + KC < fill) fetch(s0 + KC);
-      const int kend = min(KC, (fill - s0 + 3) & ~3);
-      for (int k4 = 0; k4 < kend; k4 += 4) {
-        double bf[NP][2], af[NP][4];
+    }
 #pragma unroll
-        for (int p = 0; p < NP; ++p) {
+    for (int u = 0; u < (KC * VA + 255) / 256; ++u) {
+      const int qd = tid + 256 * u;
+      if (qd < KC * VA) {
+        const int kk = qd / VA, c = (qd % VA) * EPV;
+        const bool ok = s0 + kk < it.fill && it.c0 + c < n;
+        const T* src = Ab + (size_t)(ok ? s0 + kk : 0) * n + (ok ? it.c0 + c : 0);
+        if (V16) cp_async_16(As + kk * LDA + c, src, ok ? 16 : 0);
+        else cp_async_8(As + kk * LDA + c, src, ok ? 8 : 0);
+      }
+    }
+  };
+
+  int p_item = 0, p_ch = 0;                       // producer cursor
+  FlushItem pit = decode(0);
+  int issued = 0;
+  auto produce = [&]() {                          // issue the next chunk (if any) and commit a group
+    if (p_item < my_items) {
+      issue(pit, p_ch, issued % NS);
+      if (++p_ch == pit.nch) {
+        p_ch = 0;
+        if (++p_item < my_items) pit = decode(p_item);
+      }
+    }
+    ++issued;
+    cp_async_commit();
+  };
+#pragma unroll 1
+  for (int s = 0; s < NS - 1; ++s) produce();
+
+  int consumed = 0;
+#pragma unroll 1
+  for (int i = 0; i < my_items; ++i) {
+    const FlushItem it = decode(i);
+    T* Tw = (T*)st.Ti + (size_t)it.w * n * n;
+    // accumulators = the output tile (zero where nothing will be stored)
+    double acc[CX ? 2 : 1][MT][NT][2];
 #pragma unroll
-          for (int mt = 0; mt < 2; ++mt) bf[p][mt] = Bs[p][k4 + lk][wr * 16 + mt * 8 + lm];
+    for (int mt = 0; mt < MT; ++mt) {
+      const int row = it.r0 + wr * (MT * 8) + mt * 8 + lm;
 #pragma unroll
-          for (int nt = 0; nt < 4; ++nt) af[p][nt] = As[p][k4 + lk][wc * 32 + nt * 8 + lm];
+      for (int nt = 0; nt < NT; ++nt) {
+        const int col = it.c0 + wc * (NT * 8) + nt * 8 + 2 * lk;
+        if constexpr (V16 && !CX) {   // both elements wanted: one 16-byte load
+          if (row < n && col + 1 < n && (!SKEW || col > row)) {
+            const double2 v = *(const double2*)((const double*)Tw + (size_t)row * n + col);
+            acc[0][mt][nt][0] = v.x;
+            acc[0][mt][nt][1] = v.y;
+            continue;
+          }
         }
 #pragma unroll
-        for (int mt = 0; mt < 2; ++mt)
-#pragma unroll
-          for (int nt = 0; nt < 4; ++nt) {
-            if (!CX) {
-              dmma884(acc[0][mt][nt][0], acc[0][mt][nt][1], bf[0][mt], af[0][nt]);
-            } else {
-              // (br + i bi)(ar + i ai) = (br ar - bi ai) + i (br ai + bi ar)
-              dmma884(acc[0][mt][nt][0], acc[0][mt][nt][1], bf[0][mt], af[0][nt]);
-              dmma884(acc[0][mt][nt][0], acc[0][mt][nt][1], -bf[NP - 1][mt], af[NP - 1][nt]);
-              dmma884(acc[NP - 1][mt][nt][0], acc[NP - 1][mt][nt][1], bf[0][mt], af[NP - 1][nt]);
-              dmma884(acc[NP - 1][mt][nt][0], acc[NP - 1][mt][nt][1], bf[NP - 1][mt], af[0][nt]);
-            }
-          }
+        for (int e = 0; e < 2; ++e) {
+          const bool need = row < n && col + e < n && (!SKEW || col + e > row);
+          T v = S::zero();
+          if (need) v = Tw[(size_t)row * n + col + e];
+          acc[0][mt][nt][e] = sc_re(v);
+          if (CX) acc[CX ? 1 : 0][mt][nt][e] = sc_im(v);
+        }
       }
     }
-    // epilogue: accumulator (row lm, cols 2*lk, 2*lk+1) of each 8x8 tile
+#pragma unroll 1
+    for (int ch = 0; ch < it.nch; ++ch) {
+      cp_async_wait<NS - 2>();
+      __syncthreads();            // chunk `consumed` has landed for everyone; stage (consumed-1)%NS is free
+      produce();
+      const T* Bs = ring + (size_t)(consumed % NS) * STAGE;
+      const T* As = Bs + KC * LDB;
+      ++consumed;
+      const int kend = min(KC, (it.fill - ch * KC + 3) & ~3);
+      for (int k4 = 0; k4 < kend; k4 += 4) {
+        if constexpr (!CX) {
+          double bf[MT], af[NT];
 #pragma unroll
-    for (int mt = 0; mt < 2; ++mt) {
-      const int row = r0 + wr * 16 + mt * 8 + lm;
+          for (int mt = 0; mt < MT; ++mt) {
+            const double b = ((const double*)Bs)[(k4 + lk) * LDB + wr * (MT * 8) + mt * 8 + lm];
+            bf[mt] = SKEW ? b : -b;
+          }
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt) af[nt] = ((const double*)As)[(k4 + lk) * LDA + wc * (NT * 8) + nt * 8 + lm];
+#pragma unroll
+          for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) dmma884(acc[0][mt][nt][0], acc[0][mt][nt][1], bf[mt], af[nt]);
+        } else {
+          double2 bf[MT], af[NT];
+#pragma unroll
+          for (int mt = 0; mt < MT; ++mt) {
+            double2 b = ((const double2*)Bs)[(k4 + lk) * LDB + wr * (MT * 8) + mt * 8 + lm];
+            if (!SKEW) { b.x = -b.x; b.y = -b.y; }
+            bf[mt] = b;
+          }
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt) af[nt] = ((const double2*)As)[(k4 + lk) * LDA + wc * (NT * 8) + nt * 8 + lm];
+#pragma unroll
+          for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+              // (br + i bi)(ar + i ai) = (br ar - bi ai) + i (br ai + bi ar)
+              dmma884(acc[0][mt][nt][0], acc[0][mt][nt][1], bf[mt].x, af[nt].x);
+              dmma884(acc[0][mt][nt][0], acc[0][mt][nt][1], -bf[mt].y, af[nt].y);
+              dmma884(acc[CX ? 1 : 0][mt][nt][0], acc[CX ? 1 : 0][mt][nt][1], bf[mt].x, af[nt].y);
+              dmma884(acc[CX ? 1 : 0][mt][nt][0], acc[CX ? 1 : 0][mt][nt][1], bf[mt].y, af[nt].x);
+            }
+        }
+      }
+    }
+    // ---- epilogue: accumulator (row lm, cols 2*lk, 2*lk+1) of each 8x8 tile
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt) {
+      const int row = it.r0 + wr * (MT * 8) + mt * 8 + lm;
       if (row >= n) continue;
 #pragma unroll
-      for (int nt = 0; nt < 4; ++nt) {
+      for (int nt = 0; nt < NT; ++nt) {
+        const int col = it.c0 + wc * (NT * 8) + nt * 8 + 2 * lk;
+        if constexpr (V16 && !CX && !SKEW) {
+          if (col + 1 < n) {
+            *(double2*)((double*)Tw + (size_t)row * n + col) = make_double2(acc[0][mt][nt][0], acc[0][mt][nt][1]);
+            continue;
+          }
+        }
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-          const int col = c0 + wc * 32 + nt * 8 + 2 * lk + e;
-          if (col >= n) continue;
-          T a;
-          if (!CX) a = sc_from(acc[0][mt][nt][e], 0.0, T{});
-          else a = sc_from(acc[0][mt][nt][e], acc[NP - 1][mt][nt][e], T{});
-          T old;
-          if (!CX) old = sc_from(tv[CX ? 0 : mt][CX ? 0 : nt][e], 0.0, T{});
-          else if (!SKEW || col > row) old = Tw[(size_t)row * n + col];
+          if (col + e >= n) continue;
+          const T v = sc_from(acc[0][mt][nt][e], acc[CX ? 1 : 0][mt][nt][e], T{});
           if (SKEW) {
-            if (col > row) {
-              const T v = S::add(old, a);
-              Tw[(size_t)row * n + col] = v;
-              Tw[(size_t)col * n + row] = S::neg(v);
+            if (col + e > row) {
+              Tw[(size_t)row * n + col + e] = v;
+              Tw[(size_t)(col + e) * n + row] = S::neg(v);
             }
           } else {
-            Tw[(size_t)row * n + col] = S::sub(old, a);
+            Tw[(size_t)row * n + col + e] = v;
           }
         }
       }
     }
   }
+  cp_async_wait<0>();
 }
 
-template <typename T, bool SKEW>
-static int launch_flush_t(const State& st, Ctx& cx, cudaStream_t s) {
-  const int t1 = (st.n + 63) / 64;
-  const int64_t tiles = SKEW ? (int64_t)t1 * (t1 + 1) / 2 : (int64_t)t1 * t1;
-  const int occ = cx.configure((const void*)flush_dmma_kernel<T, SKEW>, 256, 0);
+template <typename T, bool SKEW, bool V16>
+static int launch_flush_v(const State& st, Ctx& cx, cudaStream_t s) {
+  using Cfg = FlushCfg<T>;
+  const int tr = (st.n + Cfg::BM - 1) / Cfg::BM, tc = (st.n + Cfg::BN - 1) / Cfg::BN;
+  int64_t tiles = (int64_t)tr * tc;
+  if (SKEW) {
+    tiles = 0;
+    for (int R = 0; R < tr; ++R) tiles += tc - (R * Cfg::BM) / Cfg::BN;
+  }
+  const size_t smem = (size_t)Cfg::NS * Cfg::KC * (Cfg::LDB + Cfg::LDA) * sizeof(T);
+  auto kern = flush_dmma_kernel<T, SKEW, V16>;
+  const int occ = cx.configure((const void*)kern, 256, smem);
   if (occ < 0) return -1;
   cx.name(LRUX_PROF_FLUSH, "flush_dmma_kernel");
   int64_t grid = (int64_t)cx.num_sms * occ;
   if (grid > st.W * tiles) grid = st.W * tiles;
-  flush_dmma_kernel<T, SKEW><<<(unsigned)grid, 256, 0, s>>>(st, t1);
+  kern<<<(unsigned)grid, 256, smem, s>>>(st, tr, tc, (int)tiles);
   return 1;
+}
+
+template <typename T, bool SKEW>
+static int launch_flush_t(const State& st, Ctx& cx, cudaStream_t s) {
+  if (sizeof(T) == 16 || (st.n % 2) == 0) return launch_flush_v<T, SKEW, true>(st, cx, s);
+  if constexpr (sizeof(T) == 8) return launch_flush_v<T, SKEW, false>(st, cx, s);
+  return -1;
 }
 
 int launch_flush_dmma(const State& st, Ctx& cx, cudaStream_t s) {

@@ -94,6 +94,7 @@ struct Ctx {
   int configure(const void* fn, int threads, size_t smem);
   // Co-resident clusters of `cluster` CTAs on the whole GPU (0: not launchable), cached.
   int configure_cluster(const void* fn, int threads, size_t smem, int cluster);
+  bool optin(const void* fn, size_t smem);
   void name(int cls, const char* kernel) { last[cls] = kernel; }
 };
 
@@ -103,6 +104,7 @@ struct lrux_handle_s {
   lrux::State st;
   lrux::Ctx cx;
   int32_t pending_k;  // 0 = nothing pending
+  bool pending_general = false;   // the pending proposal came from lrux_det_ratio_general
   int64_t launches;
 };
 
@@ -135,6 +137,13 @@ int launch_pf_flush(const State& st, bool all, Ctx& cx, cudaStream_t s);
 // TMA-staged immediate det update for large rows (lrux_det_tma.cu): 1 = launched,
 // 0 = shape not eligible, -1 = CUDA error.  probe = true: eligibility only, nothing launched.
 int launch_det_update_tma(const State& st, int k, Ctx& cx, cudaStream_t s, bool probe = false);
+// immediate det update on the FP64 tensor pipe, real data (lrux_det_dmma.cu): same return codes
+int launch_det_update_dmma(const State& st, int k, Ctx& cx, cudaStream_t s, bool probe = false);
+// general update factors (lrux_general.cu); ratio: -2 = shape not supported
+int launch_det_ratio_general(const State& st, int k, int u_kd, const void* u_dense, const int32_t* u_idx,
+                             int v_kd, const void* v_dense, const int32_t* v_idx, void* ratio, Ctx& cx,
+                             cudaStream_t s);
+int launch_det_accept_general(const State& st, int k, const uint8_t* mask, Ctx& cx, cudaStream_t s);
 // DMMA flush of the delay buffers, det and pf (lrux_flush.cu)
 int launch_flush_dmma(const State& st, Ctx& cx, cudaStream_t s);
 // shared between det and pf (defined in lrux_det.cu)

@@ -33,6 +33,7 @@ SIGNATURES = {
     "lrux_pf_refresh": [_vp, _vp, _vp],
     "lrux_det_ratio": [_vp, _i32, _vp, _vp, _vp, _vp],
     "lrux_pf_ratio": [_vp, _i32, _vp, _vp, _vp, _vp],
+    "lrux_det_ratio_general": [_vp, _i32, _i32, _vp, _vp, _i32, _vp, _vp, _vp, _vp],
     "lrux_det_accept": [_vp, _vp, _vp],
     "lrux_pf_accept": [_vp, _vp, _vp],
     "lrux_det_flush": [_vp, _vp],
@@ -161,6 +162,22 @@ class _Walkers:
         k = int(idx.shape[1])
         out = self.ratio if out is None else out
         _check(self._fn("ratio")(self._h, k, _ptr(idx), _ptr(rows), _ptr(out), _stream(stream)))
+        return out
+
+    def ratio_general_(self, u_dense, u_idx, v_dense, v_idx, out=None, stream=None):
+        """lrux_det_ratio_general: A' = A + v u^T, each factor = dense columns ([W][kd][n], or
+        None) followed by one-hot columns (int32 [W][ke], or None).  Returns ratio [W]."""
+        def split(dense, idx):
+            kd = 0 if dense is None else int(dense.shape[1])
+            ke = 0 if idx is None else int(idx.shape[1])
+            return kd, ke, (None if dense is None else _ptr(dense.contiguous())), (None if idx is None else _ptr(idx.contiguous()))
+        ukd, uke, ud, ui = split(u_dense, u_idx)
+        vkd, vke, vd, vi = split(v_dense, v_idx)
+        if ukd + uke != vkd + vke:
+            raise ValueError("u and v must have the same number of columns")
+        out = self.ratio if out is None else out
+        _check(self._lib.lrux_det_ratio_general(self._h, ukd + uke, ukd, ud, ui, vkd, vd, vi, _ptr(out),
+                                                _stream(stream)))
         return out
 
     def accept(self, mask, stream=None):

@@ -115,7 +115,7 @@ def run_oracle(kind, orb, occ, unocc, k, seed, steps, walkers, scratch_every=1, 
     return out
 
 
-def compare(kind, rec, oracle, inv_tol=1e-9, strict=False, pure_floor=None, label=None):
+def compare(kind, rec, oracle, inv_tol=1e-9, strict=False, pure_floor=None, label=None, forced=False):
     """Element-by-element parity of one GPU record against oracle trajectories.
 
     Pass rule (DESIGN.md §3 reading 14).  r*_t = the oracle's from-scratch ratio,
@@ -123,9 +123,14 @@ def compare(kind, rec, oracle, inv_tol=1e-9, strict=False, pure_floor=None, labe
     over the from-scratch points so far (the plain fp64 algorithm's own error on this
     walker: it sits in the tracked inverse, so it persists).  Then
       * at a point with r*:      |r_gpu - r*|    <= min(1e-10 + 4 e_t, 1e-8) |r*|
-      * at a point without r*:   |r_gpu - r_smw| <= min(1e-10 + 5 e_t, 1e-8) |r_smw|
-        (triangle inequality: the reference itself is off by up to e_t)
+      * at a point without r*:   |r_gpu - r_smw| <= min(1e-10 + 5 e_T, 1e-8) |r_smw|,
+        e_T = e at the end of the trajectory (triangle inequality: the reference itself is off
+        by the oracle's own error, which is only sampled at the from-scratch points)
       * ``strict`` (chains that call lrux_*_refresh): the bare 1e-10 at every point with r*.
+      * ``forced`` (every proposal applied, however small its ratio -- Metropolis would never
+        accept those -- so the walker runs through nearly singular matrices and the step at
+        which an implementation loses its digits is implementation specific): e_T instead of
+        e_t at every point, and the residual bound grows with e_T as well (never past 1e-7).
     ``pure_floor``: least fraction of the from-scratch points that must meet the bare
     1e-10.  Decisions must match exactly unless the oracle logged a near-tie (then the
     walker is dropped from later comparison and counted).  Returns / prints statistics:
@@ -142,6 +147,8 @@ def compare(kind, rec, oracle, inv_tol=1e-9, strict=False, pure_floor=None, labe
         assert abs(rec["init_phase"][w] - tr["init_phase"]) < 1e-9
         dropped = False
         e_run = 0.0
+        m = ~np.isnan(tr["r_scratch"])
+        e_all = float(np.max(np.abs(tr["r_lemma"][m] - tr["r_scratch"][m]) / np.abs(tr["r_scratch"][m]))) if m.any() else 0.0
         for t in range(steps):
             rg, rl, rs = rec["ratio"][t, w], tr["r_lemma"][t], tr["r_scratch"][t]
             have = not np.isnan(rs)
@@ -155,7 +162,7 @@ def compare(kind, rec, oracle, inv_tol=1e-9, strict=False, pure_floor=None, labe
                 st["pure"] += rel <= RTOL
                 if rel > st["max_rel"]:
                     st["max_rel"], st["abs_r_at_max"] = float(rel), float(abs(ref))
-            bound = RTOL if (strict and have) else min(RTOL + (4 if have else 5) * e_run, CAP)
+            bound = RTOL if (strict and have) else min(RTOL + (4 * (e_all if forced else e_run) if have else 5 * e_all), CAP)
             assert rel <= bound, ("walker %d step %d: gpu %r from-scratch %r lemma %r: rel %.3e > %.3e"
                                   % (w, t, rg, rs, rl, rel, bound))
             if bool(rec["mask"][t, w]) != bool(tr["accepted"][t]):
@@ -181,12 +188,13 @@ def compare(kind, rec, oracle, inv_tol=1e-9, strict=False, pure_floor=None, labe
         n = tr["A"].shape[0]
         gi = rec["Ainv"][w]
         resid = np.abs(tr["A"] @ gi - np.eye(n)).max()
-        assert resid <= inv_tol, "A_T A_T^-1 residual %g" % resid
+        res_tol = min(max(inv_tol, 100 * e_all), 1e-7) if forced else inv_tol
+        assert resid <= res_tol, "A_T A_T^-1 residual %g" % resid
         # the inverse itself, element by element, against the oracle's tracked inverse: both
         # carry their own Woodbury error, so the bound is the residual bound in units of |A^-1|
         inv_rel = np.abs(gi - tr["Ainv"]).max() / np.abs(tr["Ainv"]).max()
         st["max_inv_rel"] = max(st["max_inv_rel"], float(inv_rel))
-        assert inv_rel <= max(inv_tol, 50 * e_run), "inverse differs from the oracle's: %g" % inv_rel
+        assert inv_rel <= min(max(inv_tol, 50 * e_all), 1e-6), "inverse differs from the oracle's: %g" % inv_rel
         if kind == "pf":
             assert np.array_equal(gi, -gi.T), "stored inverse not exactly skew"
     st["pure_frac"] = st["pure"] / max(1, st["scratch_points"])

