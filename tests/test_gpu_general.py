@@ -79,8 +79,9 @@ def test_general_factors_follow_the_oracle(name, uf, vf, n, K, cplx):
     worst = 0.0
     for t in range(steps):
         ud, ui, U = _factor(rng, W, n, uf[0], uf[1], cplx, 0.3 / np.sqrt(n))
-        vd, vi, V = _factor(rng, W, n, vf[0], vf[1], cplx, (1.0 if uf[0] else 0.3) / np.sqrt(n) if vf[0] and uf[0] else
-                            (0.3 / np.sqrt(n) if vf[0] else 1.0))
+        # sizes: v u^T ~ 0.3 |A_ij| for dense x dense; a pure column replacement (u one-hot) gets
+        # deltas of that size directly
+        vd, vi, V = _factor(rng, W, n, vf[0], vf[1], cplx, 1.0 if uf[0] else 0.3 / np.sqrt(n))
         r_gpu = wk.ratio_general_(None if ud is None else _t(ud), None if ui is None else _t(ui),
                                   None if vd is None else _t(vd), None if vi is None else _t(vi)).cpu().numpy().copy()
         mask = (rng.random(W) < 0.7).astype(np.uint8)
