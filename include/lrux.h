@@ -30,7 +30,8 @@
 extern "C" {
 #endif
 
-#define LRUX_MAX_K 8 /* largest kmax accepted by *_init */
+#define LRUX_MAX_K 64 /* largest kmax accepted by *_init; kmax > 8 (backflow-sized ranks):
+                         float64 determinants with K = 0 and even n only, else LRUX_EUNSUPPORTED */
 #define LRUX_MAX_K_GENERAL 8 /* largest rank of lrux_det_ratio_general */
 
 typedef struct lrux_handle_s* lrux_handle_t; /* small HOST object */

@@ -33,6 +33,7 @@ size_t state_layout(State* st, void* base, int64_t W, int32_t n, int32_t kmax, i
   s.pend_Rinv = take((size_t)W * kc * kc * e);
   s.pend_C = take((size_t)W * kmax * n * e);
   s.pend_N = take((size_t)W * kmax * n * e);
+  if (kind == KIND_DET && kmax > kSmallMaxK) s.pend_D = take((size_t)W * kmax * n * e);
   if (kind == KIND_DET) {
     const size_t nsplit = ((size_t)n + kRatioSlice - 1) / kRatioSlice;
     s.pend_Rpart = take((size_t)W * nsplit * kmax * kmax * e);
@@ -64,6 +65,8 @@ static lrux_status_t check_dims(int64_t W, int32_t n, int32_t kmax, int32_t K, i
   if (dt != LRUX_F64 && dt != LRUX_C128) return LRUX_EINVAL;
   if (kind == KIND_PF && (n % 2 != 0)) return LRUX_EINVAL;
   if (kmax > n) return LRUX_EINVAL;
+  // ranks above 8: float64 determinants with immediate updates and even n (tensor-pipe path)
+  if (kmax > kSmallMaxK && (kind != KIND_DET || dt != LRUX_F64 || K != 0 || (n & 1))) return LRUX_EUNSUPPORTED;
   // the delayed determinant ratio stages K*kmax coefficients per proposal row in (opt-in)
   // dynamic shared memory; the Pfaffian path has no such limit
   const size_t kt = kmax <= 1 ? 1 : kmax <= 2 ? 2 : kmax <= 4 ? 4 : 8;   // kernels' template rank
@@ -229,7 +232,10 @@ lrux_status_t lrux_det_ratio(lrux_handle_t h, int32_t k, const int32_t* d_idx, c
                              void* d_ratio, void* stream) {
   LRUX_CHECK_HANDLE(h, KIND_DET);
   if (k < 1 || k > h->st.kmax || !d_idx || !d_rows || !d_ratio) return LRUX_EINVAL;
-  LRUX_COUNT(h, launch_det_ratio(h->st, k, d_idx, d_rows, d_ratio, h->cx, (cudaStream_t)stream));
+  if (k > kSmallMaxK)
+    LRUX_COUNT(h, launch_det_ratio_big(h->st, k, d_idx, d_rows, d_ratio, h->cx, (cudaStream_t)stream));
+  else
+    LRUX_COUNT(h, launch_det_ratio(h->st, k, d_idx, d_rows, d_ratio, h->cx, (cudaStream_t)stream));
   h->pending_k = k;
   h->pending_general = false;
   return LRUX_OK;
@@ -268,6 +274,8 @@ lrux_status_t lrux_det_accept(lrux_handle_t h, const uint8_t* d_mask, void* stre
   if (h->pending_k == 0) return LRUX_ESTATE;
   if (h->pending_general)
     LRUX_COUNT(h, launch_det_accept_general(h->st, h->pending_k, d_mask, h->cx, (cudaStream_t)stream));
+  else if (h->pending_k > kSmallMaxK)
+    LRUX_COUNT(h, launch_det_accept_big(h->st, h->pending_k, d_mask, h->cx, (cudaStream_t)stream));
   else
     LRUX_COUNT(h, launch_det_accept(h->st, h->pending_k, d_mask, h->cx, (cudaStream_t)stream));
   h->pending_k = 0;

@@ -9,7 +9,7 @@
 
 namespace lrux {
 
-constexpr int kMaxK = LRUX_MAX_K;
+constexpr int kMaxK = 8;   // largest rank of the register / shared-memory kernels (k > 8: lrux_det_big.cu)
 
 // ---------------------------------------------------------------- scalars
 struct cplx {

@@ -6,6 +6,7 @@
 namespace lrux {
 
 constexpr uint64_t STREAM_SLOT = 2, STREAM_ORB = 3, STREAM_ACCEPT = 4;
+constexpr int kHMaxK = LRUX_MAX_K;   // proposals of up to this many rows
 
 // k distinct values in [0,m): rho_a in [0,m-a) with counter step*k+a, skipping
 // previously chosen values in ascending order (workload._distinct), i.e. the
@@ -32,10 +33,10 @@ det_propose_kernel(uint64_t seed, int64_t w0, int64_t step, int n, int M, int k,
                    const T* __restrict__ Phi, const int32_t* __restrict__ occ,
                    const int32_t* __restrict__ unocc, int32_t* __restrict__ idx,
                    int32_t* __restrict__ upos, T* __restrict__ rows) {
-  __shared__ int sq[kMaxK];
+  __shared__ int sq[kHMaxK];
   const int64_t w = blockIdx.x;
   if (threadIdx.x == 0) {
-    int P[kMaxK], J[kMaxK];
+    int P[kHMaxK], J[kHMaxK];
     draw_distinct(seed, (uint64_t)(w0 + w), STREAM_SLOT, (uint64_t)step, k, n, P);
     draw_distinct(seed, (uint64_t)(w0 + w), STREAM_ORB, (uint64_t)step, k, M - n, J);
     for (int a = 0; a < k; ++a) {
@@ -58,10 +59,10 @@ pf_propose_kernel(uint64_t seed, int64_t w0, int64_t step, int n, int M, int k,
                   const T* __restrict__ F, const int32_t* __restrict__ occ,
                   const int32_t* __restrict__ unocc, int32_t* __restrict__ idx,
                   int32_t* __restrict__ upos, T* __restrict__ rows) {
-  __shared__ int sq[kMaxK], sp[kMaxK];
+  __shared__ int sq[kHMaxK], sp[kHMaxK];
   const int64_t w = blockIdx.x;
   if (threadIdx.x == 0) {
-    int P[kMaxK], J[kMaxK];
+    int P[kHMaxK], J[kHMaxK];
     draw_distinct(seed, (uint64_t)(w0 + w), STREAM_SLOT, (uint64_t)step, k, n, P);
     draw_distinct(seed, (uint64_t)(w0 + w), STREAM_ORB, (uint64_t)step, k, M - n, J);
     for (int a = 0; a < k; ++a) {
@@ -112,7 +113,7 @@ __global__ void decide_kernel(uint64_t seed, int64_t w0, int64_t step, int64_t W
 using namespace lrux;
 
 static bool bad_args(int64_t W, int n, int M, int k, int dt) {
-  return W <= 0 || n <= 0 || M <= n || k < 1 || k > kMaxK || k > n || k > M - n ||
+  return W <= 0 || n <= 0 || M <= n || k < 1 || k > kHMaxK || k > n || k > M - n ||
          (dt != LRUX_F64 && dt != LRUX_C128);
 }
 

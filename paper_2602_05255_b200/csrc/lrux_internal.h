@@ -13,6 +13,8 @@ namespace lrux {
 enum Kind { KIND_DET = 0, KIND_PF = 1 };
 constexpr int kRatioSlice = 256;       // columns of A^-1[:,P] handled by one CTA of the det ratio
 constexpr int kRatioSplitMax = 64;     // => n <= 16384
+constexpr int kSmallMaxK = 8;          // largest rank of the register / shared-memory kernels (= kMaxK)
+constexpr int kBigMaxK = 64;           // largest rank (float64 determinants, K = 0, k > 8: lrux_det_big.cu)
 constexpr int kBlockedInitMin = 768;   // blocked (panel + DMMA) initialisation from this n on
 constexpr size_t kRatioCoefSmemMax = 160 * 1024;   // det delayed ratio: K*kmax*KT coefficients staged per CTA
 
@@ -38,6 +40,7 @@ struct State {
   void* pend_N;      // [W][kmax][n]  new rows
   void* pend_Y;      // pf: [W][kmax][n]  A^-1 N ; det delayed: [W][kmax][cap] N * Abuf^T
   void* pend_AN;     // pf delayed: [W][kmax][cap]  N * Abuf^T
+  void* pend_D;      // det, kmax > 8: [W][kmax][n]  N A^-1 - I[P,:], then R^-1 times it
   void* pend_Rpart;  // det: [W][kRatioSplitMax][kmax*kmax] partial R of each column slice
   int32_t* pend_cnt; // det: [W] slices of the current ratio call that have finished
   void* init_A;      // n >= kBlockedInitMin: [W][32][n] scratch of the blocked initialisation
@@ -74,6 +77,19 @@ struct ProfScope {
   ~ProfScope() {
     if (p) { cudaEventRecord(r.b, s); p->recs[cls].push_back(r); }
   }
+};
+
+// out[a][j] = sum_i N[a][i] X[j][i] (- 1 where j == idx[a]) on the FP64 tensor pipe
+// (lrux_rowdot.cu); per-walker strides and leading dimensions in elements.
+struct RowdotArgs {
+  const double* X; size_t x_stride; int rows, ldx;
+  const double* N; size_t n_stride; int ldn;
+  int n, k;
+  double* out; size_t o_stride; int ldo;
+  const int32_t* list;    // walker list (nullptr: walkers 0..W-1)
+  const int32_t* count;   // device count of listed walkers (nullptr: W)
+  int64_t W;
+  const int32_t* idx; int idx_stride;   // subtract 1 at out[a][idx[a]] (nullptr: nothing)
 };
 
 // Per-handle launch context (host only): what a launcher needs besides the state views.
@@ -144,6 +160,11 @@ int launch_det_ratio_general(const State& st, int k, int u_kd, const void* u_den
                              int v_kd, const void* v_dense, const int32_t* v_idx, void* ratio, Ctx& cx,
                              cudaStream_t s);
 int launch_det_accept_general(const State& st, int k, const uint8_t* mask, Ctx& cx, cudaStream_t s);
+int launch_rowdot_dmma(const RowdotArgs& A, Ctx& cx, cudaStream_t s);
+// ranks 8 < k <= 64, float64, K = 0 (lrux_det_big.cu)
+int launch_det_ratio_big(const State& st, int k, const int32_t* d_idx, const void* d_rows, void* d_ratio,
+                         Ctx& cx, cudaStream_t s);
+int launch_det_accept_big(const State& st, int k, const uint8_t* mask, Ctx& cx, cudaStream_t s);
 // DMMA flush of the delay buffers, det and pf (lrux_flush.cu)
 int launch_flush_dmma(const State& st, Ctx& cx, cudaStream_t s);
 // shared between det and pf (defined in lrux_det.cu)

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "lib", "liblrux.so")
 
 F64, C128 = 0, 1
 OK, EINVAL, ESTATE, EWORKSPACE, EUNSUPPORTED, ECUDA = range(6)
-MAX_K = 8
+MAX_K = 64
 PROF_RATIO, PROF_UPDATE, PROF_APPEND, PROF_FLUSH, PROF_YPASS = range(5)
 
 _vp, _i32, _i64, _u64, _sz = C.c_void_p, C.c_int32, C.c_int64, C.c_uint64, C.c_size_t

@@ -52,7 +52,14 @@ def test_state_bytes_and_arg_checks(lib):
     # misuse -> LRUX_EINVAL, nothing done
     assert lib.lrux_pf_state_bytes(4, 33, 1, 0, lrux.F64, C.byref(out)) == lrux.EINVAL   # odd n
     assert lib.lrux_det_state_bytes(0, 32, 1, 0, lrux.F64, C.byref(out)) == lrux.EINVAL
-    assert lib.lrux_det_state_bytes(4, 32, 9, 0, lrux.F64, C.byref(out)) == lrux.EINVAL  # k > MAX_K
+    assert lib.lrux_det_state_bytes(4, 128, 65, 0, lrux.F64, C.byref(out)) == lrux.EINVAL  # k > MAX_K
+    # ranks above 8: float64 determinants, K = 0, even n only
+    assert lib.lrux_det_state_bytes(4, 128, 9, 0, lrux.F64, C.byref(out)) == lrux.OK
+    assert lib.lrux_det_state_bytes(4, 128, 64, 0, lrux.F64, C.byref(out)) == lrux.OK
+    assert lib.lrux_det_state_bytes(4, 128, 9, 0, lrux.C128, C.byref(out)) == lrux.EUNSUPPORTED
+    assert lib.lrux_det_state_bytes(4, 128, 9, 4, lrux.F64, C.byref(out)) == lrux.EUNSUPPORTED
+    assert lib.lrux_det_state_bytes(4, 127, 9, 0, lrux.F64, C.byref(out)) == lrux.EUNSUPPORTED
+    assert lib.lrux_pf_state_bytes(4, 128, 9, 0, lrux.F64, C.byref(out)) == lrux.EUNSUPPORTED
     assert lib.lrux_det_state_bytes(4, 32, 1, -1, lrux.F64, C.byref(out)) == lrux.EINVAL
     assert lib.lrux_det_state_bytes(4, 32, 1, 0, 7, C.byref(out)) == lrux.EINVAL
     assert lib.lrux_det_state_bytes(4, 32, 1, 0, lrux.F64, None) == lrux.EINVAL

@@ -117,7 +117,8 @@ def test_det_large_row_paths(n, k, K, cplx, steps, kernel):
     """Immediate update / delayed append at rows >= 8 KB: each shape reaches the kernel named
     (selected by shape alone) and follows the oracle."""
     _run("det", 500 + n + k, 2, n, 2 * n, k, K, steps, cplx, walkers=[1],
-         scratch_every=steps - 1, acc_range=(0.0, 1.0), kernel={"update" if K == 0 else "append": kernel})
+         scratch_every=1 if n <= 1100 else steps - 1, acc_range=(0.0, 1.0),
+         kernel={"update" if K == 0 else "append": kernel})
 
 
 def test_det_tma_update_n4096_properties():
@@ -215,6 +216,21 @@ def test_pf_delayed_and_k8(n, k, K, cplx):
     """Pfaffian delayed kernels (pf_an / pf_y_colsum / pf_append / skew flush) above n = 50,
     and k = 8 (16 x 16 skew core), immediate and delayed."""
     _run("pf", 70 + n + k + K, 3, n, 2 * n, k, K, 20, cplx, walkers=[0, 2], scratch_every=1, forced=(k == 8))
+
+
+@pytest.mark.parametrize("n,k,steps", [(128, 9, 6), (256, 16, 4), (256, 33, 3), (512, 64, 3), (200, 24, 3)])
+def test_det_big_rank(n, k, steps):
+    """Ranks 8 < k <= 64: ratio = gather + R = N C on the tensor
+    pipe + Gauss-Jordan core, accept = row-dot pass + the k-column fold.  Every proposal applied
+    (a Metropolis chain accepts almost no rank-16+ move on these inputs); n = 200: ragged tiles."""
+    _run("det", 3000 + n + k, 3, n, 2 * n, k, 0, steps, forced=True,
+         kernel={"ratio": "rowdot_dmma_kernel", "update": "flush_dmma_kernel"})
+
+
+def test_det_big_rank_metropolis_and_mixed_ranks():
+    """One handle with kmax = 16 serving a Metropolis chain of rank-12 moves: rejected walkers stay
+    untouched, accepted ones follow the oracle."""
+    _run("det", 3111, 8, 96, 192, 12, 0, 30, kmax=16, acc_range=(0.0, 1.0))
 
 
 @pytest.mark.parametrize("kind,n,k,K", [("det", 64, 2, 0), ("det", 64, 2, 4), ("pf", 64, 1, 0), ("pf", 50, 2, 3)])
