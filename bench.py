@@ -58,6 +58,8 @@ def parse_args(argv=None):
                     help="forced: every proposal is applied (ncu captures, Fig. 2-style runs)")
     ap.add_argument("--delay", type=int, default=-1,
                     help="override the workload's delay depth K (headline variant only)")
+    ap.add_argument("--no-graph", action="store_true",
+                    help="time stream-launched steps instead of CUDA-graph replays")
     ap.add_argument("--no-extras", action="store_true",
                     help="skip forced-accept / delayed variants / DGEMM yardstick")
     return ap.parse_args(argv)
@@ -181,23 +183,33 @@ def make_chain(wk, K, seed, orb, occ, unocc, w0, device):
                     walkers=_MASTERS[K].clone())
 
 
-def timed_run(ch, warmup, steps, forced=False, sampler=None):
+def timed_run(ch, warmup, steps, forced=False, sampler=None, graph=True):
     """W untimed + K timed steps; device time by CUDA events on the launching stream,
-    barrier + synchronize on both sides.  Returns a dict of raw measurements."""
+    barrier + synchronize on both sides.  ``graph``: the timed steps are K replays of ONE
+    step captured into a CUDA graph (the step counter lives in device memory: mc.Chain.capture);
+    the warm-up steps and the profiled pass are plain stream launches of the same sequence.
+    A second pass of K more steps, stream-launched with the library's per-class CUDA events
+    switched on, gives the per-kernel durations the roofline figures use (events between
+    the launches of a replayed graph would only keep their last recording).
+    Returns a dict of raw measurements."""
     import torch
     from paper_2602_05255_b200 import lrux, shard
 
     for t in range(warmup):
         ch.step(t, forced)
     torch.cuda.synchronize()
+    launch = "stream"
+    if graph:
+        try:
+            ch.capture(warmup, forced)
+            launch = "cuda_graph"
+        except Exception as e:        # capture refused: fall back to stream launches, say so
+            launch = "stream (graph capture failed: %s)" % type(e).__name__
+    torch.cuda.synchronize()
     shard.barrier()
     torch.cuda.synchronize()
     acc0 = int(ch.naccept.item())
     l0 = ch.launches()
-    f0 = ch.walkers.flush_count() if ch.K > 0 else (0, 0)
-    ch.walkers.profile_enable(True)
-    for c in range(5):
-        ch.walkers.profile_read(c)
     if sampler:
         sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -205,8 +217,12 @@ def timed_run(ch, warmup, steps, forced=False, sampler=None):
         sampler.mark_begin()
         torch.cuda.profiler.start()   # ncu --profile-from-start off sees the timed region only
     e0.record()
-    for t in range(steps):
-        ch.step(warmup + t, forced)
+    if launch == "cuda_graph":
+        for t in range(steps):
+            ch.replay()
+    else:
+        for t in range(steps):
+            ch.step(warmup + t, forced)
     e1.record()
     torch.cuda.synchronize()
     if sampler:
@@ -215,6 +231,21 @@ def timed_run(ch, warmup, steps, forced=False, sampler=None):
     torch.cuda.synchronize()
     clocks = sampler.stop() if sampler else None
     ms = e0.elapsed_time(e1)
+    accepted = int(ch.naccept.item()) - acc0
+    launches = steps * ch.launches_per_replay if launch == "cuda_graph" else ch.launches() - l0
+
+    # ---- profiled pass: the next `steps` steps of the same chain, per-class events on
+    acc1 = int(ch.naccept.item())
+    f0 = ch.walkers.flush_count() if ch.K > 0 else (0, 0)
+    ch.walkers.profile_enable(True)
+    for c in range(5):
+        ch.walkers.profile_read(c)
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record()
+    for t in range(steps):
+        ch.step(warmup + steps + t, forced)
+    p1.record()
+    torch.cuda.synchronize()
     prof = {}
     for name, c in (("ratio", lrux.PROF_RATIO), ("update", lrux.PROF_UPDATE),
                     ("append", lrux.PROF_APPEND), ("flush", lrux.PROF_FLUSH),
@@ -226,7 +257,9 @@ def timed_run(ch, warmup, steps, forced=False, sampler=None):
     kernels = {name: ch.walkers.kernel_name(c) for name, c in
                (("ratio", lrux.PROF_RATIO), ("update", lrux.PROF_UPDATE), ("append", lrux.PROF_APPEND),
                 ("flush", lrux.PROF_FLUSH), ("ypass", lrux.PROF_YPASS))}
-    return {"ms": ms, "accepted": int(ch.naccept.item()) - acc0, "launches": ch.launches() - l0,
+    return {"ms": ms, "accepted_timed": accepted, "launches": launches, "launch": launch,
+            # the profiled pass: what the per-kernel roofline figures are computed from
+            "accepted": int(ch.naccept.item()) - acc1, "ms_profiled_pass": p0.elapsed_time(p1),
             "flushes": f1[0] - f0[0], "flush_cols": f1[1] - f0[1],
             "prof": prof, "clocks": clocks, "kernels": kernels}
 
@@ -522,7 +555,8 @@ def c4_leg(device, peak, peak_src, dgemm, rank, w0_of):
     torch.cuda.empty_cache()
     return {"workload": wk["desc"], "steps": steps, "warmup": warm, "init_s": init_s,
             "walker_updates_per_s": wk["W"] * steps / (run["ms"] * 1e-3), "ms_per_step": run["ms"] / steps,
-            "accept_frac": run["accepted"] / float(wk["W"] * steps), "info_nonzero_walkers": bad,
+            "accept_frac": run["accepted_timed"] / float(wk["W"] * steps), "info_nonzero_walkers": bad,
+            "launch": run["launch"],
             "gpu_launches": run["launches"], "flushes": run["flushes"], "flush_cols": run["flush_cols"],
             "prof_ms": {k: v["ms"] for k, v in run["prof"].items()},
             "roofline_flush": roofline_flush(wk, K, run, peak, peak_src, dgemm),
@@ -585,11 +619,11 @@ def main(argv=None):
     K0 = wk["Ks"][0]
     ch = make_chain(wk, K0, seed, orb, occ, unocc, w0, device)
     run = timed_run(ch, warmup, steps, forced=args.mode == "forced",
-                    sampler=ClockSampler(local_rank) if rank == 0 else None)
+                    sampler=ClockSampler(local_rank) if rank == 0 else None, graph=not args.no_graph)
     info_bad = int((ch.walkers.info != 0).sum().item())
     del ch
     ms_max, = shard.reduce_scalars([run["ms"]], "max", device)
-    acc_sum, launches = shard.reduce_scalars([run["accepted"], run["launches"]], "sum", device)
+    acc_sum, launches = shard.reduce_scalars([run["accepted_timed"], run["launches"]], "sum", device)
     value = W * world * steps / (ms_max * 1e-3)
 
     extras = {}
@@ -604,7 +638,7 @@ def main(argv=None):
         del chf
         extras["forced_accept"] = {
             "K": K0, "steps": fsteps, "walker_updates_per_s": W * fsteps / (rf["ms"] * 1e-3),
-            "accept_frac": rf["accepted"] / float(W * fsteps),
+            "accept_frac": rf["accepted_timed"] / float(W * fsteps),
             "roofline": roofline_update(wk, rf, peak, peak_src, dgemm) if K0 == 0 else None,
             "prof_ms": {k: v["ms"] for k, v in rf["prof"].items()}}
         for K in wk["Ks"][1:]:
@@ -613,7 +647,7 @@ def main(argv=None):
             del chk
             extras["K%d" % K] = {
                 "walker_updates_per_s": W * steps / (rk["ms"] * 1e-3), "ms_per_step": rk["ms"] / steps,
-                "accept_frac": rk["accepted"] / float(W * steps),
+                "accept_frac": rk["accepted_timed"] / float(W * steps),
                 "prof_ms": {k: v["ms"] for k, v in rk["prof"].items()},
                 "roofline_flush": roofline_flush(wk, K, rk, peak, peak_src, dgemm)}
 
@@ -652,7 +686,9 @@ def main(argv=None):
            "scaling": "weak", "vs_baseline": None, "dtype": "c128" if wk["cplx"] else "f64",
            "data": "synthetic",
            "config": {"workload": wk["desc"], "walkers_per_gpu": W, "n": wk["n"], "M": wk["M"],
-                      "k": wk["k"], "K": K0, "mode": args.mode,
+                      "k": wk["k"], "K": K0, "mode": args.mode, "launch": run["launch"],
+                      "roofline_region": "second pass of the same number of steps, stream-launched, with the "
+                                         "library's per-class CUDA events (prof_ms, ms_profiled_pass)",
                       "l2": "inputs larger than L2: %.2f GiB of inverses per GPU, no flush needed"
                             % (W * wk["n"] ** 2 * (16 if wk["cplx"] else 8) / 2 ** 30)},
            "init_s": {("K%d" % K): v for K, v in INIT_SECONDS.items()},
@@ -661,6 +697,7 @@ def main(argv=None):
            "gpu_launches": int(launches), "info_nonzero_walkers": info_bad,
            "clocks": run["clocks"],
            "prof_ms": {k: v["ms"] for k, v in run["prof"].items()},
+           "ms_profiled_pass": run["ms_profiled_pass"],
            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": ee["h2d"],
                    "d2h_bytes_per_step": ee["d2h"], "steps": e2e_steps,
                    "decision_mismatches_vs_device_chain": ee["mismatch"]},

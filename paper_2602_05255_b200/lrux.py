@@ -49,9 +49,9 @@ SIGNATURES = {
     "lrux_profile_read": [_vp, _i32, C.POINTER(C.c_double), C.POINTER(_i64)],
     "lrux_destroy": [_vp],
     "lrux_status_string": [C.c_int],
-    "lruxh_det_propose": [_u64, _i64, _i64, _i64, _i32, _i32, _i32, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
-    "lruxh_pf_propose": [_u64, _i64, _i64, _i64, _i32, _i32, _i32, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
-    "lruxh_decide": [_u64, _i64, _i64, _i64, _i32, _i32, _i32, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
+    "lruxh_det_propose": [_u64, _i64, _i64, _i64, _i32, _i32, _i32, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
+    "lruxh_pf_propose": [_u64, _i64, _i64, _i64, _i32, _i32, _i32, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
+    "lruxh_decide": [_u64, _i64, _i64, _i64, _i32, _i32, _i32, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp],
 }
 _RESTYPE = {"lrux_status_string": C.c_char_p, "lrux_kernel_name": C.c_char_p}
 
@@ -253,27 +253,33 @@ class PfWalkers(_Walkers):
 
 
 # ---------------------------------------------------------------- harness
-def det_propose(seed, w0, step, Phi, occ, unocc, idx, upos, rows, stream=None):
+def _optr(t):
+    return None if t is None else _ptr(t)
+
+
+def det_propose(seed, w0, step, Phi, occ, unocc, idx, upos, rows, d_step=None, stream=None):
     W, M, n = Phi.shape
     k = idx.shape[1]
     _check(load_library().lruxh_det_propose(seed, w0, step, W, n, M, k, _dt(Phi.dtype), _ptr(Phi),
                                             _ptr(occ), _ptr(unocc), _ptr(idx), _ptr(upos),
-                                            _ptr(rows), _stream(stream)))
+                                            _ptr(rows), _optr(d_step), _stream(stream)))
 
 
-def pf_propose(seed, w0, step, F, occ, unocc, idx, upos, rows, stream=None):
+def pf_propose(seed, w0, step, F, occ, unocc, idx, upos, rows, d_step=None, stream=None):
     W, M, _ = F.shape
     n = occ.shape[1]
     k = idx.shape[1]
     _check(load_library().lruxh_pf_propose(seed, w0, step, W, n, M, k, _dt(F.dtype), _ptr(F),
                                            _ptr(occ), _ptr(unocc), _ptr(idx), _ptr(upos),
-                                           _ptr(rows), _stream(stream)))
+                                           _ptr(rows), _optr(d_step), _stream(stream)))
 
 
-def decide(seed, w0, step, ratio, idx, upos, occ, unocc, mask, naccept, stream=None):
+def decide(seed, w0, step, ratio, idx, upos, occ, unocc, mask, naccept, d_step=None, stream=None):
+    """d_step: int64[2] device tensor ([0] step, [1] scratch = 0) read instead of ``step`` and
+    advanced by one (CUDA-graph replay), or None."""
     W, n = occ.shape
     M = n + unocc.shape[1]
     k = idx.shape[1]
     _check(load_library().lruxh_decide(seed, w0, step, W, n, M, k, _dt(ratio.dtype), _ptr(ratio),
                                        _ptr(idx), _ptr(upos), _ptr(occ), _ptr(unocc), _ptr(mask),
-                                       _ptr(naccept), _stream(stream)))
+                                       _ptr(naccept), _optr(d_step), _stream(stream)))

@@ -57,20 +57,40 @@ class Chain:
         self.force_ratio = torch.full((W,), 2.0, dtype=dt, device=dev)
         self.harness_launches = 0
 
-    def propose(self, t):
+    def propose(self, t, d_step=None):
         fn = lrux.det_propose if self.kind == "det" else lrux.pf_propose
-        fn(self.seed, self.w0, t, self.orb, self.occ, self.unocc, self.idx, self.upos, self.rows)
+        fn(self.seed, self.w0, t, self.orb, self.occ, self.unocc, self.idx, self.upos, self.rows, d_step)
         self.harness_launches += 1
 
-    def step(self, t, forced=False):
+    def step(self, t, forced=False, d_step=None):
         """One Monte-Carlo step of every walker.  ``forced``: every proposal with a
         regular R is applied (what the paper's Fig. 2 times)."""
-        self.propose(t)
+        self.propose(t, d_step)
         self.walkers.ratio_(self.idx, self.rows)
         lrux.decide(self.seed, self.w0, t, self.force_ratio if forced else self.ratio, self.idx,
-                    self.upos, self.occ, self.unocc, self.mask, self.naccept)
+                    self.upos, self.occ, self.unocc, self.mask, self.naccept, d_step)
         self.harness_launches += 1
         self.walkers.accept(self.mask)
 
+    def capture(self, t_next, forced=False):
+        """Capture ONE step (propose -> ratio -> decide -> accept) into a CUDA graph whose step
+        number lives in device memory; ``replay()`` then runs step t_next, t_next + 1, ... with
+        a single host call each.  The launch sequence of a step depends on the shape only and no
+        call synchronises, so the replayed chain is the stream-launched chain, kernel for kernel.
+        Run at least one eager step first (kernel attributes are configured on first use)."""
+        self.d_step = torch.tensor([int(t_next), 0], dtype=torch.int64, device=self.occ.device)
+        l0 = self.launches()
+        self.graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(self.graph):
+            self.step(0, forced, self.d_step)
+        self.launches_per_replay = self.launches() - l0      # enqueued while capturing, run by every replay
+        self.replays = 0
+        return self.graph
+
+    def replay(self):
+        self.graph.replay()
+        self.replays += 1
+
     def launches(self):
+        """Kernel launches enqueued by stream calls (a captured step counts once, at capture)."""
         return self.walkers.launch_count() + self.harness_launches

@@ -39,7 +39,7 @@ def _walkers_for(kind, n, cplx, budget_bytes):
 
 
 def tune_delay(kind, n, k, cplx=False, W=None, depths=DEPTHS, steps=None, mode="metropolis", seed=20260205,
-               device=None, budget_bytes=8e9):
+               device=None, budget_bytes=3e10):
     """Measure walker-updates/s of the hot path at each delay depth in ``depths`` (0 = immediate
     updates) and return {"best": K, "table": [...], "heuristic": K_paper, ...}.
 

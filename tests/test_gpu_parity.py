@@ -263,6 +263,42 @@ def test_large_delay_coefficient_staging(kmax, K, cplx):
     _run("pf", 6 + K, 2, 64, 128, 2, min(K, 32), 12, cplx, kmax=kmax)
 
 
+@pytest.mark.parametrize("kind,n,k,K", [("det", 64, 2, 0), ("det", 96, 2, 4), ("pf", 64, 1, 0), ("pf", 200, 1, 0),
+                                        ("det", 1024, 8, 0)])
+def test_cuda_graph_replay_equals_stream_launches(kind, n, k, K):
+    """mc.Chain.capture: one step captured into a CUDA graph (device-side step counter) and
+    replayed gives, bit for bit, the chain that stream launches give -- ratios, decisions,
+    inverse, amplitude.  Includes the cluster launches (pf n=200, det n=1024 k=8 at n <= 1024: no
+    cluster; pf_cluster_k1) and the delayed path with its flush."""
+    from paper_2602_05255_b200 import mc
+
+    seed = 88 + n
+    orb, occ, unocc = pu.make_inputs(kind, seed, 6, n, 2 * n)
+    dev = "cuda"
+    mk = lambda: mc.Chain(kind, torch.as_tensor(orb, device=dev), torch.as_tensor(occ, device=dev),
+                          torch.as_tensor(unocc, device=dev), k=k, K=K, seed=seed)
+    a, b = mk(), mk()
+    T, pre = 24, 3
+    ra, ma = [], []
+    for t in range(T):
+        a.step(t)
+        ra.append(a.ratio.clone())
+        ma.append(a.mask.clone())
+    for t in range(pre):
+        b.step(t)
+    b.capture(pre)
+    for t in range(pre, T):
+        b.replay()
+        assert torch.equal(b.ratio, ra[t]) and torch.equal(b.mask, ma[t]), t
+    assert int(b.d_step[0].item()) == T and int(b.d_step[1].item()) == 0
+    assert torch.equal(a.walkers.get_inverse(), b.walkers.get_inverse())
+    assert torch.equal(a.occ, b.occ) and int(a.naccept.item()) == int(b.naccept.item())
+    pa, la = a.walkers.get_amplitude()
+    pb, lb = b.walkers.get_amplitude()
+    assert torch.equal(pa, pb) and torch.equal(la, lb)
+    assert b.launches_per_replay >= 5
+
+
 def test_attach_resumes_from_a_state_copy():
     """lrux_*_attach: a byte copy of the state buffer is a checkpoint; a chain resumed
     from it reproduces the original chain bit for bit (det with a half-full delay
