@@ -14,6 +14,10 @@
 #ifndef LRUX_DMMA_MIN_KT
 #define LRUX_DMMA_MIN_KT 4
 #endif
+// ... and from which real-valued delayed appends take the row-dot DMMA pass
+#ifndef LRUX_APPEND_ROWDOT_MIN_KT
+#define LRUX_APPEND_ROWDOT_MIN_KT 8
+#endif
 
 namespace lrux {
 
@@ -804,6 +808,57 @@ det_append_dmma_kernel(State st, int k, int tiles, int rows_per_tile) {
   }
 }
 
+// Second half of the append as its own pass, for the tensor-pipe variant below: D = N A0^-1 -
+// I[P,:] is already in the pending area (pend_C, free once det_prep_kernel has copied a_tau
+// into the buffer).  b_tau^T = R^-1 (D - (N Abuf) Bbuf^T) -> Bbuf[fill .. fill+k)   (Eq. 15,
+// PAPER.md:194; reading 5b).  Work item = (accepted walker, 256 columns); thread per column.
+template <typename T, int KT>
+__global__ void __launch_bounds__(256) det_append_finish_kernel(State st, int k, int chunks) {
+  using S = Sc<T>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* NAs = (T*)smem_raw;   // [fill][KT]
+  __shared__ T Ri[KT * KT];
+  const int n = st.n, kmax = st.kmax, cap = st.cap;
+  const int tid = threadIdx.x;
+  const int count = st.counters[0];
+  for (int item = blockIdx.x; item < count * chunks; item += gridDim.x) {
+    const int w = st.list[item / chunks];
+    const int j = (item % chunks) * 256 + tid;
+    const int fill = st.fill[w];
+    __syncthreads();
+    const T* NA = (const T*)st.pend_Y + (size_t)w * kmax * cap;
+    for (int q = tid; q < fill * KT; q += 256)
+      NAs[q] = (q % KT) < k ? NA[(size_t)(q % KT) * cap + q / KT] : S::zero();
+    if (tid < KT * KT) {
+      const int a = tid / KT, b = tid % KT;
+      Ri[tid] = (a < k && b < k) ? ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + a * st.kc + b]
+                                 : S::zero();
+    }
+    __syncthreads();
+    if (j >= n) continue;
+    const T* D = (const T*)st.pend_C + (size_t)w * kmax * n;
+    T* Bb = (T*)st.Bbuf + (size_t)w * cap * n;
+    T m[KT];
+#pragma unroll
+    for (int b = 0; b < KT; ++b) m[b] = b < k ? D[(size_t)b * n + j] : S::zero();
+#pragma unroll 8
+    for (int s = 0; s < fill; ++s) {
+      const T bv = Bb[(size_t)s * n + j];
+#pragma unroll
+      for (int b = 0; b < KT; ++b) m[b] = S::fnma(NAs[s * KT + b], bv, m[b]);
+    }
+#pragma unroll
+    for (int a = 0; a < KT; ++a) {
+      if (a < k) {
+        T acc = S::zero();
+#pragma unroll
+        for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], m[b], acc);
+        Bb[(size_t)(fill + a) * n + j] = acc;
+      }
+    }
+  }
+}
+
 // post: fill += k for accepted walkers; walkers whose depth reached K (or whose
 // buffer cannot take another kmax columns) go to the flush list (reading 9).
 __global__ void post_kernel(State st, int k) {
@@ -949,6 +1004,32 @@ static int launch_append_kt(const State& st, int k, Ctx& cx, cudaStream_t s) {
     const int groups = (st.cap + 8 * kPrepRows - 1) / (8 * kPrepRows);
     const int grid = persistent_grid(cx.num_sms, 8, (int64_t)st.W * groups);
     det_prep_kernel<T, KT><<<grid, 256, 0, s>>>(st, k, groups); ++nl;
+  }
+  if constexpr (sizeof(T) == 8 && KT >= LRUX_APPEND_ROWDOT_MIN_KT) {
+    // real data, k >= 5: the k dot products per row on the FP64 tensor pipe (one read-only pass,
+    // lrux_rowdot.cu), then the buffer terms and R^-1 in a pass over the k x n result (measured
+    // at n = 1024, K = 32: k = 8 0.46 of HBM against 0.40 for the register-row pass, k = 4
+    // 0.63 against 0.67 -- so k <= 4 stays on the register-row pass)
+    if ((n & 1) == 0) {
+      RowdotArgs A{};
+      A.X = (const double*)st.Ti;      A.x_stride = (size_t)n * n;          A.rows = n;  A.ldx = n;
+      A.N = (const double*)st.pend_N;  A.n_stride = (size_t)st.kmax * n;   A.ldn = n;
+      A.n = n;  A.k = k;
+      A.out = (double*)st.pend_C;      A.o_stride = (size_t)st.kmax * n;   A.ldo = n;
+      A.list = st.list;  A.count = st.counters;  A.W = st.W;
+      A.idx = st.pend_idx;  A.idx_stride = st.kmax;
+      const int r = launch_rowdot_dmma(A, cx, s);
+      if (r < 0) return -1;
+      if (r > 0) {
+        const int chunks = (n + 255) / 256;
+        const size_t smf = (size_t)st.cap * KT * sizeof(T);
+        auto kf = det_append_finish_kernel<T, KT>;
+        if (cx.configure((const void*)kf, 256, smf) < 0) return -1;
+        kf<<<persistent_grid(cx.num_sms, 8, (int64_t)st.W * chunks), 256, smf, s>>>(st, k, chunks);
+        cx.name(LRUX_PROF_APPEND, "det_prep_kernel+rowdot_dmma_kernel+det_append_finish_kernel");
+        return nl + r + 1;
+      }
+    }
   }
   const int rows_per_tile = n >= 1024 ? 128 : 64;   // must divide the block size (256)
   const int tiles = (n + rows_per_tile - 1) / rows_per_tile;

@@ -7,10 +7,10 @@
 // per flushed walker.  sm_100a has no tcgen05 kind for f64; the FP64 tensor path is the
 // warp-level DMMA (mma.sync.m8n8k4.f64 -> SASS DMMA.8x8x4), fed from shared memory.
 //
-// Work item = (walker on the flush list, output tile); persistent grid, one CTA of 8
-// warps per SM.  float64: 128 x 128 tiles, warp tile 32 x 64 (4 x 8 MMA tiles, 12 fragment
-// loads per 32 DMMAs); complex128: 64 x 128 tiles, warp tile 16 x 64, one complex MMA = 4
-// real DMMAs on (re, im) pairs read with ONE 16-byte fragment load each -- the buffers stay
+// Work item = (walker on the flush list, output tile); persistent grid, one CTA per SM.
+// float64: 128 x 128 tiles, 8 warps, warp tile 32 x 64 (4 x 8 MMA tiles, 12 fragment loads per
+// 32 DMMAs); complex128: 64 x 64 tiles, 16 warps, warp tile 16 x 16, one complex MMA = 4 real
+// DMMAs on (re, im) pairs read with ONE 16-byte fragment load each -- the buffers stay
 // interleaved, nothing is de-interleaved while staging.
 //
 // Both buffer panels move global -> shared with 16-byte cp.async (LDGSTS) through a ring of
@@ -52,15 +52,23 @@ __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
+// Tile configurations (warps per CTA as WR x WC over the output tile).  Measured on B200
+// (profiles/r02_flush_variants.md): float64 128 x 128 with 8 warps (warp tile 32 x 64) gives
+// 0.77 of cuBLAS DGEMM at K k = 256 against 0.73 with 16 warps; complex128 64 x 64 with 16 warps
+// (warp tile 16 x 16) gives 0.62 / 0.68 (Metropolis / all walkers at once) on configs[3]
+// against 0.58 / 0.69 for 64 x 128 with 8 warps -- with ~5 walkers folding per step the
+// smaller tile wastes less of the last wave.
 template <typename T>
 struct FlushCfg;
 template <>
 struct FlushCfg<double> {   // 128 x 128, warps 4 x 2, warp tile 32 x 64
+  static constexpr int WR = 4, WC = 2;
   static constexpr int BM = 128, BN = 128, MT = 4, NT = 8, KC = 16, NS = 4, LDB = 132, LDA = 132;
 };
 template <>
-struct FlushCfg<cplx> {     // 64 x 128, warps 4 x 2, warp tile 16 x 64
-  static constexpr int BM = 64, BN = 128, MT = 2, NT = 8, KC = 8, NS = 4, LDB = 66, LDA = 130;
+struct FlushCfg<cplx> {     // 64 x 64, warps 4 x 4, warp tile 16 x 16
+  static constexpr int WR = 4, WC = 4;
+  static constexpr int BM = 64, BN = 64, MT = 2, NT = 2, KC = 16, NS = 4, LDB = 66, LDA = 66;
 };
 
 struct FlushItem {
@@ -69,9 +77,11 @@ struct FlushItem {
 
 // V16: rows of the buffers are 16-byte aligned (always for complex; real: n even)
 template <typename T, bool SKEW, bool V16>
-__global__ void __launch_bounds__(256, 1) flush_dmma_kernel(State st, int tr, int tc, int tiles) {
+__global__ void __launch_bounds__(FlushCfg<T>::WR * FlushCfg<T>::WC * 32, 1)
+flush_dmma_kernel(State st, int tr, int tc, int tiles) {
   using S = Sc<T>;
   using Cfg = FlushCfg<T>;
+  constexpr int NTHR = Cfg::WR * Cfg::WC * 32;
   constexpr int BM = Cfg::BM, BN = Cfg::BN, MT = Cfg::MT, NT = Cfg::NT, KC = Cfg::KC, NS = Cfg::NS;
   constexpr int LDB = Cfg::LDB, LDA = Cfg::LDA;
   constexpr bool CX = sizeof(T) == 16;
@@ -80,7 +90,7 @@ __global__ void __launch_bounds__(256, 1) flush_dmma_kernel(State st, int tr, in
   T* ring = (T*)smem_raw;                          // [NS][ Bs[KC][LDB] | As[KC][LDA] ]
   const int n = st.n, cap = st.cap;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int wr = warp >> 1, wc = warp & 1;         // warp position in the 4 x 2 grid
+  const int wr = warp / Cfg::WC, wc = warp % Cfg::WC;   // warp position in the WR x WC grid
   const int lm = lane >> 2, lk = lane & 3;         // fragment row / k index
   const int count = st.counters[1];
   const int64_t total = (int64_t)count * tiles;
@@ -123,8 +133,8 @@ __global__ void __launch_bounds__(256, 1) flush_dmma_kernel(State st, int tr, in
     constexpr int EPV = V16 ? (CX ? 1 : 2) : 1;            // elements per copy
     constexpr int VB = BM / EPV, VA = BN / EPV;            // copies per row
 #pragma unroll
-    for (int u = 0; u < (KC * VB + 255) / 256; ++u) {
-      const int qd = tid + 256 * u;
+    for (int u = 0; u < (KC * VB + NTHR - 1) / NTHR; ++u) {
+      const int qd = tid + NTHR * u;
       if (qd < KC * VB) {
         const int kk = qd / VB, c = (qd % VB) * EPV;
         const bool ok = s0 + kk < it.fill && it.r0 + c < n;
@@ -134,8 +144,8 @@ __global__ void __launch_bounds__(256, 1) flush_dmma_kernel(State st, int tr, in
       }
     }
 #pragma unroll
-    for (int u = 0; u < (KC * VA + 255) / 256; ++u) {
-      const int qd = tid + 256 * u;
+    for (int u = 0; u < (KC * VA + NTHR - 1) / NTHR; ++u) {
+      const int qd = tid + NTHR * u;
       if (qd < KC * VA) {
         const int kk = qd / VA, c = (qd % VA) * EPV;
         const bool ok = s0 + kk < it.fill && it.c0 + c < n;
@@ -227,14 +237,23 @@ __global__ void __launch_bounds__(256, 1) flush_dmma_kernel(State st, int tr, in
           }
 #pragma unroll
           for (int nt = 0; nt < NT; ++nt) af[nt] = ((const double2*)As)[(k4 + lk) * LDA + wc * (NT * 8) + nt * 8 + lm];
+          // (br + i bi)(ar + i ai) = (br ar - bi ai) + i (br ai + bi ar): four passes over the
+          // MT x NT tiles, so that the two DMMAs into one accumulator are 2 MT NT instructions apart
+          double nby[MT];
+#pragma unroll
+          for (int mt = 0; mt < MT; ++mt) nby[mt] = -bf[mt].y;
 #pragma unroll
           for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt) {
-              // (br + i bi)(ar + i ai) = (br ar - bi ai) + i (br ai + bi ar)
               dmma884(acc[0][mt][nt][0], acc[0][mt][nt][1], bf[mt].x, af[nt].x);
-              dmma884(acc[0][mt][nt][0], acc[0][mt][nt][1], -bf[mt].y, af[nt].y);
               dmma884(acc[CX ? 1 : 0][mt][nt][0], acc[CX ? 1 : 0][mt][nt][1], bf[mt].x, af[nt].y);
+            }
+#pragma unroll
+          for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+              dmma884(acc[0][mt][nt][0], acc[0][mt][nt][1], nby[mt], af[nt].y);
               dmma884(acc[CX ? 1 : 0][mt][nt][0], acc[CX ? 1 : 0][mt][nt][1], bf[mt].y, af[nt].x);
             }
         }
@@ -284,12 +303,13 @@ static int launch_flush_v(const State& st, Ctx& cx, cudaStream_t s) {
   }
   const size_t smem = (size_t)Cfg::NS * Cfg::KC * (Cfg::LDB + Cfg::LDA) * sizeof(T);
   auto kern = flush_dmma_kernel<T, SKEW, V16>;
-  const int occ = cx.configure((const void*)kern, 256, smem);
+  constexpr int NTHR = Cfg::WR * Cfg::WC * 32;
+  const int occ = cx.configure((const void*)kern, NTHR, smem);
   if (occ < 0) return -1;
   cx.name(LRUX_PROF_FLUSH, "flush_dmma_kernel");
   int64_t grid = (int64_t)cx.num_sms * occ;
   if (grid > st.W * tiles) grid = st.W * tiles;
-  kern<<<(unsigned)grid, 256, smem, s>>>(st, tr, tc, (int)tiles);
+  kern<<<(unsigned)grid, NTHR, smem, s>>>(st, tr, tc, (int)tiles);
   return 1;
 }
 

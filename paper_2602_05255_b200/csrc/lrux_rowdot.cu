@@ -125,10 +125,11 @@ __global__ void __launch_bounds__(256, 1) rowdot_dmma_kernel(RowdotArgs A) {
 #pragma unroll
         for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
-          for (int nt = 0; nt < NT; ++nt) {
-            dmma884r(acc[mt][nt][0], acc[mt][nt][1], af[mt].x, bf[nt].x);
-            dmma884r(acc[mt][nt][0], acc[mt][nt][1], af[mt].y, bf[nt].y);
-          }
+          for (int nt = 0; nt < NT; ++nt) dmma884r(acc[mt][nt][0], acc[mt][nt][1], af[mt].x, bf[nt].x);
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt) dmma884r(acc[mt][nt][0], acc[mt][nt][1], af[mt].y, bf[nt].y);
       }
     }
     // accumulator of tile (mt, nt): row j = .. + r8 of X, columns a = nt*8 + 2q, +1 of N

@@ -202,12 +202,21 @@ def test_flush_multichunk(kind, n, k, K, cplx):
     assert st["max_inv_rel"] < max(1e-9, 50 * st["e_oracle"])
 
 
-@pytest.mark.parametrize("n,k,K", [(512, 4, 8), (512, 8, 32), (1024, 4, 32), (1024, 8, 8)])
-def test_det_real_append_large_n(n, k, K):
-    """Real-valued delayed append (det_prep_kernel + det_append_kernel) at the sizes of the
-    configs[4] sweep; forced accept so that buffers fill and flush."""
+@pytest.mark.parametrize("n,k,K,kernel", [
+    (512, 8, 32, "rowdot_dmma_kernel+det_append_finish_kernel"),    # k >= 5: dot products on the tensor pipe
+    (1024, 8, 8, "rowdot_dmma_kernel+det_append_finish_kernel"),
+    (300, 5, 5, "rowdot_dmma_kernel+det_append_finish_kernel"),     # ragged tiles and chunks
+    (512, 4, 8, "det_prep_kernel+det_append_kernel"),               # k <= 4: register-row pass
+    (1024, 4, 32, "det_prep_kernel+det_append_kernel"),
+    (512, 2, 8, "det_prep_kernel+det_append_kernel"),               # k <= 2: register-row pass
+    (1024, 1, 32, "det_prep_kernel+det_append_kernel"),
+    (301, 4, 4, "det_prep_kernel+det_append_kernel"),               # odd n: rows not 16-byte aligned
+])
+def test_det_real_append_large_n(n, k, K, kernel):
+    """Real-valued delayed append at the sizes of the configs[4] sweep, both variants; forced
+    accept so that buffers fill and flush."""
     _run("det", 40 + n + k + K, 3, n, 2 * n, k, K, min(K, 10) + 3, walkers=[0, 2], scratch_every=1,
-         forced=True, kernel={"append": "det_append_kernel"})
+         forced=True, kernel={"append": kernel})
 
 
 @pytest.mark.parametrize("n,k,K,cplx", [(128, 1, 4, False), (512, 2, 8, False), (512, 1, 4, False),
