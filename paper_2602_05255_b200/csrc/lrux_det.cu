@@ -15,6 +15,10 @@
 #define LRUX_DMMA_MIN_KT 4
 #endif
 // ... and from which real-valued delayed appends take the row-dot DMMA pass
+// rows of A0^-1 per work item of the register-row / complex-DMMA append
+#ifndef LRUX_APPEND_TILE_ROWS
+#define LRUX_APPEND_TILE_ROWS 128
+#endif
 #ifndef LRUX_APPEND_ROWDOT_MIN_KT
 #define LRUX_APPEND_ROWDOT_MIN_KT 8
 #endif
@@ -638,12 +642,18 @@ det_append_kernel(State st, int k, int tiles, int rows_per_tile, int n_in_smem) 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
   const int count = st.counters[0];
   const int nvec = n / VEC;
-  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
+  // each CTA takes a CONTIGUOUS range of (walker, tile) items: N, R^-1 and P are staged once per
+  // walker, not once per tile, so that small tiles (an even last wave) cost nothing extra
+  const int total = count * tiles;
+  const int first = (int)((int64_t)total * blockIdx.x / gridDim.x), last = (int)((int64_t)total * (blockIdx.x + 1) / gridDim.x);
+  int cur_w = -1;
+  for (int item = first; item < last; ++item) {
     const int w = st.list[item / tiles];
     const int tile = item % tiles;
     const int fill = st.fill[w];
     __syncthreads();
-    {
+    if (w != cur_w) {
+      cur_w = w;
       const V* gN = (const V*)((const T*)st.pend_N + (size_t)w * kmax * n);
       if (n_in_smem)
         for (int q = tid; q < k * nvec; q += blockDim.x) ((V*)Ns)[q] = gN[q];
@@ -723,7 +733,8 @@ __device__ __forceinline__ void dmma884_acc(double& d0, double& d1, double a, do
                : "d"(a), "d"(b));
 }
 
-template <int KT>
+// MT = 8-row MMA tiles per warp and pass: 2 with 128-row work items, 1 with 64-row items.
+template <int KT, int MT>
 __global__ void __launch_bounds__(256, 2)
 det_append_dmma_kernel(State st, int k, int tiles, int rows_per_tile) {
   using T = cplx;
@@ -738,12 +749,17 @@ det_append_dmma_kernel(State st, int k, int tiles, int rows_per_tile) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
   const int r8 = lane >> 2, kk = lane & 3;       // A: (row, column) of the lane; B: (column kk, N-column r8)
   const int count = st.counters[0];
-  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
+  // contiguous item ranges per CTA: [Re N | Im N] is staged once per walker (see det_append_kernel)
+  const int total = count * tiles;
+  const int first = (int)((int64_t)total * blockIdx.x / gridDim.x), last = (int)((int64_t)total * (blockIdx.x + 1) / gridDim.x);
+  int cur_w = -1;
+  for (int item = first; item < last; ++item) {
     const int w = st.list[item / tiles];
     const int tile = item % tiles;
     const int fill = st.fill[w];
     __syncthreads();
-    {
+    if (w != cur_w) {
+      cur_w = w;
       const T* gN = (const T*)st.pend_N + (size_t)w * kmax * n;
       for (int q = tid; q < 4 * n; q += blockDim.x) {
         const int a = q / n, i = q % n;
@@ -761,10 +777,10 @@ det_append_dmma_kernel(State st, int k, int tiles, int rows_per_tile) {
     __syncthreads();
     const T* Tw = (const T*)st.Ti + (size_t)w * n * n;
     const int j_beg = tile * rows_per_tile, j_end = min(n, j_beg + rows_per_tile);
-    for (int j0 = j_beg + warp * 16; j0 < j_end; j0 += nw * 16) {
+    for (int j0 = j_beg + warp * (8 * MT); j0 < j_end; j0 += nw * (8 * MT)) {
       double acc[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
       const T* row0 = Tw + (size_t)min(j0 + r8, j_end - 1) * n + kk;        // rows past the tile: clamped, discarded
-      const T* row1 = Tw + (size_t)min(j0 + 8 + r8, j_end - 1) * n + kk;
+      const T* row1 = Tw + (size_t)min(j0 + 8 * (MT - 1) + r8, j_end - 1) * n + kk;
       const double* bp = Bs + kk * 8 + r8;
       const double* bq = Bs + kk * 8 + (r8 ^ 4);
       const bool lo = r8 < 4;
@@ -774,7 +790,7 @@ det_append_dmma_kernel(State st, int k, int tiles, int rows_per_tile) {
         for (int u = 0; u < UN; ++u) {
           const bool in = i0 + 4 * u < n;
           x0[u] = in ? row0[i0 + 4 * u] : S::zero();
-          x1[u] = in ? row1[i0 + 4 * u] : S::zero();
+          if (MT == 2) x1[u] = in ? row1[i0 + 4 * u] : S::zero();
         }
 #pragma unroll
         for (int u = 0; u < UN; ++u) {
@@ -784,14 +800,16 @@ det_append_dmma_kernel(State st, int k, int tiles, int rows_per_tile) {
             const double bm = lo ? -b2 : b2;          // B' = [-Im N | Re N]
             dmma884_acc(acc[0][0], acc[0][1], x0[u].re, b);
             dmma884_acc(acc[0][0], acc[0][1], x0[u].im, bm);
-            dmma884_acc(acc[1][0], acc[1][1], x1[u].re, b);
-            dmma884_acc(acc[1][0], acc[1][1], x1[u].im, bm);
+            if (MT == 2) {
+              dmma884_acc(acc[1][0], acc[1][1], x1[u].re, b);
+              dmma884_acc(acc[1][0], acc[1][1], x1[u].im, bm);
+            }
           }
         }
       }
       // D fragment: row r8, columns 2*kk, 2*kk+1 of [Re W | Im W]
 #pragma unroll
-      for (int mt = 0; mt < 2; ++mt) {
+      for (int mt = 0; mt < MT; ++mt) {
         const int j = j0 + 8 * mt + r8;
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
@@ -1005,7 +1023,8 @@ static int launch_append_kt(const State& st, int k, Ctx& cx, cudaStream_t s) {
     const int grid = persistent_grid(cx.num_sms, 8, (int64_t)st.W * groups);
     det_prep_kernel<T, KT><<<grid, 256, 0, s>>>(st, k, groups); ++nl;
   }
-  if constexpr (sizeof(T) == 8 && KT >= LRUX_APPEND_ROWDOT_MIN_KT) {
+  // (... and whenever N does not fit beside the register-row pass in shared memory: k n e > 96 KB)
+  if (sizeof(T) == 8 && (KT >= LRUX_APPEND_ROWDOT_MIN_KT || (size_t)k * n * sizeof(T) > 96 * 1024)) {
     // real data, k >= 5: the k dot products per row on the FP64 tensor pipe (one read-only pass,
     // lrux_rowdot.cu), then the buffer terms and R^-1 in a pass over the k x n result (measured
     // at n = 1024, K = 32: k = 8 0.46 of HBM against 0.40 for the register-row pass, k = 4
@@ -1031,15 +1050,15 @@ static int launch_append_kt(const State& st, int k, Ctx& cx, cudaStream_t s) {
       }
     }
   }
-  const int rows_per_tile = n >= 1024 ? 128 : 64;   // must divide the block size (256)
+  const int rows_per_tile = LRUX_APPEND_TILE_ROWS;   // must divide the block size (256)
   const int tiles = (n + rows_per_tile - 1) / rows_per_tile;
   const int n_in_smem = (size_t)k * n * sizeof(T) <= 96 * 1024;
   const size_t smem = ((n_in_smem ? (size_t)k * n : 0) + 4 * (size_t)KT * rows_per_tile) * sizeof(T);
   if constexpr (sizeof(T) == 16 && KT <= 4) {
     // complex data, k <= 4, 128-row tiles: the dot products on the FP64 tensor pipe
     const size_t smd = (size_t)n * 64 + 4 * (size_t)KT * rows_per_tile * sizeof(T);
-    if (n % 4 == 0 && rows_per_tile == 128 && smd <= 100 * 1024) {
-      auto kd = det_append_dmma_kernel<KT>;
+    if (n % 4 == 0 && n >= 1024 && smd <= 100 * 1024) {
+      auto kd = rows_per_tile >= 128 ? det_append_dmma_kernel<KT, 2> : det_append_dmma_kernel<KT, 1>;
       const int occd = cx.configure((const void*)kd, 256, smd);
       if (occd < 0) return -1;
       kd<<<persistent_grid(cx.num_sms, occd, (int64_t)st.W * tiles), 256, smd, s>>>(st, k, tiles, rows_per_tile);

@@ -216,6 +216,7 @@ def orbital_matrices_torch(seed, w0, W, M, n, var, device, complex_=False, chunk
     out = torch.empty((W, M, n), dtype=torch.complex128 if complex_ else torch.float64, device=device)
     cnt = torch.arange(M * n, dtype=torch.int64, device=device)
     s = float(np.sqrt(var))
+    chunk = max(1, min(chunk, (1 << 27) // (M * n)))      # bound the temporaries
     for c0 in range(0, W, chunk):
         c1 = min(W, c0 + chunk)
         w = torch.arange(w0 + c0, w0 + c1, dtype=torch.int64, device=device)[:, None]
@@ -235,6 +236,7 @@ def pairing_matrices_torch(seed, w0, W, M, var, device, chunk=64):
     out = torch.empty((W, M, M), dtype=torch.float64, device=device)
     cnt = torch.arange(M * M, dtype=torch.int64, device=device)
     s = float(np.sqrt(var))
+    chunk = max(1, min(chunk, (1 << 27) // (M * M)))      # bound the temporaries (~10 arrays of chunk*M*M*8 B)
     for c0 in range(0, W, chunk):
         c1 = min(W, c0 + chunk)
         w = torch.arange(w0 + c0, w0 + c1, dtype=torch.int64, device=device)[:, None]
