@@ -115,7 +115,9 @@ class _Walkers:
 
     kind = "det"
 
-    def __init__(self, A0, kmax=1, K=0, stream=None):
+    def __init__(self, A0, kmax=1, K=0, stream=None, guard=0):
+        """``guard`` > 0 (tests): that many bytes of 0xA5 before and after the state buffer,
+        checked by ``guards_intact()`` -- an out-of-bounds write detector that needs no tool."""
         lib = load_library()
         if not A0.is_cuda:
             raise ValueError("A0 must be a CUDA tensor (no CPU path)")
@@ -123,9 +125,14 @@ class _Walkers:
         self.W, self.n = int(A0.shape[0]), int(A0.shape[1])
         self.kmax, self.K, self.dtype, self.device = int(kmax), int(K), A0.dtype, A0.device
         nbytes = state_bytes(self.kind, self.W, self.n, self.kmax, self.K, self.dtype)
-        self.state = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-        off = (-self.state.data_ptr()) % 256
+        self._guard = g = (int(guard) + 255) // 256 * 256
+        self.state = torch.empty(nbytes + 256 + 2 * g, dtype=torch.uint8, device=self.device)
+        off = (-self.state.data_ptr()) % 256 + g
         self._state_ptr = self.state.data_ptr() + off
+        self._nbytes = nbytes
+        if g:
+            self.state[:off].fill_(0xA5)
+            self.state[off + nbytes:].fill_(0xA5)
         self.info = torch.zeros(self.W, dtype=torch.int32, device=self.device)
         self.ratio = torch.empty(self.W, dtype=self.dtype, device=self.device)
         self._h = C.c_void_p()
@@ -138,6 +145,7 @@ class _Walkers:
         """Independent copy of these walkers: byte copy of the state buffer + lrux_*_attach
         (no re-initialisation).  No proposal may be pending."""
         new = object.__new__(type(self))
+        new._guard, new._nbytes = 0, getattr(self, "_nbytes", 0)
         for a in ("W", "n", "kmax", "K", "dtype", "device", "_lib"):
             setattr(new, a, getattr(self, a))
         nbytes = state_bytes(self.kind, self.W, self.n, self.kmax, self.K, self.dtype)
@@ -156,6 +164,15 @@ class _Walkers:
 
     def _fn(self, name):
         return getattr(self._lib, "lrux_%s_%s" % (self.kind, name))
+
+    def guards_intact(self):
+        """True when no byte of the guard zones around the state buffer has changed
+        (``guard=`` at construction); synchronises."""
+        if not self._guard:
+            return True
+        off = self._state_ptr - self.state.data_ptr()
+        lo, hi = self.state[:off], self.state[off + self._nbytes:]
+        return bool((lo == 0xA5).all().item()) and bool((hi == 0xA5).all().item())
 
     def ratio_(self, idx, rows, out=None, stream=None):
         """lrux_*_ratio: idx int32 [W][k], rows [W][k][n]; returns ratio [W]."""

@@ -17,7 +17,7 @@ class Chain:
     occ [W][n], unocc [W][M-n] int32 device tensors are updated in place.
     """
 
-    def __init__(self, kind, orbitals, occ, unocc, k, K=0, seed=0, w0=0, kmax=None, walkers=None):
+    def __init__(self, kind, orbitals, occ, unocc, k, K=0, seed=0, w0=0, kmax=None, walkers=None, guard=0):
         assert kind in ("det", "pf")
         self.kind, self.k, self.K, self.seed, self.w0 = kind, int(k), int(K), int(seed), int(w0)
         self.orb = orbitals.contiguous()
@@ -42,7 +42,7 @@ class Chain:
             else:
                 A0[c0:c1] = self.orb[ar[:, :, None], occl[:, :, None], occl[:, None, :]]
         cls = lrux.DetWalkers if kind == "det" else lrux.PfWalkers
-        self.walkers = cls(A0, kmax=self.k if kmax is None else kmax, K=self.K)
+        self.walkers = cls(A0, kmax=self.k if kmax is None else kmax, K=self.K, guard=guard)
         del A0
         self._buffers(W, n, dt, dev)
 

@@ -206,3 +206,42 @@ def test_refresh_rebuilds_inverse_and_amplitude(kind, dtype, K):
     inv = wk.get_inverse().cpu().numpy()
     assert wk.info.cpu().numpy().tolist() == [0] * W
     assert np.abs(A[1] @ inv[1] - np.eye(n)).max() < 1e-11
+
+
+_GUARD_SHAPES = [
+    # kind, n, k, K, cplx, forced : one per kernel family the dispatcher can pick
+    ("det", 33, 1, 0, False, False), ("det", 64, 2, 4, False, False), ("det", 96, 4, 8, True, False),
+    ("det", 130, 8, 0, False, True), ("det", 128, 8, 4, False, True), ("det", 256, 3, 0, False, True),
+    ("det", 192, 4, 0, True, True), ("det", 512, 1, 16, False, False), ("det", 1026, 4, 0, False, True),
+    ("det", 128, 16, 0, False, True), ("det", 64, 5, 3, False, True), ("det", 47, 2, 5, True, True),
+    ("pf", 32, 1, 0, False, False), ("pf", 64, 2, 4, False, True), ("pf", 130, 1, 8, False, False),
+    ("pf", 96, 4, 0, False, True),
+]
+
+
+@pytest.mark.parametrize("kind,n,k,K,cplx,forced", _GUARD_SHAPES)
+def test_no_write_outside_the_state_buffer(kind, n, k, K, cplx, forced):
+    """Stand-in for compute-sanitizer (closed on this pool, profiles/r02_sanitizer.md): 4 KiB of
+    guard bytes on both sides of the state buffer stay intact over a chain that fills and
+    flushes the delay buffer, and two runs from the same inputs are bit-identical (a race or a
+    read of uninitialised memory would show up as a difference)."""
+    import parity_util as pu
+    from paper_2602_05255_b200 import mc
+
+    W, M, seed, steps = 5, 2 * n, 77 + n, 3 * max(K, 1) + 6
+    orb, occ, unocc = pu.make_inputs(kind, seed, W, n, M, cplx)
+    out = []
+    for _ in range(2):
+        ch = mc.Chain(kind, _t(orb), _t(occ), _t(unocc), k=k, K=K, seed=seed, guard=4096)
+        ratios = []
+        for t in range(steps):
+            ch.step(t, forced)
+            ratios.append(ch.ratio.clone())
+        inv = ch.walkers.get_inverse()
+        ph, la = ch.walkers.get_amplitude()
+        torch.cuda.synchronize()
+        assert ch.walkers.guards_intact()
+        out.append((torch.stack(ratios).cpu(), inv.cpu(), ph.cpu(), la.cpu(), ch.occ.cpu()))
+    for a, b in zip(*out):
+        assert torch.equal(torch.view_as_real(a) if a.is_complex() else a,
+                           torch.view_as_real(b) if b.is_complex() else b)
