@@ -8,7 +8,8 @@
  * Conventions
  *  - Every d_* pointer is DEVICE memory owned by the caller.  The library never
  *    allocates or frees device memory and holds no global state; the only host
- *    allocation is the small handle.  `d_state` and `d_info` must outlive the handle.
+ *    allocation is the small handle.  (One exception, stated at its declaration: the
+ *    fixed scratch array of lrux_det_ratio_noalloc.)  `d_state` and `d_info` must outlive the handle.
  *  - `stream` is a cudaStream_t passed as void*.  Every call is asynchronous and
  *    stream-ordered on it; no call synchronises the device.
  *  - Matrices are row-major.  LRUX_C128 data is interleaved (re,im) doubles at the
@@ -45,7 +46,8 @@ typedef enum {
                             n*(sizeof(elem)+4) > 200 KiB, i.e. n > 16384 f64 / 10240 c128; pf:
                             2*n*sizeof(elem) > 200 KiB), or a determinant delay depth with
                             K*kmax*kt*sizeof(elem) > 160 KiB (kt = kmax rounded up to 1,2,4,8) */
-  LRUX_ECUDA = 5        /* a CUDA launch failed */
+  LRUX_ECUDA = 5,       /* a CUDA launch failed */
+  LRUX_ELIMIT = 6       /* lrux_det_ratio_noalloc: problem larger than the fixed scratch array */
 } lrux_status_t;
 
 /* ---------------------------------------------------------------- determinant
@@ -205,6 +207,28 @@ lrux_status_t lrux_profile_read(lrux_handle_t h, int32_t cls, double* ms_total,
  * folded (k per determinant update, 2k per Pfaffian update).  d_out is DEVICE memory,
  * 2 x int64; stream-ordered copy.  bench.py uses it to count the flush flops exactly. */
 lrux_status_t lrux_get_flush_count(lrux_handle_t h, int64_t* d_out, void* stream);
+
+/* ---------------------------------------------------------------- allocation-free call */
+/* Rank-k determinant ratio for callers that cannot allocate (code under CUDA-graph capture,
+ * serving loops, harnesses that forbid cudaMalloc): no handle, no state buffer.
+ *     r_w = det(R_w),   R_w = N_w A_w^-1[:,P_w]     (Eq. 3-4 with one-hot v)
+ *   d_Ti    [W][n][n]  A_w^-T row-major (row j = column j of A_w^-1), the layout the handles keep
+ *   d_idx   [W][k]     int32 replaced rows P_w           d_rows [W][k][n]  the new rows N_w
+ *   d_ratio [W]        output
+ * All pointers are DEVICE memory owned by the caller; inputs are only read.  1 <= k <=
+ * LRUX_MAX_K_GENERAL.  An index outside [0,n) or a duplicate gives ratio NaN for that walker.
+ * The k x k cores R_w pass between the two kernels of the call through a fixed scratch array
+ * that lives in the library image (LRUX_NOALLOC_SCRATCH_BYTES of device memory on every GPU
+ * that loads the library, until the process exits): the call performs NO device or host
+ * allocation.  W*k*k*sizeof(elem) > LRUX_NOALLOC_SCRATCH_BYTES -> LRUX_ELIMIT, nothing done.
+ * Every call on a device shares that one array: calls whose kernels may overlap on the GPU
+ * (different streams, no dependency between them) RACE -- order them.  The array keeps the
+ * previous call's contents; every element a call reads it has written first, so nothing needs
+ * clearing.  Asynchronous, stream-ordered.  Errors: LRUX_EINVAL, LRUX_ELIMIT, LRUX_ECUDA. */
+#define LRUX_NOALLOC_SCRATCH_BYTES (1u << 20)
+lrux_status_t lrux_det_ratio_noalloc(int64_t W, int32_t n, int32_t k, lrux_dtype_t dtype,
+                                     const void* d_Ti, const int32_t* d_idx, const void* d_rows,
+                                     void* d_ratio, void* stream);
 
 /* ---------------------------------------------------------------- common */
 /* Number of kernel launches the library has enqueued through this handle so far

@@ -409,6 +409,7 @@ const char* lrux_status_string(lrux_status_t s) {
     case LRUX_EWORKSPACE: return "LRUX_EWORKSPACE: state buffer too small";
     case LRUX_EUNSUPPORTED: return "LRUX_EUNSUPPORTED";
     case LRUX_ECUDA: return "LRUX_ECUDA: CUDA error";
+    case LRUX_ELIMIT: return "LRUX_ELIMIT: W*k*k*sizeof(elem) exceeds LRUX_NOALLOC_SCRATCH_BYTES (1 MiB)";
   }
   return "LRUX_?";
 }

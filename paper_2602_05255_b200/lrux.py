@@ -15,7 +15,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "lib", "liblrux.so")
 
 F64, C128 = 0, 1
-OK, EINVAL, ESTATE, EWORKSPACE, EUNSUPPORTED, ECUDA = range(6)
+OK, EINVAL, ESTATE, EWORKSPACE, EUNSUPPORTED, ECUDA, ELIMIT = range(7)
+NOALLOC_SCRATCH_BYTES = 1 << 20
 MAX_K = 64
 PROF_RATIO, PROF_UPDATE, PROF_APPEND, PROF_FLUSH, PROF_YPASS = range(5)
 
@@ -34,6 +35,7 @@ SIGNATURES = {
     "lrux_det_ratio": [_vp, _i32, _vp, _vp, _vp, _vp],
     "lrux_pf_ratio": [_vp, _i32, _vp, _vp, _vp, _vp],
     "lrux_det_ratio_general": [_vp, _i32, _i32, _vp, _vp, _i32, _vp, _vp, _vp, _vp],
+    "lrux_det_ratio_noalloc": [_i64, _i32, _i32, C.c_int, _vp, _vp, _vp, _vp, _vp],
     "lrux_det_accept": [_vp, _vp, _vp],
     "lrux_pf_accept": [_vp, _vp, _vp],
     "lrux_det_flush": [_vp, _vp],
@@ -270,6 +272,26 @@ class PfWalkers(_Walkers):
 
 
 # ---------------------------------------------------------------- harness
+def det_ratio_noalloc(Ti, idx, rows, out, stream=None):
+    """lrux_det_ratio_noalloc: r_w = det(N_w A_w^-1[:,P_w]) with no handle and no allocation.
+    Ti [W][n][n] = A^-T, idx int32 [W][k], rows [W][k][n], out [W] (all caller-owned CUDA
+    tensors, contiguous; this wrapper creates no tensor either).  The call's scratch is a fixed
+    1 MiB array in the library: W*k*k*itemsize beyond it raises LruxError (ELIMIT); calls that
+    may overlap on the GPU race."""
+    for t in (Ti, idx, rows, out):
+        if not (t.is_cuda and t.is_contiguous()):
+            raise ValueError("det_ratio_noalloc takes contiguous CUDA tensors")
+    if idx.dtype != torch.int32 or rows.dtype != Ti.dtype or out.dtype != Ti.dtype:
+        raise TypeError("idx must be int32; rows and out must have the dtype of Ti")
+    W, n, k = int(Ti.shape[0]), int(Ti.shape[1]), int(idx.shape[1])
+    if tuple(Ti.shape) != (W, n, n) or tuple(idx.shape) != (W, k) or tuple(rows.shape) != (W, k, n) \
+            or out.numel() != W:
+        raise ValueError("shape mismatch")
+    _check(load_library().lrux_det_ratio_noalloc(W, n, k, _dt(Ti.dtype), _ptr(Ti), _ptr(idx), _ptr(rows),
+                                                 _ptr(out), _stream(stream)))
+    return out
+
+
 def _optr(t):
     return None if t is None else _ptr(t)
 
