@@ -13,7 +13,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "lib", "liblrux.so")
-SOURCES = ["lrux_api.cu", "lrux_init.cu", "lrux_init_blocked.cu", "lrux_det.cu", "lrux_det_tma.cu", "lrux_det_dmma.cu", "lrux_pf.cu", "lrux_flush.cu", "lrux_general.cu", "lrux_rowdot.cu", "lrux_det_big.cu", "lrux_harness.cu", "lrux_noalloc.cu"]
+SOURCES = ["lrux_api.cu", "lrux_init.cu", "lrux_init_blocked.cu", "lrux_det.cu", "lrux_det_tma.cu", "lrux_det_dmma.cu", "lrux_pf.cu", "lrux_pf_dmma.cu", "lrux_flush.cu", "lrux_general.cu", "lrux_rowdot.cu", "lrux_det_big.cu", "lrux_harness.cu", "lrux_noalloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

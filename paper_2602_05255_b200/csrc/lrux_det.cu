@@ -717,49 +717,55 @@ det_append_kernel(State st, int k, int tiles, int rows_per_tile, int n_in_smem) 
   }
 }
 
-// The same pass for complex128 with k <= 4 on the FP64 tensor pipe.  The k dot products per
-// row are an (rows x n)(n x k) contraction: per warp, 8 rows x 4 columns of Ti form the A
+// The same dot products for complex128 with k <= 4 on the FP64 tensor pipe.  The k dot products
+// per row are an (rows x n)(n x k) contraction: per warp, 8 rows x 4 columns of Ti form the A
 // fragment of mma.sync.m8n8k4.f64 straight from the global loads (lane = (row, column): one
 // 16-byte complex element, both halves used), and the 8 real columns [Re N | Im N] the B
 // fragment, so that  A=Re Ti, B=[Re N | Im N]  and  A=Im Ti, B'=[-Im N | Re N]  accumulate
 // [Re W | Im W] in two DMMAs per 8x4 complex elements.  Against the scalar pass: 2 tensor
 // instructions instead of 32 DFMAs + shuffles, 4 accumulator registers per lane instead of
-// 32, which leaves room for 16 loads of 16 bytes in flight per lane.  Measured at C4: 689 us per step for the
-// append class against 697 us for the scalar pass -- the pass is bound by its per-item phases and
-// the walker-count tail, not by issue; 64-row tiles (less tail, twice the per-item work) were slower (762 us).
+// 32, which leaves room for 16 loads of 16 bytes in flight per lane.
 __device__ __forceinline__ void dmma884_acc(double& d0, double& d1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                : "+d"(d0), "+d"(d1)
                : "d"(a), "d"(b));
 }
 
-// MT = 8-row MMA tiles per warp and pass: 2 with 128-row work items, 1 with 64-row items.
-template <int KT, int MT>
-__global__ void __launch_bounds__(256, 2)
-det_append_dmma_kernel(State st, int k, int tiles, int rows_per_tile) {
+// The complex k <= 4 dot-product pass as a PURE STREAM.  Both contractions of the append have
+// the same shape -- rows of a matrix against the k new rows N:
+//     D[a][j]  = sum_i N[a][i] Ti[j][i] - [j == P_a]      (N A0^-1 - I[P,:], j < n)
+//     NA[a][s] = sum_i N[a][i] Abuf[s][i]                 (N Abuf^T of Eq. 15, s < fill)
+// so one kernel streams the n rows of Ti AND the fill rows of Abuf of every accepted walker
+// (det_prep_kernel is not launched on this path).  D goes to the rows Bbuf[fill .. fill+k) that
+// b_tau will occupy (free space), NA to pend_Y; det_append_finish_kernel then copies a_tau and
+// does Eq. 15, so this kernel has no per-tile phases and no CTA barrier except when its range
+// crosses into the next walker ([Re N | Im N] restaged).  Work is split in 16-row units, the
+// ceil(cap/16) buffer units of a walker interleaved evenly among its ceil(n/16) inverse units
+// (Bresenham), so that every contiguous range holds its share of both: CTA b takes units
+// [total b / G, total (b+1) / G) of the concatenated accepted list -- with ~150 accepted
+// walkers of 72 units over 296 CTAs that is 36.5 units each instead of 4 or 5 whole 128-row
+// tiles (a 25 % tail) -- and warp (u - first) mod 8 takes unit u.
+__global__ void __launch_bounds__(256, 2) det_append_dmma_stream_kernel(State st, int k) {
   using T = cplx;
   using S = Sc<T>;
-  constexpr int UN = 8;                          // column steps of 4 per batch of loads: 2 x 8 16-byte loads in flight per lane
+  constexpr int UN = 8, MT = 2;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int n = st.n, kmax = st.kmax;
-  T* dsm = (T*)smem_raw;                         // [4][KT][rows_per_tile] partial sums
-  double* Bs = (double*)(dsm + 4 * KT * rows_per_tile);   // [n][8]  Re N (cols 0-3), Im N (cols 4-7)
-  __shared__ T Ri[KT * KT];
-  __shared__ int sidx[KT];
+  const int n = st.n, kmax = st.kmax, cap = st.cap;
+  double* Bs = (double*)smem_raw;                // [n][8]  Re N (cols 0-3), Im N (cols 4-7)
+  __shared__ int sidx[4];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
-  const int r8 = lane >> 2, kk = lane & 3;       // A: (row, column) of the lane; B: (column kk, N-column r8)
+  const int r8 = lane >> 2, kk = lane & 3;
   const int count = st.counters[0];
-  // contiguous item ranges per CTA: [Re N | Im N] is staged once per walker (see det_append_kernel)
-  const int total = count * tiles;
-  const int first = (int)((int64_t)total * blockIdx.x / gridDim.x), last = (int)((int64_t)total * (blockIdx.x + 1) / gridDim.x);
-  int cur_w = -1;
-  for (int item = first; item < last; ++item) {
-    const int w = st.list[item / tiles];
-    const int tile = item % tiles;
+  const int upt = (n + 15) >> 4, upa = (cap + 15) >> 4, upw = upt + upa;
+  const int64_t total = (int64_t)count * upw;
+  const int64_t first = total * blockIdx.x / gridDim.x, last = total * (blockIdx.x + 1) / gridDim.x;
+  for (int64_t u = first; u < last;) {
+    const int wi = (int)(u / upw);
+    const int w = st.list[wi];
     const int fill = st.fill[w];
+    const int64_t seg_end = min(last, (int64_t)(wi + 1) * upw);
     __syncthreads();
-    if (w != cur_w) {
-      cur_w = w;
+    {
       const T* gN = (const T*)st.pend_N + (size_t)w * kmax * n;
       for (int q = tid; q < 4 * n; q += blockDim.x) {
         const int a = q / n, i = q % n;
@@ -767,81 +773,93 @@ det_append_dmma_kernel(State st, int k, int tiles, int rows_per_tile) {
         Bs[i * 8 + a] = v.re;
         Bs[i * 8 + 4 + a] = v.im;
       }
-      if (tid < KT * KT) {
-        const int a = tid / KT, b = tid % KT;
-        Ri[tid] = (a < k && b < k) ? ((const T*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + a * st.kc + b]
-                                   : S::zero();
-      }
-      if (tid < KT) sidx[tid] = tid < k ? st.pend_idx[(size_t)w * kmax + tid] : -1;
+      if (tid < 4) sidx[tid] = tid < k ? st.pend_idx[(size_t)w * kmax + tid] : -1;
     }
     __syncthreads();
-    const T* Tw = (const T*)st.Ti + (size_t)w * n * n;
-    const int j_beg = tile * rows_per_tile, j_end = min(n, j_beg + rows_per_tile);
-    for (int j0 = j_beg + warp * (8 * MT); j0 < j_end; j0 += nw * (8 * MT)) {
+    const int64_t u_mine = u + ((warp - (int)((u - first) % nw)) + nw) % nw;
+    for (int64_t uu = u_mine; uu < seg_end; uu += nw) {
+      const int ul = (int)(uu - (int64_t)wi * upw);          // unit within the walker
+      const int a_before = (int)((int64_t)ul * upa / upw);
+      const bool is_a = (int)((int64_t)(ul + 1) * upa / upw) > a_before;
+      const int j0 = (is_a ? a_before : ul - a_before) * 16;
+      const int rlim = is_a ? fill : n;                     // valid rows of this matrix
+      if (j0 >= rlim) continue;                              // buffer unit past the fill
+      const T* X = is_a ? (const T*)st.Abuf + (size_t)w * cap * n : (const T*)st.Ti + (size_t)w * n * n;
       double acc[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
-      const T* row0 = Tw + (size_t)min(j0 + r8, j_end - 1) * n + kk;        // rows past the tile: clamped, discarded
-      const T* row1 = Tw + (size_t)min(j0 + 8 * (MT - 1) + r8, j_end - 1) * n + kk;
+      const T* row0 = X + (size_t)min(j0 + r8, rlim - 1) * n + kk;         // rows past the end: clamped, discarded
+      const T* row1 = X + (size_t)min(j0 + 8 + r8, rlim - 1) * n + kk;
       const double* bp = Bs + kk * 8 + r8;
       const double* bq = Bs + kk * 8 + (r8 ^ 4);
       const bool lo = r8 < 4;
       for (int i0 = 0; i0 < n; i0 += 4 * UN) {
         T x0[UN], x1[UN];
 #pragma unroll
-        for (int u = 0; u < UN; ++u) {
-          const bool in = i0 + 4 * u < n;
-          x0[u] = in ? row0[i0 + 4 * u] : S::zero();
-          if (MT == 2) x1[u] = in ? row1[i0 + 4 * u] : S::zero();
+        for (int v = 0; v < UN; ++v) {
+          const bool in = i0 + 4 * v < n;
+          x0[v] = in ? row0[i0 + 4 * v] : S::zero();
+          x1[v] = in ? row1[i0 + 4 * v] : S::zero();
         }
 #pragma unroll
-        for (int u = 0; u < UN; ++u) {
-          if (i0 + 4 * u < n) {
-            const double b = bp[(i0 + 4 * u) * 8];
-            const double b2 = bq[(i0 + 4 * u) * 8];
+        for (int v = 0; v < UN; ++v) {
+          if (i0 + 4 * v < n) {
+            const double b = bp[(i0 + 4 * v) * 8];
+            const double b2 = bq[(i0 + 4 * v) * 8];
             const double bm = lo ? -b2 : b2;          // B' = [-Im N | Re N]
-            dmma884_acc(acc[0][0], acc[0][1], x0[u].re, b);
-            dmma884_acc(acc[0][0], acc[0][1], x0[u].im, bm);
-            if (MT == 2) {
-              dmma884_acc(acc[1][0], acc[1][1], x1[u].re, b);
-              dmma884_acc(acc[1][0], acc[1][1], x1[u].im, bm);
-            }
+            dmma884_acc(acc[0][0], acc[0][1], x0[v].re, b);
+            dmma884_acc(acc[0][0], acc[0][1], x0[v].im, bm);
+            dmma884_acc(acc[1][0], acc[1][1], x1[v].re, b);
+            dmma884_acc(acc[1][0], acc[1][1], x1[v].im, bm);
           }
         }
       }
-      // D fragment: row r8, columns 2*kk, 2*kk+1 of [Re W | Im W]
+      // D fragment: row r8, columns 2*kk, 2*kk+1 of [Re | Im]
+      T* outD = (T*)st.Bbuf + ((size_t)w * cap + fill) * n;                // [a][j], row stride n
+      T* outNA = (T*)st.pend_Y + (size_t)w * kmax * cap;                   // [a][s], row stride cap
 #pragma unroll
       for (int mt = 0; mt < MT; ++mt) {
         const int j = j0 + 8 * mt + r8;
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
           const int col = 2 * kk + e, a = col & 3;
-          if (j < j_end && a < KT) {
+          if (j < rlim && a < k) {
             double v = acc[mt][e];
-            if (col < 4 && j == sidx[a]) v -= 1.0;
-            ((double*)&dsm[a * rows_per_tile + (j - j_beg)])[col >> 2] = v;
+            if (is_a) {
+              ((double*)&outNA[(size_t)a * cap + j])[col >> 2] = v;
+            } else {
+              if (col < 4 && j == sidx[a]) v -= 1.0;
+              ((double*)&outD[(size_t)a * n + j])[col >> 2] = v;
+            }
           }
         }
       }
     }
-    append_finish<T, KT>(st, w, k, fill, j_beg, j_end, rows_per_tile, dsm, Ri);
+    u = seg_end;
   }
 }
 
 // Second half of the append as its own pass, for the tensor-pipe variant below: D = N A0^-1 -
 // I[P,:] is already in the pending area (pend_C, free once det_prep_kernel has copied a_tau
 // into the buffer).  b_tau^T = R^-1 (D - (N Abuf) Bbuf^T) -> Bbuf[fill .. fill+k)   (Eq. 15,
-// PAPER.md:194; reading 5b).  Work item = (accepted walker, 256 columns); thread per column.
+// PAPER.md:194; reading 5b).  Work item = (accepted walker, 64 columns); four groups of
+// threads split the buffer rows (the loop over them is a chain of dependent loads) and meet in
+// shared memory, summed in a fixed order.
+// inplace = 1 (after det_append_dmma_stream_kernel, which ran without det_prep_kernel): D is
+// read from the rows Bbuf[fill .. fill+k) it is about to overwrite (each thread reads its k
+// values before it writes any), and a_tau = C_eff is copied into Abuf[fill .. fill+k) here.
 template <typename T, int KT>
-__global__ void __launch_bounds__(256) det_append_finish_kernel(State st, int k, int chunks) {
+__global__ void __launch_bounds__(256) det_append_finish_kernel(State st, int k, int chunks, int inplace) {
   using S = Sc<T>;
+  constexpr int CW = 64, SG = 4;               // columns per work item, groups that split the buffer rows
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  T* NAs = (T*)smem_raw;   // [fill][KT]
+  T* NAs = (T*)smem_raw;                       // [fill][KT]
+  T* red = NAs + (size_t)st.cap * KT;          // [SG-1][KT][CW] partial sums of groups 1..SG-1
   __shared__ T Ri[KT * KT];
   const int n = st.n, kmax = st.kmax, cap = st.cap;
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, jj = tid & (CW - 1), sg = tid / CW;
   const int count = st.counters[0];
   for (int item = blockIdx.x; item < count * chunks; item += gridDim.x) {
     const int w = st.list[item / chunks];
-    const int j = (item % chunks) * 256 + tid;
+    const int j = (item % chunks) * CW + jj;
     const int fill = st.fill[w];
     __syncthreads();
     const T* NA = (const T*)st.pend_Y + (size_t)w * kmax * cap;
@@ -853,25 +871,44 @@ __global__ void __launch_bounds__(256) det_append_finish_kernel(State st, int k,
                                  : S::zero();
     }
     __syncthreads();
-    if (j >= n) continue;
-    const T* D = (const T*)st.pend_C + (size_t)w * kmax * n;
     T* Bb = (T*)st.Bbuf + (size_t)w * cap * n;
+    const T* pC = (const T*)st.pend_C + (size_t)w * kmax * n;
+    const T* D = inplace ? Bb + (size_t)fill * n : pC;
     T m[KT];
 #pragma unroll
-    for (int b = 0; b < KT; ++b) m[b] = b < k ? D[(size_t)b * n + j] : S::zero();
-#pragma unroll 8
-    for (int s = 0; s < fill; ++s) {
-      const T bv = Bb[(size_t)s * n + j];
+    for (int b = 0; b < KT; ++b) m[b] = (sg == 0 && b < k && j < n) ? D[(size_t)b * n + j] : S::zero();
+    if (inplace && sg == 1 && j < n) {
+      T* Ab = (T*)st.Abuf + ((size_t)w * cap + fill) * n;
 #pragma unroll
-      for (int b = 0; b < KT; ++b) m[b] = S::fnma(NAs[s * KT + b], bv, m[b]);
+      for (int b = 0; b < KT; ++b)
+        if (b < k) Ab[(size_t)b * n + j] = pC[(size_t)b * n + j];
     }
+    if (j < n) {
+#pragma unroll 8
+      for (int s = sg; s < fill; s += SG) {
+        const T bv = Bb[(size_t)s * n + j];
 #pragma unroll
-    for (int a = 0; a < KT; ++a) {
-      if (a < k) {
-        T acc = S::zero();
+        for (int b = 0; b < KT; ++b) m[b] = S::fnma(NAs[s * KT + b], bv, m[b]);
+      }
+    }
+    if (sg > 0) {
 #pragma unroll
-        for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], m[b], acc);
-        Bb[(size_t)(fill + a) * n + j] = acc;
+      for (int b = 0; b < KT; ++b) red[((size_t)(sg - 1) * KT + b) * CW + jj] = m[b];
+    }
+    __syncthreads();
+    if (sg == 0 && j < n) {
+#pragma unroll
+      for (int b = 0; b < KT; ++b)
+#pragma unroll
+        for (int g = 0; g < SG - 1; ++g) m[b] = S::add(m[b], red[((size_t)g * KT + b) * CW + jj]);
+#pragma unroll
+      for (int a = 0; a < KT; ++a) {
+        if (a < k) {
+          T acc = S::zero();
+#pragma unroll
+          for (int b = 0; b < KT; ++b) acc = S::fma(Ri[a * KT + b], m[b], acc);
+          Bb[(size_t)(fill + a) * n + j] = acc;
+        }
       }
     }
   }
@@ -1017,6 +1054,22 @@ template <typename T, int KT>
 static int launch_append_kt(const State& st, int k, Ctx& cx, cudaStream_t s) {
   const int n = st.n;
   constexpr int VECMAX = sizeof(T) == 8 ? 2 : 1;
+  if constexpr (sizeof(T) == 16 && KT <= 4) {
+    // complex data, k <= 4: the dot products as a pure stream on the FP64 tensor pipe, Eq. 15 in a second pass
+    if (n % 4 == 0 && n >= 1024 && (size_t)n * 64 <= 100 * 1024) {
+      const size_t sms = (size_t)n * 64;
+      const int occs = cx.configure((const void*)det_append_dmma_stream_kernel, 256, sms);
+      if (occs < 0) return -1;
+      det_append_dmma_stream_kernel<<<persistent_grid(cx.num_sms, occs, (int64_t)st.W * ((n + 15) / 16)), 256, sms, s>>>(st, k);
+      const int chunks = (n + 63) / 64;
+      const size_t smf = ((size_t)st.cap * KT + 3 * KT * 64) * sizeof(T);
+      auto kf = det_append_finish_kernel<T, KT>;
+      if (cx.configure((const void*)kf, 256, smf) < 0) return -1;
+      kf<<<persistent_grid(cx.num_sms, 8, (int64_t)st.W * chunks), 256, smf, s>>>(st, k, chunks, 1);
+      cx.name(LRUX_PROF_APPEND, "det_append_dmma_stream_kernel+det_append_finish_kernel");
+      return 2;
+    }
+  }
   int nl = 0;
   {
     const int groups = (st.cap + 8 * kPrepRows - 1) / (8 * kPrepRows);
@@ -1040,11 +1093,11 @@ static int launch_append_kt(const State& st, int k, Ctx& cx, cudaStream_t s) {
       const int r = launch_rowdot_dmma(A, cx, s);
       if (r < 0) return -1;
       if (r > 0) {
-        const int chunks = (n + 255) / 256;
-        const size_t smf = (size_t)st.cap * KT * sizeof(T);
+        const int chunks = (n + 63) / 64;
+        const size_t smf = ((size_t)st.cap * KT + 3 * KT * 64) * sizeof(T);
         auto kf = det_append_finish_kernel<T, KT>;
         if (cx.configure((const void*)kf, 256, smf) < 0) return -1;
-        kf<<<persistent_grid(cx.num_sms, 8, (int64_t)st.W * chunks), 256, smf, s>>>(st, k, chunks);
+        kf<<<persistent_grid(cx.num_sms, 8, (int64_t)st.W * chunks), 256, smf, s>>>(st, k, chunks, 0);
         cx.name(LRUX_PROF_APPEND, "det_prep_kernel+rowdot_dmma_kernel+det_append_finish_kernel");
         return nl + r + 1;
       }
@@ -1054,18 +1107,6 @@ static int launch_append_kt(const State& st, int k, Ctx& cx, cudaStream_t s) {
   const int tiles = (n + rows_per_tile - 1) / rows_per_tile;
   const int n_in_smem = (size_t)k * n * sizeof(T) <= 96 * 1024;
   const size_t smem = ((n_in_smem ? (size_t)k * n : 0) + 4 * (size_t)KT * rows_per_tile) * sizeof(T);
-  if constexpr (sizeof(T) == 16 && KT <= 4) {
-    // complex data, k <= 4, 128-row tiles: the dot products on the FP64 tensor pipe
-    const size_t smd = (size_t)n * 64 + 4 * (size_t)KT * rows_per_tile * sizeof(T);
-    if (n % 4 == 0 && n >= 1024 && smd <= 100 * 1024) {
-      auto kd = rows_per_tile >= 128 ? det_append_dmma_kernel<KT, 2> : det_append_dmma_kernel<KT, 1>;
-      const int occd = cx.configure((const void*)kd, 256, smd);
-      if (occd < 0) return -1;
-      kd<<<persistent_grid(cx.num_sms, occd, (int64_t)st.W * tiles), 256, smd, s>>>(st, k, tiles, rows_per_tile);
-      cx.name(LRUX_PROF_APPEND, "det_prep_kernel+det_append_dmma_kernel");
-      return nl + 1;
-    }
-  }
   const bool vec = (n % VECMAX) == 0 && VECMAX == 2;
   auto kern = vec ? det_append_kernel<T, KT, VECMAX, 2> : det_append_kernel<T, KT, 1, 2>;
   const int occ = cx.configure((const void*)kern, 256, smem);

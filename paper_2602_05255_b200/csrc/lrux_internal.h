@@ -138,6 +138,7 @@ static inline int round_kt(int k) { return k <= 1 ? 1 : k <= 2 ? 2 : k <= 4 ? 4 
 
 // launchers (each returns the number of kernels it enqueued, or -1 on a CUDA error)
 int launch_det_init(const State& st, const void* d_A0, Ctx& cx, cudaStream_t s);
+int launch_pf_update_dmma(const State& st, int k, Ctx& cx, cudaStream_t s, bool probe = false);
 int launch_pf_init(const State& st, const void* d_A0, Ctx& cx, cudaStream_t s);
 int launch_refresh(const State& st, const void* d_A, Ctx& cx, cudaStream_t s);
 // blocked in-place inverse of st.Ti (lrux_init_blocked.cu); 0 = not applicable

@@ -17,6 +17,16 @@
 #include <cooperative_groups.h>
 #include <algorithm>
 
+#ifndef LRUX_PF_DMMA
+#define LRUX_PF_DMMA 1
+#endif
+#ifndef LRUX_PF_Y_ROWDOT_MIN_K
+#define LRUX_PF_Y_ROWDOT_MIN_K 3
+#endif
+#ifndef LRUX_PF_DMMA_MIN_K
+#define LRUX_PF_DMMA_MIN_K 2
+#endif
+
 namespace lrux {
 
 constexpr int kMaxC = 2 * kMaxK;  // largest core size
@@ -1291,6 +1301,24 @@ static int launch_y(const State& st, int k, int use_list, Ctx& cx, cudaStream_t 
     pf_an_kernel<T><<<persistent_grid(cx.num_sms, 4, st.W), 256, 0, s>>>(st, k, use_list); ++nl;
   }
   const int kt = round_kt(k);
+  if (sizeof(T) == 8 && !st.cap && k >= LRUX_PF_Y_ROWDOT_MIN_K && (st.n & 1) == 0) {
+    // real data, K = 0, k >= 3: by skewness Y[a][i] = sum_j Ti[i][j] N[a][j] is the row-dot
+    // contraction of lrux_rowdot.cu on the FP64 tensor pipe (the column-sum kernel spends k
+    // DFMAs and k shared-memory operands per element: 0.68 of its k = 2 rate at k = 4)
+    RowdotArgs A{};
+    A.X = (const double*)st.Ti;      A.x_stride = (size_t)st.n * st.n;        A.rows = st.n;  A.ldx = st.n;
+    A.N = (const double*)st.pend_N;  A.n_stride = (size_t)st.kmax * st.n;     A.ldn = st.n;
+    A.n = st.n;  A.k = k;
+    A.out = (double*)st.pend_Y;      A.o_stride = (size_t)st.kmax * st.n;     A.ldo = st.n;
+    A.list = use_list ? st.list : nullptr;  A.count = use_list ? st.counters : nullptr;  A.W = st.W;
+    A.idx = nullptr;  A.idx_stride = 0;
+    const int r = launch_rowdot_dmma(A, cx, s);
+    if (r < 0) return -1;
+    if (r > 0) {
+      cx.name(LRUX_PROF_YPASS, "rowdot_dmma_kernel");
+      return nl + r;
+    }
+  }
   {
     // column sums (no warp reductions) whenever N fits in shared memory
     constexpr int VE = sizeof(T) == 8 ? 2 : 1;
@@ -1438,6 +1466,15 @@ static int launch_pf_resident(const State& st, int k, Ctx& cx, cudaStream_t s) {
 template <typename T>
 static int pf_accept_impl(const State& st, int k, const uint8_t* mask, Ctx& cx, cudaStream_t s) {
   int nl = launch_select(st, mask, s);
+#if LRUX_PF_DMMA
+  if (st.K == 0 && sizeof(T) == 8 && k >= LRUX_PF_DMMA_MIN_K && launch_pf_update_dmma(st, k, cx, s, true) > 0) {
+    // real data, k >= 2 (Y is already in the pending area): 8-row strips on the FP64 tensor pipe
+    ProfScope ps(&cx.prof, LRUX_PROF_UPDATE, s);
+    const int r = launch_pf_update_dmma(st, k, cx, s);
+    if (r < 0) return -1;
+    if (r > 0) return cudaGetLastError() == cudaSuccess ? nl + r : -1;
+  }
+#endif
   if (st.K == 0) {
     const int r = launch_pf_resident<T>(st, k, cx, s);
     if (r < 0) return -1;
@@ -1451,7 +1488,16 @@ static int pf_accept_impl(const State& st, int k, const uint8_t* mask, Ctx& cx, 
   if (st.K == 0) {
     ProfScope ps(&cx.prof, LRUX_PROF_UPDATE, s);
     const size_t sm = 4 * (size_t)k * st.n * sizeof(T);   // Y' and g
-    if (sm <= 160 * 1024) {
+    int rd = 0;
+#if LRUX_PF_DMMA
+    if (sizeof(T) == 8 && k < LRUX_PF_DMMA_MIN_K && launch_pf_update_dmma(st, k, cx, s, true) > 0) {   // k = 1 beyond the resident kernels
+      rd = launch_pf_update_dmma(st, k, cx, s);
+      if (rd < 0) return -1;
+      nl += rd;
+    }
+#endif
+    if (rd > 0) {
+    } else if (sm <= 160 * 1024) {
       auto kern = k <= 1 ? pf_update_stream_kernel<T, 2> : k <= 2 ? pf_update_stream_kernel<T, 4>
                 : k <= 4 ? pf_update_stream_kernel<T, 8> : pf_update_stream_kernel<T, 16>;
       const int occ = cx.configure((const void*)kern, 256, sm);

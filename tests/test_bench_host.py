@@ -77,6 +77,6 @@ def test_oracle_sample_takes_out_the_initialisation():
 def test_roofline_append_counts_one_read_pass():
     c4 = bench.parse_workload("c4")
     run = {"accepted": 100, "prof": {"append": {"ms": 4.0, "launches": 2}, "ypass": {"ms": 0.0, "launches": 0}},
-           "kernels": {"append": "det_prep_kernel+det_append_dmma_kernel", "ypass": ""}}
+           "kernels": {"append": "det_append_dmma_stream_kernel+det_append_finish_kernel", "ypass": ""}}
     r = bench.roofline_append(c4, run, 6460.9, "m")
     assert r["achieved"] == pytest.approx(1024 * 1024 * 16 * 100 / 4e-3 / 1e9) and r["bound"] == "hbm"

@@ -163,16 +163,40 @@ def test_pf_large_n_paths(n, k):
     (140, 1, False, "pf_resident_k1_kernel"),     # ... 5 chunk buffers
     (200, 1, False, "pf_cluster_k1_kernel"),      # 8-CTA cluster, run-time sizes
     (256, 1, False, "pf_cluster_k1_kernel"),      # 8-CTA cluster, unrolled instance
-    (128, 2, False, "pf_cluster_update_kernel"),  # generic cluster kernel, 4-CTA
-    (96, 1, True, "pf_cluster_update_kernel"),    # complex
-    (320, 1, False, "pf_update_stream_kernel"),   # Y pass + streaming update
-    (320, 2, True, "pf_update_stream_kernel"),
+    (128, 2, False, "pf_update_dmma_kernel"),     # real k >= 2: 8-row strips on the FP64 tensor pipe (2 DMMAs / block)
+    (64, 1, True, "pf_cluster_update_kernel"),    # complex: generic cluster kernel, 4-CTA
+    (128, 2, True, "pf_cluster_update_kernel"),   # ... 8-CTA, k = 2
+    (96, 1, True, "pf_cluster_update_kernel"),
+    (320, 1, False, "pf_update_dmma_kernel"),     # k = 1 beyond the cluster kernels: Y pass + DMMA strips (1 DMMA / block)
+    (320, 2, True, "pf_update_stream_kernel"),    # complex: Y pass + streaming update
+    (34, 2, False, "pf_update_dmma_kernel"),      # ragged: n not a multiple of 8, two strips straddle walkers
+    (520, 2, False, "pf_update_dmma_kernel"),     # 16 warps
 ])
 def test_pf_update_kernel_by_shape(n, k, cplx, name):
     """Every immediate Pfaffian update kernel, reached by its SHAPE (there is no environment
     switch): same trajectory as the oracle."""
     _run("pf", 171 + n + k, 4, n, 2 * n, k, 0, 24, cplx, walkers=[0, 3], scratch_every=4,
          kernel={"update": name})
+
+
+@pytest.mark.parametrize("n,k", [
+    (250, 3),      # 2k = 6 padded to 8
+    (256, 4),      # 2 DMMAs per block, 4 blocks per warp
+    (130, 8),      # 2k = 16: 4 DMMAs per block
+    (512, 4),      # 8 blocks per warp (the shape VERDICT r1 item 7 names)
+])
+def test_pf_update_dmma_larger_ranks(n, k):
+    """pf_update_dmma_kernel with 2 and 4 DMMAs per 8 x 8 block, every proposal applied (rank >= 3
+    proposals are rarely accepted by the Metropolis test); the stored inverse must stay EXACTLY
+    skew (parity_util.compare checks Ti == -Ti^T bit for bit)."""
+    _run("pf", 1900 + n + k, 3, n, 2 * n, k, 0, 8, walkers=[0, 2], scratch_every=2, forced=True,
+         kernel={"update": "pf_update_dmma_kernel"})
+
+
+def test_pf_update_stream_kernel_real_beyond_dmma():
+    """Real data with n > 1024: past the DMMA strips' instances -> Y pass + streaming update."""
+    _run("pf", 1813, 2, 1040, 2080, 1, 0, 5, walkers=[1], scratch_every=4,
+         kernel={"update": "pf_update_stream_kernel"})
 
 
 def test_pf_update_tile_kernel_large_k():
@@ -217,6 +241,18 @@ def test_det_real_append_large_n(n, k, K, kernel):
     accept so that buffers fill and flush."""
     _run("det", 40 + n + k + K, 3, n, 2 * n, k, K, min(K, 10) + 3, walkers=[0, 2], scratch_every=1,
          forced=True, kernel={"append": kernel})
+
+
+@pytest.mark.parametrize("n,k,K", [
+    (1024, 4, 6),      # the configs[3] shape (k = 4), shallow buffer: flushes inside the run
+    (1028, 3, 5),      # n a multiple of 4 but not of 16: part-filled last unit; cap = 15: part-filled buffer unit
+    (1024, 1, 9),      # k = 1 through the 4-column fragments
+])
+def test_det_complex_append_stream(n, k, K):
+    """Complex delayed append at n >= 1024: det_append_dmma_stream_kernel (rows of A0^-1 and of
+    Abuf against N on the FP64 tensor pipe, no det_prep_kernel) + the in-place finish pass."""
+    _run("det", 60 + n + k + K, 3, n, 2 * n, k, K, K + 4, cplx=True, walkers=[0, 2], scratch_every=1,
+         forced=True, kernel={"append": "det_append_dmma_stream_kernel+det_append_finish_kernel"})
 
 
 @pytest.mark.parametrize("n,k,K,cplx", [(128, 1, 4, False), (512, 2, 8, False), (512, 1, 4, False),
