@@ -163,6 +163,58 @@ __device__ inline T small_det_inv(T* a, T* inv, int k, int ld, bool* ok) {
   return det;
 }
 
+// The same elimination executed by ONE WARP (all 32 lanes call it; a, inv in shared memory):
+// lane l < 2k owns column l of the augmented matrix [a | inv].  Every element goes through the
+// operations of small_det_inv in the same order, so det and inv are bit-identical to the
+// serial routine -- at k = 8 the serial one was the longest phase of the ratio kernel.
+template <typename T>
+__device__ inline T warp_det_inv(T* a, T* inv, int k, int ld, bool* ok, int lane) {
+  using S = Sc<T>;
+  constexpr int KM = 2 * kMaxK;
+  const bool act = lane < 2 * k;
+  T* col = lane < k ? a + lane : inv + (lane - k);   // this lane's column, stride ld
+  if (act && lane >= k)
+    for (int i = 0; i < k; ++i) col[i * ld] = (i == lane - k) ? S::one() : S::zero();
+  __syncwarp();
+  T det = S::one();
+  bool good = true;
+  for (int c = 0; c < k; ++c) {
+    int p = c;
+    double best = S::abs2(a[c * ld + c]);
+    for (int r = c + 1; r < k; ++r) {
+      const double v = S::abs2(a[r * ld + c]);
+      if (v > best) { best = v; p = r; }
+    }
+    if (!(best > 0.0) || !isfinite(best)) { good = false; det = S::zero(); break; }   // uniform
+    __syncwarp();
+    if (p != c) {
+      if (act) { const T t = col[c * ld]; col[c * ld] = col[p * ld]; col[p * ld] = t; }
+      det = S::neg(det);
+      __syncwarp();
+    }
+    const T d = a[c * ld + c];
+    det = S::mul(det, d);
+    const T di = S::inv(d);
+    __syncwarp();                      // every lane has d before lane c rescales it
+    if (act) col[c * ld] = S::mul(col[c * ld], di);
+    __syncwarp();
+    T f[KM];
+#pragma unroll
+    for (int r = 0; r < KM; ++r) f[r] = r < k ? a[r * ld + c] : S::zero();
+    __syncwarp();                      // ... and the multipliers before column c is eliminated
+    if (act) {
+      const T pc = col[c * ld];
+#pragma unroll
+      for (int r = 0; r < KM; ++r)
+        if (r < k && r != c) col[r * ld] = S::fnma(f[r], pc, col[r * ld]);
+    }
+    __syncwarp();
+  }
+  if (good && !S::finite(det)) good = false;
+  *ok = good;
+  return det;
+}
+
 // Pfaffian of an exactly skew m x m matrix (m even, m <= 2*kMaxK) by
 // Parlett-Reid elimination with pivoting, ONE thread, destroys `a`.
 template <typename T>
@@ -200,6 +252,48 @@ __device__ inline T small_pf(T* a, int m, int ld) {
         a[c * ld + r] = S::neg(v);
       }
     }
+  }
+  return pf;
+}
+
+// small_pf executed by ONE WARP (all 32 lanes call it; `a` in shared memory).  The (r, c)
+// updates of one elimination step are independent of each other, and the swaps keep the
+// serial order (rows, then columns): bit-identical to small_pf.
+template <typename T>
+__device__ inline T warp_pf(T* a, int m, int ld, int lane) {
+  using S = Sc<T>;
+  T pf = S::one();
+  for (int j = 0; j + 1 < m; j += 2) {
+    int p = j + 1;
+    double best = S::abs2(a[(j + 1) * ld + j]);
+    for (int r = j + 2; r < m; ++r) {
+      const double v = S::abs2(a[r * ld + j]);
+      if (v > best) { best = v; p = r; }
+    }
+    if (!(best > 0.0)) return S::zero();   // uniform
+    __syncwarp();
+    if (p != j + 1) {
+      if (lane < m) { const T t = a[(j + 1) * ld + lane]; a[(j + 1) * ld + lane] = a[p * ld + lane]; a[p * ld + lane] = t; }
+      __syncwarp();
+      if (lane < m) { const T t = a[lane * ld + j + 1]; a[lane * ld + j + 1] = a[lane * ld + p]; a[lane * ld + p] = t; }
+      __syncwarp();
+      pf = S::neg(pf);
+    }
+    const T piv = a[j * ld + j + 1];
+    pf = S::mul(pf, piv);
+    const T pi = S::inv(piv);
+    for (int r = j + 2; r < m; ++r) {
+      const int c = r + 1 + lane;
+      if (c < m) {
+        const T tr = S::mul(a[j * ld + r], pi), tc = S::mul(a[j * ld + c], pi);
+        T v = a[r * ld + c];
+        v = S::fma(tr, a[c * ld + j + 1], v);
+        v = S::fnma(a[r * ld + j + 1], tc, v);
+        a[r * ld + c] = v;
+        a[c * ld + r] = S::neg(v);
+      }
+    }
+    __syncwarp();
   }
   return pf;
 }

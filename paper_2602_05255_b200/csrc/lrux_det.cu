@@ -16,6 +16,9 @@
 #endif
 // ... and from which real-valued delayed appends take the row-dot DMMA pass
 // rows of A0^-1 per work item of the register-row / complex-DMMA append
+#ifndef LRUX_RATIO_FLY_MAX_KT
+#define LRUX_RATIO_FLY_MAX_KT 4
+#endif
 #ifndef LRUX_APPEND_TILE_ROWS
 #define LRUX_APPEND_TILE_ROWS 128
 #endif
@@ -33,14 +36,16 @@ namespace lrux {
 // (b_t^T v = Bbuf[s][P[a]] is a warp-uniform load).  C_eff and N are stashed for
 // accept.  R = N C_eff (Eq. 4 / Eq. 13): every slice writes its partial k x k sum
 // (accumulated on the fly), and the slice that finishes last adds the partials in slice
-// order (deterministic) -- or, for complex128 with KT = 8, forms R from the complete stash --
+// order (deterministic) -- or, with KT = 8, forms R from the complete stash --
 // and evaluates r = det R by a k x k LU in one thread.
 template <typename T, int KT, int EPT>
 __global__ void __launch_bounds__(256)
 det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __restrict__ rows,
                  T* __restrict__ ratio_out) {
   using S = Sc<T>;
-  constexpr bool FLY = KT <= 4 || sizeof(T) == 8;   // k x k accumulators in registers
+  // k x k accumulators in registers up to k = 4; at k = 8 the 64 accumulators cost 161 registers
+  // (one CTA per SM, 4.2 ms per step at n = 512, W = 8192): R comes from the complete stash instead
+  constexpr bool FLY = KT <= LRUX_RATIO_FLY_MAX_KT;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* Bp = (T*)smem_raw;  // [fill][KT]: b_t^T v = Bbuf[s][P[a]]
   __shared__ T Rs[kMaxK * kMaxK];
@@ -201,17 +206,19 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
     }
   }
   __syncthreads();
-  if (tid == 0) {
+  if (warp == 0) {   // k x k elimination by one warp (bit-identical to the serial small_det_inv)
     bool ok;
-    T det = small_det_inv(Rs, Ri, k, kMaxK, &ok);
-    ratio_out[w] = det;
-    ((T*)st.pend_ratio)[w] = det;
-    st.pend_ok[w] = ok ? 1 : 0;
-    T* pR = (T*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
-    for (int a = 0; a < k; ++a) {
-      st.pend_idx[(size_t)w * kmax + a] = P[a];
-      for (int b = 0; b < k; ++b) pR[a * st.kc + b] = Ri[a * kMaxK + b];
+    const T det = warp_det_inv(Rs, Ri, k, kMaxK, &ok, lane);
+    if (lane == 0) {
+      ratio_out[w] = det;
+      ((T*)st.pend_ratio)[w] = det;
+      st.pend_ok[w] = ok ? 1 : 0;
     }
+    T* pR = (T*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
+    for (int q = lane; q < k * k; q += 32) pR[(q / k) * st.kc + (q % k)] = Ri[(q / k) * kMaxK + (q % k)];
+#pragma unroll
+    for (int a = 0; a < KT; ++a)
+      if (lane == a && a < k) st.pend_idx[(size_t)w * kmax + a] = P[a];
   }
 }
 

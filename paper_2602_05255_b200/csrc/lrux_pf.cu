@@ -403,23 +403,35 @@ pf_core_kernel(State st, int k, T* __restrict__ ratio_out) {
   __syncthreads();
   for (int q = tid; q < kMaxC * kMaxC; q += nt) R2[q] = R[q];
   __syncthreads();
-  if (tid == 0) {
-    T pfv = small_pf(R2, m, kMaxC);
-    if ((k * (k - 1) / 2) & 1) pfv = S::neg(pfv);
+  // warp 0: R'^-1 by Gauss-Jordan, warp 1: pf R' by Parlett-Reid, side by side (each bit-identical
+  // to the serial small_det_inv / small_pf, which at k = 8 cost more than the update pass)
+  __shared__ T pf_s;
+  __shared__ int ok_s;
+  if (warp == 0) {
     bool ok;
-    small_det_inv(R, Ri, m, kMaxC, &ok);
-    ok = ok && S::finite(pfv) && !S::is_zero(pfv);
+    warp_det_inv(R, Ri, m, kMaxC, &ok, lane);
+    if (lane == 0) ok_s = ok ? 1 : 0;
+  } else if (warp == 1) {
+    T pfv = warp_pf(R2, m, kMaxC, lane);
+    if ((k * (k - 1) / 2) & 1) pfv = S::neg(pfv);
+    if (lane == 0) pf_s = pfv;
+  }
+  __syncthreads();
+  const T pfv = pf_s;
+  const bool ok = ok_s && S::finite(pfv) && !S::is_zero(pfv);
+  if (tid == 0) {
     ratio_out[w] = pfv;
     ((T*)st.pend_ratio)[w] = pfv;
     st.pend_ok[w] = ok ? 1 : 0;
-    T* pR = (T*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
-    for (int a = 0; a < m; ++a) {
-      pR[a * st.kc + a] = S::zero();
-      for (int b = a + 1; b < m; ++b) {
-        const T v = ok ? S::scale(S::sub(Ri[a * kMaxC + b], Ri[b * kMaxC + a]), 0.5) : S::zero();
-        pR[a * st.kc + b] = v;
-        pR[b * st.kc + a] = S::neg(v);
-      }
+  }
+  T* pR = (T*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
+  for (int q = tid; q < m * m; q += nt) {
+    const int a = q / m, b = q % m;
+    if (a == b) pR[a * st.kc + a] = S::zero();
+    else if (a < b) {
+      const T v = ok ? S::scale(S::sub(Ri[a * kMaxC + b], Ri[b * kMaxC + a]), 0.5) : S::zero();
+      pR[a * st.kc + b] = v;
+      pR[b * st.kc + a] = S::neg(v);
     }
   }
 }
