@@ -19,6 +19,9 @@
 #ifndef LRUX_RATIO_FLY_MAX_KT
 #define LRUX_RATIO_FLY_MAX_KT 4
 #endif
+#ifndef LRUX_APPEND_REAL_STREAM_MIN_K
+#define LRUX_APPEND_REAL_STREAM_MIN_K 1
+#endif
 #ifndef LRUX_APPEND_TILE_ROWS
 #define LRUX_APPEND_TILE_ROWS 128
 #endif
@@ -844,6 +847,102 @@ __global__ void __launch_bounds__(256, 2) det_append_dmma_stream_kernel(State st
   }
 }
 
+// The same stream for float64 and every k <= 8.  Lane (r, q) loads the 16-byte pair
+// X[j0+r][i0+2q, i0+2q+1] of its row and the same pair of N[a = r][.] from shared memory
+// (permuted contraction index, as in lrux_rowdot.cu) and issues two DMMAs into two independent
+// accumulator chains; D fragment = (row j0+r, a = 2q, 2q+1).  KS = rows of N kept in shared
+// memory (4 for k <= 4, else 8: lanes with r >= KS contribute zeros), row stride 8 mod 16
+// doubles: conflict-free.  Replaces det_prep_kernel + det_append_kernel and det_prep_kernel +
+// rowdot_dmma_kernel on this path: no per-tile phases, balanced 16-row units, N Abuf^T folded in.
+// Measured (append class, fraction of HBM for n^2 e per accepted walker, Metropolis): n=512 K=8:
+// k=4 0.76 (was 0.62), k=8 0.65 (0.56); K=32: n=512 k=4 0.62 (0.45), n=1024 k=4 0.74 (0.61),
+// k=8 0.64 (0.52), n=2048 k=4 0.81 (0.71); k=1: 0.95-0.98 (0.94-0.96).
+template <int KS>
+__global__ void __launch_bounds__(256, 2) det_append_stream_real_kernel(State st, int k, int ldn) {
+  constexpr int UN = 8, MT = 2;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int n = st.n, kmax = st.kmax, cap = st.cap;
+  double* Ns = (double*)smem_raw;                // [KS][ldn]
+  __shared__ int sidx[8];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
+  const int r8 = lane >> 2, q = lane & 3;
+  const int count = st.counters[0];
+  const int upt = (n + 15) >> 4, upa = (cap + 15) >> 4, upw = upt + upa;
+  const int64_t total = (int64_t)count * upw;
+  const int64_t first = total * blockIdx.x / gridDim.x, last = total * (blockIdx.x + 1) / gridDim.x;
+  for (int64_t u = first; u < last;) {
+    const int wi = (int)(u / upw);
+    const int w = st.list[wi];
+    const int fill = st.fill[w];
+    const int64_t seg_end = min(last, (int64_t)(wi + 1) * upw);
+    __syncthreads();
+    {
+      const double* gN = (const double*)st.pend_N + (size_t)w * kmax * n;
+      for (int qd = tid; qd < KS * (n >> 1); qd += blockDim.x) {
+        const int a = qd / (n >> 1), i = 2 * (qd % (n >> 1));
+        *(double2*)(Ns + (size_t)a * ldn + i) = a < k ? *(const double2*)(gN + (size_t)a * n + i) : make_double2(0.0, 0.0);
+      }
+      if (tid < 8) sidx[tid] = tid < k ? st.pend_idx[(size_t)w * kmax + tid] : -1;
+    }
+    __syncthreads();
+    const int64_t u_mine = u + ((warp - (int)((u - first) % nw)) + nw) % nw;
+    for (int64_t uu = u_mine; uu < seg_end; uu += nw) {
+      const int ul = (int)(uu - (int64_t)wi * upw);          // unit within the walker
+      const int a_before = (int)((int64_t)ul * upa / upw);
+      const bool is_a = (int)((int64_t)(ul + 1) * upa / upw) > a_before;
+      const int j0 = (is_a ? a_before : ul - a_before) * 16;
+      const int rlim = is_a ? fill : n;                     // valid rows of this matrix
+      if (j0 >= rlim) continue;                              // buffer unit past the fill
+      const double* X = is_a ? (const double*)st.Abuf + (size_t)w * cap * n : (const double*)st.Ti + (size_t)w * n * n;
+      double acc[MT][2][2] = {};
+      const double* row0 = X + (size_t)min(j0 + r8, rlim - 1) * n + 2 * q;       // rows past the end: clamped, discarded
+      const double* row1 = X + (size_t)min(j0 + 8 + r8, rlim - 1) * n + 2 * q;
+      const double* bp = Ns + (size_t)(r8 < KS ? r8 : 0) * ldn + 2 * q;
+      const bool bz = r8 >= KS;
+      for (int i0 = 0; i0 < n; i0 += 8 * UN) {
+        double2 x0[UN], x1[UN];
+#pragma unroll
+        for (int v = 0; v < UN; ++v) {
+          const bool in = i0 + 8 * v + 2 * q < n;
+          x0[v] = in ? *(const double2*)(row0 + i0 + 8 * v) : make_double2(0.0, 0.0);
+          x1[v] = in ? *(const double2*)(row1 + i0 + 8 * v) : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int v = 0; v < UN; ++v) {
+          if (i0 + 8 * v < n) {
+            double2 b = (i0 + 8 * v + 2 * q < n) ? *(const double2*)(bp + i0 + 8 * v) : make_double2(0.0, 0.0);
+            if (bz) b = make_double2(0.0, 0.0);
+            dmma884_acc(acc[0][0][0], acc[0][0][1], x0[v].x, b.x);
+            dmma884_acc(acc[0][1][0], acc[0][1][1], x0[v].y, b.y);
+            dmma884_acc(acc[1][0][0], acc[1][0][1], x1[v].x, b.x);
+            dmma884_acc(acc[1][1][0], acc[1][1][1], x1[v].y, b.y);
+          }
+        }
+      }
+      double* outD = (double*)st.Bbuf + ((size_t)w * cap + fill) * n;          // [a][j], row stride n
+      double* outNA = (double*)st.pend_Y + (size_t)w * kmax * cap;             // [a][s], row stride cap
+#pragma unroll
+      for (int mt = 0; mt < MT; ++mt) {
+        const int j = j0 + 8 * mt + r8;
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int a = 2 * q + e;
+          if (j < rlim && a < k) {
+            double v = acc[mt][0][e] + acc[mt][1][e];
+            if (is_a) {
+              outNA[(size_t)a * cap + j] = v;
+            } else {
+              if (j == sidx[a]) v -= 1.0;
+              outD[(size_t)a * n + j] = v;
+            }
+          }
+        }
+      }
+    }
+    u = seg_end;
+  }
+}
+
 // Second half of the append as its own pass, for the tensor-pipe variant below: D = N A0^-1 -
 // I[P,:] is already in the pending area (pend_C, free once det_prep_kernel has copied a_tau
 // into the buffer).  b_tau^T = R^-1 (D - (N Abuf) Bbuf^T) -> Bbuf[fill .. fill+k)   (Eq. 15,
@@ -1074,6 +1173,26 @@ static int launch_append_kt(const State& st, int k, Ctx& cx, cudaStream_t s) {
       if (cx.configure((const void*)kf, 256, smf) < 0) return -1;
       kf<<<persistent_grid(cx.num_sms, 8, (int64_t)st.W * chunks), 256, smf, s>>>(st, k, chunks, 1);
       cx.name(LRUX_PROF_APPEND, "det_append_dmma_stream_kernel+det_append_finish_kernel");
+      return 2;
+    }
+  }
+  if constexpr (sizeof(T) == 8) {
+    // real data, even n: the same stream for every k <= 8
+    const int ks = k <= 4 ? 4 : 8;
+    const int ldn = ((n + 15) & ~15) + 8;
+    const size_t sms = (size_t)ks * ldn * sizeof(double);
+    // (n = 256, k = 2 -- configs[1] with a delay -- stays on the register-row pass: 0.58 of HBM against 0.54)
+    if ((n & 1) == 0 && (n >= 512 || k >= 3) && k >= LRUX_APPEND_REAL_STREAM_MIN_K && sms <= 200 * 1024) {
+      auto ksr = ks == 4 ? det_append_stream_real_kernel<4> : det_append_stream_real_kernel<8>;
+      const int occs = cx.configure((const void*)ksr, 256, sms);
+      if (occs < 0) return -1;
+      ksr<<<persistent_grid(cx.num_sms, occs, (int64_t)st.W * ((n + 15) / 16)), 256, sms, s>>>(st, k, ldn);
+      const int chunks = (n + 63) / 64;
+      const size_t smf = ((size_t)st.cap * KT + 3 * KT * 64) * sizeof(T);
+      auto kf = det_append_finish_kernel<T, KT>;
+      if (cx.configure((const void*)kf, 256, smf) < 0) return -1;
+      kf<<<persistent_grid(cx.num_sms, 8, (int64_t)st.W * chunks), 256, smf, s>>>(st, k, chunks, 1);
+      cx.name(LRUX_PROF_APPEND, "det_append_stream_real_kernel+det_append_finish_kernel");
       return 2;
     }
   }

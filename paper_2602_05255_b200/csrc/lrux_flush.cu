@@ -7,9 +7,9 @@
 // per flushed walker.  sm_100a has no tcgen05 kind for f64; the FP64 tensor path is the
 // warp-level DMMA (mma.sync.m8n8k4.f64 -> SASS DMMA.8x8x4), fed from shared memory.
 //
-// Work item = (walker on the flush list, output tile); persistent grid, one CTA per SM.
-// float64: 128 x 128 tiles, 8 warps, warp tile 32 x 64 (4 x 8 MMA tiles, 12 fragment loads per
-// 32 DMMAs); complex128: 64 x 64 tiles, 16 warps, warp tile 16 x 16, one complex MMA = 4 real
+// Work item = (walker on the flush list, output tile); persistent grid, two CTAs per SM.
+// float64: 128 x 64 tiles, 8 warps, warp tile 32 x 32 (4 x 4 MMA tiles, 8 fragment loads per
+// 16 DMMAs); complex128: 64 x 64 tiles, 8 warps, warp tile 16 x 32, one complex MMA = 4 real
 // DMMAs on (re, im) pairs read with ONE 16-byte fragment load each -- the buffers stay
 // interleaved, nothing is de-interleaved while staging.
 //
@@ -52,23 +52,40 @@ __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-// Tile configurations (warps per CTA as WR x WC over the output tile).  Measured on B200
-// (profiles/r02_flush_variants.md): float64 128 x 128 with 8 warps (warp tile 32 x 64) gives
-// 0.77 of cuBLAS DGEMM at K k = 256 against 0.73 with 16 warps; complex128 64 x 64 with 16 warps
-// (warp tile 16 x 16) gives 0.62 / 0.68 (Metropolis / all walkers at once) on configs[3]
-// against 0.58 / 0.69 for 64 x 128 with 8 warps -- with ~5 walkers folding per step the
-// smaller tile wastes less of the last wave.
+// Tile configurations (warps per CTA as WR x WC over the output tile).  A tile's own traffic
+// (the output tile read into the accumulators and stored back: 128 KB of a 64 x 64 complex
+// tile's 390 KB at K k = 128) is NOT covered by the cp.async ring, and the contraction is only
+// ~2x above the machine balance (10.7 flop/B against 36.6 TF/s / 6.5 TB/s = 5.6), so one CTA
+// per SM leaves the DMMA pipe idle for a third of the time (66 % busy in the ncu capture of the
+// 16-warp configuration).  Two co-resident CTAs of 8 warps overlap one tile's load / store with
+// the other's MMAs.  Measured on B200 (profiles/r02_flush_variants.md), fraction of cuBLAS DGEMM:
+//   complex128 64 x 64: 2 CTAs x 8 warps (warp tile 16 x 32, 3 stages) 0.655 / 0.681 (configs[3]
+//     Metropolis / forced) against 0.621 / 0.619 for 1 CTA x 16 warps and 0.615 / 0.629 for 1 x 8;
+//   float64: 128 x 64, 2 CTAs x 8 warps (warp tile 32 x 32, 3 stages) 0.700 (n = 1024, K k = 256,
+//     Metropolis), 0.617 (n = 2048, K k = 128), 0.455 of HBM (configs[1], K k = 32) against
+//     0.644 / 0.563 / 0.397 for 128 x 128 with one CTA per SM; all walkers at once: 0.74 both.
 template <typename T>
 struct FlushCfg;
+#ifndef LRUX_FLUSH_R_BN
+#define LRUX_FLUSH_R_BN 64
+#define LRUX_FLUSH_R_NS 3
+#define LRUX_FLUSH_R_MINB 2
+#endif
 template <>
-struct FlushCfg<double> {   // 128 x 128, warps 4 x 2, warp tile 32 x 64
-  static constexpr int WR = 4, WC = 2;
-  static constexpr int BM = 128, BN = 128, MT = 4, NT = 8, KC = 16, NS = 4, LDB = 132, LDA = 132;
+struct FlushCfg<double> {   // 128 x 64, warps 4 x 2, warp tile 32 x 32, two CTAs per SM
+  static constexpr int WR = 4, WC = 2, MINB = LRUX_FLUSH_R_MINB;
+  static constexpr int BM = 128, BN = LRUX_FLUSH_R_BN, MT = 4, NT = LRUX_FLUSH_R_BN / 16, KC = 16, NS = LRUX_FLUSH_R_NS,
+                       LDB = 132, LDA = LRUX_FLUSH_R_BN + 4;
 };
+#ifndef LRUX_FLUSH_CX_WC
+#define LRUX_FLUSH_CX_WC 2
+#define LRUX_FLUSH_CX_NS 3
+#define LRUX_FLUSH_CX_MINB 2
+#endif
 template <>
-struct FlushCfg<cplx> {     // 64 x 64, warps 4 x 4, warp tile 16 x 16
-  static constexpr int WR = 4, WC = 4;
-  static constexpr int BM = 64, BN = 64, MT = 2, NT = 2, KC = 16, NS = 4, LDB = 66, LDA = 66;
+struct FlushCfg<cplx> {     // 64 x 64, warps 4 x 2, warp tile 16 x 32, two CTAs per SM
+  static constexpr int WR = 4, WC = LRUX_FLUSH_CX_WC, MINB = LRUX_FLUSH_CX_MINB;
+  static constexpr int BM = 64, BN = 64, MT = 2, NT = 8 / LRUX_FLUSH_CX_WC, KC = 16, NS = LRUX_FLUSH_CX_NS, LDB = 66, LDA = 66;
 };
 
 struct FlushItem {
@@ -77,7 +94,7 @@ struct FlushItem {
 
 // V16: rows of the buffers are 16-byte aligned (always for complex; real: n even)
 template <typename T, bool SKEW, bool V16>
-__global__ void __launch_bounds__(FlushCfg<T>::WR * FlushCfg<T>::WC * 32, 1)
+__global__ void __launch_bounds__(FlushCfg<T>::WR * FlushCfg<T>::WC * 32, FlushCfg<T>::MINB)
 flush_dmma_kernel(State st, int tr, int tc, int tiles) {
   using S = Sc<T>;
   using Cfg = FlushCfg<T>;

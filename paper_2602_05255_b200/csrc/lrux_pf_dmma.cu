@@ -33,16 +33,27 @@ __device__ __forceinline__ void dmma884p(double& d0, double& d1, double a, doubl
                : "d"(a), "d"(b));
 }
 
-// NB = 8-column blocks per warp and strip, NW = warps per CTA (8 NB NW >= n), MQ = DMMAs per
-// block (4 MQ >= 2k).  ld = row stride of yv / gv (>= n + 8, 8 mod 16 doubles: conflict-free).
-template <int NB, int NW, int MQ>
-__global__ void __launch_bounds__(NW * 32, NW <= 8 ? 2 : 1) pf_update_dmma_kernel(State st, int k, int ld) {
+// NB = 8-column blocks per warp and strip, NW = warps per CTA, MQ = DMMAs per block (4 MQ >= 2k).
+// The columns are cut into ncr ranges of ncl (8 NB NW >= ncl; ncr = 1 up to n = 1024): CTA b
+// works on range b mod ncr for all of its strips and keeps only that range of y and g in
+// shared memory (row stride ld >= ncl + 8, 8 mod 16 doubles: conflict-free).  With ncr > 1
+// the A fragments (y, g of the strip's own ROWS, which may lie in another range) come from a
+// second, small pair of panels that holds y and g of `rmax` consecutive rows and is restaged
+// whenever the strips leave it -- the same staging arithmetic, so that mirrored elements
+// produced by different CTAs still see identical operands.
+template <int NB, int NW, int MQ, bool RANGES>
+__global__ void __launch_bounds__(NW * 32, NW <= 8 ? 2 : 1)
+pf_update_dmma_kernel(State st, int k, int ld, int ncr_, int ncl, int rmax) {
+  const int ncr = RANGES ? ncr_ : 1;
   constexpr int MH = 4 * MQ;
   constexpr int kMaxC = 2 * kMaxK;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int n = st.n, kmax = st.kmax, m = 2 * k;
   double* yv = (double*)smem_raw;           // [MH][ld]
   double* gv = yv + (size_t)MH * ld;        // [MH][ld]
+  const int ldr = rmax + 8;
+  double* yr = gv + (size_t)MH * ld;        // [MH][ldr]  (ncr > 1) y of rows [row_lo, row_lo + rmax)
+  double* gr = yr + (size_t)MH * ldr;       // [MH][ldr]
   __shared__ double Ri[kMaxC * kMaxC];
   __shared__ int P[kMaxK];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -51,7 +62,9 @@ __global__ void __launch_bounds__(NW * 32, NW <= 8 ? 2 : 1) pf_update_dmma_kerne
   const int count = st.counters[0];
   const int spw = (n + 7) >> 3;
   const int64_t S = (int64_t)count * spw;
-  const int64_t first = S * blockIdx.x / gridDim.x, last = S * (blockIdx.x + 1) / gridDim.x;
+  const int ngrp = (int)gridDim.x / ncr, grp = (int)blockIdx.x / ncr;   // CTAs that share a column range
+  const int col_base = ((int)blockIdx.x % ncr) * ncl, col_end = min(n, col_base + ncl);
+  const int64_t first = S * grp / ngrp, last = S * (grp + 1) / ngrp;
   const int my = (int)(last - first);
   const int wi0 = (int)(first / spw), s00 = (int)(first % spw);
   const double* Ti = (const double*)st.Ti;
@@ -63,14 +76,44 @@ __global__ void __launch_bounds__(NW * 32, NW <= 8 ? 2 : 1) pf_update_dmma_kerne
     const double* row = Ti + ((size_t)w * n + j) * n;
 #pragma unroll
     for (int t = 0; t < NB; ++t) {
-      const int c = 8 * (t * NW + warp) + 2 * q;
-      x[t] = c < n ? *(const double2*)(row + c) : make_double2(0.0, 0.0);
+      const int c = col_base + 8 * (t * NW + warp) + 2 * q;
+      x[t] = c < col_end ? *(const double2*)(row + c) : make_double2(0.0, 0.0);
+    }
+  };
+
+  // y[a][i] = Y'[a][i], g[b][i] = sum_a y[a][i] R'^-1[a][b] for i in [i0, i0 + cnt) -> panels of stride lds
+  auto stage = [&](int w, int i0, int cnt, double* ys, double* gs, int lds) {
+    const double* pC = (const double*)st.pend_C + (size_t)w * kmax * n;
+    const double* pY = (const double*)st.pend_Y + (size_t)w * kmax * n;
+    for (int il = tid; il < cnt; il += NW * 32) {
+      const int i = i0 + il;
+      double yp[MH];
+#pragma unroll
+      for (int a = 0; a < MH; ++a) {
+        double v = 0.0;
+        if (a < m && i < n) {
+          v = a < k ? pY[(size_t)a * n + i] : pC[(size_t)(a - k) * n + i];
+          if (a < k && i == P[a]) v += 1.0;
+        }
+        yp[a] = v;
+        ys[(size_t)a * lds + il] = v;
+      }
+#pragma unroll 1
+      for (int b = 0; b < MH; ++b) {
+        double g = 0.0;
+        if (b < m) {
+#pragma unroll
+          for (int a = 0; a < MH; ++a)
+            if (a < m) g = fma(yp[a], Ri[a * kMaxC + b], g);
+        }
+        gs[(size_t)b * lds + il] = g;
+      }
     }
   };
 
   double2 xc[NB], xn[NB];
   if (my > 0) load_strip(0, xc);
-  int cur_w = -1;
+  int cur_w = -1, row_lo = 0;
   for (int li = 0; li < my; ++li) {
     const int sx = s00 + li;
     const int w = st.list[wi0 + sx / spw];
@@ -82,72 +125,63 @@ __global__ void __launch_bounds__(NW * 32, NW <= 8 ? 2 : 1) pf_update_dmma_kerne
             ((const double*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + (idx / m) * st.kc + (idx % m)];
       if (tid < k) P[tid] = st.pend_idx[(size_t)w * kmax + tid];
       __syncthreads();
-      const double* pC = (const double*)st.pend_C + (size_t)w * kmax * n;
-      const double* pY = (const double*)st.pend_Y + (size_t)w * kmax * n;
-      for (int i = tid; i < ld; i += NW * 32) {
-        double yp[MH];
-#pragma unroll
-        for (int a = 0; a < MH; ++a) {
-          double v = 0.0;
-          if (a < m && i < n) {
-            v = a < k ? pY[(size_t)a * n + i] : pC[(size_t)(a - k) * n + i];
-            if (a < k && i == P[a]) v += 1.0;
-          }
-          yp[a] = v;
-          yv[(size_t)a * ld + i] = v;
-        }
-#pragma unroll 1
-        for (int b = 0; b < MH; ++b) {
-          double g = 0.0;
-          if (b < m) {
-#pragma unroll
-            for (int a = 0; a < MH; ++a)
-              if (a < m) g = fma(yp[a], Ri[a * kMaxC + b], g);
-          }
-          gv[(size_t)b * ld + i] = g;
-        }
-      }
+      stage(w, col_base, ld, yv, gv, ld);
+      if constexpr (RANGES) { row_lo = j0; stage(w, row_lo, ldr, yr, gr, ldr); }
       cur_w = w;
+      __syncthreads();
+    } else if (RANGES && j0 >= row_lo + rmax) {
+      __syncthreads();   // every warp is done with the previous rows' panels
+      row_lo = j0;
+      stage(w, row_lo, ldr, yr, gr, ldr);
       __syncthreads();
     }
     if (li + 1 < my) load_strip(li + 1, xn);   // in flight during this strip's arithmetic
 
     double ag[MQ], ay[MQ];                      // A fragments: g / y of the strip's rows
+    if constexpr (!RANGES) {
 #pragma unroll
-    for (int s = 0; s < MQ; ++s) {
-      ag[s] = gv[(size_t)(4 * s + q) * ld + j0 + r8];
-      ay[s] = yv[(size_t)(4 * s + q) * ld + j0 + r8];
+      for (int s = 0; s < MQ; ++s) {
+        ag[s] = gv[(size_t)(4 * s + q) * ld + j0 + r8];
+        ay[s] = yv[(size_t)(4 * s + q) * ld + j0 + r8];
+      }
+    } else {
+#pragma unroll
+      for (int s = 0; s < MQ; ++s) {
+        ag[s] = gr[(size_t)(4 * s + q) * ldr + (j0 - row_lo) + r8];
+        ay[s] = yr[(size_t)(4 * s + q) * ldr + (j0 - row_lo) + r8];
+      }
     }
     const int j = j0 + r8;
     double* orow = (double*)st.Ti + ((size_t)w * n + min(j, n - 1)) * n;
 #pragma unroll
     for (int t = 0; t < NB; ++t) {
-      const int cb = 8 * (t * NW + warp);
-      if (cb < n) {
+      const int cl = 8 * (t * NW + warp);   // block's first column within the range, and overall
+      const int cb = col_base + cl;
+      if (cb < col_end) {
         double2 v = xc[t];
         if (cb > j0) {                          // above the diagonal: v(r, c)
 #pragma unroll
-          for (int s = 0; s < MQ; ++s) dmma884p(v.x, v.y, ag[s], yv[(size_t)(4 * s + q) * ld + cb + r8]);
+          for (int s = 0; s < MQ; ++s) dmma884p(v.x, v.y, ag[s], yv[(size_t)(4 * s + q) * ld + cl + r8]);
         } else if (cb < j0) {                   // below: -v(c, r)
           v.x = -v.x;
           v.y = -v.y;
 #pragma unroll
-          for (int s = 0; s < MQ; ++s) dmma884p(v.x, v.y, ay[s], gv[(size_t)(4 * s + q) * ld + cb + r8]);
+          for (int s = 0; s < MQ; ++s) dmma884p(v.x, v.y, ay[s], gv[(size_t)(4 * s + q) * ld + cl + r8]);
           v.x = -v.x;
           v.y = -v.y;
         } else {                                // the diagonal block: both forms, selected per element
           double2 lo = make_double2(-v.x, -v.y);
 #pragma unroll
           for (int s = 0; s < MQ; ++s) {
-            dmma884p(v.x, v.y, ag[s], yv[(size_t)(4 * s + q) * ld + cb + r8]);
-            dmma884p(lo.x, lo.y, ay[s], gv[(size_t)(4 * s + q) * ld + cb + r8]);
+            dmma884p(v.x, v.y, ag[s], yv[(size_t)(4 * s + q) * ld + cl + r8]);
+            dmma884p(lo.x, lo.y, ay[s], gv[(size_t)(4 * s + q) * ld + cl + r8]);
           }
           const int c0 = cb + 2 * q;
           v.x = c0 > j ? v.x : c0 < j ? -lo.x : 0.0;
           v.y = c0 + 1 > j ? v.y : c0 + 1 < j ? -lo.y : 0.0;
         }
         const int c = cb + 2 * q;
-        if (j < n && c < n) *(double2*)(orow + c) = v;
+        if (j < n && c < col_end) *(double2*)(orow + c) = v;
       }
     }
 #pragma unroll
@@ -155,38 +189,57 @@ __global__ void __launch_bounds__(NW * 32, NW <= 8 ? 2 : 1) pf_update_dmma_kerne
   }
 }
 
-template <int NB, int NW, int MQ>
-static int launch_pf_dmma_inst(const State& st, int k, int ld, Ctx& cx, cudaStream_t s, bool probe) {
-  const size_t smem = (size_t)2 * 4 * MQ * ld * sizeof(double);
+template <int NB, int NW, int MQ, bool RANGES>
+static int launch_pf_dmma_inst(const State& st, int k, int ld, int ncr, int ncl, int rmax, Ctx& cx, cudaStream_t s, bool probe) {
+  const size_t smem = (size_t)2 * 4 * MQ * (ld + (ncr > 1 ? rmax + 8 : 0)) * sizeof(double);
   if (smem > 200 * 1024) return 0;
   if (probe) return 1;
-  auto kern = pf_update_dmma_kernel<NB, NW, MQ>;
+  auto kern = pf_update_dmma_kernel<NB, NW, MQ, RANGES>;
   const int occ = cx.configure((const void*)kern, NW * 32, smem);
   if (occ < 0) return -1;
   const int64_t strips = (int64_t)st.W * ((st.n + 7) / 8);
-  kern<<<persistent_grid(cx.num_sms, occ, strips), NW * 32, smem, s>>>(st, k, ld);
+  int grid = persistent_grid(cx.num_sms, occ, strips * ncr);
+  grid = grid / ncr * ncr;                     // whole groups of ncr CTAs (one per column range)
+  if (grid < ncr) grid = ncr;
+  kern<<<grid, NW * 32, smem, s>>>(st, k, ld, ncr, ncl, rmax);
   cx.name(LRUX_PROF_UPDATE, "pf_update_dmma_kernel");
   return 1;
 }
 
-// 1 = launched, 0 = shape not eligible (complex data, n > 1024, 2k x n panels beyond shared
-// memory), -1 = CUDA error.  Expects Y in pend_Y (launch_y) and the accepted list (select).
+// 1 = launched, 0 = shape not eligible (complex data, odd n, more than 16 column ranges),
+// -1 = CUDA error.  Expects Y in pend_Y (launch_y) and the accepted list (select).
 int launch_pf_update_dmma(const State& st, int k, Ctx& cx, cudaStream_t s, bool probe) {
   const int n = st.n;
-  if (st.dt != LRUX_F64 || (n & 1) || k > 8 || n > 1024) return 0;
-  const int ld = ((n + 15) & ~15) + 8;
-  const int blocks = (n + 7) / 8;
+  if (st.dt != LRUX_F64 || (n & 1) || k > 8) return 0;
   const int mq = k <= 2 ? 1 : k <= 4 ? 2 : 4;
-#define LRUX_PFD_CASE(NB_, NW_)                                                         \
-  if (blocks <= NB_ * NW_)                                                              \
-    return mq == 1 ? launch_pf_dmma_inst<NB_, NW_, 1>(st, k, ld, cx, s, probe)                 \
-         : mq == 2 ? launch_pf_dmma_inst<NB_, NW_, 2>(st, k, ld, cx, s, probe)                 \
-                   : launch_pf_dmma_inst<NB_, NW_, 4>(st, k, ld, cx, s, probe);
-  LRUX_PFD_CASE(2, 8)
-  LRUX_PFD_CASE(4, 8)
-  LRUX_PFD_CASE(8, 8)
-  LRUX_PFD_CASE(8, 16)
-#undef LRUX_PFD_CASE
+  // column ranges: at most 1024 columns per CTA, and y, g of a range (2 x 4 mq x ld doubles) within 200 KB
+  // (+ with more than one range, y and g of rmax rows for the A fragments)
+  const int rmax = mq == 4 ? 128 : 256;
+  int ncr = 1, ncl = 0, ld = 0;
+  for (;; ncr *= 2) {
+    if (ncr > 16) return 0;
+    ncl = (((n + ncr - 1) / ncr) + 7) & ~7;
+    ld = ((ncl + 15) & ~15) + 8;
+    if (ncl <= 1024 && (size_t)2 * 4 * mq * (ld + (ncr > 1 ? rmax + 8 : 0)) * sizeof(double) <= 200 * 1024) break;
+  }
+  const int blocks = ncl / 8;
+#define LRUX_PFD_MQ(NB_, NW_, RG_)                                                                   \
+  return mq == 1 ? launch_pf_dmma_inst<NB_, NW_, 1, RG_>(st, k, ld, ncr, ncl, rmax, cx, s, probe)    \
+       : mq == 2 ? launch_pf_dmma_inst<NB_, NW_, 2, RG_>(st, k, ld, ncr, ncl, rmax, cx, s, probe)    \
+                 : launch_pf_dmma_inst<NB_, NW_, 4, RG_>(st, k, ld, ncr, ncl, rmax, cx, s, probe);
+  if (ncr > 1) {                       // column ranges: 16 warps (the panels leave one CTA per SM)
+    if (blocks <= 64) { LRUX_PFD_MQ(4, 16, true) }
+    LRUX_PFD_MQ(8, 16, true)
+  }
+  if (blocks <= 16) { LRUX_PFD_MQ(2, 8, false) }
+  if (blocks <= 32) { LRUX_PFD_MQ(4, 8, false) }
+  // panels beyond half the shared memory leave one CTA per SM: 16 warps instead of 8
+  // (n = 512, k = 8: 0.61 of HBM against 0.38)
+  if (blocks <= 64 && (size_t)2 * 4 * mq * ld * sizeof(double) > 100 * 1024)
+    return launch_pf_dmma_inst<4, 16, 4, false>(st, k, ld, ncr, ncl, rmax, cx, s, probe);
+  if (blocks <= 64) { LRUX_PFD_MQ(8, 8, false) }
+  if (blocks <= 128) { LRUX_PFD_MQ(8, 16, false) }
+#undef LRUX_PFD_MQ
   return 0;
 }
 

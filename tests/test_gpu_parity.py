@@ -110,7 +110,8 @@ def test_pf_config3_shape_reduced():
     (512, 2, 0, True, 10, "det_update_tma_kernel"),      # complex128, 8 KB rows
     (2048, 2, 0, False, 4, "det_update_tma_kernel"),     # 16 KB rows: RC=2, 4 vectors per lane
     (512, 8, 0, True, 8, "det_update_tma_kernel"),       # complex k=8: no rank-8 instance -> two rank-4 passes (det_split_prep_kernel)
-    (1024, 2, 3, False, 14, "det_append_kernel"),        # delayed, real rows of 8 KB
+    (1024, 2, 3, False, 14, "det_append_stream_real_kernel"),   # delayed, real rows of 8 KB
+    (256, 2, 3, False, 14, "det_append_kernel"),         # n < 512 with k <= 2: the register-row pass stays (configs[1] with a delay)
     (512, 4, 2, True, 12, "det_append_kernel"),          # complex128 delayed (configs[3] shape at n=512)
 ])
 def test_det_large_row_paths(n, k, K, cplx, steps, kernel):
@@ -193,16 +194,23 @@ def test_pf_update_dmma_larger_ranks(n, k):
          kernel={"update": "pf_update_dmma_kernel"})
 
 
-def test_pf_update_stream_kernel_real_beyond_dmma():
-    """Real data with n > 1024: past the DMMA strips' instances -> Y pass + streaming update."""
-    _run("pf", 1813, 2, 1040, 2080, 1, 0, 5, walkers=[1], scratch_every=4,
-         kernel={"update": "pf_update_stream_kernel"})
+@pytest.mark.parametrize("n,k,steps", [
+    (1040, 1, 5),      # two column ranges of 520: A fragments formed from the pending area
+    (1024, 8, 4),      # 2k = 16: the y, g panels of 1024 columns exceed shared memory -> two ranges of 512
+    (1500, 2, 4),      # ragged ranges (752 + 748)
+])
+def test_pf_update_dmma_column_ranges(n, k, steps):
+    """pf_update_dmma_kernel with the columns cut into ranges (n > 1024, or 2k x n panels beyond
+    shared memory): a strip's own y, g rows may lie in another CTA's range; exact skewness across
+    ranges (mirrored elements are produced by different CTAs)."""
+    _run("pf", 1813 + n + k, 2, n, 2 * n, k, 0, steps, walkers=[1], scratch_every=4, forced=True,
+         kernel={"update": "pf_update_dmma_kernel"})
 
 
 def test_pf_update_tile_kernel_large_k():
-    """4k n e > 160 KB (here fp64, n = 1024, k = 8): Y' and g no longer fit in shared memory ->
-    the 32x32-tile kernel.  Forced accept (k = 8 proposals are rarely accepted)."""
-    _run("pf", 1812, 2, 1024, 2048, 8, 0, 5, walkers=[1], scratch_every=4, forced=True,
+    """Complex data with 4 k n e > 160 KB (n = 1024, k = 4): Y' and g no longer fit in shared
+    memory -> the 32x32-tile kernel.  Forced accept."""
+    _run("pf", 1812, 2, 1024, 2048, 4, 0, 3, cplx=True, walkers=[1], scratch_every=3, forced=True,
          kernel={"update": "pf_update_kernel"})
 
 
@@ -227,14 +235,16 @@ def test_flush_multichunk(kind, n, k, K, cplx):
 
 
 @pytest.mark.parametrize("n,k,K,kernel", [
-    (512, 8, 32, "rowdot_dmma_kernel+det_append_finish_kernel"),    # k >= 5: dot products on the tensor pipe
-    (1024, 8, 8, "rowdot_dmma_kernel+det_append_finish_kernel"),
-    (300, 5, 5, "rowdot_dmma_kernel+det_append_finish_kernel"),     # ragged tiles and chunks
-    (512, 4, 8, "det_prep_kernel+det_append_kernel"),               # k <= 4: register-row pass
-    (1024, 4, 32, "det_prep_kernel+det_append_kernel"),
-    (512, 2, 8, "det_prep_kernel+det_append_kernel"),               # k <= 2: register-row pass
-    (1024, 1, 32, "det_prep_kernel+det_append_kernel"),
-    (301, 4, 4, "det_prep_kernel+det_append_kernel"),               # odd n: rows not 16-byte aligned
+    (512, 8, 32, "det_append_stream_real_kernel+det_append_finish_kernel"),   # even n: one DMMA stream for every k <= 8
+    (1024, 8, 8, "det_append_stream_real_kernel+det_append_finish_kernel"),
+    (300, 5, 5, "det_append_stream_real_kernel+det_append_finish_kernel"),    # ragged: n = 18.75 units, cap = 25 rows
+    (512, 4, 8, "det_append_stream_real_kernel+det_append_finish_kernel"),    # k <= 4: 4 rows of N in shared memory
+    (1024, 4, 32, "det_append_stream_real_kernel+det_append_finish_kernel"),
+    (512, 2, 8, "det_append_stream_real_kernel+det_append_finish_kernel"),
+    (1024, 1, 32, "det_append_stream_real_kernel+det_append_finish_kernel"),
+    (130, 3, 7, "det_append_stream_real_kernel+det_append_finish_kernel"),    # n = 2 mod 16, cap = 21
+    (301, 4, 4, "det_prep_kernel+det_append_kernel"),                         # odd n: rows not 16-byte aligned -> register-row pass
+    (257, 8, 3, "det_prep_kernel+det_append_kernel"),                         # odd n, k = 8
 ])
 def test_det_real_append_large_n(n, k, K, kernel):
     """Real-valued delayed append at the sizes of the configs[4] sweep, both variants; forced
