@@ -13,7 +13,8 @@
  *  - `stream` is a cudaStream_t passed as void*.  Every call is asynchronous and
  *    stream-ordered on it; no call synchronises the device.
  *  - Matrices are row-major.  LRUX_C128 data is interleaved (re,im) doubles at the
- *    ABI.  All transposes in the method are plain, never conjugate.
+ *    ABI; every LRUX_C128 array must be 16-byte aligned (the kernels move a complex
+ *    element with one 16-byte access).  All transposes in the method are plain, never conjugate.
  *  - Host-detectable misuse returns a status and does nothing.  Conditions only
  *    visible on the device set sticky bits in d_info[w] and never trap:
  *      1 = singular A0 at init (zero pivot)

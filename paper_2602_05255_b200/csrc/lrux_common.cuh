@@ -12,7 +12,13 @@ namespace lrux {
 constexpr int kMaxK = 8;   // largest rank of the register / shared-memory kernels (k > 8: lrux_det_big.cu)
 
 // ---------------------------------------------------------------- scalars
-struct cplx {
+// 16-byte aligned: one LDG.128 / STG.128 per element instead of two 8-byte accesses (the ncu
+// capture of the complex flush showed 8 of every 32-byte sector used per store instruction).
+// Every complex array at the ABI must therefore be 16-byte aligned (include/lrux.h).
+#ifndef LRUX_CPLX_ALIGN
+#define LRUX_CPLX_ALIGN 16
+#endif
+struct __align__(LRUX_CPLX_ALIGN) cplx {
   double re, im;
 };
 
@@ -167,10 +173,9 @@ __device__ inline T small_det_inv(T* a, T* inv, int k, int ld, bool* ok) {
 // lane l < 2k owns column l of the augmented matrix [a | inv].  Every element goes through the
 // operations of small_det_inv in the same order, so det and inv are bit-identical to the
 // serial routine -- at k = 8 the serial one was the longest phase of the ratio kernel.
-template <typename T>
+template <typename T, int KM = 2 * kMaxK>   // KM >= k: size of the per-lane multiplier array
 __device__ inline T warp_det_inv(T* a, T* inv, int k, int ld, bool* ok, int lane) {
   using S = Sc<T>;
-  constexpr int KM = 2 * kMaxK;
   const bool act = lane < 2 * k;
   T* col = lane < k ? a + lane : inv + (lane - k);   // this lane's column, stride ld
   if (act && lane >= k)

@@ -19,6 +19,13 @@
 #ifndef LRUX_RATIO_FLY_MAX_KT
 #define LRUX_RATIO_FLY_MAX_KT 4
 #endif
+// CTAs per SM the ratio kernel is compiled for (64 registers; complex k = 8 keeps 128: it would spill)
+#ifndef LRUX_RATIO_MINB
+#define LRUX_RATIO_MINB 4
+#endif
+#ifndef LRUX_RATIO_FLY_MAX_KT_CX
+#define LRUX_RATIO_FLY_MAX_KT_CX 2
+#endif
 #ifndef LRUX_APPEND_REAL_STREAM_MIN_K
 #define LRUX_APPEND_REAL_STREAM_MIN_K 1
 #endif
@@ -42,13 +49,15 @@ namespace lrux {
 // order (deterministic) -- or, with KT = 8, forms R from the complete stash --
 // and evaluates r = det R by a k x k LU in one thread.
 template <typename T, int KT, int EPT>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, (sizeof(T) == 16 && KT == 8) ? 2 : LRUX_RATIO_MINB)
 det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __restrict__ rows,
                  T* __restrict__ ratio_out) {
   using S = Sc<T>;
   // k x k accumulators in registers up to k = 4; at k = 8 the 64 accumulators cost 161 registers
   // (one CTA per SM, 4.2 ms per step at n = 512, W = 8192): R comes from the complete stash instead
-  constexpr bool FLY = KT <= LRUX_RATIO_FLY_MAX_KT;
+  // (complex: up to k = 2 -- at k = 4 the 32 accumulator doubles meant 102 registers, two CTAs per SM and
+  // 6.9 waves for configs[3]: 180 us per step)
+  constexpr bool FLY = KT <= (sizeof(T) == 8 ? LRUX_RATIO_FLY_MAX_KT : LRUX_RATIO_FLY_MAX_KT_CX);
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* Bp = (T*)smem_raw;  // [fill][KT]: b_t^T v = Bbuf[s][P[a]]
   __shared__ T Rs[kMaxK * kMaxK];
@@ -211,7 +220,7 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
   __syncthreads();
   if (warp == 0) {   // k x k elimination by one warp (bit-identical to the serial small_det_inv)
     bool ok;
-    const T det = warp_det_inv(Rs, Ri, k, kMaxK, &ok, lane);
+    const T det = warp_det_inv<T, KT>(Rs, Ri, k, kMaxK, &ok, lane);
     if (lane == 0) {
       ratio_out[w] = det;
       ((T*)st.pend_ratio)[w] = det;

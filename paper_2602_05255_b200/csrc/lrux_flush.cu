@@ -64,6 +64,9 @@ __device__ __forceinline__ void cp_async_wait() {
 //   float64: 128 x 64, 2 CTAs x 8 warps (warp tile 32 x 32, 3 stages) 0.700 (n = 1024, K k = 256,
 //     Metropolis), 0.617 (n = 2048, K k = 128), 0.455 of HBM (configs[1], K k = 32) against
 //     0.644 / 0.563 / 0.397 for 128 x 128 with one CTA per SM; all walkers at once: 0.74 both.
+#ifndef LRUX_FLUSH_PREFETCH
+#define LRUX_FLUSH_PREFETCH 1
+#endif
 template <typename T>
 struct FlushCfg;
 #ifndef LRUX_FLUSH_R_BN
@@ -195,6 +198,19 @@ flush_dmma_kernel(State st, int tr, int tc, int tiles) {
   for (int i = 0; i < my_items; ++i) {
     const FlushItem it = decode(i);
     T* Tw = (T*)st.Ti + (size_t)it.w * n * n;
+#if LRUX_FLUSH_PREFETCH
+    // the NEXT item's output tile on its way into L2 while this one is contracted: its
+    // accumulator loads (outside the cp.async ring) then hit L2 instead of waiting on DRAM
+    if (i + 1 < my_items) {
+      const FlushItem nx = decode(i + 1);
+      const T* Tn = (const T*)st.Ti + (size_t)nx.w * n * n;
+      constexpr int LPR = BN * (int)sizeof(T) / 128;          // 128-byte lines per tile row
+      for (int qd = tid; qd < BM * LPR; qd += NTHR) {
+        const int r = nx.r0 + qd / LPR, c = nx.c0 + (qd % LPR) * (128 / (int)sizeof(T));
+        if (r < n && c < n) asm volatile("prefetch.global.L2 [%0];" ::"l"(Tn + (size_t)r * n + c));
+      }
+    }
+#endif
     // accumulators = the output tile (zero where nothing will be stored)
     double acc[CX ? 2 : 1][MT][NT][2];
 #pragma unroll
@@ -214,10 +230,12 @@ flush_dmma_kernel(State st, int tr, int tc, int tiles) {
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
           const bool need = row < n && col + e < n && (!SKEW || col + e > row);
-          T v = S::zero();
-          if (need) v = Tw[(size_t)row * n + col + e];
-          acc[0][mt][nt][e] = sc_re(v);
-          if (CX) acc[CX ? 1 : 0][mt][nt][e] = sc_im(v);
+          // component-wise 8-byte accesses on purpose: the DMMA accumulators keep the re and im
+          // planes in separate register pairs, a 16-byte access would need a staging quad
+          // (spills at the 128-register cap of two CTAs per SM)
+          const double* src = (const double*)(Tw + (size_t)row * n + col + e);
+          acc[0][mt][nt][e] = need ? src[0] : 0.0;
+          if (CX) acc[CX ? 1 : 0][mt][nt][e] = need ? src[1] : 0.0;
         }
       }
     }
@@ -293,14 +311,17 @@ flush_dmma_kernel(State st, int tr, int tc, int tiles) {
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
           if (col + e >= n) continue;
-          const T v = sc_from(acc[0][mt][nt][e], acc[CX ? 1 : 0][mt][nt][e], T{});
+          double* dst = (double*)(Tw + (size_t)row * n + col + e);
           if (SKEW) {
             if (col + e > row) {
-              Tw[(size_t)row * n + col + e] = v;
-              Tw[(size_t)(col + e) * n + row] = S::neg(v);
+              double* mir = (double*)(Tw + (size_t)(col + e) * n + row);
+              dst[0] = acc[0][mt][nt][e];
+              mir[0] = -acc[0][mt][nt][e];
+              if (CX) { dst[1] = acc[CX ? 1 : 0][mt][nt][e]; mir[1] = -acc[CX ? 1 : 0][mt][nt][e]; }
             }
           } else {
-            Tw[(size_t)row * n + col + e] = v;
+            dst[0] = acc[0][mt][nt][e];
+            if (CX) dst[1] = acc[CX ? 1 : 0][mt][nt][e];
           }
         }
       }

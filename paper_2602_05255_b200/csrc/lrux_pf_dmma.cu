@@ -220,6 +220,7 @@ int launch_pf_update_dmma(const State& st, int k, Ctx& cx, cudaStream_t s, bool 
     if (ncr > 16) return 0;
     ncl = (((n + ncr - 1) / ncr) + 7) & ~7;
     ld = ((ncl + 15) & ~15) + 8;
+    // (2k = 16 with ranges narrow enough for two CTAs per SM was measured too: no gain, 0.53-0.67 either way)
     if (ncl <= 1024 && (size_t)2 * 4 * mq * (ld + (ncr > 1 ? rmax + 8 : 0)) * sizeof(double) <= 200 * 1024) break;
   }
   const int blocks = ncl / 8;
