@@ -63,10 +63,8 @@ __device__ __forceinline__ void cp_async_wait() {
 //     Metropolis / forced) against 0.621 / 0.619 for 1 CTA x 16 warps and 0.615 / 0.629 for 1 x 8;
 //   float64: 128 x 64, 2 CTAs x 8 warps (warp tile 32 x 32, 3 stages) 0.700 (n = 1024, K k = 256,
 //     Metropolis), 0.617 (n = 2048, K k = 128), 0.455 of HBM (configs[1], K k = 32) against
-//     0.644 / 0.563 / 0.397 for 128 x 128 with one CTA per SM; all walkers at once: 0.74 both.
-#ifndef LRUX_FLUSH_PREFETCH
-#define LRUX_FLUSH_PREFETCH 1
-#endif
+//     0.644 / 0.563 / 0.397 for 128 x 128 with one CTA per SM; all walkers at once: 0.67-0.74 both.
+// (An L2 prefetch of the next item's output tile was measured too: no difference.)
 template <typename T>
 struct FlushCfg;
 #ifndef LRUX_FLUSH_R_BN
@@ -198,19 +196,6 @@ flush_dmma_kernel(State st, int tr, int tc, int tiles) {
   for (int i = 0; i < my_items; ++i) {
     const FlushItem it = decode(i);
     T* Tw = (T*)st.Ti + (size_t)it.w * n * n;
-#if LRUX_FLUSH_PREFETCH
-    // the NEXT item's output tile on its way into L2 while this one is contracted: its
-    // accumulator loads (outside the cp.async ring) then hit L2 instead of waiting on DRAM
-    if (i + 1 < my_items) {
-      const FlushItem nx = decode(i + 1);
-      const T* Tn = (const T*)st.Ti + (size_t)nx.w * n * n;
-      constexpr int LPR = BN * (int)sizeof(T) / 128;          // 128-byte lines per tile row
-      for (int qd = tid; qd < BM * LPR; qd += NTHR) {
-        const int r = nx.r0 + qd / LPR, c = nx.c0 + (qd % LPR) * (128 / (int)sizeof(T));
-        if (r < n && c < n) asm volatile("prefetch.global.L2 [%0];" ::"l"(Tn + (size_t)r * n + c));
-      }
-    }
-#endif
     // accumulators = the output tile (zero where nothing will be stored)
     double acc[CX ? 2 : 1][MT][NT][2];
 #pragma unroll
