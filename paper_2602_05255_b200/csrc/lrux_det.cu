@@ -29,6 +29,12 @@
 #ifndef LRUX_APPEND_REAL_STREAM_MIN_K
 #define LRUX_APPEND_REAL_STREAM_MIN_K 1
 #endif
+#ifndef LRUX_APPEND_REAL_STREAM_MIN_N
+#define LRUX_APPEND_REAL_STREAM_MIN_N 2
+#endif
+#ifndef LRUX_APPEND_PW_SMEM_KB
+#define LRUX_APPEND_PW_SMEM_KB 100
+#endif
 #ifndef LRUX_APPEND_TILE_ROWS
 #define LRUX_APPEND_TILE_ROWS 128
 #endif
@@ -62,7 +68,9 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
   T* Bp = (T*)smem_raw;  // [fill][KT]: b_t^T v = Bbuf[s][P[a]]
   __shared__ T Rs[kMaxK * kMaxK];
   __shared__ T Ri[kMaxK * kMaxK];
-  __shared__ T red[8][FLY ? KT * KT : 1];
+  // real k = 8: the slice's partial R by DMMA from the stash this CTA has just written (n even)
+  constexpr bool DM = !FLY && sizeof(T) == 8 && KT == 8;
+  __shared__ T red[8][(FLY || DM) ? KT * KT : 1];
   __shared__ int sP[KT];
   __shared__ int is_last;
   const int w = blockIdx.x, sp = blockIdx.y, nsplit = gridDim.y;
@@ -154,6 +162,32 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
     }
   }
   T* part = (T*)st.pend_Rpart + ((size_t)w * nsplit + sp) * kmax * kmax;
+  const bool dm = DM && (n & 1) == 0;
+  if constexpr (DM) {
+    if (dm) {
+      // R[b][a] = sum_i N[b][i] C[a][i] over this slice's columns: lane (r, q) reads the 16-byte pairs
+      // N[r][c + 2q, +1] and C[r][c + 2q, +1] (permuted contraction index), two DMMAs per 8 columns;
+      // the warps take the slice's 8-column blocks in turn.  D fragment = R[r][2q, 2q + 1].
+      __syncthreads();   // the CTA's own stores to pN / pC are visible to all of its threads
+      const int r8 = lane >> 2, q = lane & 3;
+      const int i0 = sp * kRatioSlice;
+      double d0 = 0.0, d1 = 0.0, e0 = 0.0, e1 = 0.0;
+      for (int c8 = warp * 8; c8 < kRatioSlice; c8 += nw * 8) {
+        const int col = i0 + c8 + 2 * q;
+        double2 nv = make_double2(0.0, 0.0), cv = nv;
+        if (col < n && r8 < k) {
+          nv = *(const double2*)((const double*)pN + (size_t)r8 * n + col);
+          cv = *(const double2*)((const double*)pC + (size_t)r8 * n + col);
+        }
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                     : "+d"(d0), "+d"(d1) : "d"(nv.x), "d"(cv.x));
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                     : "+d"(e0), "+d"(e1) : "d"(nv.y), "d"(cv.y));
+      }
+      ((double*)&red[warp][r8 * KT + 2 * q])[0] = d0 + e0;
+      ((double*)&red[warp][r8 * KT + 2 * q + 1])[0] = d1 + e1;
+    }
+  }
   if constexpr (FLY) {
 #pragma unroll
     for (int b = 0; b < KT; ++b)
@@ -162,6 +196,8 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
         const T v = warp_sum(racc[b][a]);
         if (lane == 0) red[warp][b * KT + a] = v;
       }
+  }
+  if (FLY || dm) {
     __syncthreads();
     if (tid < KT * KT) {
       T v = red[0][tid];
@@ -170,7 +206,7 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
       else if (tid / KT < k && tid % KT < k) part[(tid / KT) * kmax + (tid % KT)] = v;
     }
   }
-  if (nsplit > 1 || !FLY) {
+  if (nsplit > 1 || !(FLY || dm)) {
     // make this slice's stash / partial visible, then find out whether we are last
     __threadfence();
     __syncthreads();
@@ -182,7 +218,7 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
     __syncthreads();
     if (!is_last) return;
     __threadfence();
-    if constexpr (FLY) {
+    if (FLY || dm) {
       if (tid < KT * KT && tid / KT < k && tid % KT < k) {
         const T* p0 = (const T*)st.pend_Rpart + (size_t)w * nsplit * kmax * kmax +
                       (tid / KT) * kmax + (tid % KT);
@@ -866,36 +902,41 @@ __global__ void __launch_bounds__(256, 2) det_append_dmma_stream_kernel(State st
 // Measured (append class, fraction of HBM for n^2 e per accepted walker, Metropolis): n=512 K=8:
 // k=4 0.76 (was 0.62), k=8 0.65 (0.56); K=32: n=512 k=4 0.62 (0.45), n=1024 k=4 0.74 (0.61),
 // k=8 0.64 (0.52), n=2048 k=4 0.81 (0.71); k=1: 0.95-0.98 (0.94-0.96).
-template <int KS>
+// PW (small n: eight copies of N fit in shared memory): every WARP owns a contiguous range of
+// units and its own copy of N -- no CTA barrier at all.  With one shared copy a walker of 18 units
+// (n = 256) keeps the 8 warps busy for 2 or 3 units each between two barriers: 75 % at best.
+template <int KS, bool PW>
 __global__ void __launch_bounds__(256, 2) det_append_stream_real_kernel(State st, int k, int ldn) {
   constexpr int UN = 8, MT = 2;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n = st.n, kmax = st.kmax, cap = st.cap;
-  double* Ns = (double*)smem_raw;                // [KS][ldn]
-  __shared__ int sidx[8];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
+  double* Ns = (double*)smem_raw + (PW ? (size_t)warp * KS * ldn : 0);   // [KS][ldn] (per warp when PW)
+  __shared__ int sidx_s[PW ? 8 : 1][8];
+  int* sidx = sidx_s[PW ? warp : 0];
   const int r8 = lane >> 2, q = lane & 3;
   const int count = st.counters[0];
   const int upt = (n + 15) >> 4, upa = (cap + 15) >> 4, upw = upt + upa;
   const int64_t total = (int64_t)count * upw;
-  const int64_t first = total * blockIdx.x / gridDim.x, last = total * (blockIdx.x + 1) / gridDim.x;
+  const int64_t me = PW ? (int64_t)blockIdx.x * nw + warp : blockIdx.x, parts = PW ? (int64_t)gridDim.x * nw : gridDim.x;
+  const int64_t first = total * me / parts, last = total * (me + 1) / parts;
   for (int64_t u = first; u < last;) {
     const int wi = (int)(u / upw);
     const int w = st.list[wi];
     const int fill = st.fill[w];
     const int64_t seg_end = min(last, (int64_t)(wi + 1) * upw);
-    __syncthreads();
+    if (PW) __syncwarp(); else __syncthreads();
     {
       const double* gN = (const double*)st.pend_N + (size_t)w * kmax * n;
-      for (int qd = tid; qd < KS * (n >> 1); qd += blockDim.x) {
+      for (int qd = PW ? lane : tid; qd < KS * (n >> 1); qd += PW ? 32 : blockDim.x) {
         const int a = qd / (n >> 1), i = 2 * (qd % (n >> 1));
         *(double2*)(Ns + (size_t)a * ldn + i) = a < k ? *(const double2*)(gN + (size_t)a * n + i) : make_double2(0.0, 0.0);
       }
-      if (tid < 8) sidx[tid] = tid < k ? st.pend_idx[(size_t)w * kmax + tid] : -1;
+      if ((PW ? lane : tid) < 8) sidx[PW ? lane : tid] = (PW ? lane : tid) < k ? st.pend_idx[(size_t)w * kmax + (PW ? lane : tid)] : -1;
     }
-    __syncthreads();
-    const int64_t u_mine = u + ((warp - (int)((u - first) % nw)) + nw) % nw;
-    for (int64_t uu = u_mine; uu < seg_end; uu += nw) {
+    if (PW) __syncwarp(); else __syncthreads();
+    const int64_t u_mine = PW ? u : u + ((warp - (int)((u - first) % nw)) + nw) % nw;
+    for (int64_t uu = u_mine; uu < seg_end; uu += PW ? 1 : nw) {
       const int ul = (int)(uu - (int64_t)wi * upw);          // unit within the walker
       const int a_before = (int)((int64_t)ul * upa / upw);
       const bool is_a = (int)((int64_t)(ul + 1) * upa / upw) > a_before;
@@ -1189,10 +1230,11 @@ static int launch_append_kt(const State& st, int k, Ctx& cx, cudaStream_t s) {
     // real data, even n: the same stream for every k <= 8
     const int ks = k <= 4 ? 4 : 8;
     const int ldn = ((n + 15) & ~15) + 8;
-    const size_t sms = (size_t)ks * ldn * sizeof(double);
-    // (n = 256, k = 2 -- configs[1] with a delay -- stays on the register-row pass: 0.58 of HBM against 0.54)
-    if ((n & 1) == 0 && (n >= 512 || k >= 3) && k >= LRUX_APPEND_REAL_STREAM_MIN_K && sms <= 200 * 1024) {
-      auto ksr = ks == 4 ? det_append_stream_real_kernel<4> : det_append_stream_real_kernel<8>;
+    const bool pw = (size_t)8 * ks * ldn * sizeof(double) <= LRUX_APPEND_PW_SMEM_KB * 1024;   // a copy of N per warp
+    const size_t sms = (size_t)(pw ? 8 : 1) * ks * ldn * sizeof(double);
+    if ((n & 1) == 0 && (n >= LRUX_APPEND_REAL_STREAM_MIN_N || k >= 3) && k >= LRUX_APPEND_REAL_STREAM_MIN_K && sms <= 200 * 1024) {
+      auto ksr = pw ? (ks == 4 ? det_append_stream_real_kernel<4, true> : det_append_stream_real_kernel<8, true>)
+                    : (ks == 4 ? det_append_stream_real_kernel<4, false> : det_append_stream_real_kernel<8, false>);
       const int occs = cx.configure((const void*)ksr, 256, sms);
       if (occs < 0) return -1;
       ksr<<<persistent_grid(cx.num_sms, occs, (int64_t)st.W * ((n + 15) / 16)), 256, sms, s>>>(st, k, ldn);
