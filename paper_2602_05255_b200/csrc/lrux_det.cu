@@ -29,11 +29,10 @@
 #ifndef LRUX_APPEND_REAL_STREAM_MIN_K
 #define LRUX_APPEND_REAL_STREAM_MIN_K 1
 #endif
-#ifndef LRUX_APPEND_REAL_STREAM_MIN_N
-#define LRUX_APPEND_REAL_STREAM_MIN_N 2
-#endif
+// per-warp copies of N in the real stream append up to this much shared memory (n <= 256 with k <= 4:
+// n=128 k=2 0.49 of HBM against 0.40, n=256 k=4 0.57 / 0.55; beyond -- n=384, or k > 4 -- the shared copy wins)
 #ifndef LRUX_APPEND_PW_SMEM_KB
-#define LRUX_APPEND_PW_SMEM_KB 100
+#define LRUX_APPEND_PW_SMEM_KB 68
 #endif
 #ifndef LRUX_APPEND_TILE_ROWS
 #define LRUX_APPEND_TILE_ROWS 128
@@ -1232,7 +1231,9 @@ static int launch_append_kt(const State& st, int k, Ctx& cx, cudaStream_t s) {
     const int ldn = ((n + 15) & ~15) + 8;
     const bool pw = (size_t)8 * ks * ldn * sizeof(double) <= LRUX_APPEND_PW_SMEM_KB * 1024;   // a copy of N per warp
     const size_t sms = (size_t)(pw ? 8 : 1) * ks * ldn * sizeof(double);
-    if ((n & 1) == 0 && (n >= LRUX_APPEND_REAL_STREAM_MIN_N || k >= 3) && k >= LRUX_APPEND_REAL_STREAM_MIN_K && sms <= 200 * 1024) {
+    // (k <= 2 at 128 < n < 512 -- configs[1] with a delay -- stays on the register-row pass: 0.57-0.61 of HBM
+    // against 0.56-0.58 for the stream)
+    if ((n & 1) == 0 && (n >= 512 || n <= 128 || k >= 3) && k >= LRUX_APPEND_REAL_STREAM_MIN_K && sms <= 200 * 1024) {
       auto ksr = pw ? (ks == 4 ? det_append_stream_real_kernel<4, true> : det_append_stream_real_kernel<8, true>)
                     : (ks == 4 ? det_append_stream_real_kernel<4, false> : det_append_stream_real_kernel<8, false>);
       const int occs = cx.configure((const void*)ksr, 256, sms);
