@@ -339,9 +339,28 @@ det_update_kernel(State st, int k, int tiles, int rows_per_tile) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nw = blockDim.x >> 5;
   const int count = st.counters[0];
   const int nvec = n / VEC;  // vectors per row
-  for (int item = blockIdx.x; item < count * tiles; item += gridDim.x) {
-    const int w = st.list[item / tiles];
-    const int tile = item % tiles;
+  // Work unit = one pass of the CTA's warps (nw * RW rows); every CTA takes a CONTIGUOUS, equal
+  // range of the units of the concatenated accepted list, so that N, C, R^-1 are staged once per
+  // walker and CTA (they were staged per 64-row tile: 8 KB of staging per 128 KB of rows at
+  // configs[1]) and the last wave is a fraction of a unit, not of a tile.
+  (void)tiles; (void)rows_per_tile;
+  const int rpu = nw * RW;
+  const int upw = (n + rpu - 1) / rpu;
+  const int64_t total = (int64_t)count * upw;
+  const int64_t first = total * blockIdx.x / gridDim.x, last = total * (blockIdx.x + 1) / gridDim.x;
+  int wi = (int)(first / upw), ul = (int)(first % upw);   // 32-bit running (walker, unit) from here on
+  const int my = (int)(last - first);
+  bool fresh = true;
+  int w = my > 0 ? st.list[wi] : 0;
+  for (int it = 0; it < my;) {
+    if (ul == upw) { ul = 0; w = st.list[++wi]; fresh = true; }
+    // up to 4 units of the same walker in an inner loop without a barrier (the compiler overlaps
+    // their loads; one unit per barrier-carrying iteration cost 5 % at configs[1]: 0.87 of HBM
+    // against 0.94); n <= 128 -- a walker is 4-8 units -- is faster one unit at a time (0.93 / 0.89
+    // at n = 128 / 64 against 0.89 / 0.86)
+    const int nun = min(min(n <= 128 ? 1 : 4, upw - ul), my - it);
+    if (fresh) {
+    fresh = false;
     __syncthreads();
     {
       const V* gN = (const V*)((const T*)st.pend_N + (size_t)w * kmax * n);
@@ -358,9 +377,13 @@ det_update_kernel(State st, int k, int tiles, int rows_per_tile) {
       if (tid < KT) sidx[tid] = tid < k ? st.pend_idx[(size_t)w * kmax + tid] : -1;
     }
     __syncthreads();
+    }
     T* Tw = (T*)st.Ti + (size_t)w * n * n;
-    const int j_end = min(n, (tile + 1) * rows_per_tile);
-    for (int j0 = tile * rows_per_tile + warp * RW; j0 < j_end; j0 += nw * RW) {
+    const int j_end = min(n, (ul + nun) * rpu);
+    const int j_beg = ul * rpu + warp * RW;
+    ul += nun;
+    it += nun;
+    for (int j0 = j_beg; j0 < j_end; j0 += rpu) {
       V x[RW][CH];
       T d[RW][KT];
 #pragma unroll
