@@ -39,6 +39,10 @@
 #define LRUX_DMMA_MAXCOLS 1024
 #endif
 
+#ifndef LRUX_DMMA_WARP_STRIPS
+#define LRUX_DMMA_WARP_STRIPS 1
+#endif
+
 namespace lrux {
 
 namespace cg = cooperative_groups;
@@ -208,6 +212,130 @@ __global__ void __launch_bounds__(NW * 32, NW <= 8 ? 2 : 1) det_update_dmma_kern
   if constexpr (CLUSTER) cg::this_cluster().sync();   // no CTA exits while a peer may still write its cpart
 }
 
+// Narrow matrices (n <= 128): ONE WARP owns a whole 8-row strip (NB <= 16 blocks of 8 columns), so
+// the dots need no exchange and there is no barrier per strip -- only one per walker, when N and C
+// are restaged.  With the strip split over 8 warps a strip of n = 128 is 8 KB of work per CTA
+// barrier (0.31 / 0.56 of HBM at n = 64 / 128, k = 4).  Strips of a walker go round-robin to the
+// 8 warps of the CTA that holds the walker's N, C; CTAs take contiguous balanced strip ranges.
+template <int NB>
+__global__ void __launch_bounds__(256, 2) det_update_dmma_warp_kernel(State st, int k, int ncl) {
+  constexpr int KT = 8, NW = 8;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int n = st.n, kmax = st.kmax;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int r8 = lane >> 2, q = lane & 3;
+  const int ldn = ncl + 8, ldc = ncl + 2;
+  double* Ns = (double*)smem_raw;                          // [KT][ldn]
+  double* Cs2 = Ns + (size_t)KT * ldn;                     // [KT/2][ldc][2]
+  __shared__ double Ris[KT * KT];
+  __shared__ int sidx[KT];
+  const int count = st.counters[0];
+  const int spw = (n + 7) >> 3;
+  const int64_t S = (int64_t)count * spw;
+  const int64_t first = S * blockIdx.x / gridDim.x, last = S * (blockIdx.x + 1) / gridDim.x;
+  const double* Ti = (const double*)st.Ti;
+  for (int64_t u = first; u < last;) {
+    const int wi = (int)(u / spw);
+    const int w = st.list[wi];
+    const int s_beg = (int)(u - (int64_t)wi * spw);
+    const int s_end = (int)(min(last, (int64_t)(wi + 1) * spw) - (int64_t)wi * spw);
+    __syncthreads();   // every warp is done with the previous walker's N, C
+    {
+      const double* gN = (const double*)st.pend_N + (size_t)w * kmax * n;
+      const double* gC = (const double*)st.pend_C + (size_t)w * kmax * n;
+      for (int idx = tid; idx < KT * (ncl >> 1); idx += NW * 32) {
+        const int a = idx / (ncl >> 1), c = 2 * (idx % (ncl >> 1));
+        double2 nv = make_double2(0.0, 0.0), cv = nv;
+        if (a < k && c < n) {
+          nv = *(const double2*)(gN + (size_t)a * n + c);
+          cv = *(const double2*)(gC + (size_t)a * n + c);
+        }
+        *(double2*)(Ns + (size_t)a * ldn + c) = nv;
+        Cs2[((size_t)(a >> 1) * ldc + c) * 2 + (a & 1)] = cv.x;
+        Cs2[((size_t)(a >> 1) * ldc + c + 1) * 2 + (a & 1)] = cv.y;
+      }
+      if (tid < KT * KT) {
+        const int a = tid / KT, b = tid % KT;
+        Ris[tid] = (a < k && b < k) ? ((const double*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + a * st.kc + b] : 0.0;
+      }
+      if (tid < KT) sidx[tid] = tid < k ? st.pend_idx[(size_t)w * kmax + tid] : -1;
+    }
+    __syncthreads();
+    const double ri0 = Ris[r8 * KT + 2 * q], ri1 = Ris[r8 * KT + 2 * q + 1];
+    double* Tw = (double*)st.Ti + (size_t)w * n * n;
+    auto load_strip = [&](int sx, double2 (&x)[NB]) {
+      const int j = min(sx * 8 + r8, n - 1);               // rows past the end: clamped, never stored
+      const double* row = Ti + ((size_t)w * n + j) * n;
+#pragma unroll
+      for (int t = 0; t < NB; ++t) {
+        const int c = 8 * t + 2 * q;
+        x[t] = c < n ? *(const double2*)(row + c) : make_double2(0.0, 0.0);
+      }
+    };
+    constexpr bool PF = NB <= 8;       // a second strip in registers only where it fits (n <= 64)
+    double2 xc[NB], xn[PF ? NB : 1];
+    if (PF && s_beg + warp < s_end) load_strip(s_beg + warp, xc);
+    for (int sx = s_beg + warp; sx < s_end; sx += NW) {
+      if constexpr (PF) {
+        if (sx + NW < s_end) load_strip(sx + NW, (double2(&)[NB])xn);   // in flight during this strip's arithmetic
+      } else {
+        load_strip(sx, xc);
+      }
+      const int j0 = sx * 8;
+      double d0 = 0.0, d1 = 0.0, e0 = 0.0, e1 = 0.0;
+#pragma unroll
+      for (int t = 0; t < NB; ++t) {
+        if (8 * t < ncl) {
+          const double2 nv = *(const double2*)(Ns + (size_t)r8 * ldn + 8 * t + 2 * q);
+          dmma884u(d0, d1, xc[t].x, nv.x);
+          dmma884u(e0, e1, xc[t].y, nv.y);
+        }
+      }
+      d0 += e0;
+      d1 += e1;
+      if (j0 + r8 == sidx[2 * q]) d0 -= 1.0;
+      if (j0 + r8 == sidx[2 * q + 1]) d1 -= 1.0;
+      double g0 = 0.0, g1 = 0.0;
+      dmma884u(g0, g1, d0, ri0);
+      dmma884u(g0, g1, d1, ri1);
+      g0 = -g0;
+      g1 = -g1;
+      const int j = j0 + r8;
+      double* orow = Tw + (size_t)min(j, n - 1) * n;
+#pragma unroll
+      for (int t = 0; t < NB; ++t) {
+        const int cb = 8 * t;
+        if (cb < ncl) {
+          const double2 cv = *(const double2*)(Cs2 + ((size_t)q * ldc + cb + r8) * 2);
+          double2 v = xc[t];
+          dmma884u(v.x, v.y, g0, cv.x);
+          dmma884u(v.x, v.y, g1, cv.y);
+          const int c = cb + 2 * q;
+          if (j < n && c < n) *(double2*)(orow + c) = v;
+        }
+      }
+      if constexpr (PF) {
+#pragma unroll
+        for (int t = 0; t < NB; ++t) xc[t] = xn[t];
+      }
+    }
+    u = (int64_t)wi * spw + s_end;
+  }
+}
+
+template <int NB>
+static int launch_dmma_warp(const State& st, int k, int ncl, Ctx& cx, cudaStream_t s, bool probe) {
+  const size_t smem = ((size_t)8 * (ncl + 8) + (size_t)8 * (ncl + 2)) * sizeof(double);
+  if (probe) return 1;
+  auto kern = det_update_dmma_warp_kernel<NB>;
+  const int occ = cx.configure((const void*)kern, 256, smem);
+  if (occ < 0) return -1;
+  const int64_t strips = (int64_t)st.W * ((st.n + 7) / 8);
+  kern<<<persistent_grid(cx.num_sms, occ, (strips + 7) / 8), 256, smem, s>>>(st, k, ncl);
+  cx.name(LRUX_PROF_UPDATE, "det_update_dmma_warp_kernel");
+  return 1;
+}
+
 // ---------------------------------------------------------------- launcher
 // 1 = launched, 0 = shape not eligible (complex data, odd n, no instance), -1 = CUDA error.
 template <int NB, int NW>
@@ -256,6 +384,10 @@ int launch_det_update_dmma(const State& st, int k, Ctx& cx, cudaStream_t s, bool
   if (CL > 8) return 0;
   const int ncl = (((n + CL - 1) / CL) + 7) & ~7;
   const int blocks = ncl / 8;
+#if LRUX_DMMA_WARP_STRIPS
+  if (blocks <= 8) return launch_dmma_warp<8>(st, k, ncl, cx, s, probe);     // n <= 64
+  if (blocks <= 16) return launch_dmma_warp<16>(st, k, ncl, cx, s, probe);   // n <= 128
+#endif
 #define LRUX_DMMA_CASE(NB_, NW_) \
   if (blocks <= NB_ * NW_) return launch_dmma_inst<NB_, NW_>(st, k, CL, ncl, cx, s, probe);
   LRUX_DMMA_CASE(1, 8)
