@@ -25,6 +25,10 @@
 #include "lrux_common.cuh"
 #include "lrux_internal.h"
 
+#ifndef LRUX_PF_DMMA_WARP_STRIPS
+#define LRUX_PF_DMMA_WARP_STRIPS 1
+#endif
+
 namespace lrux {
 
 __device__ __forceinline__ void dmma884p(double& d0, double& d1, double a, double b) {
@@ -189,6 +193,144 @@ pf_update_dmma_kernel(State st, int k, int ld, int ncr_, int ncl, int rmax) {
   }
 }
 
+// Narrow matrices (n <= 128): ONE WARP owns a whole 8-row strip (NB <= 16 blocks) and the strips of a
+// walker go round-robin to the 8 warps of the CTA that holds the walker's y, g -- with the strip
+// split over 8 warps each warp had 1-2 blocks (0.5-1 KB) of work per loop iteration.  CTAs take
+// contiguous balanced strip ranges; the only barriers are those around the staging of y, g.
+template <int NB, int MQ>
+__global__ void __launch_bounds__(256, 2) pf_update_dmma_warp_kernel(State st, int k, int ld) {
+  constexpr int MH = 4 * MQ, NW = 8;
+  constexpr int kMaxC = 2 * kMaxK;
+  constexpr bool PF = NB <= 8;                  // a second strip in registers only where it fits
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int n = st.n, kmax = st.kmax, m = 2 * k;
+  double* yv = (double*)smem_raw;           // [MH][ld]
+  double* gv = yv + (size_t)MH * ld;        // [MH][ld]
+  __shared__ double Ri[kMaxC * kMaxC];
+  __shared__ int P[kMaxK];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int r8 = lane >> 2, q = lane & 3;
+  const int count = st.counters[0];
+  const int spw = (n + 7) >> 3;
+  const int64_t S = (int64_t)count * spw;
+  const int64_t first = S * blockIdx.x / gridDim.x, last = S * (blockIdx.x + 1) / gridDim.x;
+  for (int64_t u = first; u < last;) {
+    const int wi = (int)(u / spw);
+    const int w = st.list[wi];
+    const int s_beg = (int)(u - (int64_t)wi * spw);
+    const int s_end = (int)(min(last, (int64_t)(wi + 1) * spw) - (int64_t)wi * spw);
+    __syncthreads();   // every warp is done with the previous walker's y, g
+    for (int idx = tid; idx < m * m; idx += NW * 32)
+      Ri[(idx / m) * kMaxC + (idx % m)] =
+          ((const double*)st.pend_Rinv)[(size_t)w * st.kc * st.kc + (idx / m) * st.kc + (idx % m)];
+    if (tid < k) P[tid] = st.pend_idx[(size_t)w * kmax + tid];
+    __syncthreads();
+    {
+      const double* pC = (const double*)st.pend_C + (size_t)w * kmax * n;
+      const double* pY = (const double*)st.pend_Y + (size_t)w * kmax * n;
+      for (int i = tid; i < ld; i += NW * 32) {
+        double yp[MH];
+#pragma unroll
+        for (int a = 0; a < MH; ++a) {
+          double v = 0.0;
+          if (a < m && i < n) {
+            v = a < k ? pY[(size_t)a * n + i] : pC[(size_t)(a - k) * n + i];
+            if (a < k && i == P[a]) v += 1.0;
+          }
+          yp[a] = v;
+          yv[(size_t)a * ld + i] = v;
+        }
+#pragma unroll 1
+        for (int b = 0; b < MH; ++b) {
+          double g = 0.0;
+          if (b < m) {
+#pragma unroll
+            for (int a = 0; a < MH; ++a)
+              if (a < m) g = fma(yp[a], Ri[a * kMaxC + b], g);
+          }
+          gv[(size_t)b * ld + i] = g;
+        }
+      }
+    }
+    __syncthreads();
+    double* Tw = (double*)st.Ti + (size_t)w * n * n;
+    auto load_strip = [&](int sx, double2 (&x)[NB]) {
+      const int j = min(sx * 8 + r8, n - 1);               // rows past the end: clamped, never stored
+      const double* row = Tw + (size_t)j * n;
+#pragma unroll
+      for (int t = 0; t < NB; ++t) {
+        const int c = 8 * t + 2 * q;
+        x[t] = c < n ? *(const double2*)(row + c) : make_double2(0.0, 0.0);
+      }
+    };
+    double2 xc[NB], xn[PF ? NB : 1];
+    if (PF && s_beg + warp < s_end) load_strip(s_beg + warp, xc);
+    for (int sx = s_beg + warp; sx < s_end; sx += NW) {
+      if constexpr (PF) {
+        if (sx + NW < s_end) load_strip(sx + NW, (double2(&)[NB])xn);
+      } else {
+        load_strip(sx, xc);
+      }
+      const int j0 = sx * 8, j = j0 + r8;
+      double ag[MQ], ay[MQ];
+#pragma unroll
+      for (int s2 = 0; s2 < MQ; ++s2) {
+        ag[s2] = gv[(size_t)(4 * s2 + q) * ld + j0 + r8];
+        ay[s2] = yv[(size_t)(4 * s2 + q) * ld + j0 + r8];
+      }
+      double* orow = Tw + (size_t)min(j, n - 1) * n;
+#pragma unroll
+      for (int t = 0; t < NB; ++t) {
+        const int cb = 8 * t;
+        if (cb < n) {
+          double2 v = xc[t];
+          if (cb > j0) {                          // above the diagonal: v(r, c)
+#pragma unroll
+            for (int s2 = 0; s2 < MQ; ++s2) dmma884p(v.x, v.y, ag[s2], yv[(size_t)(4 * s2 + q) * ld + cb + r8]);
+          } else if (cb < j0) {                   // below: -v(c, r)
+            v.x = -v.x;
+            v.y = -v.y;
+#pragma unroll
+            for (int s2 = 0; s2 < MQ; ++s2) dmma884p(v.x, v.y, ay[s2], gv[(size_t)(4 * s2 + q) * ld + cb + r8]);
+            v.x = -v.x;
+            v.y = -v.y;
+          } else {                                // the diagonal block: both forms, selected per element
+            double2 lo = make_double2(-v.x, -v.y);
+#pragma unroll
+            for (int s2 = 0; s2 < MQ; ++s2) {
+              dmma884p(v.x, v.y, ag[s2], yv[(size_t)(4 * s2 + q) * ld + cb + r8]);
+              dmma884p(lo.x, lo.y, ay[s2], gv[(size_t)(4 * s2 + q) * ld + cb + r8]);
+            }
+            const int c0 = cb + 2 * q;
+            v.x = c0 > j ? v.x : c0 < j ? -lo.x : 0.0;
+            v.y = c0 + 1 > j ? v.y : c0 + 1 < j ? -lo.y : 0.0;
+          }
+          const int c = cb + 2 * q;
+          if (j < n && c < n) *(double2*)(orow + c) = v;
+        }
+      }
+      if constexpr (PF) {
+#pragma unroll
+        for (int t = 0; t < NB; ++t) xc[t] = xn[t];
+      }
+    }
+    u = (int64_t)wi * spw + s_end;
+  }
+}
+
+template <int NB, int MQ>
+static int launch_pf_dmma_warp(const State& st, int k, int ld, Ctx& cx, cudaStream_t s, bool probe) {
+  const size_t smem = (size_t)2 * 4 * MQ * ld * sizeof(double);
+  if (probe) return 1;
+  auto kern = pf_update_dmma_warp_kernel<NB, MQ>;
+  const int occ = cx.configure((const void*)kern, 256, smem);
+  if (occ < 0) return -1;
+  const int64_t strips = (int64_t)st.W * ((st.n + 7) / 8);
+  kern<<<persistent_grid(cx.num_sms, occ, (strips + 7) / 8), 256, smem, s>>>(st, k, ld);
+  cx.name(LRUX_PROF_UPDATE, "pf_update_dmma_warp_kernel");
+  return 1;
+}
+
 template <int NB, int NW, int MQ, bool RANGES>
 static int launch_pf_dmma_inst(const State& st, int k, int ld, int ncr, int ncl, int rmax, Ctx& cx, cudaStream_t s, bool probe) {
   const size_t smem = (size_t)2 * 4 * MQ * (ld + (ncr > 1 ? rmax + 8 : 0)) * sizeof(double);
@@ -232,6 +374,14 @@ int launch_pf_update_dmma(const State& st, int k, Ctx& cx, cudaStream_t s, bool 
     if (blocks <= 64) { LRUX_PFD_MQ(4, 16, true) }
     LRUX_PFD_MQ(8, 16, true)
   }
+#if LRUX_PF_DMMA_WARP_STRIPS
+  if (blocks <= 8)
+    return mq == 1 ? launch_pf_dmma_warp<8, 1>(st, k, ld, cx, s, probe)
+         : mq == 2 ? launch_pf_dmma_warp<8, 2>(st, k, ld, cx, s, probe) : launch_pf_dmma_warp<8, 4>(st, k, ld, cx, s, probe);
+  if (blocks <= 16)
+    return mq == 1 ? launch_pf_dmma_warp<16, 1>(st, k, ld, cx, s, probe)
+         : mq == 2 ? launch_pf_dmma_warp<16, 2>(st, k, ld, cx, s, probe) : launch_pf_dmma_warp<16, 4>(st, k, ld, cx, s, probe);
+#endif
   if (blocks <= 16) { LRUX_PFD_MQ(2, 8, false) }
   if (blocks <= 32) { LRUX_PFD_MQ(4, 8, false) }
   // panels beyond half the shared memory leave one CTA per SM: 16 warps instead of 8

@@ -172,13 +172,14 @@ def test_pf_large_n_paths(n, k):
     (140, 1, False, "pf_resident_k1_kernel"),     # ... 5 chunk buffers
     (200, 1, False, "pf_cluster_k1_kernel"),      # 8-CTA cluster, run-time sizes
     (256, 1, False, "pf_cluster_k1_kernel"),      # 8-CTA cluster, unrolled instance
-    (128, 2, False, "pf_update_dmma_kernel"),     # real k >= 2: 8-row strips on the FP64 tensor pipe (2 DMMAs / block)
+    (128, 2, False, "pf_update_dmma_warp_kernel"),    # real k >= 2, n <= 128: warp-owned 8-row strips on the FP64 tensor pipe
+    (136, 2, False, "pf_update_dmma_kernel"),     # n > 128: strips split over the 8 warps
     (64, 1, True, "pf_cluster_update_kernel"),    # complex: generic cluster kernel, 4-CTA
     (128, 2, True, "pf_cluster_update_kernel"),   # ... 8-CTA, k = 2
     (96, 1, True, "pf_cluster_update_kernel"),
     (320, 1, False, "pf_update_dmma_kernel"),     # k = 1 beyond the cluster kernels: Y pass + DMMA strips (1 DMMA / block)
     (320, 2, True, "pf_update_stream_kernel"),    # complex: Y pass + streaming update
-    (34, 2, False, "pf_update_dmma_kernel"),      # ragged: n not a multiple of 8, two strips straddle walkers
+    (34, 2, False, "pf_update_dmma_warp_kernel"), # ragged: n not a multiple of 8, strips of two walkers in one range
     (520, 2, False, "pf_update_dmma_kernel"),     # 16 warps
 ])
 def test_pf_update_kernel_by_shape(n, k, cplx, name):
@@ -193,13 +194,16 @@ def test_pf_update_kernel_by_shape(n, k, cplx, name):
     (256, 4),      # 2 DMMAs per block, 4 blocks per warp
     (130, 8),      # 2k = 16: 4 DMMAs per block
     (512, 4),      # 8 blocks per warp (the shape VERDICT r1 item 7 names)
+    (64, 4),       # n <= 128: warp-owned strips (pf_update_dmma_warp_kernel), 8 blocks, prefetched
+    (128, 8),      # ... 16 blocks, 4 DMMAs per block
+    (100, 3),      # ... ragged
 ])
 def test_pf_update_dmma_larger_ranks(n, k):
     """pf_update_dmma_kernel with 2 and 4 DMMAs per 8 x 8 block, every proposal applied (rank >= 3
     proposals are rarely accepted by the Metropolis test); the stored inverse must stay EXACTLY
     skew (parity_util.compare checks Ti == -Ti^T bit for bit)."""
     _run("pf", 1900 + n + k, 3, n, 2 * n, k, 0, 8, walkers=[0, 2], scratch_every=2, forced=True,
-         kernel={"update": "pf_update_dmma_kernel"})
+         kernel={"update": "pf_update_dmma_warp_kernel" if n <= 128 else "pf_update_dmma_kernel"})
 
 
 @pytest.mark.parametrize("n,k,steps", [
