@@ -20,6 +20,9 @@
 #define LRUX_RATIO_FLY_MAX_KT 4
 #endif
 // CTAs per SM the ratio kernel is compiled for (64 registers; complex k = 8 keeps 128: it would spill)
+#ifndef LRUX_RATIO_WARP
+#define LRUX_RATIO_WARP 1
+#endif
 #ifndef LRUX_RATIO_MINB
 #define LRUX_RATIO_MINB 4
 #endif
@@ -267,6 +270,118 @@ det_ratio_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __re
     for (int a = 0; a < KT; ++a)
       if (lane == a && a < k) st.pend_idx[(size_t)w * kmax + a] = P[a];
   }
+}
+
+// Narrow matrices (n <= 128): ONE WARP per walker, 8 walkers per CTA.  With one CTA per walker the
+// ratio had become the step at these sizes (n = 64, k = 8, W = 32768: 306 us of ratio for 77 us of
+// update -- one small CTA, two barriers and a single-warp tail per walker).  Lane l owns the
+// columns l, l + 32, ... (EPT of them) of the k gathered columns; the delay buffer is walked as in
+// det_ratio_kernel (Eq. 14), C_eff and N are stashed, R = N C_eff comes from k^2 warp reductions
+// and the elimination is warp_det_inv on the warp's own 2 x KT x KT doubles of shared memory.
+template <typename T, int KT, int EPT>
+__global__ void __launch_bounds__(256)
+det_ratio_warp_kernel(State st, int k, const int32_t* __restrict__ idx, const T* __restrict__ rows,
+                      T* __restrict__ ratio_out) {
+  using S = Sc<T>;
+  __shared__ T Rs[8][KT * KT];
+  __shared__ T Ri[8][KT * KT];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t w = (int64_t)blockIdx.x * 8 + warp;
+  const int n = st.n, kmax = st.kmax;
+  if (blockIdx.x == 0 && threadIdx.x == 0) st.counters[0] = 0;
+  if (w >= st.W) return;
+  int P[KT];
+  bool bad = false;
+#pragma unroll
+  for (int a = 0; a < KT; ++a) {
+    P[a] = a < k ? idx[(size_t)w * k + a] : -1 - a;
+    if (a < k && (P[a] < 0 || P[a] >= n)) bad = true;
+#pragma unroll
+    for (int c = 0; c < a; ++c)
+      if (a < k && P[c] == P[a]) bad = true;
+  }
+  if (bad) {
+    if (lane == 0) {
+      ratio_out[w] = S::nan();
+      ((T*)st.pend_ratio)[w] = S::nan();
+      st.pend_ok[w] = 0;
+      atomicOr(&st.info[w], 2);
+    }
+    return;
+  }
+  const int fill = st.cap ? st.fill[w] : 0;
+  const T* Tw = (const T*)st.Ti + (size_t)w * n * n;
+  const T* Ab = st.cap ? (const T*)st.Abuf + (size_t)w * st.cap * n : nullptr;
+  const T* Bb = st.cap ? (const T*)st.Bbuf + (size_t)w * st.cap * n : nullptr;
+  T* pC = (T*)st.pend_C + (size_t)w * kmax * n;
+  T* pN = (T*)st.pend_N + (size_t)w * kmax * n;
+  T c[KT][EPT];
+#pragma unroll
+  for (int e = 0; e < EPT; ++e) {
+    const int i = lane + 32 * e;
+#pragma unroll
+    for (int a = 0; a < KT; ++a) c[a][e] = (a < k && i < n) ? Tw[(size_t)P[a] * n + i] : S::zero();
+  }
+  for (int s2 = 0; s2 < fill; ++s2) {
+    T av[EPT];
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+      const int i = lane + 32 * e;
+      av[e] = i < n ? Ab[(size_t)s2 * n + i] : S::zero();
+    }
+#pragma unroll
+    for (int a = 0; a < KT; ++a) {
+      if (a < k) {
+        const T bp = Bb[(size_t)s2 * n + P[a]];          // b_t^T v: the same address for the whole warp
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) c[a][e] = S::fnma(bp, av[e], c[a][e]);
+      }
+    }
+  }
+#pragma unroll
+  for (int e = 0; e < EPT; ++e) {
+    const int i = lane + 32 * e;
+    if (i < n) {
+#pragma unroll
+      for (int a = 0; a < KT; ++a)
+        if (a < k) pC[(size_t)a * n + i] = c[a][e];
+    }
+  }
+#pragma unroll
+  for (int b = 0; b < KT; ++b) {
+    if (b < k) {
+      T x[EPT];
+#pragma unroll
+      for (int e = 0; e < EPT; ++e) {
+        const int i = lane + 32 * e;
+        x[e] = i < n ? rows[((size_t)w * k + b) * n + i] : S::zero();
+        if (i < n) pN[(size_t)b * n + i] = x[e];
+      }
+#pragma unroll
+      for (int a = 0; a < KT; ++a) {
+        if (a < k) {
+          T v = S::zero();
+#pragma unroll
+          for (int e = 0; e < EPT; ++e) v = S::fma(x[e], c[a][e], v);
+          v = warp_sum(v);
+          if (lane == 0) Rs[warp][b * KT + a] = v;
+        }
+      }
+    }
+  }
+  __syncwarp();
+  bool ok;
+  const T det = warp_det_inv<T, KT>(Rs[warp], Ri[warp], k, KT, &ok, lane);
+  if (lane == 0) {
+    ratio_out[w] = det;
+    ((T*)st.pend_ratio)[w] = det;
+    st.pend_ok[w] = ok ? 1 : 0;
+  }
+  T* pR = (T*)st.pend_Rinv + (size_t)w * st.kc * st.kc;
+  for (int q = lane; q < k * k; q += 32) pR[(q / k) * st.kc + (q % k)] = Ri[warp][(q / k) * KT + (q % k)];
+#pragma unroll
+  for (int a = 0; a < KT; ++a)
+    if (lane == a && a < k) st.pend_idx[(size_t)w * kmax + a] = P[a];
 }
 
 // ---------------------------------------------------------------- select + amplitude (a8)
@@ -1377,6 +1492,17 @@ static int launch_ratio_kt(const State& st, int k, const int32_t* d_idx, const v
   // one CTA per 256-column slice: 128 threads x 2 elements (n <= 256: a single slice,
   // 1 element per thread when n <= 128), else 256 threads x 1 element
   const int n = st.n;
+#if LRUX_RATIO_WARP
+  // one warp per walker, 8 walkers per CTA: k <= 4 without a delay buffer, k <= 2 with one (measured at
+  // n = 64 / 128, ratio time per step: k=1 0.38x / 0.49x, k=4 0.49x / 0.66x of the CTA kernel's; k=8 0.76x /
+  // 0.93x -- not worth a second arithmetic order --; with K = 8: k=1 0.49x, k=4 1.29x)
+  if (n <= 128 && KT <= 4 && (st.cap == 0 || KT <= 2)) {
+    auto kw = n <= 32 ? det_ratio_warp_kernel<T, KT, 1> : n <= 64 ? det_ratio_warp_kernel<T, KT, 2>
+                                                                  : det_ratio_warp_kernel<T, KT, 4>;
+    kw<<<(unsigned)((st.W + 7) / 8), 256, 0, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
+    return 1;
+  }
+#endif
   const int nsplit = (n + kRatioSlice - 1) / kRatioSlice;
   const dim3 grid((unsigned)st.W, (unsigned)nsplit);
   const size_t sm = (size_t)st.cap * KT * sizeof(T);   // <= kRatioCoefSmemMax (checked at init)
@@ -1402,7 +1528,7 @@ static int launch_ratio_t(const State& st, int k, const int32_t* d_idx, const vo
 int launch_det_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
                      void* d_ratio, Ctx& cx, cudaStream_t s) {
   ProfScope ps(&cx.prof, LRUX_PROF_RATIO, s);
-  cx.name(LRUX_PROF_RATIO, "det_ratio_kernel");
+  cx.name(LRUX_PROF_RATIO, (LRUX_RATIO_WARP && st.n <= 128 && k <= 4 && (st.cap == 0 || k <= 2)) ? "det_ratio_warp_kernel" : "det_ratio_kernel");
   const int r = st.dt == LRUX_F64 ? launch_ratio_t<double>(st, k, d_idx, d_rows, d_ratio, cx, s)
                                   : launch_ratio_t<cplx>(st, k, d_idx, d_rows, d_ratio, cx, s);
   return (r > 0 && cudaGetLastError() == cudaSuccess) ? r : -1;

@@ -130,6 +130,21 @@ def test_det_update_dmma_warp_strips(n, k):
          acc_range=(0.0, 1.0), kernel={"update": "det_update_dmma_warp_kernel"})
 
 
+@pytest.mark.parametrize("n,k,K,cplx,name", [
+    (64, 1, 0, False, "det_ratio_warp_kernel"),    # n <= 128: one warp per walker, 8 walkers per CTA
+    (128, 4, 0, False, "det_ratio_warp_kernel"),
+    (100, 3, 0, False, "det_ratio_warp_kernel"),   # ragged: 100 = 3 x 32 + 4 columns
+    (33, 2, 0, True, "det_ratio_warp_kernel"),     # complex, odd n
+    (96, 2, 4, False, "det_ratio_warp_kernel"),    # with a delay buffer: k <= 2
+    (64, 4, 4, False, "det_ratio_kernel"),         # k = 4 with a delay buffer, and k = 8: one CTA per walker
+    (64, 8, 0, False, "det_ratio_kernel"),
+])
+def test_det_ratio_kernel_by_shape(n, k, K, cplx, name):
+    """The two determinant ratio kernels, each reached by its shape and checked by name."""
+    _run("det", 7100 + n + k + K, 9, n, 2 * n, k, K, 30, cplx, walkers=[0, 4, 8], scratch_every=1,
+         forced=(k == 8), acc_range=(0.0, 1.0), kernel={"ratio": name})
+
+
 def test_det_tma_update_n4096_properties():
     """n=4096 (32 KB rows, one row per bulk copy): the oracle is too slow here, so check
     what holds at any size: A_T A_T^-1 = 1 and the tracked amplitude against a library
