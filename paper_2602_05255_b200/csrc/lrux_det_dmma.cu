@@ -39,8 +39,10 @@
 #define LRUX_DMMA_MAXCOLS 1024
 #endif
 
+// 1: warp-owned strips for n <= 128; 2: also for n <= 256 (32 blocks per warp, one CTA per SM: n=256 k=4 / 8
+// 0.88 / 0.87 of HBM against 0.81 / 0.80 with the strip split over the 8 warps)
 #ifndef LRUX_DMMA_WARP_STRIPS
-#define LRUX_DMMA_WARP_STRIPS 1
+#define LRUX_DMMA_WARP_STRIPS 2
 #endif
 
 namespace lrux {
@@ -212,13 +214,13 @@ __global__ void __launch_bounds__(NW * 32, NW <= 8 ? 2 : 1) det_update_dmma_kern
   if constexpr (CLUSTER) cg::this_cluster().sync();   // no CTA exits while a peer may still write its cpart
 }
 
-// Narrow matrices (n <= 128): ONE WARP owns a whole 8-row strip (NB <= 16 blocks of 8 columns), so
+// Narrow matrices (n <= 256): ONE WARP owns a whole 8-row strip (NB <= 32 blocks of 8 columns), so
 // the dots need no exchange and there is no barrier per strip -- only one per walker, when N and C
 // are restaged.  With the strip split over 8 warps a strip of n = 128 is 8 KB of work per CTA
 // barrier (0.31 / 0.56 of HBM at n = 64 / 128, k = 4).  Strips of a walker go round-robin to the
 // 8 warps of the CTA that holds the walker's N, C; CTAs take contiguous balanced strip ranges.
 template <int NB>
-__global__ void __launch_bounds__(256, 2) det_update_dmma_warp_kernel(State st, int k, int ncl) {
+__global__ void __launch_bounds__(256, NB <= 16 ? 2 : 1) det_update_dmma_warp_kernel(State st, int k, int ncl) {
   constexpr int KT = 8, NW = 8;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int n = st.n, kmax = st.kmax;
@@ -387,6 +389,9 @@ int launch_det_update_dmma(const State& st, int k, Ctx& cx, cudaStream_t s, bool
 #if LRUX_DMMA_WARP_STRIPS
   if (blocks <= 8) return launch_dmma_warp<8>(st, k, ncl, cx, s, probe);     // n <= 64
   if (blocks <= 16) return launch_dmma_warp<16>(st, k, ncl, cx, s, probe);   // n <= 128
+#if LRUX_DMMA_WARP_STRIPS >= 2
+  if (blocks <= 32) return launch_dmma_warp<32>(st, k, ncl, cx, s, probe);   // n <= 256: one CTA per SM
+#endif
 #endif
 #define LRUX_DMMA_CASE(NB_, NW_) \
   if (blocks <= NB_ * NW_) return launch_dmma_inst<NB_, NW_>(st, k, CL, ncl, cx, s, probe);

@@ -25,6 +25,8 @@
 #include "lrux_common.cuh"
 #include "lrux_internal.h"
 
+// 1: warp-owned strips for n <= 128; 2: also for n <= 256 (32 blocks per warp, one CTA per SM) -- measured at
+// n = 256: k=2 0.80 (same), k=4 0.72 against 0.73-0.77, k=8 0.53 against 0.58: not shipped
 #ifndef LRUX_PF_DMMA_WARP_STRIPS
 #define LRUX_PF_DMMA_WARP_STRIPS 1
 #endif
@@ -198,7 +200,7 @@ pf_update_dmma_kernel(State st, int k, int ld, int ncr_, int ncl, int rmax) {
 // split over 8 warps each warp had 1-2 blocks (0.5-1 KB) of work per loop iteration.  CTAs take
 // contiguous balanced strip ranges; the only barriers are those around the staging of y, g.
 template <int NB, int MQ>
-__global__ void __launch_bounds__(256, 2) pf_update_dmma_warp_kernel(State st, int k, int ld) {
+__global__ void __launch_bounds__(256, NB <= 16 ? 2 : 1) pf_update_dmma_warp_kernel(State st, int k, int ld) {
   constexpr int MH = 4 * MQ, NW = 8;
   constexpr int kMaxC = 2 * kMaxK;
   constexpr bool PF = NB <= 8;                  // a second strip in registers only where it fits
@@ -381,6 +383,11 @@ int launch_pf_update_dmma(const State& st, int k, Ctx& cx, cudaStream_t s, bool 
   if (blocks <= 16)
     return mq == 1 ? launch_pf_dmma_warp<16, 1>(st, k, ld, cx, s, probe)
          : mq == 2 ? launch_pf_dmma_warp<16, 2>(st, k, ld, cx, s, probe) : launch_pf_dmma_warp<16, 4>(st, k, ld, cx, s, probe);
+#if LRUX_PF_DMMA_WARP_STRIPS >= 2
+  if (blocks <= 32)     // n <= 256: 32 blocks per warp, one CTA per SM
+    return mq == 1 ? launch_pf_dmma_warp<32, 1>(st, k, ld, cx, s, probe)
+         : mq == 2 ? launch_pf_dmma_warp<32, 2>(st, k, ld, cx, s, probe) : launch_pf_dmma_warp<32, 4>(st, k, ld, cx, s, probe);
+#endif
 #endif
   if (blocks <= 16) { LRUX_PFD_MQ(2, 8, false) }
   if (blocks <= 32) { LRUX_PFD_MQ(4, 8, false) }

@@ -122,9 +122,9 @@ def test_det_large_row_paths(n, k, K, cplx, steps, kernel):
          kernel={"update" if K == 0 else "append": kernel})
 
 
-@pytest.mark.parametrize("n,k", [(64, 4), (128, 8), (100, 3), (34, 5), (128, 4)])
+@pytest.mark.parametrize("n,k", [(64, 4), (128, 8), (100, 3), (34, 5), (128, 4), (256, 8), (200, 5)])
 def test_det_update_dmma_warp_strips(n, k):
-    """Real k >= 3 at n <= 128: one warp owns a whole 8-row strip (det_update_dmma_warp_kernel);
+    """Real k >= 3 at n <= 256: one warp owns a whole 8-row strip (det_update_dmma_warp_kernel);
     n = 100 / 34: ragged last block and last strip, strips of two walkers in one CTA's range."""
     _run("det", 6400 + n + k, 5, n, 2 * n, k, 0, 12, walkers=[0, 2, 4], scratch_every=1, forced=(k > 4),
          acc_range=(0.0, 1.0), kernel={"update": "det_update_dmma_warp_kernel"})
