@@ -216,6 +216,14 @@ _GUARD_SHAPES = [
     ("det", 128, 16, 0, False, True), ("det", 64, 5, 3, False, True), ("det", 47, 2, 5, True, True),
     ("pf", 32, 1, 0, False, False), ("pf", 64, 2, 4, False, True), ("pf", 130, 1, 8, False, False),
     ("pf", 96, 4, 0, False, True),
+    # kernels added late in round 2
+    ("det", 1028, 3, 5, True, True),      # det_append_dmma_stream_kernel + in-place finish (ragged units)
+    ("det", 516, 4, 6, False, True),      # det_append_stream_real_kernel, shared copy of N
+    ("det", 100, 3, 4, False, True),      # ... per-warp copies of N; det_ratio_kernel with a delay buffer
+    ("det", 72, 4, 0, False, True),       # det_update_dmma_warp_kernel, det_ratio_warp_kernel
+    ("det", 250, 8, 0, False, True),      # 32 blocks per warp, DMMA partial R in the ratio
+    ("pf", 100, 3, 0, False, True),       # pf_update_dmma_warp_kernel, row-dot Y pass
+    ("pf", 1040, 2, 0, False, True),      # pf_update_dmma_kernel with column ranges
 ]
 
 
