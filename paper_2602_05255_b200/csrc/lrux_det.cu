@@ -20,8 +20,10 @@
 #define LRUX_RATIO_FLY_MAX_KT 4
 #endif
 // CTAs per SM the ratio kernel is compiled for (64 registers; complex k = 8 keeps 128: it would spill)
+// 1: one warp per walker in the ratio for n <= 128; 2: also n <= 256 with k <= 2 and no delay buffer (configs[1]:
+// ratio 22.5 -> 19.1 us per step, 18.88 M -> 19.10 M walker-updates/s; with K = 16 the CTA kernel is faster)
 #ifndef LRUX_RATIO_WARP
-#define LRUX_RATIO_WARP 1
+#define LRUX_RATIO_WARP 2
 #endif
 #ifndef LRUX_RATIO_MINB
 #define LRUX_RATIO_MINB 4
@@ -1496,9 +1498,9 @@ static int launch_ratio_kt(const State& st, int k, const int32_t* d_idx, const v
   // one warp per walker, 8 walkers per CTA: k <= 4 without a delay buffer, k <= 2 with one (measured at
   // n = 64 / 128, ratio time per step: k=1 0.38x / 0.49x, k=4 0.49x / 0.66x of the CTA kernel's; k=8 0.76x /
   // 0.93x -- not worth a second arithmetic order --; with K = 8: k=1 0.49x, k=4 1.29x)
-  if (n <= 128 && KT <= 4 && (st.cap == 0 || KT <= 2)) {
+  if ((n <= 128 && KT <= 4 && (st.cap == 0 || KT <= 2)) || (LRUX_RATIO_WARP >= 2 && n <= 256 && KT <= 2 && st.cap == 0)) {
     auto kw = n <= 32 ? det_ratio_warp_kernel<T, KT, 1> : n <= 64 ? det_ratio_warp_kernel<T, KT, 2>
-                                                                  : det_ratio_warp_kernel<T, KT, 4>;
+            : n <= 128 ? det_ratio_warp_kernel<T, KT, 4> : det_ratio_warp_kernel<T, (KT <= 2 ? KT : 2), 8>;
     kw<<<(unsigned)((st.W + 7) / 8), 256, 0, s>>>(st, k, d_idx, (const T*)d_rows, (T*)d_ratio);
     return 1;
   }
@@ -1528,7 +1530,7 @@ static int launch_ratio_t(const State& st, int k, const int32_t* d_idx, const vo
 int launch_det_ratio(const State& st, int k, const int32_t* d_idx, const void* d_rows,
                      void* d_ratio, Ctx& cx, cudaStream_t s) {
   ProfScope ps(&cx.prof, LRUX_PROF_RATIO, s);
-  cx.name(LRUX_PROF_RATIO, (LRUX_RATIO_WARP && st.n <= 128 && k <= 4 && (st.cap == 0 || k <= 2)) ? "det_ratio_warp_kernel" : "det_ratio_kernel");
+  cx.name(LRUX_PROF_RATIO, (LRUX_RATIO_WARP && ((st.n <= 128 && k <= 4 && (st.cap == 0 || k <= 2)) || (LRUX_RATIO_WARP >= 2 && st.n <= 256 && k <= 2 && st.cap == 0))) ? "det_ratio_warp_kernel" : "det_ratio_kernel");
   const int r = st.dt == LRUX_F64 ? launch_ratio_t<double>(st, k, d_idx, d_rows, d_ratio, cx, s)
                                   : launch_ratio_t<cplx>(st, k, d_idx, d_rows, d_ratio, cx, s);
   return (r > 0 && cudaGetLastError() == cudaSuccess) ? r : -1;

@@ -136,6 +136,8 @@ def test_det_update_dmma_warp_strips(n, k):
     (100, 3, 0, False, "det_ratio_warp_kernel"),   # ragged: 100 = 3 x 32 + 4 columns
     (33, 2, 0, True, "det_ratio_warp_kernel"),     # complex, odd n
     (96, 2, 4, False, "det_ratio_warp_kernel"),    # with a delay buffer: k <= 2
+    (256, 2, 0, False, "det_ratio_warp_kernel"),   # configs[1] shape: n <= 256, k <= 2, no delay buffer
+    (256, 2, 4, False, "det_ratio_kernel"),        # ... with a delay buffer: one CTA per walker
     (64, 4, 4, False, "det_ratio_kernel"),         # k = 4 with a delay buffer, and k = 8: one CTA per walker
     (64, 8, 0, False, "det_ratio_kernel"),
 ])
