@@ -27,6 +27,9 @@
 
 // 1: warp-owned strips for n <= 128; 2: also for n <= 256 (32 blocks per warp, one CTA per SM) -- measured at
 // n = 256: k=2 0.80 (same), k=4 0.72 against 0.73-0.77, k=8 0.53 against 0.58: not shipped
+#ifndef LRUX_PF_DMMA_PAD
+#define LRUX_PF_DMMA_PAD 4
+#endif
 #ifndef LRUX_PF_DMMA_WARP_STRIPS
 #define LRUX_PF_DMMA_WARP_STRIPS 1
 #endif
@@ -42,7 +45,9 @@ __device__ __forceinline__ void dmma884p(double& d0, double& d1, double a, doubl
 // NB = 8-column blocks per warp and strip, NW = warps per CTA, MQ = DMMAs per block (4 MQ >= 2k).
 // The columns are cut into ncr ranges of ncl (8 NB NW >= ncl; ncr = 1 up to n = 1024): CTA b
 // works on range b mod ncr for all of its strips and keeps only that range of y and g in
-// shared memory (row stride ld >= ncl + 8, 8 mod 16 doubles: conflict-free).  With ncr > 1
+// shared memory (row stride ld >= ncl, 4 mod 16 doubles: the 8-byte fragment loads of a half-warp --
+// rows q = 0..3, columns r = 0..3 -- then fall into 16 different bank pairs; with 8 mod 16 the ncu capture at
+// 2k = 16 showed 1.8 bank conflicts per shared load).  With ncr > 1
 // the A fragments (y, g of the strip's own ROWS, which may lie in another range) come from a
 // second, small pair of panels that holds y and g of `rmax` consecutive rows and is restaged
 // whenever the strips leave it -- the same staging arithmetic, so that mirrored elements
@@ -57,7 +62,7 @@ pf_update_dmma_kernel(State st, int k, int ld, int ncr_, int ncl, int rmax) {
   const int n = st.n, kmax = st.kmax, m = 2 * k;
   double* yv = (double*)smem_raw;           // [MH][ld]
   double* gv = yv + (size_t)MH * ld;        // [MH][ld]
-  const int ldr = rmax + 8;
+  const int ldr = rmax + LRUX_PF_DMMA_PAD;
   double* yr = gv + (size_t)MH * ld;        // [MH][ldr]  (ncr > 1) y of rows [row_lo, row_lo + rmax)
   double* gr = yr + (size_t)MH * ldr;       // [MH][ldr]
   __shared__ double Ri[kMaxC * kMaxC];
@@ -363,7 +368,7 @@ int launch_pf_update_dmma(const State& st, int k, Ctx& cx, cudaStream_t s, bool 
   for (;; ncr *= 2) {
     if (ncr > 16) return 0;
     ncl = (((n + ncr - 1) / ncr) + 7) & ~7;
-    ld = ((ncl + 15) & ~15) + 8;
+    ld = ((ncl + 15) & ~15) + LRUX_PF_DMMA_PAD;
     // (2k = 16 with ranges narrow enough for two CTAs per SM was measured too: no gain, 0.53-0.67 either way)
     if (ncl <= 1024 && (size_t)2 * 4 * mq * (ld + (ncr > 1 ? rmax + 8 : 0)) * sizeof(double) <= 200 * 1024) break;
   }
